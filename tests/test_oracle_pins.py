@@ -1,0 +1,479 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (no GPU).
+
+Every pin compares ``oracle/`` with something that is NOT the oracle: numbers the paper prints
+(tests/golden/), brute-force numerical differentiation of Eq. 22, quadrature of the defining k-integral,
+textbook free-space limits, Hasimoto's periodic-array constant, and structural invariants
+(xi-independence, symmetry, positive definiteness, spectral convergence of O2 to O1).
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def _gold(name):
+    with open(os.path.join(GOLD, name)) as fh:
+        rows = [ln.split() for ln in fh if ln.strip() and not ln.startswith("#")]
+    return [float(v) for v in rows[0]]
+
+
+def _rel(a, b):
+    return float(np.linalg.norm(np.asarray(a) - np.asarray(b)) / np.linalg.norm(np.asarray(b)))
+
+
+def _ewald_cut(xi, L, digits=6.5):
+    """(nimg, kmax) so that exp(-xi^2 r^2) and exp(-k^2/4xi^2) are below exp(-digits^2) at the cut."""
+    nimg = int(math.ceil(digits / xi / L)) + 1
+    kmax = int(math.ceil(xi * L / (2 * math.pi) * 2 * digits)) + 1
+    return nimg, kmax
+
+
+# ------------------------------------------------------------------------------------------------
+# Printed value: Eq. 37
+# ------------------------------------------------------------------------------------------------
+def test_eq37_self_term_printed_coefficients(oracle):
+    c0, c2, c4, den = _gold("eq37_self_term.txt")
+    for a, xi, eta0 in [(1.0, 0.5, 1.0), (2.0, 0.31, 0.7), (0.5, 1.9, 2.5)]:
+        want = xi * (c0 + c2 * (a * xi) ** 2 + c4 * (a * xi) ** 4) / (den * eta0 * math.pi ** 1.5)
+        assert oracle.self_coeffs(a, xi, eta0)[0] == pytest.approx(want, rel=1e-14)
+
+
+def test_self_terms_equal_the_k_integral(oracle):
+    """The i=j term of the unrestricted wave sum (Eq. 35) in the continuum limit sum_k/V -> int d^3k/(2pi)^3,
+    with the angular averages <I - kk> = 2/3 I, <k_a k_c> = delta/3, <k_a k_b k_c k_d> = (dd+dd+dd)/15:
+      UF: (1/3 pi^2 eta0) int H (1 - cF k^2)^2 dk;  Omega-T: (1/12 pi^2 eta0) int k^2 H dk;
+      ES: (1/10 pi^2 eta0) int k^2 H (1 - cS k^2)^2 dk,   H = (1 + k^2/4xi^2) exp(-k^2/4xi^2)  (Eq. 23, 36)."""
+    from scipy.integrate import quad
+    for a, xi, eta0 in [(1.0, 0.6, 1.0), (1.7, 0.9, 0.4)]:
+        H = lambda k: (1 + k * k / (4 * xi * xi)) * math.exp(-k * k / (4 * xi * xi))
+        cF, cS = a * a / 6, a * a / 10
+        uf = quad(lambda k: H(k) * (1 - cF * k * k) ** 2, 0, 40 * xi, epsabs=0, epsrel=1e-13)[0] / (3 * math.pi ** 2 * eta0)
+        wt = quad(lambda k: k * k * H(k), 0, 40 * xi, epsabs=0, epsrel=1e-13)[0] / (12 * math.pi ** 2 * eta0)
+        es = quad(lambda k: k * k * H(k) * (1 - cS * k * k) ** 2, 0, 40 * xi, epsabs=0, epsrel=1e-13)[0] / (10 * math.pi ** 2 * eta0)
+        got = oracle.self_coeffs(a, xi, eta0)
+        assert got[0] == pytest.approx(uf, rel=1e-11)
+        assert got[1] == pytest.approx(wt, rel=1e-11)
+        assert got[2] == pytest.approx(es, rel=1e-11)
+
+
+# ------------------------------------------------------------------------------------------------
+# Eq. 22 and everything generated from it, against brute-force numerical differentiation
+# ------------------------------------------------------------------------------------------------
+def _mp_setup(xi):
+    import mpmath as mp
+    mp.mp.dps = 32
+    xim = mp.mpf(xi)
+
+    def phi(x, y, z):
+        r = mp.sqrt(x * x + y * y + z * z)
+        return r * mp.erfc(xim * r) - mp.exp(-xim * xim * r * r) / (xim * mp.sqrt(mp.pi))
+
+    def chi(x, y, z):
+        r = mp.sqrt(x * x + y * y + z * z)
+        return mp.erfc(xim * r) / r
+
+    return mp, phi, chi
+
+
+def test_radial_chain_against_numerical_derivatives_of_eq22(oracle):
+    """Families B, C, D = lap^n Phi and ((1/r)d/dr)^n of each, against mpmath derivatives of Eq. 22."""
+    import mpmath as mp
+    xi = 0.7
+    mp.mp.dps = 50
+    xim = mp.mpf(xi)
+    phi_r = lambda r: r * mp.erfc(xim * r) - mp.exp(-xim * xim * r * r) / (xim * mp.sqrt(mp.pi))
+    chi_r = lambda r: mp.erfc(xim * r) / r
+
+    def lap(f):
+        return lambda r: mp.diff(f, r, 2) + 2 * mp.diff(f, r, 1) / r
+
+    def D1(f):
+        return lambda r: mp.diff(f, r, 1) / r
+
+    fams = {0: phi_r, 1: lap(phi_r), 4: chi_r, 5: lap(chi_r)}
+    for r in (0.9, 2.3):
+        for fam, f in fams.items():
+            g = f
+            for n in range(0, 3):
+                want = float(g(mp.mpf(r)))
+                got = oracle.radial(fam, n, xi, r)
+                assert got == pytest.approx(want, rel=1e-11, abs=1e-13), (fam, n, r)
+                g = D1(g)
+    # closed forms that follow from Eq. 22 by hand (checked here against the mechanical chain)
+    for r in (0.7, 1.9, 4.0):
+        g = math.exp(-xi * xi * r * r)
+        sp = math.sqrt(math.pi)
+        assert oracle.radial(0, 1, xi, r) == pytest.approx(math.erfc(xi * r) / r, rel=1e-13)
+        assert oracle.radial(1, 0, xi, r) == pytest.approx(2 * math.erfc(xi * r) / r - 2 * xi / sp * g, rel=1e-13)
+        assert oracle.radial(2, 0, xi, r) == pytest.approx(4 * xi ** 3 / sp * (5 - 2 * xi * xi * r * r) * g, rel=1e-12)
+        assert oracle.radial(3, 0, xi, r) == pytest.approx(
+            8 * xi ** 5 / sp * (-21 + 24 * xi ** 2 * r ** 2 - 4 * xi ** 4 * r ** 4) * g, rel=1e-12)
+        assert oracle.radial(5, 0, xi, r) == pytest.approx(4 * xi ** 3 / sp * g, rel=1e-12)
+
+
+def _operator_apply(poly, base, point, cache):
+    """Apply a polynomial in (dx,dy,dz) (sympy Poly) to the scalar function ``base`` at ``point``."""
+    import mpmath as mp
+    total = mp.mpf(0)
+    for (nx, ny, nz), coeff in poly.terms():
+        key = (id(base), nx, ny, nz)
+        if key not in cache:
+            cache[key] = mp.diff(base, point, (nx, ny, nz)) if (nx + ny + nz) else base(*point)
+        total += mp.mpf(float(coeff)) * cache[key]
+    return total
+
+
+def test_pair_couplings_against_cartesian_differentiation_of_the_definition(oracle):
+    """All real-space couplings of one pair (U,Omega,E,p <- F,T,S,s), from the definition
+    (Eq. 13-15 Faxen, Eq. 17 multipoles, Eq. 22 Phi, Eq. 26/29-31/34 compressible part) written as
+    polynomials in the Cartesian derivative operators acting on Phi and chi, evaluated by brute-force
+    high-precision numerical differentiation -- no radial reduction, no tensor identities."""
+    import mpmath as mp
+    import sympy as sp
+    xi, eta0 = 0.8, 1.3
+    ai, aj = 1.2, 0.7
+    xvec = (0.9, -1.4, 0.6)
+    rng = np.random.default_rng(5)
+    F, T, S5, s = rng.standard_normal(3), rng.standard_normal(3), rng.standard_normal(5), 0.83
+    S = np.array([[S5[0], S5[1], S5[2]], [S5[1], S5[3], S5[4]], [S5[2], S5[4], -(S5[0] + S5[3])]])
+
+    mp_, phi, chi = _mp_setup(xi)
+    d = sp.symbols("dx dy dz")
+    lap = d[0] ** 2 + d[1] ** 2 + d[2] ** 2
+    eps = sp.LeviCivita
+    k0 = sp.Rational(1) / (8 * sp.pi * sp.Float(eta0, 30))
+    cFi, cFj, cSi, cSj = [sp.Float(v, 30) for v in (ai * ai / 6, aj * aj / 6, ai * ai / 10, aj * aj / 10)]
+    Jop = lambda a, b: (lap if a == b else 0) - d[a] * d[b]
+    Ff, Tf, Sf = [sp.Float(v, 30) for v in F], [sp.Float(v, 30) for v in T], [[sp.Float(v, 30) for v in row] for row in S]
+    # disturbance velocity of source j (operators on Phi), Eq. 17 with J -> J_R
+    v_phi = []
+    for a in range(3):
+        e = 0
+        for b in range(3):
+            e += Jop(a, b) * (1 + cFj * lap) * Ff[b]
+            for g in range(3):
+                e += -d[g] * Jop(a, b) * (1 + cSj * lap) * Sf[b][g]
+        for g in range(3):
+            for m in range(3):
+                e += sp.Rational(1, 2) * eps(a, g, m) * d[g] * lap * Tf[m]
+        v_phi.append(k0 * e)
+    # source flow of the pressure moment (operators on chi), Eq. 26/34: v = grad(psi_R) s, psi_R = -chi/(16 pi eta0)
+    kq = -sp.Rational(1) / (16 * sp.pi * sp.Float(eta0, 30))
+    v_chi = [kq * d[a] * sp.Float(s, 30) for a in range(3)]
+
+    point = tuple(mp.mpf(v) for v in xvec)
+    cache = {}
+
+    def ev(op_phi, op_chi):
+        tot = mp.mpf(0)
+        if op_phi != 0:
+            tot += _operator_apply(sp.Poly(sp.expand(op_phi), *d), phi, point, cache)
+        if op_chi != 0:
+            tot += _operator_apply(sp.Poly(sp.expand(op_chi), *d), chi, point, cache)
+        return float(tot)
+
+    U = [ev((1 + cFi * lap) * v_phi[a], (1 + cFi * lap) * v_chi[a]) for a in range(3)]                 # Eq. 13
+    W = [ev(sum(sp.Rational(1, 2) * eps(a, p, q) * d[p] * v_phi[q] for p in range(3) for q in range(3)),
+            sum(sp.Rational(1, 2) * eps(a, p, q) * d[p] * v_chi[q] for p in range(3) for q in range(3)))
+         for a in range(3)]                                                                           # Eq. 14
+    E = np.array([[ev((1 + cSi * lap) * sp.Rational(1, 2) * (d[a] * v_phi[b] + d[b] * v_phi[a]),
+                      (1 + cSi * lap) * sp.Rational(1, 2) * (d[a] * v_chi[b] + d[b] * v_chi[a]))
+                   for b in range(3)] for a in range(3)])                                             # Eq. 15
+    E -= np.eye(3) * np.trace(E) / 3
+    # pressure, Eq. 29-31: p' = -(1/4pi)[(1+cF_j lap) d_b chi F_b - (1+cS_j lap) d_b d_g chi S_bg]
+    p_op = 0
+    for b in range(3):
+        p_op += -(1 + cFj * lap) * d[b] * Ff[b]
+        for g in range(3):
+            p_op += (1 + cSj * lap) * d[b] * d[g] * Sf[b][g]
+    p = ev(0, p_op / (4 * sp.pi))
+
+    # oracle: N=2, only the n=0 image, real part only; target particle 0 at xvec, source particle 1 at 0
+    pos = np.array([xvec, (0.0, 0.0, 0.0)])
+    rad = np.array([ai, aj])
+    Fz, Tz, Sz, sz = np.zeros((2, 3)), np.zeros((2, 3)), np.zeros((2, 5)), np.zeros(2)
+    Fz[1], Tz[1], Sz[1], sz[1] = F, T, S5, s
+    Uo, Wo, Eo, so = oracle.o1_apply(pos, rad, 1.0e3, xi, Fz, Tz, Sz, sz, eta0=eta0, nimg=0, kmax=0,
+                                     parts=oracle.PART_REAL)
+    assert Uo[0] == pytest.approx(U, rel=1e-10, abs=1e-13)
+    assert Wo[0] == pytest.approx(W, rel=1e-10, abs=1e-13)
+    assert Eo[0] == pytest.approx([E[0, 0], E[0, 1], E[0, 2], E[1, 1], E[1, 2]], rel=1e-10, abs=1e-13)
+    assert so[0] == pytest.approx(4 * math.pi * ai ** 3 * p, rel=1e-10, abs=1e-13)
+
+
+# ------------------------------------------------------------------------------------------------
+# Textbook free-space limits (xi -> 0 in the n=0 real-space term: Phi -> r + const)
+# ------------------------------------------------------------------------------------------------
+def test_free_space_limits(oracle):
+    xi, eta0 = 1.0e-7, 1.0
+    a1, a2 = 1.3, 0.8
+    x = np.array([2.5, -1.0, 3.0])
+    r = np.linalg.norm(x)
+    rh = x / r
+    k0 = 1 / (8 * math.pi * eta0)
+    pos = np.array([x, np.zeros(3)])
+    rad = np.array([a1, a2])
+    Z3, Z5 = np.zeros((2, 3)), np.zeros((2, 5))
+
+    def app(F=None, T=None, S=None, s=None):
+        Fz, Tz, Sz, sz = Z3.copy(), Z3.copy(), Z5.copy(), np.zeros(2)
+        if F is not None: Fz[1] = F
+        if T is not None: Tz[1] = T
+        if S is not None: Sz[1] = S
+        if s is not None: sz[1] = s
+        return oracle.o1_apply(pos, rad, 1.0e4, xi, Fz, Tz, Sz, sz, eta0=eta0, nimg=0, kmax=0, parts=oracle.PART_REAL)
+
+    F = np.array([0.3, -1.1, 0.7])
+    U, W, E, so = app(F=F)
+    s2 = a1 * a1 + a2 * a2
+    rp = k0 * ((1 / r + s2 / (3 * r ** 3)) * F + (1 / r - s2 / r ** 3) * rh * (rh @ F))          # Rotne-Prager, unequal spheres
+    assert U[0] == pytest.approx(rp, rel=1e-6)
+    assert W[0] == pytest.approx(k0 * np.cross(F, x) / r ** 3, rel=1e-6)                        # (1/2) curl of the Stokeslet
+    assert so[0] == pytest.approx(4 * math.pi * a1 ** 3 * (x @ F) / (4 * math.pi * r ** 3), rel=1e-6)  # Eq. 29-30: p = x.F/(4 pi r^3)
+
+    T = np.array([-0.4, 0.9, 1.2])
+    U, W, E, so = app(T=T)
+    assert U[0] == pytest.approx(k0 * np.cross(T, x) / r ** 3, rel=1e-6)                        # rotlet
+    assert W[0] == pytest.approx(0.5 * k0 * (3 * rh * (rh @ T) - T) / r ** 3, rel=1e-6)
+
+    S5 = np.array([0.5, -0.2, 0.8, -1.0, 0.3])
+    S = np.array([[S5[0], S5[1], S5[2]], [S5[1], S5[3], S5[4]], [S5[2], S5[4], -(S5[0] + S5[3])]])
+    U, W, E, so = app(S=S5)
+    xSx = x @ S @ x
+    u_pt = 3 * k0 * x * xSx / r ** 5                                                            # point stresslet
+    # finite-size corrections (a1^2/6 + a2^2/10) lap of the point-stresslet field:
+    # lap[x xSx / r^5] = (2 S.x r^2 - 5 x xSx)... taken numerically instead
+    h = 1e-3
+    f = lambda y: 3 * k0 * y * (y @ S @ y) / np.linalg.norm(y) ** 5
+    lapf = sum(f(x + h * e) + f(x - h * e) - 2 * f(x) for e in np.eye(3)) / h ** 2
+    assert U[0] == pytest.approx(u_pt + (a1 * a1 / 6 + a2 * a2 / 10) * lapf, rel=2e-5)
+
+    U, W, E, so = app(s=1.7)
+    assert U[0] == pytest.approx(1.7 * x / (16 * math.pi * eta0 * r ** 3), rel=1e-6)             # Eq. 26
+    assert np.abs(W[0]).max() < 1e-12
+
+
+# ------------------------------------------------------------------------------------------------
+# Hasimoto's periodic array (N = 1)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("a_over_L", [0.05, 0.1, 0.2])
+def test_hasimoto_periodic_array(oracle, a_over_L):
+    hconst, printed = _gold("hasimoto_constant.txt")
+    assert hconst / (4 * math.pi / 3) ** (1 / 3) == pytest.approx(printed, abs=5e-3)     # Eq. 81's 1.76
+    a, L = 1.0, 1.0 / a_over_L
+    pos, rad = np.array([[0.3, 0.1, 0.7]]) * L, np.array([a])
+    F, T, S = np.array([[1.0, 0, 0]]), np.array([[0, 1.0, 0]]), np.zeros((1, 5))
+    vals = []
+    for xi in (5.0 / L, 8.0 / L):
+        nimg, kmax = _ewald_cut(xi, L)
+        U, W, E, _ = oracle.o1_apply(pos, rad, L, xi, F, T, S, nimg=nimg, kmax=kmax)
+        vals.append((6 * math.pi * a * U[0, 0], 8 * math.pi * a ** 3 * W[0, 1]))
+    tt = 1 - hconst * a_over_L + 4 * math.pi / 3 * a_over_L ** 3
+    rr = 1 - 4 * math.pi / 3 * a_over_L ** 3
+    assert vals[0][0] == pytest.approx(tt, abs=2e-7 + 30 * a_over_L ** 6)
+    assert vals[0][1] == pytest.approx(rr, abs=1e-11)
+    assert vals[0][0] == pytest.approx(vals[1][0], abs=1e-12)
+    assert vals[0][1] == pytest.approx(vals[1][1], abs=1e-12)
+
+
+# ------------------------------------------------------------------------------------------------
+# Structure of the assembled grand mobility (tiny N, polydisperse)
+# ------------------------------------------------------------------------------------------------
+@pytest.fixture(scope="module")
+def small_matrices(oracle, workloads):
+    sysm = workloads.random_small_system(1, 4, 8.0)
+    mats = {}
+    for xi in (0.5, 0.95):
+        nimg, kmax = _ewald_cut(xi, sysm["L"])
+        mats[xi] = oracle.o1_matrix(sysm["pos"], sysm["radii"], sysm["L"], xi, nimg=nimg, kmax=kmax)
+    return sysm, mats
+
+
+def test_total_is_independent_of_the_splitting_parameter(small_matrices):
+    sysm, mats = small_matrices
+    A, B = mats[0.5], mats[0.95]
+    N = sysm["N"]
+    rows = {"U": range(0, 3), "W": range(3, 6), "E": range(6, 11), "p": range(11, 12)}
+    for rn, rr in rows.items():
+        for cn, cc in rows.items():
+            ri = [12 * i + c for i in range(N) for c in rr]
+            ci = [12 * i + c for i in range(N) for c in cc]
+            a, b = A[np.ix_(ri, ci)], B[np.ix_(ri, ci)]
+            scale = np.abs(a).max()
+            if scale < 1e-15:         # Omega<-s, p<-T, p<-s vanish identically (rounding residue only)
+                assert np.abs(b).max() < 1e-15
+                continue
+            assert np.abs(a - b).max() / scale < 1e-12, (rn, cn)
+
+
+def test_removing_the_self_term_breaks_xi_independence(oracle, workloads):
+    sysm = workloads.random_small_system(1, 4, 8.0)
+    out = []
+    for xi in (0.5, 0.95):
+        nimg, kmax = _ewald_cut(xi, sysm["L"])
+        U, *_ = oracle.o1_apply(sysm["pos"], sysm["radii"], sysm["L"], xi, sysm["F"], sysm["T"], sysm["S"],
+                                nimg=nimg, kmax=kmax, parts=oracle.PART_ALL & ~oracle.PART_SELF)
+        out.append(U)
+    assert _rel(out[0], out[1]) > 1e-3
+
+
+def _gram(N):
+    """Frobenius Gram matrix of the stored 5-component basis (xx,xy,xz,yy,yz; zz implied)."""
+    def full(s5):
+        return np.array([[s5[0], s5[1], s5[2]], [s5[1], s5[3], s5[4]], [s5[2], s5[4], -(s5[0] + s5[3])]])
+    e = np.eye(5)
+    B5 = np.array([[np.sum(full(e[a]) * full(e[b])) for b in range(5)] for a in range(5)])
+    G = np.zeros((11 * N, 11 * N))
+    for i in range(N):
+        G[11 * i:11 * i + 6, 11 * i:11 * i + 6] = np.eye(6)
+        G[11 * i + 6:11 * i + 11, 11 * i + 6:11 * i + 11] = B5
+    return G
+
+
+def test_grand_mobility_is_symmetric_positive_definite(small_matrices):
+    """the grand mobility is positive definite (Lorentz reciprocal theorem) -- incompressible
+    (F,T,S) level; the dissipation is F.U + T.Omega + S:E with the Frobenius product on S, E."""
+    import scipy.linalg as sl
+    sysm, mats = small_matrices
+    N = sysm["N"]
+    idx = [12 * i + c for i in range(N) for c in range(11)]
+    A = mats[0.5][np.ix_(idx, idx)]
+    G = _gram(N)
+    Q = G @ A
+    assert np.abs(Q - Q.T).max() / np.abs(Q).max() < 1e-13
+    ev = sl.eigh(0.5 * (Q + Q.T), G, eigvals_only=True)
+    assert ev.min() > 0
+
+
+def test_rate_of_strain_rows_are_traceless_and_real_part_is_reciprocal(oracle, workloads):
+    sysm = workloads.random_small_system(3, 3, 9.0)
+    xi = 0.6
+    # block(i,j) at x equals block(j,i)^T at -x: swap the two particles' roles through the full matrix symmetry
+    nimg, kmax = _ewald_cut(xi, sysm["L"])
+    A = oracle.o1_matrix(sysm["pos"], sysm["radii"], sysm["L"], xi, nimg=nimg, kmax=kmax, parts=oracle.PART_REAL)
+    N = sysm["N"]
+    idx = [12 * i + c for i in range(N) for c in range(11)]
+    Q = _gram(N) @ A[np.ix_(idx, idx)]
+    assert np.abs(Q - Q.T).max() / np.abs(Q).max() < 1e-13
+
+
+# ------------------------------------------------------------------------------------------------
+# O2 (the algorithm) against O1 (the definition)
+# ------------------------------------------------------------------------------------------------
+def test_o2_wave_part_converges_spectrally_to_o1(oracle, workloads):
+    """Eq. 79: at m = sqrt(pi P) the wave-space error decays like exp(-P pi/2)."""
+    _, rate = _gold("paper_accuracy_claims.txt")
+    sysm = workloads.random_small_system(2, 10, 10.0)
+    xi = 0.6
+    nimg, kmax = _ewald_cut(xi, sysm["L"])
+    a = (sysm["pos"], sysm["radii"], sysm["L"], xi)
+    mom = (sysm["F"], sysm["T"], sysm["S"], sysm["s"])
+    ref = oracle.o1_apply(*a, *mom, nimg=nimg, kmax=kmax, parts=oracle.PART_WAVE)
+    errs = {}
+    for P in (8, 12, 16, 20, 24):
+        r = oracle.o2_apply(*a, 0.5 * sysm["L"], 32, P, *mom, parts=oracle.PART_WAVE)
+        errs[P] = max(_rel(r["U"], ref[0]), _rel(r["Omega"], ref[1]), _rel(r["E"], ref[2]), _rel(r["s_out"], ref[3]))
+    slope = -math.log(errs[20] / errs[8]) / 12.0
+    assert 0.8 * rate < slope < 1.2 * rate, (errs, slope)
+    assert errs[24] < 5e-11
+    # decoupled errors: a finer grid does not change the P-limited error much
+    r48 = oracle.o2_apply(*a, 0.5 * sysm["L"], 48, 24, *mom, parts=oracle.PART_WAVE)
+    assert max(_rel(r48["U"], ref[0]), _rel(r48["E"], ref[2])) < 5e-11
+
+
+def test_o2_full_product_matches_o1_when_converged(oracle, workloads):
+    sysm = workloads.random_small_system(2, 10, 10.0)
+    xi = 1.0
+    L = sysm["L"]
+    nimg, kmax = _ewald_cut(xi, L)
+    a = (sysm["pos"], sysm["radii"], L, xi)
+    mom = (sysm["F"], sysm["T"], sysm["S"], sysm["s"])
+    ref = oracle.o1_apply(*a, *mom, nimg=nimg, kmax=kmax)
+    r = oracle.o2_apply(*a, 0.5 * L, 64, 24, *mom)
+    # real-space truncation at r_c = L/2: exp(-xi^2 r_c^2) = 1e-11
+    assert _rel(r["U"], ref[0]) < 1e-8 and _rel(r["Omega"], ref[1]) < 1e-8
+    assert _rel(r["E"], ref[2]) < 1e-8 and _rel(r["s_out"], ref[3]) < 1e-8
+
+
+def test_o2_real_part_equals_o1_nearest_images(oracle, workloads):
+    sysm = workloads.random_small_system(4, 12, 9.0)
+    xi, L = 2.0, sysm["L"]        # exp(-xi^2 (L/2)^2) (xi L/2)^8 << 1e-16: images beyond L/2 are negligible
+    a = (sysm["pos"], sysm["radii"], L, xi)
+    mom = (sysm["F"], sysm["T"], sysm["S"], sysm["s"])
+    ref = oracle.o1_apply(*a, *mom, nimg=1, kmax=0, parts=oracle.PART_REAL)
+    r = oracle.o2_apply(*a, 0.5 * L, 16, 4, *mom, parts=oracle.PART_REAL)
+    for k, v in zip(("U", "Omega", "E", "s_out"), ref):
+        assert _rel(r[k], v) < 1e-12, k
+
+
+def test_o2_cell_list_equals_brute_force(oracle, workloads):
+    wl = workloads.make_workload("c2")
+    tg = np.arange(0, wl.N, 37)
+    s = np.linspace(-1, 1, wl.N)
+    full = oracle.o2_apply(wl.pos, wl.radii, wl.L, wl.xi, wl.rc, 16, 4, wl.F, wl.T, wl.S, s, parts=oracle.PART_REAL)
+    U, W, E, so = oracle.o2_real_targets(wl.pos, wl.radii, wl.L, wl.xi, wl.rc, wl.F, wl.T, wl.S, tg, s)
+    assert _rel(full["U"][tg], U) < 1e-13 and _rel(full["Omega"][tg], W) < 1e-13
+    assert _rel(full["E"][tg], E) < 1e-13 and _rel(full["s_out"][tg], so) < 1e-13
+
+
+def test_o2_spread_conserves_total_force_and_invariances(oracle, workloads):
+    wl = workloads.make_workload("c1")
+    args = dict(L=wl.L, xi=wl.xi, rc=wl.rc, M=wl.M, P=wl.P)
+    base = oracle.o2_apply(wl.pos, wl.radii, F=wl.F, T=wl.T, S=wl.S, want_grids=True, **args)
+    Delta = wl.L / wl.M
+    # reading 12: sum_n H(x_n) Delta^3 = sum_j F_j up to the SE quadrature error (torque and stresslet
+    # terms are total derivatives and integrate to zero)
+    tot = base["gridH"].reshape(3, -1).sum(axis=1) * Delta ** 3
+    assert tot == pytest.approx(wl.F.sum(axis=0), abs=2e-3 * np.abs(wl.F).sum())
+    # returned grids are divergence-free fields with zero mean (k=0 removed)
+    assert np.abs(base["gridOut"].reshape(6, -1).mean(axis=1)).max() < 1e-12
+    # exact invariance under a shift by a multiple of Delta and under periodic wrap
+    shift = np.array([3, -5, 40]) * Delta
+    sh = oracle.o2_apply(wl.pos + shift, wl.radii, F=wl.F, T=wl.T, S=wl.S, **args)
+    for k in ("U", "Omega", "E"):
+        assert _rel(sh[k], base[k]) < 1e-11
+    # permutation invariance
+    perm = np.random.default_rng(0).permutation(wl.N)
+    pr = oracle.o2_apply(wl.pos[perm], wl.radii[perm], F=wl.F[perm], T=wl.T[perm], S=wl.S[perm], **args)
+    for k in ("U", "Omega", "E"):
+        assert _rel(pr[k], base[k][perm]) < 1e-12
+    # linearity and zero in -> zero out
+    two = oracle.o2_apply(wl.pos, wl.radii, F=2 * wl.F, T=2 * wl.T, S=2 * wl.S, **args)
+    assert _rel(two["E"], 2 * base["E"]) < 1e-14
+    z = oracle.o2_apply(wl.pos, wl.radii, F=0 * wl.F, T=0 * wl.T, S=0 * wl.S, **args)
+    assert np.abs(z["U"]).max() == 0 and np.abs(z["E"]).max() == 0
+    # E is traceless by construction of the 5-component storage; without pressure moments the
+    # compressible rows contribute exactly nothing (a9)
+    s0 = oracle.o2_apply(wl.pos, wl.radii, F=wl.F, T=wl.T, S=wl.S, s=np.zeros(wl.N), **args)
+    for k in ("U", "Omega", "E"):
+        assert np.array_equal(s0[k], base[k])
+
+
+def test_paper_accuracy_system_wave_error_ladder(oracle, workloads):
+    """PAPER.md L491-508 (Fig. 2b): N=50 bidisperse, phi=0.05, M=64, xi a1=0.1, hybrid variant.  With the
+    support-counting convention of DESIGN.md reading 11 the error e_inf,r(E) (Eq. 78) crosses 1e-4 within
+    +-2 of the paper's P=13 and decays at the rate of Eq. 79."""
+    p_paper, rate = _gold("paper_accuracy_claims.txt")
+    sysm = workloads.make_accuracy_system()
+    xi, L = 0.1, sysm["L"]
+    assert L == pytest.approx(23.5, abs=0.01)               # L/a1 = 23.5
+    _, kmax = _ewald_cut(xi, L)
+    a = (sysm["pos"], sysm["radii"], L, xi)
+    mom = (sysm["F"], sysm["T"], sysm["S"])
+    ref = oracle.o1_apply(*a, *mom, nimg=0, kmax=kmax, parts=oracle.PART_WAVE)[2]
+
+    def einf(E):
+        full = lambda e: np.sqrt(e[:, 0] ** 2 + e[:, 3] ** 2 + (e[:, 0] + e[:, 3]) ** 2 + 2 * (e[:, 1] ** 2 + e[:, 2] ** 2 + e[:, 4] ** 2))
+        return float((full(E - ref) / full(ref)).max())
+
+    best = {}
+    for P in (9, 11, 13, 15, 17):
+        best[P] = min(einf(oracle.o2_apply(*a, 0.5 * L, 64, P, *mom, m=m, parts=oracle.PART_WAVE)["E"])
+                      for m in np.arange(0.8, 1.11, 0.1) * math.sqrt(math.pi * P))
+    p_cross = min(P for P, e in best.items() if e < 1e-4)
+    assert abs(p_cross - p_paper) <= 2, best
+    slope = -math.log(best[17] / best[9]) / 8.0
+    assert 0.75 * rate < slope < 1.25 * rate, best
