@@ -1,0 +1,148 @@
+/* se_mobility.h -- C ABI of the B200-native far-field mobility product of SEASD.
+ *
+ * One operation: the far-field grand-mobility product  M.[F,T,S] -> [U,Omega,E]  for N polydisperse
+ * spheres in a cubic, triply periodic box, by the Ewald split of Wang & Brady, arXiv 1506.08481
+ * ("PAPER.md"): a real-space pair sum with cutoff r_c over a cell list (Sec. 3.3, Eq. 22 with
+ * the Faxen laws Eq. 13-15 and the multipole expansion Eq. 17) plus a Spectral-Ewald wave-space sum in
+ * the hybrid size-effect variant (Sec. 3.1-3.2: Eq. 41-46, 48, 50-52), minus the wave-space self terms
+ * (Eq. 37) plus the one-body Faxen terms (Eq. 13-15).
+ *
+ * Conventions: inputs are the moments the particles exert ON THE FLUID, (F,T,S) = -(F^H,T^H,S^H) of
+ * Eq. 7-9; outputs are (U - U^inf, Omega - Omega^inf, -E^inf) of Eq. 11, so that the operator is the
+ * symmetric positive definite grand mobility of PAPER.md L92.  S and E are symmetric and traceless and
+ * are stored as 5 components (xx, xy, xz, yy, yz); zz = -(xx+yy).  Everything is IEEE double.
+ *
+ * Every entry point returns an se_status and never throws, aborts or prints.  The library has no CPU
+ * fallback: without a CUDA device every compute call returns SE_ERR_CUDA.
+ *
+ * Threading/streams: a plan owns one workspace, so at most one apply per plan may be in flight;
+ * different plans may be used concurrently on different streams.
+ */
+#ifndef SE_MOBILITY_H
+#define SE_MOBILITY_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct se_plan se_plan;       /* opaque; created, owned and freed by the library */
+
+typedef enum {
+    SE_OK = 0,
+    SE_ERR_INVALID_ARG = 1,           /* bad size/parameter or NULL pointer; nothing was launched    */
+    SE_ERR_UNSUPPORTED = 2,           /* valid request this build does not implement (e.g. P > 24)   */
+    SE_ERR_ALLOC = 3,                 /* host or device allocation failed                            */
+    SE_ERR_CUDA = 4,                  /* CUDA runtime error (text in se_last_error)                  */
+    SE_ERR_CUFFT = 5                  /* cuFFT error                                                 */
+} se_status;
+
+/* flags for se_plan_set_flags (staged parity and profiling; default 0 = the full product) */
+#define SE_SKIP_REAL     0x1u         /* leave out the real-space pair sum (a2)                       */
+#define SE_SKIP_WAVE     0x2u         /* leave out the Spectral-Ewald wave-space sum (a3-a7)          */
+#define SE_SKIP_SELF     0x4u         /* do not subtract the wave-space self terms (Eq. 37)           */
+#define SE_SKIP_ONEBODY  0x8u         /* do not add the one-body Faxen terms (Eq. 13-15)              */
+#define SE_TIMING        0x10u        /* record CUDA events between stages (se_plan_get_timings)      */
+
+/* stage indices of se_plan_get_timings */
+enum {
+    SE_STAGE_SORT = 0,                /* a1: wrap, counting sorts by real-space cell and grid tile, packing */
+    SE_STAGE_REAL = 1,                /* a2: real-space pair sum                                      */
+    SE_STAGE_SPREAD = 2,              /* a3: Gaussian spreading onto the grid                         */
+    SE_STAGE_FFT_FWD = 3,             /* a4: forward FFTs (cuFFT)                                     */
+    SE_STAGE_KSPACE = 4,              /* a5: fused k-space scaling                                    */
+    SE_STAGE_FFT_INV = 5,             /* a6: inverse FFTs (cuFFT)                                     */
+    SE_STAGE_GATHER = 6,              /* a7: Gaussian gather                                          */
+    SE_STAGE_EPILOGUE = 7,            /* a8: self / one-body terms, sum, un-permute                   */
+    SE_NUM_STAGES = 8
+};
+
+/* Create a plan.  Derives Delta = L/M, the Gaussian shape (Eq. 41, 46) with shape
+ * parameter m = sqrt(pi P) (Eq. 79) unless changed by se_plan_set_shape, cell and tile grids, creates
+ * the cuFFT plans and allocates every workspace on the CURRENT CUDA device.
+ *   out     receives the plan (set to NULL on failure)
+ *   N       number of particles, >= 1
+ *   L       edge of the cubic periodic box [0,L)^3, > 0
+ *   radii   HOST pointer, N entries, each > 0; copied                        (a_i)
+ *   xi      Ewald splitting parameter, > 0 (Beenakker convention)
+ *   r_c     real-space cutoff: pairs with minimum-image distance r < r_c;  0 < r_c <= L/2  (L330)
+ *   M       grid points per axis, even, >= P
+ *   P       support points of the Gaussian per axis, 2 <= P <= 24
+ *   eta0    solvent viscosity, > 0
+ * Errors: SE_ERR_INVALID_ARG for any violated bound or NULL; SE_ERR_UNSUPPORTED for P > 24;
+ * SE_ERR_ALLOC / SE_ERR_CUDA / SE_ERR_CUFFT when resources cannot be had. */
+se_status se_plan_create(se_plan **out, int64_t N, double L, const double *radii,
+                         double xi, double r_c, int M, int P, double eta0);
+
+/* Gaussian shape parameter m of Eq. 46 (h ~ exp(-m^2/2) at the edge of the support), m > 0. */
+se_status se_plan_set_shape(se_plan *plan, double m);
+
+/* Bitwise OR of the SE_* flags above. */
+se_status se_plan_set_flags(se_plan *plan, unsigned flags);
+
+/* The product.  All pointers are DEVICE pointers to arrays the caller owns:
+ *   pos    [N][3] row-major particle centres, any real value (wrapped into the box internally)
+ *   F, T   [N][3] force and torque on the fluid
+ *   S      [N][5] stresslet on the fluid, (xx,xy,xz,yy,yz)
+ *   U, Omega [N][3], E [N][5]  outputs, OVERWRITTEN (never accumulated into)
+ *   cuda_stream   a cudaStream_t (NULL = default stream); the work is enqueued and the call returns
+ *                 without synchronising.  Inputs must stay valid until the stream reaches the end.
+ * Errors: SE_ERR_INVALID_ARG for NULL pointers; SE_ERR_CUDA / SE_ERR_CUFFT on launch failure. */
+se_status far_mobility_apply(se_plan *plan, const double *pos, const double *F, const double *T,
+                             const double *S, double *U, double *Omega, double *E, void *cuda_stream);
+
+/* Compressible-solvent extension (Sec. 2.3, Eq. 24-34).  As far_mobility_apply with
+ *   s_in   [N] DEVICE pressure moments S^H_j (paper's Eq. 25-26 sign), or NULL for none
+ *   s_out  [N] DEVICE interaction part 4 pi a_i^3 p'(r_i) of the pressure Faxen law (Eq. 28), or NULL
+ * With s_in == NULL the outputs U, Omega, E equal those of far_mobility_apply. */
+se_status far_mobility_apply_compressible(se_plan *plan, const double *pos, const double *F,
+                                          const double *T, const double *S, const double *s_in,
+                                          double *U, double *Omega, double *E, double *s_out,
+                                          void *cuda_stream);
+
+/* End-to-end convenience: the same product with HOST arrays (pinned or pageable).  Copies the inputs
+ * to plan-owned device buffers, runs far_mobility_apply on cuda_stream, copies the outputs back and
+ * synchronises the stream before returning. */
+se_status far_mobility_apply_host(se_plan *plan, const double *pos, const double *F, const double *T,
+                                  const double *S, double *U, double *Omega, double *E, void *cuda_stream);
+
+/* Staged outputs for parity tests (valid after the stream of the last apply has been synchronised).
+ * which = 0: the three spread grids H_x,H_y,H_z, [3][M][M][M];  which = 1: the six returned grids
+ * u~ (3), w~ (3), [6][M][M][M].  dst is a HOST pointer with room for the whole array.  The spread
+ * grids share storage with the returned grids and are only available from an apply made with flag
+ * SE_SKIP_WAVE cleared and read through which = 0 BEFORE a later apply; tests use se_plan_debug_stop. */
+se_status se_plan_copy_grids(se_plan *plan, int which, double *dst);
+
+/* Debug: stop the wave pipeline after stage `stage` (SE_STAGE_SPREAD .. SE_STAGE_GATHER), or -1 for
+ * the normal full run.  Used with se_plan_copy_grids for per-stage parity. */
+se_status se_plan_debug_stop(se_plan *plan, int stage);
+
+/* CUDA-event times in milliseconds of the stages of the last apply made with SE_TIMING set;
+ * synchronises on the last event.  ms has SE_NUM_STAGES entries. */
+se_status se_plan_get_timings(se_plan *plan, double *ms);
+
+/* Number of kernel launches (own kernels, cuFFT excluded) the last apply enqueued. */
+int se_plan_last_launch_count(const se_plan *plan);
+
+/* Device bytes held by the plan (grids, sorted copies, cell tables, cuFFT work areas). */
+size_t se_plan_workspace_bytes(const se_plan *plan);
+
+/* Derived constants, for tests: out[0..5] = Delta, eta_se, alpha, m, cells per axis of the real-space
+ * cell grid (as double), number of sweep segments of the spreading kernel (as double). */
+se_status se_plan_get_constants(const se_plan *plan, double *out);
+
+/* Text of the last error on this plan ("" if none); owned by the plan. */
+const char *se_last_error(const se_plan *plan);
+
+/* Release everything.  NULL is allowed. */
+se_status se_plan_destroy(se_plan *plan);
+
+/* Library version string, e.g. "se_mobility 0.1 (sm_100a)". */
+const char *se_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SE_MOBILITY_H */

@@ -1,0 +1,12 @@
+"""B200-native far-field mobility product of Spectral Ewald Accelerated Stokesian Dynamics.
+
+Thin Python binding (argument marshalling only) over the C-ABI library ``libse_mobility.so``
+(``include/se_mobility.h``); every step of the path runs in the library's CUDA kernels.  PyTorch is
+used for device memory and streams only.  There is no CPU fallback: importing works anywhere, but
+creating a plan without the built library or without a CUDA device raises.
+"""
+from .binding import (SE_NUM_STAGES, SE_SKIP_ONEBODY, SE_SKIP_REAL, SE_SKIP_SELF, SE_SKIP_WAVE, SE_TIMING,
+                      STAGE_NAMES, SeError, SePlan, declared_symbols, load_library, version)
+
+__all__ = ["SePlan", "SeError", "load_library", "declared_symbols", "version", "SE_SKIP_REAL", "SE_SKIP_WAVE",
+           "SE_SKIP_SELF", "SE_SKIP_ONEBODY", "SE_TIMING", "SE_NUM_STAGES", "STAGE_NAMES"]

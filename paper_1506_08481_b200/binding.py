@@ -1,0 +1,183 @@
+"""ctypes binding of include/se_mobility.h -- same names, argument marshalling only."""
+from __future__ import annotations
+
+import ctypes
+import os
+import re
+
+import numpy as np
+
+from . import build as _build
+
+SE_SKIP_REAL, SE_SKIP_WAVE, SE_SKIP_SELF, SE_SKIP_ONEBODY, SE_TIMING = 0x1, 0x2, 0x4, 0x8, 0x10
+SE_NUM_STAGES = 8
+STAGE_NAMES = ("sort", "real", "spread", "fft_fwd", "kspace", "fft_inv", "gather", "epilogue")
+_STATUS = {0: "SE_OK", 1: "SE_ERR_INVALID_ARG", 2: "SE_ERR_UNSUPPORTED", 3: "SE_ERR_ALLOC", 4: "SE_ERR_CUDA",
+           5: "SE_ERR_CUFFT"}
+
+_HEADER = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "include", "se_mobility.h")
+
+
+class SeError(RuntimeError):
+    def __init__(self, status: int, where: str, detail: str = ""):
+        self.status = status
+        super().__init__(f"{where}: {_STATUS.get(status, status)} {detail}".strip())
+
+
+def declared_symbols() -> list[str]:
+    """Names of the functions include/se_mobility.h declares."""
+    text = open(_HEADER).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b((?:se_|far_mobility_)\w+)\s*\(", text)))
+
+
+_lib = None
+
+
+def load_library(build_if_missing: bool = True):
+    """dlopen libse_mobility.so (building it with nvcc if sources are newer); fails loudly."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if build_if_missing and _build.needs_build():
+        _build.build()
+    if not os.path.exists(_build.LIB_PATH):
+        raise ImportError(f"{_build.LIB_PATH} is missing: run `python -m paper_1506_08481_b200.build`")
+    L = ctypes.CDLL(_build.LIB_PATH)
+    D, I64, INT, U, P, SZ = ctypes.c_double, ctypes.c_int64, ctypes.c_int, ctypes.c_uint, ctypes.c_void_p, ctypes.c_size_t
+    L.se_plan_create.restype = INT
+    L.se_plan_create.argtypes = [ctypes.POINTER(P), I64, D, P, D, D, INT, INT, D]
+    L.se_plan_set_shape.restype = INT
+    L.se_plan_set_shape.argtypes = [P, D]
+    L.se_plan_set_flags.restype = INT
+    L.se_plan_set_flags.argtypes = [P, U]
+    L.far_mobility_apply.restype = INT
+    L.far_mobility_apply.argtypes = [P] * 9
+    L.far_mobility_apply_compressible.restype = INT
+    L.far_mobility_apply_compressible.argtypes = [P] * 11
+    L.far_mobility_apply_host.restype = INT
+    L.far_mobility_apply_host.argtypes = [P] * 9
+    L.se_plan_copy_grids.restype = INT
+    L.se_plan_copy_grids.argtypes = [P, INT, P]
+    L.se_plan_debug_stop.restype = INT
+    L.se_plan_debug_stop.argtypes = [P, INT]
+    L.se_plan_get_timings.restype = INT
+    L.se_plan_get_timings.argtypes = [P, P]
+    L.se_plan_last_launch_count.restype = INT
+    L.se_plan_last_launch_count.argtypes = [P]
+    L.se_plan_workspace_bytes.restype = SZ
+    L.se_plan_workspace_bytes.argtypes = [P]
+    L.se_plan_get_constants.restype = INT
+    L.se_plan_get_constants.argtypes = [P, P]
+    L.se_last_error.restype = ctypes.c_char_p
+    L.se_last_error.argtypes = [P]
+    L.se_plan_destroy.restype = INT
+    L.se_plan_destroy.argtypes = [P]
+    L.se_version.restype = ctypes.c_char_p
+    L.se_version.argtypes = []
+    _lib = L
+    return L
+
+
+def version() -> str:
+    return load_library().se_version().decode()
+
+
+def _dptr(t, n, name):
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous() or t.numel() != n:
+        raise ValueError(f"{name}: expected a contiguous CUDA float64 tensor with {n} elements")
+    return t.data_ptr()
+
+
+def _hptr(a, n, name):
+    if not isinstance(a, np.ndarray) or a.dtype != np.float64 or not a.flags.c_contiguous or a.size != n:
+        raise ValueError(f"{name}: expected a C-contiguous float64 numpy array with {n} elements")
+    return a.ctypes.data
+
+
+class SePlan:
+    """se_plan_create / far_mobility_apply / se_plan_destroy with the header's argument meaning."""
+
+    def __init__(self, N, L, radii, xi, r_c, M, P, eta0=1.0):
+        self._lib = load_library()
+        self._h = ctypes.c_void_p()
+        rad = np.ascontiguousarray(radii, dtype=np.float64)
+        if rad.size != N:
+            raise ValueError("radii must have N entries")
+        st = self._lib.se_plan_create(ctypes.byref(self._h), int(N), float(L), rad.ctypes.data, float(xi), float(r_c),
+                                      int(M), int(P), float(eta0))
+        if st != 0:
+            self._h = ctypes.c_void_p()
+            raise SeError(st, "se_plan_create")
+        self.N, self.L, self.M, self.P = int(N), float(L), int(M), int(P)
+
+    # -- helpers --
+    def _check(self, st, where):
+        if st != 0:
+            raise SeError(st, where, self._lib.se_last_error(self._h).decode())
+
+    def set_shape(self, m):
+        self._check(self._lib.se_plan_set_shape(self._h, float(m)), "se_plan_set_shape")
+
+    def set_flags(self, flags):
+        self._check(self._lib.se_plan_set_flags(self._h, int(flags)), "se_plan_set_flags")
+
+    def debug_stop(self, stage):
+        self._check(self._lib.se_plan_debug_stop(self._h, int(stage)), "se_plan_debug_stop")
+
+    def apply(self, pos, F, T, S, U, Omega, E, stream=None):
+        """far_mobility_apply on CUDA float64 tensors; enqueues on ``stream`` (default: torch's current)."""
+        import torch
+        N = self.N
+        sp = (torch.cuda.current_stream() if stream is None else stream).cuda_stream
+        st = self._lib.far_mobility_apply(self._h, _dptr(pos, 3 * N, "pos"), _dptr(F, 3 * N, "F"), _dptr(T, 3 * N, "T"),
+                                          _dptr(S, 5 * N, "S"), _dptr(U, 3 * N, "U"), _dptr(Omega, 3 * N, "Omega"),
+                                          _dptr(E, 5 * N, "E"), sp)
+        self._check(st, "far_mobility_apply")
+
+    def apply_raw(self, pos, F, T, S, U, Omega, E, stream_ptr=0):
+        """far_mobility_apply on raw device addresses (ints); used to test NULL handling."""
+        return self._lib.far_mobility_apply(self._h, pos, F, T, S, U, Omega, E, stream_ptr)
+
+    def apply_host(self, pos, F, T, S, U, Omega, E, stream=None):
+        """far_mobility_apply_host on numpy float64 arrays (copies in, computes, copies out, synchronises)."""
+        import torch
+        N = self.N
+        sp = (torch.cuda.current_stream() if stream is None else stream).cuda_stream
+        st = self._lib.far_mobility_apply_host(self._h, _hptr(pos, 3 * N, "pos"), _hptr(F, 3 * N, "F"), _hptr(T, 3 * N, "T"),
+                                               _hptr(S, 5 * N, "S"), _hptr(U, 3 * N, "U"), _hptr(Omega, 3 * N, "Omega"),
+                                               _hptr(E, 5 * N, "E"), sp)
+        self._check(st, "far_mobility_apply_host")
+
+    def copy_grids(self, which):
+        out = np.empty((3 if which == 0 else 6, self.M, self.M, self.M))
+        self._check(self._lib.se_plan_copy_grids(self._h, int(which), out.ctypes.data), "se_plan_copy_grids")
+        return out
+
+    def timings(self):
+        ms = np.zeros(SE_NUM_STAGES)
+        self._check(self._lib.se_plan_get_timings(self._h, ms.ctypes.data), "se_plan_get_timings")
+        return dict(zip(STAGE_NAMES, ms.tolist()))
+
+    def last_launch_count(self):
+        return int(self._lib.se_plan_last_launch_count(self._h))
+
+    def workspace_bytes(self):
+        return int(self._lib.se_plan_workspace_bytes(self._h))
+
+    def constants(self):
+        out = np.zeros(6)
+        self._check(self._lib.se_plan_get_constants(self._h, out.ctypes.data), "se_plan_get_constants")
+        return dict(Delta=out[0], eta_se=out[1], alpha=out[2], m=out[3], real_cells=int(out[4]), spread_segments=int(out[5]))
+
+    def destroy(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            self._lib.se_plan_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

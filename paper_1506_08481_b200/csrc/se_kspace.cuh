@@ -1,0 +1,40 @@
+// a5: fused k-space pass (Eq. 43 with the kernel g1 of Eq. 36; hybrid variant Eq. 50-51 with the
+// bracket replaced by H_k, L326).  One HBM pass: reads the three spectra H_k, writes the six spectra
+//   u_k = s(k) (H_k - k (k.H_k)/k^2),   s(k) = [Delta^3/(eta0 V)] (1 + k^2/4xi^2) exp(-(1-eta_se) k^2/4xi^2)/k^2
+//   w_k = -k^2 u_k
+// (Green's function scale and Gaussian deconvolution e^{+eta_se k^2/4xi^2} folded into one factor);
+// zero at k = 0 (Eq. 43) and on the Nyquist planes (reading 13).
+// Layout: half spectra [M][M][M/2+1] complex (cuFFT D2Z), last index fastest.
+#pragma once
+#include "se_common.cuh"
+
+#define KSPACE_THREADS 256
+
+__global__ void __launch_bounds__(KSPACE_THREADS) k_kspace(SeConst c, const double2 *__restrict__ Hk, double2 *__restrict__ Gk)
+{
+    const int M = c.M, Zc = M / 2 + 1;
+    const size_t Gc = (size_t)M * M * Zc;
+    const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= Gc) return;
+    const int iz = (int)(q % Zc);
+    const size_t t = q / Zc;
+    const int iy = (int)(t % M), ix = (int)(t / M);
+    const int jx = ix < M / 2 ? ix : ix - M, jy = iy < M / 2 ? iy : iy - M, jz = iz;
+    double2 u0 = make_double2(0.0, 0.0), u1 = u0, u2 = u0, w0 = u0, w1 = u0, w2 = u0;
+    const bool zero = (ix == 0 && iy == 0 && iz == 0) || ix == M / 2 || iy == M / 2 || iz == M / 2;
+    if (!zero) {
+        const double kx = c.twopiL * jx, ky = c.twopiL * jy, kz = c.twopiL * jz;
+        const double k2 = kx * kx + ky * ky + kz * kz;
+        const double sc = c.scale0 * (1.0 + k2 * c.inv4xi2) * exp(-c.dec * k2) / k2;
+        const double2 h0 = Hk[q], h1 = Hk[Gc + q], h2 = Hk[2 * Gc + q];
+        const double pr = (kx * h0.x + ky * h1.x + kz * h2.x) / k2, pi = (kx * h0.y + ky * h1.y + kz * h2.y) / k2;
+        u0 = make_double2(sc * (h0.x - kx * pr), sc * (h0.y - kx * pi));
+        u1 = make_double2(sc * (h1.x - ky * pr), sc * (h1.y - ky * pi));
+        u2 = make_double2(sc * (h2.x - kz * pr), sc * (h2.y - kz * pi));
+        w0 = make_double2(-k2 * u0.x, -k2 * u0.y);
+        w1 = make_double2(-k2 * u1.x, -k2 * u1.y);
+        w2 = make_double2(-k2 * u2.x, -k2 * u2.y);
+    }
+    Gk[q] = u0; Gk[Gc + q] = u1; Gk[2 * Gc + q] = u2;
+    Gk[3 * Gc + q] = w0; Gk[4 * Gc + q] = w1; Gk[5 * Gc + q] = w2;
+}

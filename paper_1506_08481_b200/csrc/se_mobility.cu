@@ -1,0 +1,429 @@
+// C-ABI of the far-field mobility product (include/se_mobility.h): plan, orchestration, cuFFT calls.
+// Hand-written CUDA for sm_100a; cuFFT is used for the 3-D transforms only (a4, a6).
+#include "../../include/se_mobility.h"
+
+#include <cuda_runtime.h>
+#include <cufft.h>
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include "se_common.cuh"
+#include "se_sort.cuh"
+#include "se_real.cuh"
+#include "se_spread.cuh"
+#include "se_kspace.cuh"
+#include "se_gather.cuh"
+
+#ifndef M_PI
+#define M_PI 3.14159265358979323846
+#endif
+
+struct se_plan {
+    SeConst c;
+    double m;                      // Gaussian shape parameter
+    unsigned flags;
+    int debug_stop;
+    int last_launches;
+    size_t bytes;
+    char err[256];
+    // device buffers
+    double *d_radii;
+    int *d_key_r, *d_rank_r, *d_cnt_r, *d_start_r;
+    int *d_key_s, *d_rank_s, *d_cnt_s, *d_start_s;
+    int *d_bsum;
+    int ncell_r, ncell_s;
+    double4 *d_rs_pos;
+    double *d_rs_mom;
+    int *d_rs_orig;
+    double *d_recs;
+    double *d_real;                // [6][M^3]; the first three double as the spread grids H
+    double2 *d_Hk;                 // [3][M][M][M/2+1]
+    double2 *d_Gk;                 // [6][M][M][M/2+1]
+    double *d_out_real, *d_out_wave;      // [N][11] in caller order
+    // host-API staging
+    double *d_io;                  // pos3 F3 T3 S5 U3 W3 E5 = 25 N doubles
+    cufftHandle fft_fwd, fft_inv;
+    bool have_fwd, have_inv;
+    size_t fft_bytes;
+    cudaEvent_t ev[SE_NUM_STAGES + 1];
+    bool have_events, timed;
+};
+
+static se_status fail(se_plan *p, se_status st, const char *what, const char *detail)
+{
+    if (p) snprintf(p->err, sizeof(p->err), "%s: %s", what, detail ? detail : "");
+    return st;
+}
+
+#define CUDA_TRY(p, call)                                                              \
+    do {                                                                               \
+        cudaError_t e_ = (call);                                                       \
+        if (e_ != cudaSuccess) return fail((p), SE_ERR_CUDA, #call, cudaGetErrorString(e_)); \
+    } while (0)
+
+#define CUFFT_TRY(p, call)                                                             \
+    do {                                                                               \
+        cufftResult r_ = (call);                                                       \
+        if (r_ != CUFFT_SUCCESS) {                                                     \
+            char b_[32]; snprintf(b_, sizeof(b_), "cufftResult %d", (int)r_);          \
+            return fail((p), SE_ERR_CUFFT, #call, b_);                                 \
+        }                                                                              \
+    } while (0)
+
+template <typename Tp>
+static se_status dev_alloc(se_plan *p, Tp **ptr, size_t count)
+{
+    *ptr = nullptr;
+    const size_t nb = count * sizeof(Tp);
+    cudaError_t e = cudaMalloc((void **)ptr, nb ? nb : 16);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(p, e == cudaErrorMemoryAllocation ? SE_ERR_ALLOC : SE_ERR_CUDA, "cudaMalloc", cudaGetErrorString(e));
+    }
+    p->bytes += nb;
+    return SE_OK;
+}
+
+// Derived constants (oracle step 1 restated independently): Delta = L/M,
+// eta_se = (P Delta xi/m)^2 [= theta L^2/4pi^2 of Eq. 46], alpha = 2 xi^2/eta_se (Eq. 41).
+static void derive_constants(se_plan *p)
+{
+    SeConst &c = p->c;
+    c.MoverL = (double)c.M / c.L;
+    c.Delta = c.L / c.M;
+    const double t = c.P * c.Delta * c.xi / p->m;
+    c.eta_se = t * t;
+    c.alpha = 2.0 * c.xi * c.xi / c.eta_se;
+    c.gnorm = pow(c.alpha / M_PI, 1.5);
+    c.q = 2.0 * c.xi / sqrt(M_PI);
+    c.x2 = c.xi * c.xi; c.x4 = c.x2 * c.x2; c.x6 = c.x4 * c.x2; c.x8 = c.x4 * c.x4; c.x10 = c.x8 * c.x2; c.x12 = c.x6 * c.x6;
+    c.k0 = 1.0 / (8.0 * M_PI * c.eta0);
+    const double V = c.L * c.L * c.L;
+    c.D3 = c.Delta * c.Delta * c.Delta;
+    c.scale0 = c.D3 / (c.eta0 * V);
+    c.inv4xi2 = 1.0 / (4.0 * c.xi * c.xi);
+    c.dec = (1.0 - c.eta_se) / (4.0 * c.xi * c.xi);
+    c.twopiL = 2.0 * M_PI / c.L;
+}
+
+extern "C" const char *se_version(void) { return "se_mobility 0.1 (sm_100a)"; }
+
+extern "C" const char *se_last_error(const se_plan *plan) { return plan ? plan->err : "null plan"; }
+
+extern "C" se_status se_plan_destroy(se_plan *p)
+{
+    if (!p) return SE_OK;
+    cudaFree(p->d_radii);
+    cudaFree(p->d_key_r); cudaFree(p->d_rank_r); cudaFree(p->d_cnt_r); cudaFree(p->d_start_r);
+    cudaFree(p->d_key_s); cudaFree(p->d_rank_s); cudaFree(p->d_cnt_s); cudaFree(p->d_start_s);
+    cudaFree(p->d_bsum);
+    cudaFree(p->d_rs_pos); cudaFree(p->d_rs_mom); cudaFree(p->d_rs_orig); cudaFree(p->d_recs);
+    cudaFree(p->d_real); cudaFree(p->d_Hk); cudaFree(p->d_Gk);
+    cudaFree(p->d_out_real); cudaFree(p->d_out_wave); cudaFree(p->d_io);
+    if (p->have_fwd) cufftDestroy(p->fft_fwd);
+    if (p->have_inv) cufftDestroy(p->fft_inv);
+    if (p->have_events) for (int k = 0; k <= SE_NUM_STAGES; ++k) cudaEventDestroy(p->ev[k]);
+    cudaGetLastError();
+    free(p);
+    return SE_OK;
+}
+
+extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const double *radii,
+                                    double xi, double r_c, int M, int P, double eta0)
+{
+    if (!out) return SE_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!radii || N < 1 || N > (int64_t)1 << 30 || !(L > 0.0) || !(xi > 0.0) || !(r_c > 0.0) || r_c > 0.5 * L ||
+        M < 2 || (M & 1) || M > 2048 || P < 2 || P > M || !(eta0 > 0.0))
+        return SE_ERR_INVALID_ARG;
+    if (P > SE_PMAX) return SE_ERR_UNSUPPORTED;
+    for (int64_t i = 0; i < N; ++i) if (!(radii[i] > 0.0)) return SE_ERR_INVALID_ARG;
+
+    se_plan *p = (se_plan *)calloc(1, sizeof(se_plan));
+    if (!p) return SE_ERR_ALLOC;
+    p->debug_stop = -1;
+    SeConst &c = p->c;
+    c.N = (int)N; c.M = M; c.P = P; c.L = L; c.xi = xi; c.rc2 = r_c * r_c; c.eta0 = eta0;
+    p->m = sqrt(M_PI * P);
+    derive_constants(p);
+
+    // real-space cell grid: edge >= r_c, at least 3 cells per axis, else all pairs (one cell)
+    int ncr = (int)floor(L / r_c);
+    if (ncr < 3) ncr = 1;
+    if (ncr > 1024) ncr = 1024;
+    c.ncr = ncr;
+    c.hr = L / ncr;
+    p->ncell_r = ncr * ncr * ncr;
+    // spreading tile bins (plane-thin): M x ceil(M/4) x ceil(M/8)
+    c.NBY = (M + SE_TILE_Y - 1) / SE_TILE_Y;
+    c.NBZ = (M + SE_TILE_Z - 1) / SE_TILE_Z;
+    p->ncell_s = M * c.NBY * c.NBZ;
+    c.rec_stride = (SE_REC_HDR + 3 * P + 1) & ~1;
+    // sweep segments: enough warps to fill 148 SMs several times, segments no shorter than 32 planes
+    {
+        const int npatch = c.NBY * c.NBZ;
+        int nseg = (148 * 48 + npatch - 1) / npatch;
+        const int maxseg = M / 32 > 1 ? M / 32 : 1;
+        if (nseg > maxseg) nseg = maxseg;
+        if (nseg < 1) nseg = 1;
+        c.seg_len = (M + nseg - 1) / nseg;
+        c.nseg = (M + c.seg_len - 1) / c.seg_len;
+    }
+
+    se_status st = SE_OK;
+    const size_t G = (size_t)M * M * M, Gc = (size_t)M * M * (M / 2 + 1);
+    const int nscan = (p->ncell_s > p->ncell_r ? p->ncell_s : p->ncell_r);
+#define ALLOC(ptr, count) if (st == SE_OK) st = dev_alloc(p, &(ptr), (size_t)(count))
+    ALLOC(p->d_radii, N);
+    ALLOC(p->d_key_r, N); ALLOC(p->d_rank_r, N); ALLOC(p->d_cnt_r, p->ncell_r); ALLOC(p->d_start_r, p->ncell_r + 1);
+    ALLOC(p->d_key_s, N); ALLOC(p->d_rank_s, N); ALLOC(p->d_cnt_s, p->ncell_s); ALLOC(p->d_start_s, p->ncell_s + 1);
+    ALLOC(p->d_bsum, (nscan + SCAN_BLOCK - 1) / SCAN_BLOCK + 1);
+    ALLOC(p->d_rs_pos, N); ALLOC(p->d_rs_mom, 12 * (size_t)N); ALLOC(p->d_rs_orig, N);
+    ALLOC(p->d_recs, (size_t)N * c.rec_stride);
+    ALLOC(p->d_real, 6 * G); ALLOC(p->d_Hk, 3 * Gc); ALLOC(p->d_Gk, 6 * Gc);
+    ALLOC(p->d_out_real, 11 * (size_t)N); ALLOC(p->d_out_wave, 11 * (size_t)N);
+    ALLOC(p->d_io, 25 * (size_t)N);
+#undef ALLOC
+    if (st != SE_OK) { se_plan_destroy(p); return st; }
+    if (cudaMemcpy(p->d_radii, radii, sizeof(double) * (size_t)N, cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemset(p->d_out_real, 0, sizeof(double) * 11 * (size_t)N) != cudaSuccess ||
+        cudaMemset(p->d_out_wave, 0, sizeof(double) * 11 * (size_t)N) != cudaSuccess) {
+        se_plan_destroy(p);
+        return SE_ERR_CUDA;
+    }
+
+    // cuFFT: batched D2Z (3 grids) and Z2D (6 grids), out of place, contiguous batches
+    int n3[3] = { M, M, M };
+    size_t ws = 0;
+    cufftResult r = cufftCreate(&p->fft_fwd);
+    if (r == CUFFT_SUCCESS) { p->have_fwd = true; r = cufftMakePlanMany(p->fft_fwd, 3, n3, NULL, 1, 0, NULL, 1, 0, CUFFT_D2Z, 3, &ws); p->fft_bytes += ws; }
+    if (r == CUFFT_SUCCESS) r = cufftCreate(&p->fft_inv);
+    if (r == CUFFT_SUCCESS) { p->have_inv = true; r = cufftMakePlanMany(p->fft_inv, 3, n3, NULL, 1, 0, NULL, 1, 0, CUFFT_Z2D, 6, &ws); p->fft_bytes += ws; }
+    if (r != CUFFT_SUCCESS) { se_plan_destroy(p); return r == CUFFT_ALLOC_FAILED ? SE_ERR_ALLOC : SE_ERR_CUFFT; }
+    p->bytes += p->fft_bytes;
+
+    for (int k = 0; k <= SE_NUM_STAGES; ++k)
+        if (cudaEventCreate(&p->ev[k]) != cudaSuccess) { p->have_events = (k > 0); se_plan_destroy(p); return SE_ERR_CUDA; }
+    p->have_events = true;
+    *out = p;
+    return SE_OK;
+}
+
+extern "C" se_status se_plan_set_shape(se_plan *p, double m)
+{
+    if (!p || !(m > 0.0)) return SE_ERR_INVALID_ARG;
+    p->m = m;
+    derive_constants(p);
+    return SE_OK;
+}
+
+extern "C" se_status se_plan_set_flags(se_plan *p, unsigned flags)
+{
+    if (!p || (flags & ~0x1fu)) return SE_ERR_INVALID_ARG;
+    p->flags = flags;
+    return SE_OK;
+}
+
+extern "C" se_status se_plan_debug_stop(se_plan *p, int stage)
+{
+    if (!p || stage < -1 || stage >= SE_NUM_STAGES) return SE_ERR_INVALID_ARG;
+    p->debug_stop = stage;
+    return SE_OK;
+}
+
+extern "C" int se_plan_last_launch_count(const se_plan *p) { return p ? p->last_launches : 0; }
+extern "C" size_t se_plan_workspace_bytes(const se_plan *p) { return p ? p->bytes : 0; }
+
+extern "C" se_status se_plan_get_constants(const se_plan *p, double *out)
+{
+    if (!p || !out) return SE_ERR_INVALID_ARG;
+    out[0] = p->c.Delta; out[1] = p->c.eta_se; out[2] = p->c.alpha; out[3] = p->m;
+    out[4] = (double)p->c.ncr; out[5] = (double)p->c.nseg;
+    return SE_OK;
+}
+
+static se_status scan_cells(se_plan *p, const int *cnt, int *start, int n, cudaStream_t s)
+{
+    const int nb = (n + SCAN_BLOCK - 1) / SCAN_BLOCK;
+    k_scan_local<<<nb, SCAN_THREADS, 0, s>>>(cnt, start, p->d_bsum, n);
+    k_scan_sums<<<1, SCAN_THREADS, 0, s>>>(p->d_bsum, nb);
+    k_scan_add<<<nb, SCAN_THREADS, 0, s>>>(start, p->d_bsum, n, p->c.N);
+    p->last_launches += 3;
+    CUDA_TRY(p, cudaGetLastError());
+    return SE_OK;
+}
+
+template <int P>
+static void launch_spread(se_plan *p, cudaStream_t s)
+{
+    const SeConst &c = p->c;
+    const long long warps = (long long)c.NBY * c.NBZ * c.nseg;
+    const int blocks = (int)((warps + SPREAD_WARPS - 1) / SPREAD_WARPS);
+    k_spread<P><<<blocks, SPREAD_WARPS * 32, 0, s>>>(c, p->d_recs, p->d_start_s, p->d_real);
+}
+
+template <int P>
+static void launch_gather(se_plan *p, cudaStream_t s)
+{
+    const SeConst &c = p->c;
+    const int blocks = (c.N + GATHER_WARPS - 1) / GATHER_WARPS;
+    k_gather<P><<<blocks, GATHER_WARPS * 32, 0, s>>>(c, p->d_recs, p->d_real, p->d_out_wave);
+}
+
+#define FOR_EACH_P(X) \
+    X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15) X(16) X(17) X(18) X(19) X(20) X(21) X(22) X(23) X(24)
+
+static void dispatch_spread(se_plan *p, cudaStream_t s)
+{
+    switch (p->c.P) {
+#define X(v) case v: launch_spread<v>(p, s); break;
+        FOR_EACH_P(X)
+#undef X
+    }
+}
+
+static void dispatch_gather(se_plan *p, cudaStream_t s)
+{
+    switch (p->c.P) {
+#define X(v) case v: launch_gather<v>(p, s); break;
+        FOR_EACH_P(X)
+#undef X
+    }
+}
+
+extern "C" se_status far_mobility_apply(se_plan *p, const double *pos, const double *F, const double *T,
+                                        const double *S, double *U, double *Omega, double *E, void *cuda_stream)
+{
+    if (!p) return SE_ERR_INVALID_ARG;
+    if (!pos || !F || !T || !S || !U || !Omega || !E) return fail(p, SE_ERR_INVALID_ARG, "far_mobility_apply", "null pointer");
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const SeConst &c = p->c;
+    const unsigned fl = p->flags;
+    const bool timing = (fl & SE_TIMING) != 0;
+    const bool do_real = !(fl & SE_SKIP_REAL), do_wave = !(fl & SE_SKIP_WAVE);
+    const int stop = p->debug_stop;
+    auto on = [&](int stage) { return do_wave && (stop < 0 || stage <= stop); };
+    p->last_launches = 0;
+    p->timed = false;
+    p->err[0] = 0;
+    const int TB = 128, nbN = (c.N + TB - 1) / TB;
+    int evi = 0;
+#define MARK() do { if (timing) CUDA_TRY(p, cudaEventRecord(p->ev[evi], s)); ++evi; } while (0)
+    MARK();
+    // ---- a1: wrap + counting sorts + packing ----
+    CUDA_TRY(p, cudaMemsetAsync(p->d_cnt_r, 0, sizeof(int) * (size_t)p->ncell_r, s));
+    CUDA_TRY(p, cudaMemsetAsync(p->d_cnt_s, 0, sizeof(int) * (size_t)p->ncell_s, s));
+    k_keys<<<nbN, TB, 0, s>>>(c, pos, p->d_key_r, p->d_rank_r, p->d_cnt_r, p->d_key_s, p->d_rank_s, p->d_cnt_s);
+    p->last_launches += 1;
+    se_status st = scan_cells(p, p->d_cnt_r, p->d_start_r, p->ncell_r, s);
+    if (st != SE_OK) return st;
+    st = scan_cells(p, p->d_cnt_s, p->d_start_s, p->ncell_s, s);
+    if (st != SE_OK) return st;
+    k_scatter<<<nbN, TB, 0, s>>>(c, pos, p->d_radii, F, T, S, p->d_key_r, p->d_rank_r, p->d_start_r,
+                                 p->d_key_s, p->d_rank_s, p->d_start_s, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig, p->d_recs);
+    p->last_launches += 1;
+    CUDA_TRY(p, cudaGetLastError());
+    MARK();
+    // ---- a2: real-space pair sum ----
+    if (do_real) {
+        k_real<<<(c.N + REAL_WARPS - 1) / REAL_WARPS, REAL_WARPS * 32, 0, s>>>(c, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig,
+                                                                                p->d_start_r, p->d_out_real);
+        p->last_launches += 1;
+        CUDA_TRY(p, cudaGetLastError());
+    }
+    MARK();
+    // ---- a3..a7: Spectral Ewald wave-space sum ----
+    bool wave_done = false;
+    if (on(SE_STAGE_SPREAD)) {
+        dispatch_spread(p, s);
+        p->last_launches += 1;
+        CUDA_TRY(p, cudaGetLastError());
+    }
+    MARK();
+    if (on(SE_STAGE_FFT_FWD)) {
+        CUFFT_TRY(p, cufftSetStream(p->fft_fwd, s));
+        CUFFT_TRY(p, cufftExecD2Z(p->fft_fwd, p->d_real, (cufftDoubleComplex *)p->d_Hk));
+    }
+    MARK();
+    if (on(SE_STAGE_KSPACE)) {
+        const size_t Gc = (size_t)c.M * c.M * (c.M / 2 + 1);
+        k_kspace<<<(unsigned)((Gc + KSPACE_THREADS - 1) / KSPACE_THREADS), KSPACE_THREADS, 0, s>>>(c, p->d_Hk, p->d_Gk);
+        p->last_launches += 1;
+        CUDA_TRY(p, cudaGetLastError());
+    }
+    MARK();
+    if (on(SE_STAGE_FFT_INV)) {
+        CUFFT_TRY(p, cufftSetStream(p->fft_inv, s));
+        CUFFT_TRY(p, cufftExecZ2D(p->fft_inv, (cufftDoubleComplex *)p->d_Gk, p->d_real));
+    }
+    MARK();
+    if (on(SE_STAGE_GATHER)) {
+        dispatch_gather(p, s);
+        p->last_launches += 1;
+        CUDA_TRY(p, cudaGetLastError());
+        wave_done = true;
+    }
+    MARK();
+    // ---- a8: epilogue ----
+    k_epilogue<<<nbN, TB, 0, s>>>(c, fl | (wave_done ? 0u : SE_SKIP_WAVE), p->d_radii, F, T, S, p->d_out_real, p->d_out_wave, U, Omega, E);
+    p->last_launches += 1;
+    CUDA_TRY(p, cudaGetLastError());
+    MARK();
+#undef MARK
+    p->timed = timing;
+    return SE_OK;
+}
+
+extern "C" se_status far_mobility_apply_compressible(se_plan *p, const double *pos, const double *F, const double *T,
+                                                     const double *S, const double *s_in, double *U, double *Omega,
+                                                     double *E, double *s_out, void *cuda_stream)
+{
+    if (!p) return SE_ERR_INVALID_ARG;
+    if (s_in || s_out) return fail(p, SE_ERR_UNSUPPORTED, "far_mobility_apply_compressible", "pressure moments not built yet");
+    return far_mobility_apply(p, pos, F, T, S, U, Omega, E, cuda_stream);
+}
+
+extern "C" se_status far_mobility_apply_host(se_plan *p, const double *pos, const double *F, const double *T,
+                                             const double *S, double *U, double *Omega, double *E, void *cuda_stream)
+{
+    if (!p) return SE_ERR_INVALID_ARG;
+    if (!pos || !F || !T || !S || !U || !Omega || !E) return fail(p, SE_ERR_INVALID_ARG, "far_mobility_apply_host", "null pointer");
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const size_t N = (size_t)p->c.N, B = sizeof(double);
+    double *d = p->d_io;
+    double *dpos = d, *dF = d + 3 * N, *dT = d + 6 * N, *dS = d + 9 * N, *dU = d + 14 * N, *dW = d + 17 * N, *dE = d + 20 * N;
+    CUDA_TRY(p, cudaMemcpyAsync(dpos, pos, 3 * N * B, cudaMemcpyHostToDevice, s));
+    CUDA_TRY(p, cudaMemcpyAsync(dF, F, 3 * N * B, cudaMemcpyHostToDevice, s));
+    CUDA_TRY(p, cudaMemcpyAsync(dT, T, 3 * N * B, cudaMemcpyHostToDevice, s));
+    CUDA_TRY(p, cudaMemcpyAsync(dS, S, 5 * N * B, cudaMemcpyHostToDevice, s));
+    se_status st = far_mobility_apply(p, dpos, dF, dT, dS, dU, dW, dE, cuda_stream);
+    if (st != SE_OK) return st;
+    CUDA_TRY(p, cudaMemcpyAsync(U, dU, 3 * N * B, cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(p, cudaMemcpyAsync(Omega, dW, 3 * N * B, cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(p, cudaMemcpyAsync(E, dE, 5 * N * B, cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(p, cudaStreamSynchronize(s));
+    return SE_OK;
+}
+
+extern "C" se_status se_plan_copy_grids(se_plan *p, int which, double *dst)
+{
+    if (!p || !dst || which < 0 || which > 1) return SE_ERR_INVALID_ARG;
+    const size_t G = (size_t)p->c.M * p->c.M * p->c.M;
+    CUDA_TRY(p, cudaMemcpy(dst, p->d_real, sizeof(double) * (which == 0 ? 3 : 6) * G, cudaMemcpyDeviceToHost));
+    return SE_OK;
+}
+
+extern "C" se_status se_plan_get_timings(se_plan *p, double *ms)
+{
+    if (!p || !ms) return SE_ERR_INVALID_ARG;
+    if (!p->timed) return fail(p, SE_ERR_INVALID_ARG, "se_plan_get_timings", "last apply was not made with SE_TIMING");
+    CUDA_TRY(p, cudaEventSynchronize(p->ev[SE_NUM_STAGES]));
+    for (int k = 0; k < SE_NUM_STAGES; ++k) {
+        float t = 0.f;
+        CUDA_TRY(p, cudaEventElapsedTime(&t, p->ev[k], p->ev[k + 1]));
+        ms[k] = (double)t;
+    }
+    return SE_OK;
+}

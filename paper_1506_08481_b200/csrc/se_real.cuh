@@ -1,0 +1,192 @@
+// a2: real-space Ewald pair sum, matrix-free (Sec. 3.3; Eq. 22 with Eq. 13-15 and Eq. 17).
+//
+// Every coupling is a Cartesian derivative of two radial functions built from the Hasimoto screening
+// function Phi(r) = r erfc(xi r) - exp(-xi^2 r^2)/(xi sqrt(pi)) (Eq. 22):
+//     Psi = Phi + (ci+cj) B + ci cj C,   Lambda = lap Psi = B + (ci+cj) C + ci cj D,
+//     B = lap Phi, C = lap^2 Phi, D = lap^3 Phi,   ci, cj in {a^2/6, a^2/10, 0} per coupling.
+// Here the derivative tensors are contracted by hand with x, F, T, S (f_n = ((1/r) d/dr)^n f):
+//   U  = k0 { (L0-Ps1) F - Ps2 (x.F) x            [UF: (cFi,cFj)]
+//            + (1/2) L1 x^T                        [UT: (cFi,0)]
+//            - (L1-2Ps2) S.x + Ps3 (x.S.x) x }     [US: (cFi,cSj)]
+//   Om = k0 { (1/2) L1 x^F                         [OF: (0,cFj)]
+//            + (1/4) [(B1-C0) T + B2 (x.T) x]      [OT]
+//            - (1/2) L2 x^(S.x) }                  [OS: (0,cSj)]
+//   E  = k0 { x w + w x + a4 S + beta x x + kappa I },  w = a1 F + a2 (x^T) + a3 S.x
+//        a1 = L1/2 - Ps2, beta -= Ps3 (x.F), kappa -= Ps2 (x.F)       [EF: (cSi,cFj)]
+//        a2 = L2/4                                                     [ET: (cSi,0)]
+//        a3 = -(L2/2 - 2 Ps3), a4 = -(L1 - 2 Ps2), beta += Ps4 (x.S.x), kappa += Ps3 (x.S.x)   [ES: (cSi,cSj)]
+// with x = r_i - r_j (minimum image), k0 = 1/(8 pi eta0).
+#pragma once
+#include "se_common.cuh"
+
+#define REAL_WARPS 4
+#define REAL_QCAP 64
+
+// acc[0..2] U, [3..5] Omega, [6..10] E (xx,xy,xz,yy,yz); everything still to be multiplied by k0.
+__device__ __forceinline__ void pair_real(const SeConst &c, double x, double y, double z, double r2,
+                                          double cFi, double cSi, double aj, const double *__restrict__ mj,
+                                          double acc[11])
+{
+    const double cFj = aj * aj * (1.0 / 6.0), cSj = aj * aj * 0.1;
+    const double r = sqrt(r2), ir = 1.0 / r, ir2 = ir * ir;
+    const double xr = c.xi * r;
+    const double Ec = erfc(xr), qg = c.q * exp(-xr * xr);
+    const double ir3 = ir2 * ir, ir4 = ir2 * ir2, ir5 = ir4 * ir, ir6 = ir4 * ir2, ir7 = ir6 * ir, ir8 = ir4 * ir4, ir9 = ir8 * ir;
+    // Phi_n = ((1/r) d/dr)^n Phi
+    const double P1 = Ec * ir;
+    const double P2 = -(Ec * ir3 + qg * ir2);
+    const double P3 = 3.0 * Ec * ir5 + qg * (3.0 * ir4 + 2.0 * c.x2 * ir2);
+    const double P4 = -(15.0 * Ec * ir7 + qg * (15.0 * ir6 + 10.0 * c.x2 * ir4 + 4.0 * c.x4 * ir2));
+    const double P5 = 105.0 * Ec * ir9 + qg * (105.0 * ir8 + 70.0 * c.x2 * ir6 + 28.0 * c.x4 * ir4 + 8.0 * c.x6 * ir2);
+    // B_n: B = 2 Phi_1 - q g
+    const double B0 = 2.0 * P1 - qg;
+    const double B1 = 2.0 * P2 + 2.0 * c.x2 * qg;
+    const double B2 = 2.0 * P3 - 4.0 * c.x4 * qg;
+    const double B3 = 2.0 * P4 + 8.0 * c.x6 * qg;
+    const double B4 = 2.0 * P5 - 16.0 * c.x8 * qg;
+    // C_n, D_n: polynomials in s = r^2 times q g
+    const double C0 = qg * (10.0 * c.x2 - 4.0 * c.x4 * r2);
+    const double C1 = qg * (-28.0 * c.x4 + 8.0 * c.x6 * r2);
+    const double C2 = qg * (72.0 * c.x6 - 16.0 * c.x8 * r2);
+    const double C3 = qg * (-176.0 * c.x8 + 32.0 * c.x10 * r2);
+    const double C4 = qg * (416.0 * c.x10 - 64.0 * c.x12 * r2);
+    const double D0 = qg * (-84.0 * c.x4 + (96.0 * c.x6 - 16.0 * c.x8 * r2) * r2);
+    const double D1 = qg * (360.0 * c.x6 + (-256.0 * c.x8 + 32.0 * c.x10 * r2) * r2);
+    const double D2 = qg * (-1232.0 * c.x8 + (640.0 * c.x10 - 64.0 * c.x12 * r2) * r2);
+
+    const double Fx = mj[0], Fy = mj[1], Fz = mj[2], Tx = mj[3], Ty = mj[4], Tz = mj[5];
+    const double Sxx = mj[6], Sxy = mj[7], Sxz = mj[8], Syy = mj[9], Syz = mj[10], Szz = -(Sxx + Syy);
+    const double xF = x * Fx + y * Fy + z * Fz, xT = x * Tx + y * Ty + z * Tz;
+    const double Sx0 = Sxx * x + Sxy * y + Sxz * z, Sx1 = Sxy * x + Syy * y + Syz * z, Sx2 = Sxz * x + Syz * y + Szz * z;
+    const double xSx = x * Sx0 + y * Sx1 + z * Sx2;
+    const double cT0 = y * Tz - z * Ty, cT1 = z * Tx - x * Tz, cT2 = x * Ty - y * Tx;       // x ^ T
+    const double cF0 = y * Fz - z * Fy, cF1 = z * Fx - x * Fz, cF2 = x * Fy - y * Fx;       // x ^ F
+    const double cS0 = y * Sx2 - z * Sx1, cS1 = z * Sx0 - x * Sx2, cS2 = x * Sx1 - y * Sx0; // x ^ (S.x)
+
+    double s, p;
+    // ---- U ----
+    s = cFi + cFj; p = cFi * cFj;
+    const double uf_a = (B0 + s * C0 + p * D0) - (P1 + s * B1 + p * C1);
+    const double uf_b = -(P2 + s * B2 + p * C2) * xF;
+    const double ut = 0.5 * (B1 + cFi * C1);
+    s = cFi + cSj; p = cFi * cSj;
+    const double us_Ps2 = P2 + s * B2 + p * C2;
+    const double us_a = -((B1 + s * C1 + p * D1) - 2.0 * us_Ps2);
+    const double us_b = (P3 + s * B3 + p * C3) * xSx;
+    const double ux = uf_b + us_b;
+    acc[0] += uf_a * Fx + ux * x + ut * cT0 + us_a * Sx0;
+    acc[1] += uf_a * Fy + ux * y + ut * cT1 + us_a * Sx1;
+    acc[2] += uf_a * Fz + ux * z + ut * cT2 + us_a * Sx2;
+    // ---- Omega ----
+    const double of = 0.5 * (B1 + cFj * C1);
+    const double ot_a = 0.25 * (B1 - C0), ot_b = 0.25 * B2 * xT;
+    const double os = -0.5 * (B2 + cSj * C2);
+    acc[3] += of * cF0 + ot_a * Tx + ot_b * x + os * cS0;
+    acc[4] += of * cF1 + ot_a * Ty + ot_b * y + os * cS1;
+    acc[5] += of * cF2 + ot_a * Tz + ot_b * z + os * cS2;
+    // ---- E ----
+    s = cSi + cFj; p = cSi * cFj;
+    const double ef_Ps2 = P2 + s * B2 + p * C2, ef_Ps3 = P3 + s * B3 + p * C3;
+    const double a1 = 0.5 * (B1 + s * C1 + p * D1) - ef_Ps2;
+    const double a2 = 0.25 * (B2 + cSi * C2);
+    s = cSi + cSj; p = cSi * cSj;
+    const double es_Ps2 = P2 + s * B2 + p * C2, es_Ps3 = P3 + s * B3 + p * C3, es_Ps4 = P4 + s * B4 + p * C4;
+    const double a3 = -(0.5 * (B2 + s * C2 + p * D2) - 2.0 * es_Ps3);
+    const double a4 = -((B1 + s * C1 + p * D1) - 2.0 * es_Ps2);
+    const double beta = es_Ps4 * xSx - ef_Ps3 * xF;
+    const double kappa = es_Ps3 * xSx - ef_Ps2 * xF;
+    const double w0 = a1 * Fx + a2 * cT0 + a3 * Sx0, w1 = a1 * Fy + a2 * cT1 + a3 * Sx1, w2 = a1 * Fz + a2 * cT2 + a3 * Sx2;
+    acc[6] += 2.0 * x * w0 + a4 * Sxx + beta * x * x + kappa;
+    acc[7] += x * w1 + y * w0 + a4 * Sxy + beta * x * y;
+    acc[8] += x * w2 + z * w0 + a4 * Sxz + beta * x * z;
+    acc[9] += 2.0 * y * w1 + a4 * Syy + beta * y * y + kappa;
+    acc[10] += y * w2 + z * w1 + a4 * Syz + beta * y * z;
+}
+
+// One warp per target particle i (cell order).  Lanes scan the particles of the 27 neighbour cells
+// (or all particles when the box holds fewer than 3 cells per axis), hits are compacted through a
+// per-warp shared-memory queue so that the expensive pair evaluation always runs on full warps.
+__global__ void __launch_bounds__(REAL_WARPS * 32) k_real(SeConst c, const double4 *__restrict__ rs_pos,
+                                                          const double *__restrict__ rs_mom, const int *__restrict__ rs_orig,
+                                                          const int *__restrict__ start_r, double *__restrict__ out_real)
+{
+    __shared__ double4 qd[REAL_WARPS][REAL_QCAP];      // (dx, dy, dz, a_j)
+    __shared__ int qj[REAL_WARPS][REAL_QCAP];
+    const int wl = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int i = blockIdx.x * REAL_WARPS + wl;
+    if (i >= c.N) return;
+    const double4 pi = rs_pos[i];
+    const double cFi = pi.w * pi.w * (1.0 / 6.0), cSi = pi.w * pi.w * 0.1;
+    double acc[11];
+#pragma unroll
+    for (int k = 0; k < 11; ++k) acc[k] = 0.0;
+    int qn = 0;
+
+    const int nc = c.ncr;
+    int ci[3] = { 0, 0, 0 };
+    if (nc > 1) {
+        ci[0] = se_mod((int)floor(pi.x / c.hr), nc);
+        ci[1] = se_mod((int)floor(pi.y / c.hr), nc);
+        ci[2] = se_mod((int)floor(pi.z / c.hr), nc);
+    }
+    const int nrow = nc > 1 ? 9 : 1;
+    for (int row = 0; row < nrow; ++row) {
+        // neighbour cells (cx+dx, cy+dy, cz-1..cz+1): contiguous in memory except across the z wrap
+        int s0, e0, s1 = 0, e1 = 0;
+        if (nc > 1) {
+            const int cx = se_mod(ci[0] + row / 3 - 1, nc), cy = se_mod(ci[1] + row % 3 - 1, nc);
+            const int base = (cx * nc + cy) * nc;
+            const int zlo = ci[2] - 1, zhi = ci[2] + 1;
+            if (zlo < 0) { s0 = start_r[base]; e0 = start_r[base + zhi + 1]; s1 = start_r[base + nc - 1]; e1 = start_r[base + nc]; }
+            else if (zhi >= nc) { s0 = start_r[base + zlo]; e0 = start_r[base + nc]; s1 = start_r[base]; e1 = start_r[base + 1]; }
+            else { s0 = start_r[base + zlo]; e0 = start_r[base + zhi + 1]; }
+        } else { s0 = 0; e0 = c.N; }
+        for (int part = 0; part < 2; ++part) {
+            const int s = part ? s1 : s0, e = part ? e1 : e0;
+            for (int jb = s; jb < e; jb += 32) {
+                const int j = jb + lane;
+                bool hit = false;
+                double dx = 0, dy = 0, dz = 0, aj = 0;
+                if (j < e && j != i) {
+                    const double4 pj = rs_pos[j];
+                    dx = pi.x - pj.x; dy = pi.y - pj.y; dz = pi.z - pj.z;
+                    dx -= c.L * rint(dx / c.L); dy -= c.L * rint(dy / c.L); dz -= c.L * rint(dz / c.L);
+                    const double r2 = dx * dx + dy * dy + dz * dz;
+                    hit = (r2 < c.rc2) && (r2 > 0.0);
+                    aj = pj.w;
+                }
+                const unsigned mask = __ballot_sync(0xffffffffu, hit);
+                if (hit) {
+                    const int slot = qn + __popc(mask & ((1u << lane) - 1u));
+                    qd[wl][slot] = make_double4(dx, dy, dz, aj);
+                    qj[wl][slot] = j;
+                }
+                qn += __popc(mask);
+                __syncwarp();
+                if (qn >= 32) {
+                    const double4 d = qd[wl][qn - 32 + lane];
+                    const int jj = qj[wl][qn - 32 + lane];
+                    pair_real(c, d.x, d.y, d.z, d.x * d.x + d.y * d.y + d.z * d.z, cFi, cSi, d.w, rs_mom + 12 * (size_t)jj, acc);
+                    qn -= 32;
+                    __syncwarp();
+                }
+            }
+        }
+    }
+    if (lane < qn) {
+        const double4 d = qd[wl][lane];
+        pair_real(c, d.x, d.y, d.z, d.x * d.x + d.y * d.y + d.z * d.z, cFi, cSi, d.w, rs_mom + 12 * (size_t)qj[wl][lane], acc);
+    }
+#pragma unroll
+    for (int k = 0; k < 11; ++k) {
+        double v = acc[k];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        acc[k] = v;
+    }
+    if (lane == 0) {
+        double *o = out_real + 11 * (size_t)rs_orig[i];
+#pragma unroll
+        for (int k = 0; k < 11; ++k) o[k] = c.k0 * acc[k];
+    }
+}

@@ -1,0 +1,158 @@
+// a1: wrap, counting sorts (by real-space cell and by spreading tile), packed per-particle records.
+// PAPER.md Sec. 3.3 (cells slightly larger than r_c, 27-cell search) and Sec. 3.4 (per-grid-point
+// particle lists, replaced here by a counting sort by grid tile).
+#pragma once
+#include "se_common.cuh"
+
+__device__ __forceinline__ double se_wrap(double x, double L) { return x - L * floor(x / L); }
+
+// One thread per particle: cell keys and the rank inside each cell (atomic counter).
+__global__ void k_keys(SeConst c, const double *__restrict__ pos, int *__restrict__ key_r, int *__restrict__ rank_r,
+                       int *__restrict__ cnt_r, int *__restrict__ key_s, int *__restrict__ rank_s, int *__restrict__ cnt_s)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= c.N) return;
+    int cc[3], n0[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const double xw = se_wrap(pos[3 * (size_t)i + d], c.L);
+        cc[d] = se_mod((int)floor(xw / c.hr), c.ncr);
+        n0[d] = se_mod(se_support_start(xw * c.MoverL, c.P), c.M);
+    }
+    const int kr = (cc[0] * c.ncr + cc[1]) * c.ncr + cc[2];
+    const int ks = (n0[0] * c.NBY + n0[1] / SE_TILE_Y) * c.NBZ + n0[2] / SE_TILE_Z;
+    key_r[i] = kr;
+    key_s[i] = ks;
+    rank_r[i] = atomicAdd(&cnt_r[kr], 1);
+    rank_s[i] = atomicAdd(&cnt_s[ks], 1);
+}
+
+// ---- exclusive prefix sum over n ints (three small kernels; n up to a few million) ----
+#define SCAN_THREADS 256
+#define SCAN_ITEMS 8
+#define SCAN_BLOCK (SCAN_THREADS * SCAN_ITEMS)
+
+__device__ __forceinline__ int block_exclusive_scan(int v, int *total)
+{
+    __shared__ int wsum[SCAN_THREADS / 32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    int inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) wsum[w] = inc;
+    __syncthreads();
+    if (w == 0) {
+        int s = lane < SCAN_THREADS / 32 ? wsum[lane] : 0;
+#pragma unroll
+        for (int o = 1; o < SCAN_THREADS / 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, s, o);
+            if (lane >= o) s += t;
+        }
+        if (lane < SCAN_THREADS / 32) wsum[lane] = s;
+    }
+    __syncthreads();
+    const int base = w ? wsum[w - 1] : 0;
+    *total = wsum[SCAN_THREADS / 32 - 1];
+    __syncthreads();
+    return base + inc - v;
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_local(const int *__restrict__ in, int *__restrict__ out,
+                                                            int *__restrict__ bsum, int n)
+{
+    const int base = blockIdx.x * SCAN_BLOCK + threadIdx.x * SCAN_ITEMS;
+    int v[SCAN_ITEMS], s = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) { v[k] = (base + k < n) ? in[base + k] : 0; s += v[k]; }
+    int total;
+    int off = block_exclusive_scan(s, &total);
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) { if (base + k < n) out[base + k] = off; off += v[k]; }
+    if (threadIdx.x == 0) bsum[blockIdx.x] = total;
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_sums(int *__restrict__ bsum, int nb)
+{
+    int carry = 0;
+    for (int b0 = 0; b0 < nb; b0 += SCAN_THREADS) {
+        const int idx = b0 + threadIdx.x;
+        const int v = idx < nb ? bsum[idx] : 0;
+        int total;
+        const int ex = block_exclusive_scan(v, &total);
+        if (idx < nb) bsum[idx] = carry + ex;
+        carry += total;
+    }
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_add(int *__restrict__ out, const int *__restrict__ bsum, int n, int total)
+{
+    const int base = blockIdx.x * SCAN_BLOCK + threadIdx.x * SCAN_ITEMS;
+    const int add = bsum[blockIdx.x];
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) if (base + k < n) out[base + k] += add;
+    if (blockIdx.x == 0 && threadIdx.x == 0) out[n] = total;      // sentinel: start[n] = N
+}
+
+// One thread per particle: write the real-space packed copy (cell order) and the spreading/gather
+// record (tile order) with the per-axis Gaussian tables (Eq. 41 in physical coordinates; the paper's
+// fast Gaussian gridding, Eq. 47, is replaced by P direct exponentials per axis, done once here).
+__global__ void k_scatter(SeConst c, const double *__restrict__ pos, const double *__restrict__ radii,
+                          const double *__restrict__ F, const double *__restrict__ T, const double *__restrict__ S,
+                          const int *__restrict__ key_r, const int *__restrict__ rank_r, const int *__restrict__ start_r,
+                          const int *__restrict__ key_s, const int *__restrict__ rank_s, const int *__restrict__ start_s,
+                          double4 *__restrict__ rs_pos, double *__restrict__ rs_mom, int *__restrict__ rs_orig,
+                          double *__restrict__ recs)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= c.N) return;
+    const size_t i3 = 3 * (size_t)i, i5 = 5 * (size_t)i;
+    const double a = radii[i];
+    double xw[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) xw[d] = se_wrap(pos[i3 + d], c.L);
+    const double f[3] = { F[i3], F[i3 + 1], F[i3 + 2] }, t[3] = { T[i3], T[i3 + 1], T[i3 + 2] };
+    const double s[5] = { S[i5], S[i5 + 1], S[i5 + 2], S[i5 + 3], S[i5 + 4] };
+
+    // real-space copy
+    const int dr = start_r[key_r[i]] + rank_r[i];
+    rs_pos[dr] = make_double4(xw[0], xw[1], xw[2], a);
+    double *m = rs_mom + 12 * (size_t)dr;
+    m[0] = f[0]; m[1] = f[1]; m[2] = f[2]; m[3] = t[0]; m[4] = t[1]; m[5] = t[2];
+    m[6] = s[0]; m[7] = s[1]; m[8] = s[2]; m[9] = s[3]; m[10] = s[4]; m[11] = 0.0;
+    rs_orig[dr] = i;
+
+    // spreading / gather record
+    const int ds = start_s[key_s[i]] + rank_s[i];
+    double *r = recs + (size_t)ds * c.rec_stride;
+    int n0w[3];
+    double d0[3];
+    const double cF = a * a / 6.0, cS = a * a / 10.0, al = c.alpha;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const double u = xw[d] * c.MoverL;
+        const int n0 = se_support_start(u, c.P);
+        n0w[d] = se_mod(n0, c.M);
+        d0[d] = ((double)n0 - u) * c.Delta;
+        double *g = r + SE_REC_HDR + d * c.P;
+        for (int k = 0; k < c.P; ++k) {
+            const double dk = ((double)(n0 + k) - u) * c.Delta;
+            const double e = exp(-al * dk * dk);
+            g[k] = d == 0 ? c.gnorm * e : e;
+        }
+    }
+    reinterpret_cast<int2 *>(r)[0] = make_int2(n0w[1], n0w[2]);
+    reinterpret_cast<int2 *>(r)[1] = make_int2(n0w[0], i);
+    r[REC_D0] = d0[0]; r[REC_D0 + 1] = d0[1]; r[REC_D0 + 2] = d0[2];
+    r[REC_POLY] = 1.0 - 6.0 * al * cF;
+    r[REC_POLY + 1] = 4.0 * al * al * cF;
+    r[REC_POLY + 2] = 2.0 * al * (1.0 - 10.0 * al * cS);
+    r[REC_POLY + 3] = 8.0 * al * al * al * cS;
+    r[REC_F] = f[0]; r[REC_F + 1] = f[1]; r[REC_F + 2] = f[2];
+    r[REC_T] = t[0]; r[REC_T + 1] = t[1]; r[REC_T + 2] = t[2];
+    r[REC_S] = s[0]; r[REC_S + 1] = s[1]; r[REC_S + 2] = s[2]; r[REC_S + 3] = s[3]; r[REC_S + 4] = s[4];
+    r[REC_S + 5] = -(s[0] + s[3]);
+    r[REC_CF] = cF; r[REC_CS] = cS; r[REC_A] = a;
+}
