@@ -1,0 +1,247 @@
+"""Parity of the CUDA path (through the C-ABI) against the CPU oracle O2, element by element, on the same
+seeded inputs.  Tolerance: relative L2 <= 1e-11 per output block (BASELINE.json north_star); per-stage
+checks use 1e-12.  Run with ``-m gpu`` on a B200."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11          # north_star: "relative L2 error <= 1e-11 on the same seeded inputs and parameters"
+TOL_STAGE = 1e-12
+
+
+def _rel(a, b):
+    return float(np.linalg.norm(np.asarray(a) - np.asarray(b)) / np.linalg.norm(np.asarray(b)))
+
+
+@pytest.fixture(scope="module")
+def pk():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_1506_08481_b200 as pk
+    pk.load_library()
+    return pk
+
+
+class Runner:
+    """Holds the device copies of one workload and a plan."""
+
+    def __init__(self, pk, wl, M=None, P=None, rc=None, xi=None):
+        import torch
+        self.pk, self.wl, self.torch = pk, wl, torch
+        self.M, self.P = M or wl.M, P or wl.P
+        self.rc, self.xi = rc or wl.rc, xi or wl.xi
+        self.plan = pk.SePlan(wl.N, wl.L, wl.radii, self.xi, self.rc, self.M, self.P, wl.eta0)
+        dev = torch.device("cuda:0")
+        t = lambda a: torch.tensor(np.ascontiguousarray(a), device=dev, dtype=torch.float64)
+        self.pos, self.F, self.T, self.S = t(wl.pos), t(wl.F), t(wl.T), t(wl.S)
+        self.U = torch.full((wl.N, 3), float("nan"), device=dev, dtype=torch.float64)
+        self.W = torch.full((wl.N, 3), float("nan"), device=dev, dtype=torch.float64)
+        self.E = torch.full((wl.N, 5), float("nan"), device=dev, dtype=torch.float64)
+
+    def run(self, flags=0, stop=-1, pos=None, F=None, T=None, S=None):
+        self.plan.set_flags(flags)
+        self.plan.debug_stop(stop)
+        self.plan.apply(self.pos if pos is None else pos, self.F if F is None else F, self.T if T is None else T,
+                        self.S if S is None else S, self.U, self.W, self.E)
+        self.torch.cuda.synchronize()
+        return self.U.cpu().numpy(), self.W.cpu().numpy(), self.E.cpu().numpy()
+
+    def oracle(self, O, parts=None, want_grids=False):
+        wl = self.wl
+        return O.o2_apply(wl.pos, wl.radii, wl.L, self.xi, self.rc, self.M, self.P, wl.F, wl.T, wl.S,
+                          parts=O.PART_ALL if parts is None else parts, want_grids=want_grids)
+
+
+def _check_blocks(got, ref, tol):
+    U, W, E = got
+    assert _rel(U, ref["U"]) <= tol and _rel(W, ref["Omega"]) <= tol and _rel(E, ref["E"]) <= tol, \
+        (_rel(U, ref["U"]), _rel(W, ref["Omega"]), _rel(E, ref["E"]))
+    allg = np.concatenate([U, W, E], axis=1)
+    allr = np.concatenate([ref["U"], ref["Omega"], ref["E"]], axis=1)
+    assert _rel(allg, allr) <= tol
+
+
+# ------------------------------------------------------------------------------------------------
+# T9: per-stage parity on the configs the oracle finishes in seconds (several tiles, ragged tails)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["c1", "c2", "c3"])
+def test_stage_parity(pk, oracle, workloads, name):
+    wl = workloads.make_workload(name)
+    r = Runner(pk, wl)
+    ref = r.oracle(oracle, want_grids=True)
+    # a2 real-space part alone
+    ref_real = r.oracle(oracle, parts=oracle.PART_REAL)
+    _check_blocks(r.run(flags=pk.SE_SKIP_WAVE | pk.SE_SKIP_SELF | pk.SE_SKIP_ONEBODY), ref_real, TOL_STAGE)
+    # a3 spread grids
+    r.run(stop=2)
+    assert _rel(r.plan.copy_grids(0), ref["gridH"]) <= TOL_STAGE
+    # a4-a6 returned grids u~, w~
+    r.run(stop=5)
+    Gr = r.plan.copy_grids(1)
+    for g in range(6):
+        assert _rel(Gr[g], ref["gridOut"][g]) <= TOL_STAGE, g
+    # a7 wave part alone (gather of the returned grids)
+    ref_wave = r.oracle(oracle, parts=oracle.PART_WAVE)
+    _check_blocks(r.run(flags=pk.SE_SKIP_REAL | pk.SE_SKIP_SELF | pk.SE_SKIP_ONEBODY), ref_wave, TOL_STAGE)
+    # a8 self + one-body alone
+    ref_so = r.oracle(oracle, parts=oracle.PART_SELF | oracle.PART_ONEBODY)
+    _check_blocks(r.run(flags=pk.SE_SKIP_REAL | pk.SE_SKIP_WAVE), ref_so, TOL_STAGE)
+    # full product; E traceless by storage, outputs overwritten (they were NaN-filled)
+    got = r.run()
+    _check_blocks(got, ref, TOL)
+    assert np.isfinite(got[0]).all() and np.isfinite(got[2]).all()
+
+
+# ------------------------------------------------------------------------------------------------
+# T10: full product at full size
+# ------------------------------------------------------------------------------------------------
+def test_full_product_c4(pk, oracle, workloads):
+    wl = workloads.make_workload("c4")
+    r = Runner(pk, wl)
+    got = r.run()
+    _check_blocks(got, r.oracle(oracle), TOL)
+    # Eq. 78 error metric of the GPU against the oracle (reported, bounded)
+    ref = r.oracle(oracle)["E"]
+    full = lambda e: np.sqrt(e[:, 0] ** 2 + e[:, 3] ** 2 + (e[:, 0] + e[:, 3]) ** 2 + 2 * (e[:, 1] ** 2 + e[:, 2] ** 2 + e[:, 4] ** 2))
+    assert (full(got[2] - ref) / full(ref)).max() < 1e-9
+
+
+@pytest.mark.slow
+def test_full_product_c5(pk, oracle, workloads):
+    """N = 1e6, M = 512: the real-space part on sampled particles against the one-by-one brute-force
+    oracle, and the full product against the full oracle run."""
+    wl = workloads.make_workload("c5")
+    r = Runner(pk, wl)
+    tg = np.arange(0, wl.N, wl.N // 96)
+    Ur, Wr, Er, _ = oracle.o2_real_targets(wl.pos, wl.radii, wl.L, wl.xi, wl.rc, wl.F, wl.T, wl.S, tg)
+    U, W, E = r.run(flags=pk.SE_SKIP_WAVE | pk.SE_SKIP_SELF | pk.SE_SKIP_ONEBODY)
+    assert _rel(U[tg], Ur) <= TOL_STAGE and _rel(W[tg], Wr) <= TOL_STAGE and _rel(E[tg], Er) <= TOL_STAGE
+    got = r.run()
+    _check_blocks(got, r.oracle(oracle), TOL)
+
+
+# ------------------------------------------------------------------------------------------------
+# Edge cases and invariances (T8, T12)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("P", [2, 5, 8, 9, 13, 16, 21, 24])
+def test_every_support_size_even_and_odd(pk, oracle, workloads, P):
+    wl = workloads.make_workload("c1")
+    r = Runner(pk, wl, M=32, P=P)
+    _check_blocks(r.run(), r.oracle(oracle), TOL)
+
+
+@pytest.mark.parametrize("M", [12, 26, 36, 50])
+def test_grid_sizes_that_are_not_multiples_of_the_tile(pk, oracle, workloads, M):
+    """Ragged tile bins (M % 8 != 0, M % 4 != 0) and supports that wrap onto themselves (P = M)."""
+    wl = workloads.make_workload("c1")
+    r = Runner(pk, wl, M=M, P=min(12, M))
+    ref = r.oracle(oracle, want_grids=True)
+    r.run(stop=2)
+    assert _rel(r.plan.copy_grids(0), ref["gridH"]) <= TOL_STAGE
+    _check_blocks(r.run(), ref, TOL)
+
+
+def test_tiny_systems_all_pairs_path_and_single_particle(pk, oracle, workloads):
+    # fewer than 3 cells per axis -> all-pairs minimum-image loop
+    sysm = workloads.random_small_system(7, 12, 9.0)
+    import workloads as W
+    wl = W.Workload(name="tiny", N=12, L=9.0, radii=sysm["radii"], pos=sysm["pos"], F=sysm["F"], T=sysm["T"], S=sysm["S"],
+                    xi=0.9, rc=4.5, M=24, P=10, m=0.0)
+    r = Runner(pk, wl)
+    assert r.plan.constants()["real_cells"] == 1
+    _check_blocks(r.run(), r.oracle(oracle), TOL)
+    # N = 1: only self-image wave part + self + one-body
+    wl1 = W.Workload(name="one", N=1, L=9.0, radii=sysm["radii"][:1], pos=sysm["pos"][:1], F=sysm["F"][:1], T=sysm["T"][:1],
+                     S=sysm["S"][:1], xi=0.9, rc=4.5, M=24, P=10, m=0.0)
+    r1 = Runner(pk, wl1)
+    _check_blocks(r1.run(), r1.oracle(oracle), TOL)
+
+
+def test_unwrapped_positions_and_box_edges(pk, oracle, workloads):
+    """Positions far outside [0,L), exactly on the faces, and a tiny negative value that wraps to L."""
+    import torch
+    wl = workloads.make_workload("c1")
+    pos = wl.pos.copy()
+    rng = np.random.default_rng(3)
+    pos += wl.L * rng.integers(-3, 4, size=pos.shape)
+    pos[0] = [0.0, wl.L, -1e-18]
+    pos[1, 0] = -wl.L
+    wl.pos = pos
+    r = Runner(pk, wl)
+    _check_blocks(r.run(), r.oracle(oracle), TOL)
+
+
+def test_zero_input_linearity_and_shift_invariance(pk, workloads):
+    import torch
+    wl = workloads.make_workload("c2")
+    r = Runner(pk, wl)
+    base = [x.copy() for x in r.run()]
+    z = torch.zeros_like
+    zero = r.run(F=z(r.F), T=z(r.T), S=z(r.S))
+    assert all(np.abs(x).max() == 0.0 for x in zero)
+    two = r.run(F=2 * r.F, T=2 * r.T, S=2 * r.S)
+    for a, b in zip(two, base):
+        assert _rel(a, 2 * b) <= 1e-13
+    Delta = wl.L / wl.M
+    shift = torch.tensor([3 * Delta, -7 * Delta, 64 * Delta], device=r.pos.device, dtype=torch.float64)
+    sh = r.run(pos=r.pos + shift)
+    for a, b in zip(sh, base):
+        assert _rel(a, b) <= 1e-11
+
+
+def test_host_entry_point_and_stage_timings(pk, oracle, workloads):
+    wl = workloads.make_workload("c2")
+    r = Runner(pk, wl)
+    ref = r.oracle(oracle)
+    U, W, E = np.empty((wl.N, 3)), np.empty((wl.N, 3)), np.empty((wl.N, 5))
+    r.plan.set_flags(pk.SE_TIMING)
+    r.plan.apply_host(wl.pos, wl.F, wl.T, wl.S, U, W, E)
+    _check_blocks((U, W, E), ref, TOL)
+    tm = r.plan.timings()
+    assert set(tm) == set(pk.STAGE_NAMES) and all(v >= 0 for v in tm.values()) and sum(tm.values()) > 0
+    assert r.plan.last_launch_count() == 13
+    assert r.plan.workspace_bytes() > 6 * 8 * wl.M ** 3
+
+
+def test_api_errors_on_device(pk, workloads):
+    wl = workloads.make_workload("c1")
+    r = Runner(pk, wl)
+    ptrs = [t.data_ptr() for t in (r.pos, r.F, r.T, r.S, r.U, r.W, r.E)]
+    for k in range(7):
+        a = list(ptrs); a[k] = None
+        assert r.plan.apply_raw(*a) == 1          # SE_ERR_INVALID_ARG, nothing launched
+    with pytest.raises(pk.SeError):
+        r.plan.set_flags(0x100)
+    with pytest.raises(pk.SeError):
+        r.plan.set_shape(-1.0)
+    with pytest.raises(pk.SeError):
+        r.plan.timings()                          # last apply was not timed
+    with pytest.raises(ValueError):
+        r.plan.apply(r.pos.float(), r.F, r.T, r.S, r.U, r.W, r.E)
+
+
+def test_shape_parameter_and_two_plans_on_two_streams(pk, oracle, workloads):
+    import torch
+    wl = workloads.make_workload("c1")
+    a, b = Runner(pk, wl), Runner(pk, wl)
+    a.plan.set_shape(4.2)
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    for _ in range(3):
+        a.plan.apply(a.pos, a.F, a.T, a.S, a.U, a.W, a.E, stream=sa)
+        b.plan.apply(b.pos, b.F, b.T, b.S, b.U, b.W, b.E, stream=sb)
+    torch.cuda.synchronize()
+    ref_a = oracle.o2_apply(wl.pos, wl.radii, wl.L, wl.xi, wl.rc, wl.M, wl.P, wl.F, wl.T, wl.S, m=4.2)
+    _check_blocks((a.U.cpu().numpy(), a.W.cpu().numpy(), a.E.cpu().numpy()), ref_a, TOL)
+    _check_blocks((b.U.cpu().numpy(), b.W.cpu().numpy(), b.E.cpu().numpy()), b.oracle(oracle), TOL)
+
+
+def test_overlapping_and_coincident_particles(pk, oracle, workloads):
+    """Overlap is not an error (formulas regular for r > 0); exactly coincident particles are skipped."""
+    wl = workloads.make_workload("c1")
+    wl.pos = wl.pos.copy()
+    wl.pos[1] = wl.pos[0] + np.array([0.3, 0.1, -0.2])     # overlapping
+    wl.pos[3] = wl.pos[2]                                   # coincident
+    r = Runner(pk, wl)
+    _check_blocks(r.run(), r.oracle(oracle), TOL)
