@@ -133,6 +133,12 @@ size_t se_plan_workspace_bytes(const se_plan *plan);
  * cell grid (as double), number of sweep segments of the spreading kernel (as double). */
 se_status se_plan_get_constants(const se_plan *plan, double *out);
 
+/* Measurement aid for the "alu" roofline of the real-space kernel: runs independent double-precision FMA
+ * chains on every SM of the current device on cuda_stream (NULL = default), times them with CUDA events and
+ * writes the sustained rate in TFLOP/s (2 flop per FMA) to *tflops.  Synchronises the stream.
+ * Errors: SE_ERR_INVALID_ARG for NULL, SE_ERR_CUDA without a device. */
+se_status se_measure_fp64_peak(double *tflops, void *cuda_stream);
+
 /* Text of the last error on this plan ("" if none); owned by the plan. */
 const char *se_last_error(const se_plan *plan);
 

@@ -73,6 +73,8 @@ def load_library(build_if_missing: bool = True):
     L.se_last_error.argtypes = [P]
     L.se_plan_destroy.restype = INT
     L.se_plan_destroy.argtypes = [P]
+    L.se_measure_fp64_peak.restype = INT
+    L.se_measure_fp64_peak.argtypes = [P, P]
     L.se_version.restype = ctypes.c_char_p
     L.se_version.argtypes = []
     _lib = L
@@ -81,6 +83,17 @@ def load_library(build_if_missing: bool = True):
 
 def version() -> str:
     return load_library().se_version().decode()
+
+
+def measure_fp64_peak(stream=None) -> float:
+    """se_measure_fp64_peak: sustained independent-DFMA rate of the current device in TFLOP/s."""
+    import torch
+    sp = (torch.cuda.current_stream() if stream is None else stream).cuda_stream
+    out = ctypes.c_double(0.0)
+    st = load_library().se_measure_fp64_peak(ctypes.byref(out), sp)
+    if st != 0:
+        raise SeError(st, "se_measure_fp64_peak")
+    return float(out.value)
 
 
 def _dptr(t, n, name):

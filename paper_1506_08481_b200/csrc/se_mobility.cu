@@ -415,6 +415,54 @@ extern "C" se_status se_plan_copy_grids(se_plan *p, int which, double *dst)
     return SE_OK;
 }
 
+// Independent DFMA chains: 8 accumulators per thread, 4096 rounds, 8 CTAs of 256 threads per SM.
+__global__ void __launch_bounds__(256) k_fp64_peak(double *sink, double a, double b, int rounds)
+{
+    double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+    for (int r = 0; r < rounds; ++r) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+            x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+        }
+    }
+    const double s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+    if (s == 123.456) sink[0] = s;           // never true; keeps the chains alive
+}
+
+extern "C" se_status se_measure_fp64_peak(double *tflops, void *cuda_stream)
+{
+    if (!tflops) return SE_ERR_INVALID_ARG;
+    *tflops = 0.0;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return SE_ERR_CUDA;
+    }
+    double *sink = nullptr;
+    cudaEvent_t e0, e1;
+    if (cudaMalloc((void **)&sink, 8) != cudaSuccess) { cudaGetLastError(); return SE_ERR_CUDA; }
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int rounds = 4096, blocks = sms * 8;
+    float best = 1e30f;
+    cudaError_t e = cudaSuccess;
+    for (int rep = 0; rep < 4 && e == cudaSuccess; ++rep) {       // first repetition warms up
+        cudaEventRecord(e0, s);
+        k_fp64_peak<<<blocks, 256, 0, s>>>(sink, 0.999999, 1e-9, rounds);
+        cudaEventRecord(e1, s);
+        e = cudaEventSynchronize(e1);
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+    if (e != cudaSuccess) { cudaGetLastError(); return SE_ERR_CUDA; }
+    const double fma_count = (double)blocks * 256.0 * rounds * 64.0;
+    *tflops = 2.0 * fma_count / (best * 1e-3) / 1e12;
+    return SE_OK;
+}
+
 extern "C" se_status se_plan_get_timings(se_plan *p, double *ms)
 {
     if (!p || !ms) return SE_ERR_INVALID_ARG;
