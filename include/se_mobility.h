@@ -79,6 +79,10 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, const double *radii
 /* Gaussian shape parameter m of Eq. 46 (h ~ exp(-m^2/2) at the edge of the support), m > 0. */
 se_status se_plan_set_shape(se_plan *plan, double m);
 
+/* Performance knob: number of segments the x-sweeps of the spreading and gather kernels are cut into
+ * (0 = the plan's own choice).  Results do not depend on it beyond summation order. */
+se_status se_plan_set_tuning(se_plan *plan, int spread_segments, int gather_segments);
+
 /* Bitwise OR of the SE_* flags above. */
 se_status se_plan_set_flags(se_plan *plan, unsigned flags);
 
@@ -129,8 +133,8 @@ int se_plan_last_launch_count(const se_plan *plan);
 /* Device bytes held by the plan (grids, sorted copies, cell tables, cuFFT work areas). */
 size_t se_plan_workspace_bytes(const se_plan *plan);
 
-/* Derived constants, for tests: out[0..5] = Delta, eta_se, alpha, m, cells per axis of the real-space
- * cell grid (as double), number of sweep segments of the spreading kernel (as double). */
+/* Derived constants, for tests: out[0..6] = Delta, eta_se, alpha, m, cells per axis of the real-space
+ * cell grid (as double), number of sweep segments of the spreading and of the gather kernel (as double). */
 se_status se_plan_get_constants(const se_plan *plan, double *out);
 
 /* Measurement aid for the "alu" roofline of the real-space kernel: runs independent double-precision FMA

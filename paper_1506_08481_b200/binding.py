@@ -49,6 +49,8 @@ def load_library(build_if_missing: bool = True):
     L.se_plan_create.argtypes = [ctypes.POINTER(P), I64, D, P, D, D, INT, INT, D]
     L.se_plan_set_shape.restype = INT
     L.se_plan_set_shape.argtypes = [P, D]
+    L.se_plan_set_tuning.restype = INT
+    L.se_plan_set_tuning.argtypes = [P, INT, INT]
     L.se_plan_set_flags.restype = INT
     L.se_plan_set_flags.argtypes = [P, U]
     L.far_mobility_apply.restype = INT
@@ -133,6 +135,9 @@ class SePlan:
     def set_shape(self, m):
         self._check(self._lib.se_plan_set_shape(self._h, float(m)), "se_plan_set_shape")
 
+    def set_tuning(self, spread_segments=0, gather_segments=0):
+        self._check(self._lib.se_plan_set_tuning(self._h, int(spread_segments), int(gather_segments)), "se_plan_set_tuning")
+
     def set_flags(self, flags):
         self._check(self._lib.se_plan_set_flags(self._h, int(flags)), "se_plan_set_flags")
 
@@ -180,9 +185,10 @@ class SePlan:
         return int(self._lib.se_plan_workspace_bytes(self._h))
 
     def constants(self):
-        out = np.zeros(6)
+        out = np.zeros(7)
         self._check(self._lib.se_plan_get_constants(self._h, out.ctypes.data), "se_plan_get_constants")
-        return dict(Delta=out[0], eta_se=out[1], alpha=out[2], m=out[3], real_cells=int(out[4]), spread_segments=int(out[5]))
+        return dict(Delta=out[0], eta_se=out[1], alpha=out[2], m=out[3], real_cells=int(out[4]), spread_segments=int(out[5]),
+                    gather_segments=int(out[6]))
 
     def destroy(self):
         if getattr(self, "_h", None) is not None and self._h:

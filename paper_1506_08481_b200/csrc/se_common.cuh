@@ -32,6 +32,7 @@ struct SeConst {
 //   [9..11] F  [12..14] T  [15..20] S (xx,xy,xz,yy,yz,zz)
 //   [21] cF = a^2/6  [22] cS = a^2/10  [23] radius a
 //   [24..24+P) gx * (al/pi)^{3/2}   [24+P..24+2P) gy   [24+2P..24+3P) gz     per-axis Gaussians
+//   [24+3P..24+6P)  gx dx, gx dx^2, gx dx^3 with dx_k = d0x + k Delta     x-moment tables (P each)
 #define REC_D0 2
 #define REC_POLY 5
 #define REC_F 9

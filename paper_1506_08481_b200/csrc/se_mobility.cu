@@ -34,6 +34,7 @@ struct se_plan {
     int *d_key_s, *d_rank_s, *d_cnt_s, *d_start_s;
     int *d_bsum;
     int ncell_r, ncell_s;
+    int gseg, gseg_len;            // gather sweep segments (spreading's are in c.nseg, c.seg_len)
     double4 *d_rs_pos;
     double *d_rs_mom;
     int *d_rs_orig;
@@ -41,7 +42,8 @@ struct se_plan {
     double *d_real;                // [6][M^3]; the first three double as the spread grids H
     double2 *d_Hk;                 // [3][M][M][M/2+1]
     double2 *d_Gk;                 // [6][M][M][M/2+1]
-    double *d_out_real, *d_out_wave;      // [N][11] in caller order
+    double *d_out_real;            // [N][11] real-space part in caller order
+    double *d_moments;             // [N][24] gathered wave-space sums in caller order
     // host-API staging
     double *d_io;                  // pos3 F3 T3 S5 U3 W3 E5 = 25 N doubles
     cufftHandle fft_fwd, fft_inv;
@@ -108,6 +110,31 @@ static void derive_constants(se_plan *p)
     c.twopiL = 2.0 * M_PI / c.L;
 }
 
+// Sweep segments along x.  Spreading re-processes the particles of the P-1 planes before a segment, the
+// gather re-reads P-1 planes per segment, so segments are long; they exist only to fill the machine:
+// aim at >= 148 SMs x 16 resident warps, segments no shorter than 32 planes.
+static void choose_segments(se_plan *p, int spread_segments, int gather_segments)
+{
+    SeConst &c = p->c;
+    const int npatch = c.NBY * c.NBZ, M = c.M;
+    const int maxseg = M / 32 > 1 ? M / 32 : 1;
+    auto pick = [&](int want, int warps_per_seg) {
+        int nseg = want > 0 ? want : (148 * 16 + warps_per_seg - 1) / warps_per_seg;
+        if (nseg > maxseg && want <= 0) nseg = maxseg;
+        if (nseg > M) nseg = M;
+        if (nseg < 1) nseg = 1;
+        return nseg;
+    };
+    int ns = pick(spread_segments, npatch);
+    c.seg_len = (M + ns - 1) / ns;
+    c.nseg = (M + c.seg_len - 1) / c.seg_len;
+    int ng = pick(gather_segments, 2 * npatch);
+    p->gseg_len = (M + ng - 1) / ng;
+    p->gseg = (M + p->gseg_len - 1) / p->gseg_len;
+}
+
+static cudaError_t dispatch_prepare(int P, size_t smem);
+
 extern "C" const char *se_version(void) { return "se_mobility 0.1 (sm_100a)"; }
 
 extern "C" const char *se_last_error(const se_plan *plan) { return plan ? plan->err : "null plan"; }
@@ -121,7 +148,7 @@ extern "C" se_status se_plan_destroy(se_plan *p)
     cudaFree(p->d_bsum);
     cudaFree(p->d_rs_pos); cudaFree(p->d_rs_mom); cudaFree(p->d_rs_orig); cudaFree(p->d_recs);
     cudaFree(p->d_real); cudaFree(p->d_Hk); cudaFree(p->d_Gk);
-    cudaFree(p->d_out_real); cudaFree(p->d_out_wave); cudaFree(p->d_io);
+    cudaFree(p->d_out_real); cudaFree(p->d_moments); cudaFree(p->d_io);
     if (p->have_fwd) cufftDestroy(p->fft_fwd);
     if (p->have_inv) cufftDestroy(p->fft_inv);
     if (p->have_events) for (int k = 0; k <= SE_NUM_STAGES; ++k) cudaEventDestroy(p->ev[k]);
@@ -160,17 +187,8 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
     c.NBY = (M + SE_TILE_Y - 1) / SE_TILE_Y;
     c.NBZ = (M + SE_TILE_Z - 1) / SE_TILE_Z;
     p->ncell_s = M * c.NBY * c.NBZ;
-    c.rec_stride = (SE_REC_HDR + 3 * P + 1) & ~1;
-    // sweep segments: enough warps to fill 148 SMs several times, segments no shorter than 32 planes
-    {
-        const int npatch = c.NBY * c.NBZ;
-        int nseg = (148 * 48 + npatch - 1) / npatch;
-        const int maxseg = M / 32 > 1 ? M / 32 : 1;
-        if (nseg > maxseg) nseg = maxseg;
-        if (nseg < 1) nseg = 1;
-        c.seg_len = (M + nseg - 1) / nseg;
-        c.nseg = (M + c.seg_len - 1) / c.seg_len;
-    }
+    c.rec_stride = (SE_REC_HDR + 6 * P + 1) & ~1;
+    choose_segments(p, 0, 0);
 
     se_status st = SE_OK;
     const size_t G = (size_t)M * M * M, Gc = (size_t)M * M * (M / 2 + 1);
@@ -183,13 +201,13 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
     ALLOC(p->d_rs_pos, N); ALLOC(p->d_rs_mom, 12 * (size_t)N); ALLOC(p->d_rs_orig, N);
     ALLOC(p->d_recs, (size_t)N * c.rec_stride);
     ALLOC(p->d_real, 6 * G); ALLOC(p->d_Hk, 3 * Gc); ALLOC(p->d_Gk, 6 * Gc);
-    ALLOC(p->d_out_real, 11 * (size_t)N); ALLOC(p->d_out_wave, 11 * (size_t)N);
+    ALLOC(p->d_out_real, 11 * (size_t)N); ALLOC(p->d_moments, GATHER_SUMS * (size_t)N);
     ALLOC(p->d_io, 25 * (size_t)N);
 #undef ALLOC
     if (st != SE_OK) { se_plan_destroy(p); return st; }
     if (cudaMemcpy(p->d_radii, radii, sizeof(double) * (size_t)N, cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMemset(p->d_out_real, 0, sizeof(double) * 11 * (size_t)N) != cudaSuccess ||
-        cudaMemset(p->d_out_wave, 0, sizeof(double) * 11 * (size_t)N) != cudaSuccess) {
+        cudaMemset(p->d_moments, 0, sizeof(double) * GATHER_SUMS * (size_t)N) != cudaSuccess) {
         se_plan_destroy(p);
         return SE_ERR_CUDA;
     }
@@ -207,6 +225,7 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
     for (int k = 0; k <= SE_NUM_STAGES; ++k)
         if (cudaEventCreate(&p->ev[k]) != cudaSuccess) { p->have_events = (k > 0); se_plan_destroy(p); return SE_ERR_CUDA; }
     p->have_events = true;
+    if (dispatch_prepare(P, sweep_smem_bytes(c.rec_stride)) != cudaSuccess) { cudaGetLastError(); se_plan_destroy(p); return SE_ERR_CUDA; }
     *out = p;
     return SE_OK;
 }
@@ -216,6 +235,13 @@ extern "C" se_status se_plan_set_shape(se_plan *p, double m)
     if (!p || !(m > 0.0)) return SE_ERR_INVALID_ARG;
     p->m = m;
     derive_constants(p);
+    return SE_OK;
+}
+
+extern "C" se_status se_plan_set_tuning(se_plan *p, int spread_segments, int gather_segments)
+{
+    if (!p || spread_segments < 0 || gather_segments < 0) return SE_ERR_INVALID_ARG;
+    choose_segments(p, spread_segments, gather_segments);
     return SE_OK;
 }
 
@@ -240,7 +266,7 @@ extern "C" se_status se_plan_get_constants(const se_plan *p, double *out)
 {
     if (!p || !out) return SE_ERR_INVALID_ARG;
     out[0] = p->c.Delta; out[1] = p->c.eta_se; out[2] = p->c.alpha; out[3] = p->m;
-    out[4] = (double)p->c.ncr; out[5] = (double)p->c.nseg;
+    out[4] = (double)p->c.ncr; out[5] = (double)p->c.nseg; out[6] = (double)p->gseg;
     return SE_OK;
 }
 
@@ -260,16 +286,26 @@ static void launch_spread(se_plan *p, cudaStream_t s)
 {
     const SeConst &c = p->c;
     const long long warps = (long long)c.NBY * c.NBZ * c.nseg;
-    const int blocks = (int)((warps + SPREAD_WARPS - 1) / SPREAD_WARPS);
-    k_spread<P><<<blocks, SPREAD_WARPS * 32, 0, s>>>(c, p->d_recs, p->d_start_s, p->d_real);
+    const int blocks = (int)((warps + SWEEP_WARPS - 1) / SWEEP_WARPS);
+    k_spread<P><<<blocks, SWEEP_WARPS * 32, sweep_smem_bytes(c.rec_stride), s>>>(c, p->d_recs, p->d_start_s, p->d_real);
 }
 
 template <int P>
 static void launch_gather(se_plan *p, cudaStream_t s)
 {
-    const SeConst &c = p->c;
-    const int blocks = (c.N + GATHER_WARPS - 1) / GATHER_WARPS;
-    k_gather<P><<<blocks, GATHER_WARPS * 32, 0, s>>>(c, p->d_recs, p->d_real, p->d_out_wave);
+    SeConst c = p->c;
+    c.nseg = p->gseg; c.seg_len = p->gseg_len;
+    const long long warps = (long long)c.NBY * c.NBZ * c.nseg * 2;
+    const int blocks = (int)((warps + SWEEP_WARPS - 1) / SWEEP_WARPS);
+    k_gather<P><<<blocks, SWEEP_WARPS * 32, sweep_smem_bytes(c.rec_stride), s>>>(c, p->d_recs, p->d_start_s, p->d_real, p->d_moments);
+}
+
+template <int P>
+static cudaError_t prepare_sweeps(size_t smem)
+{
+    cudaError_t e = cudaFuncSetAttribute(k_spread<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gather<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    return e;
 }
 
 #define FOR_EACH_P(X) \
@@ -282,6 +318,16 @@ static void dispatch_spread(se_plan *p, cudaStream_t s)
         FOR_EACH_P(X)
 #undef X
     }
+}
+
+static cudaError_t dispatch_prepare(int P, size_t smem)
+{
+    switch (P) {
+#define X(v) case v: return prepare_sweeps<v>(smem);
+        FOR_EACH_P(X)
+#undef X
+    }
+    return cudaErrorInvalidValue;
 }
 
 static void dispatch_gather(se_plan *p, cudaStream_t s)
@@ -328,7 +374,7 @@ extern "C" se_status far_mobility_apply(se_plan *p, const double *pos, const dou
     MARK();
     // ---- a2: real-space pair sum ----
     if (do_real) {
-        k_real<<<(c.N + REAL_WARPS - 1) / REAL_WARPS, REAL_WARPS * 32, 0, s>>>(c, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig,
+        k_real<<<c.ncr > 1 ? p->ncell_r : (c.N + 31) / 32, REAL_WARPS * 32, 0, s>>>(c, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig,
                                                                                 p->d_start_r, p->d_out_real);
         p->last_launches += 1;
         CUDA_TRY(p, cudaGetLastError());
@@ -360,6 +406,7 @@ extern "C" se_status far_mobility_apply(se_plan *p, const double *pos, const dou
     }
     MARK();
     if (on(SE_STAGE_GATHER)) {
+        CUDA_TRY(p, cudaMemsetAsync(p->d_moments, 0, sizeof(double) * GATHER_SUMS * (size_t)c.N, s));
         dispatch_gather(p, s);
         p->last_launches += 1;
         CUDA_TRY(p, cudaGetLastError());
@@ -367,7 +414,7 @@ extern "C" se_status far_mobility_apply(se_plan *p, const double *pos, const dou
     }
     MARK();
     // ---- a8: epilogue ----
-    k_epilogue<<<nbN, TB, 0, s>>>(c, fl | (wave_done ? 0u : SE_SKIP_WAVE), p->d_radii, F, T, S, p->d_out_real, p->d_out_wave, U, Omega, E);
+    k_epilogue<<<nbN, TB, 0, s>>>(c, fl | (wave_done ? 0u : SE_SKIP_WAVE), p->d_radii, F, T, S, p->d_out_real, p->d_moments, U, Omega, E);
     p->last_launches += 1;
     CUDA_TRY(p, cudaGetLastError());
     MARK();

@@ -103,56 +103,94 @@ __device__ __forceinline__ void pair_real(const SeConst &c, double x, double y, 
     acc[10] += y * w2 + z * w1 + a4 * Syz + beta * y * z;
 }
 
-// One warp per target particle i (cell order).  Lanes scan the particles of the 27 neighbour cells
-// (or all particles when the box holds fewer than 3 cells per axis), hits are compacted through a
-// per-warp shared-memory queue so that the expensive pair evaluation always runs on full warps.
+// One CTA per real-space cell (or, when the box holds fewer than 3 cells per axis, per slice of all
+// particles).  The positions and radii of the particles of the 27 neighbour cells are staged once in
+// shared memory (chunks of REAL_STAGE), then each warp takes target particles of the cell in turn: its lanes
+// scan the staged candidates, hits are compacted through a per-warp shared-memory queue so that the expensive
+// pair evaluation always runs on full warps, and the 11 sums are reduced over the warp at the end.
+// Minimum image as in the oracle, x = d - L rint(d/L), with d/L formed as d * (1/L).
+#define REAL_STAGE 1024
+
 __global__ void __launch_bounds__(REAL_WARPS * 32) k_real(SeConst c, const double4 *__restrict__ rs_pos,
                                                           const double *__restrict__ rs_mom, const int *__restrict__ rs_orig,
                                                           const int *__restrict__ start_r, double *__restrict__ out_real)
 {
+    __shared__ double4 cand[REAL_STAGE];               // (x, y, z, a) of staged candidates
+    __shared__ int cand_j[REAL_STAGE];                 // their index in cell order
     __shared__ double4 qd[REAL_WARPS][REAL_QCAP];      // (dx, dy, dz, a_j)
     __shared__ int qj[REAL_WARPS][REAL_QCAP];
-    const int wl = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int i = blockIdx.x * REAL_WARPS + wl;
-    if (i >= c.N) return;
-    const double4 pi = rs_pos[i];
-    const double cFi = pi.w * pi.w * (1.0 / 6.0), cSi = pi.w * pi.w * 0.1;
-    double acc[11];
-#pragma unroll
-    for (int k = 0; k < 11; ++k) acc[k] = 0.0;
-    int qn = 0;
-
+    __shared__ int seg_s[27], seg_o[28];               // neighbour cell ranges: first particle, exclusive offsets
+    const int wl = threadIdx.x >> 5, lane = threadIdx.x & 31, tid = threadIdx.x;
     const int nc = c.ncr;
-    int ci[3] = { 0, 0, 0 };
+    const double invL = 1.0 / c.L;
+
+    // targets of this CTA and its candidate segments
+    int t0, t1, nsegs;
     if (nc > 1) {
-        ci[0] = se_mod((int)floor(pi.x / c.hr), nc);
-        ci[1] = se_mod((int)floor(pi.y / c.hr), nc);
-        ci[2] = se_mod((int)floor(pi.z / c.hr), nc);
+        const int cell = blockIdx.x;
+        t0 = start_r[cell]; t1 = start_r[cell + 1];
+        if (t0 == t1) return;
+        nsegs = 27;
+        if (tid < 27) {
+            const int cz = cell % nc, cy = (cell / nc) % nc, cx = cell / (nc * nc);
+            const int nx = se_mod(cx + tid / 9 - 1, nc), ny = se_mod(cy + (tid / 3) % 3 - 1, nc), nz = se_mod(cz + tid % 3 - 1, nc);
+            const int nb = (nx * nc + ny) * nc + nz;
+            seg_s[tid] = start_r[nb];
+            seg_o[tid + 1] = start_r[nb + 1] - start_r[nb];
+        }
+    } else {
+        const int per = (c.N + gridDim.x - 1) / gridDim.x;
+        t0 = blockIdx.x * per; t1 = min(t0 + per, c.N);
+        if (t0 >= t1) return;
+        nsegs = 1;
+        if (tid == 0) { seg_s[0] = 0; seg_o[1] = c.N; }
     }
-    const int nrow = nc > 1 ? 9 : 1;
-    for (int row = 0; row < nrow; ++row) {
-        // neighbour cells (cx+dx, cy+dy, cz-1..cz+1): contiguous in memory except across the z wrap
-        int s0, e0, s1 = 0, e1 = 0;
-        if (nc > 1) {
-            const int cx = se_mod(ci[0] + row / 3 - 1, nc), cy = se_mod(ci[1] + row % 3 - 1, nc);
-            const int base = (cx * nc + cy) * nc;
-            const int zlo = ci[2] - 1, zhi = ci[2] + 1;
-            if (zlo < 0) { s0 = start_r[base]; e0 = start_r[base + zhi + 1]; s1 = start_r[base + nc - 1]; e1 = start_r[base + nc]; }
-            else if (zhi >= nc) { s0 = start_r[base + zlo]; e0 = start_r[base + nc]; s1 = start_r[base]; e1 = start_r[base + 1]; }
-            else { s0 = start_r[base + zlo]; e0 = start_r[base + zhi + 1]; }
-        } else { s0 = 0; e0 = c.N; }
-        for (int part = 0; part < 2; ++part) {
-            const int s = part ? s1 : s0, e = part ? e1 : e0;
-            for (int jb = s; jb < e; jb += 32) {
-                const int j = jb + lane;
+    __syncthreads();
+    if (tid == 0) {
+        int run = 0;
+        seg_o[0] = 0;
+        for (int k = 0; k < nsegs; ++k) { const int n = seg_o[k + 1]; seg_o[k + 1] = run + n; run += n; }
+        // now seg_o[k] = exclusive offset of segment k, seg_o[nsegs] = total
+    }
+    __syncthreads();
+    const int ncand = seg_o[nsegs];
+    const int ntgt = t1 - t0;
+    const int rounds = (ntgt + REAL_WARPS - 1) / REAL_WARPS;
+
+    for (int base = 0; base < ncand; base += REAL_STAGE) {
+        const int nst = min(REAL_STAGE, ncand - base);
+        __syncthreads();                               // previous chunk fully consumed
+        for (int q = tid; q < nst; q += REAL_WARPS * 32) {
+            const int f = base + q;
+            int k = 0;
+            while (k + 1 < nsegs && seg_o[k + 1] <= f) ++k;
+            const int j = seg_s[k] + (f - seg_o[k]);
+            cand[q] = rs_pos[j];
+            cand_j[q] = j;
+        }
+        __syncthreads();
+
+        for (int rd = 0; rd < rounds; ++rd) {
+            const int i = t0 + rd * REAL_WARPS + wl;
+            if (i >= t1) break;
+            const double4 pi = rs_pos[i];
+            const double cFi = pi.w * pi.w * (1.0 / 6.0), cSi = pi.w * pi.w * 0.1;
+            double acc[11];
+#pragma unroll
+            for (int k = 0; k < 11; ++k) acc[k] = 0.0;
+            int qn = 0;
+            for (int qb = 0; qb < nst; qb += 32) {
+                const int q = qb + lane;
                 bool hit = false;
                 double dx = 0, dy = 0, dz = 0, aj = 0;
-                if (j < e && j != i) {
-                    const double4 pj = rs_pos[j];
+                int j = -1;
+                if (q < nst) {
+                    const double4 pj = cand[q];
+                    j = cand_j[q];
                     dx = pi.x - pj.x; dy = pi.y - pj.y; dz = pi.z - pj.z;
-                    dx -= c.L * rint(dx / c.L); dy -= c.L * rint(dy / c.L); dz -= c.L * rint(dz / c.L);
+                    dx -= c.L * rint(dx * invL); dy -= c.L * rint(dy * invL); dz -= c.L * rint(dz * invL);
                     const double r2 = dx * dx + dy * dy + dz * dz;
-                    hit = (r2 < c.rc2) && (r2 > 0.0);
+                    hit = (j != i) && (r2 < c.rc2) && (r2 > 0.0);
                     aj = pj.w;
                 }
                 const unsigned mask = __ballot_sync(0xffffffffu, hit);
@@ -171,22 +209,29 @@ __global__ void __launch_bounds__(REAL_WARPS * 32) k_real(SeConst c, const doubl
                     __syncwarp();
                 }
             }
+            if (lane < qn) {
+                const double4 d = qd[wl][lane];
+                pair_real(c, d.x, d.y, d.z, d.x * d.x + d.y * d.y + d.z * d.z, cFi, cSi, d.w, rs_mom + 12 * (size_t)qj[wl][lane], acc);
+            }
+            __syncwarp();
+#pragma unroll
+            for (int k = 0; k < 11; ++k) {
+                double v = acc[k];
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                acc[k] = v;
+            }
+            if (lane == 0) {
+                double *o = out_real + 11 * (size_t)rs_orig[i];
+                if (base == 0) {
+#pragma unroll
+                    for (int k = 0; k < 11; ++k) o[k] = c.k0 * acc[k];
+                } else {
+#pragma unroll
+                    for (int k = 0; k < 11; ++k) o[k] += c.k0 * acc[k];
+                }
+            }
         }
     }
-    if (lane < qn) {
-        const double4 d = qd[wl][lane];
-        pair_real(c, d.x, d.y, d.z, d.x * d.x + d.y * d.y + d.z * d.z, cFi, cSi, d.w, rs_mom + 12 * (size_t)qj[wl][lane], acc);
-    }
-#pragma unroll
-    for (int k = 0; k < 11; ++k) {
-        double v = acc[k];
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-        acc[k] = v;
-    }
-    if (lane == 0) {
-        double *o = out_real + 11 * (size_t)rs_orig[i];
-#pragma unroll
-        for (int k = 0; k < 11; ++k) o[k] = c.k0 * acc[k];
-    }
+    // a cell without any candidate at all cannot occur (it contains its own targets), so every target was written
 }

@@ -141,6 +141,11 @@ __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const doubl
             const double dk = ((double)(n0 + k) - u) * c.Delta;
             const double e = exp(-al * dk * dk);
             g[k] = d == 0 ? c.gnorm * e : e;
+            if (d == 0) {                                   // x-moment tables gx dx^n, n = 1..3
+                double *xm = r + SE_REC_HDR + 3 * c.P;
+                const double g1 = g[k] * dk, g2 = g1 * dk;
+                xm[k] = g1; xm[c.P + k] = g2; xm[2 * c.P + k] = g2 * dk;
+            }
         }
     }
     reinterpret_cast<int2 *>(r)[0] = make_int2(n0w[1], n0w[2]);
