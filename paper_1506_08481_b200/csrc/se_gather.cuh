@@ -2,177 +2,223 @@
 //   U_i  = D^3 sum_n gamma(d) (u~ + cF_i w~)
 //   Om_i = D^3 sum_n al gamma(d) d x u~
 //   E_i  = traceless part of D^3 sum_n al gamma(d) (d q + q d),  q = u~ + cS_i w~,   d = x_n - r_i
-// over the same P^3 support as the spreading.
+// over the same P^3 support as the spreading.  All of it follows from four sums per returned grid g,
+//     A0[g] = sum gamma g,  A1[g] = sum gamma dx g,  Ay[g] = sum gamma dy g,  Az[g] = sum gamma dz g,
+// which this kernel writes to moments[N][24] (caller order); a8 combines them per particle.
 //
-// Design: the mirror of the spreading sweep (se_sweep.cuh).  A thread owns one grid column (y,z) and sweeps
-// along x with a window of P planes of three grids in registers, so every grid value is read from HBM once
-// per segment, in coalesced 64-byte rows.  Two "roles" share the work: role 0 sweeps u~ (grids 0-2), role 1
-// sweeps w~ = lap u~ (grids 3-5).  For every particle whose support starts at the window's first plane and
-// covers the column, the thread reduces along x,
-//     m0[g] = sum_k gx(k) g(p+k),   m1[g] = sum_k gx(k) dx_k g(p+k),
-// and weights them with the (y,z) Gaussian: the twelve sums  gyz {m0, m1, dy m0, dz m0}[g]  are all that
-// U, Omega and E need.  They are reduced over the warp (reduce-scatter: 18 shuffles for 12 values) and added
-// with one fp64 reduction per value into moments[N][24] (caller order); a8 combines them per particle.
+// Design ("plane ring"): a CTA owns one returned grid, one (y,z) tile of TY x TZ support origins and one
+// segment of x.  It streams the planes of its haloed tile, (TY+P-1) x (TZ+P-1) columns, through a ring of R
+// planes in shared memory: two producer warps copy it with 16-byte cp.async (completion counted by the slot's
+// mbarrier), R-P planes ahead of the consumers, so every grid value crosses L2->SM once per tile and is then
+// read from shared memory.  The particles whose support starts in the tile are sorted by starting plane (a1,
+// second counting sort); the eight consumer warps take them round-robin, ONE WARP PER PARTICLE: the lanes
+// own the P^2 columns of the footprint (all lanes busy), reduce along x in registers,
+//     m0 = sum_k gx(k) g(x0+k),   m1 = sum_k gx(k) dx_k g(x0+k),
+// weight with the (y,z) Gaussian and reduce over the warp once per particle.  Every (particle, grid) pair
+// is produced by exactly one warp in a fixed order: no atomics, no zero-fill, bitwise reproducible.
+// Rows are padded to WZ = P (mod 16) doubles so that the footprint columns of a half-warp fall in
+// distinct shared-memory banks.  Planes are released through per-slot "empty" mbarriers (one arrival per
+// consumer warp), so warps run up to R-P planes apart without CTA-wide barriers.
 #pragma once
 #include "se_sweep.cuh"
+#include "se_sort.cuh"
 
-#define GATHER_SUMS 24             // per particle: role 0 (u~) sums 0..11, role 1 (w~) sums 12..23
+#define GATHER_SUMS 24             // per particle: slot (g/3)*12 + kind*3 + g%3, kind = 0 (1), 1 (dx), 2 (dy), 3 (dz)
+#define GR_WARPS 8                 // consumer warps
+// Two CTAs per SM hide each other's pipeline bubbles; supports up to GR_P2MAX keep the register budget for it.
+#define GR_P2MAX 14
+#define GR_PROD 2                  // producer warps (GR_WARPS, GR_WARPS + 1)
 
-// Warp reduce-scatter of v[0..11]: returns in every lane the total of value (lane>>4)*6 + ((lane>>3)&1)*3 + t
-// for t = 0,1,2 in out[t].
-__device__ __forceinline__ void warp_reduce12(const double (&v)[12], int lane, double (&out)[3])
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
 {
-    const bool hi16 = (lane & 16) != 0, hi8 = (lane & 8) != 0;
-    double a[6];
-#pragma unroll
-    for (int i = 0; i < 6; ++i) {
-        const double keep = hi16 ? v[i + 6] : v[i], send = hi16 ? v[i] : v[i + 6];
-        a[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
-    }
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-        const double keep = hi8 ? a[i + 3] : a[i], send = hi8 ? a[i] : a[i + 3];
-        double t = keep + __shfl_xor_sync(0xffffffffu, send, 8);
-        t += __shfl_xor_sync(0xffffffffu, t, 4);
-        t += __shfl_xor_sync(0xffffffffu, t, 2);
-        t += __shfl_xor_sync(0xffffffffu, t, 1);
-        out[i] = t;
-    }
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void *src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+// Arrive on `bar` once all cp.async of this thread issued so far have landed (counted in the barrier's init count).
+__device__ __forceinline__ void cp_async_arrive(uint32_t bar)
+{
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
 }
 
 template <int P>
-__device__ __forceinline__ void gather_hit(const SeConst &c, const double *__restrict__ rec, int y, int z, bool active,
-                                           const double (&win)[P][3], int role, int lane, double *__restrict__ moments)
+__global__ void __launch_bounds__((GR_WARPS + GR_PROD) * 32, (P <= GR_P2MAX ? 2 : 1))
+k_gather(SeConst c, GatherGeom g, const double *__restrict__ recs, const int *__restrict__ gperm,
+         const int *__restrict__ start_g, const double *__restrict__ Gr, int ngrids, double *__restrict__ moments)
 {
-    const int M = c.M;
-    const int2 yz = *reinterpret_cast<const int2 *>(rec);
-    int ry = y - yz.x, rz = z - yz.y;
-    ry += ry < 0 ? M : 0;
-    rz += rz < 0 ? M : 0;
-    const bool hit = active && ry < P && rz < P;
-    if (!__any_sync(0xffffffffu, hit)) return;
-    double v[12];
-#pragma unroll
-    for (int i = 0; i < 12; ++i) v[i] = 0.0;
-    if (hit) {
-        const double Delta = c.Delta;
-        // two partial sums per moment (even / odd planes) keep the FP64 pipe busy with few resident warps
-        double m0[2][3] = { { 0.0, 0.0, 0.0 }, { 0.0, 0.0, 0.0 } }, m1[2][3] = { { 0.0, 0.0, 0.0 }, { 0.0, 0.0, 0.0 } };
-        const double *__restrict__ X0 = rec + SE_REC_HDR, *__restrict__ X1 = rec + SE_REC_HDR + 3 * P;
-#pragma unroll
-        for (int k = 0; k < P; ++k) {
-            const double gx = X0[k], gxd = X1[k];
-#pragma unroll
-            for (int g = 0; g < 3; ++g) {
-                m0[k & 1][g] = fma(gx, win[k][g], m0[k & 1][g]);
-                m1[k & 1][g] = fma(gxd, win[k][g], m1[k & 1][g]);
-            }
-        }
-        const double dy = rec[REC_D0 + 1] + ry * Delta, dz = rec[REC_D0 + 2] + rz * Delta;
-        const double gyz = rec[SE_REC_HDR + P + ry] * rec[SE_REC_HDR + 2 * P + rz];
-        const double wy = gyz * dy, wz = gyz * dz;
-#pragma unroll
-        for (int g = 0; g < 3; ++g) {
-            const double s0 = m0[0][g] + m0[1][g], s1 = m1[0][g] + m1[1][g];
-            v[g] = gyz * s0;
-            v[3 + g] = gyz * s1;
-            v[6 + g] = wy * s0;
-            v[9 + g] = wz * s0;
-        }
-    }
-    double tot[3];
-    warp_reduce12(v, lane, tot);
-    const int orig = reinterpret_cast<const int2 *>(rec)[1].y;
-    const int t = lane & 7;
-    if (t < 3) {
-        const int q = (lane >> 4) * 6 + ((lane >> 3) & 1) * 3;
-        atomicAdd(moments + (size_t)orig * GATHER_SUMS + role * 12 + q + t, t == 0 ? tot[0] : (t == 1 ? tot[1] : tot[2]));
-    }
-}
+    extern __shared__ __align__(16) unsigned char gsm[];
+    constexpr int PP = P * P, NI = (PP + 31) / 32;
+    constexpr int NREC = SE_REC_HDR + 4 * P, NR = (NREC + 31) / 32;      // record prefix the gather needs
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int M = c.M, stride = c.rec_stride, R = g.R;
+    const int ntile = g.NTY * g.NTZ;
+    int item = blockIdx.x;
+    const int tile = item % ntile; item /= ntile;
+    const int grid = item % ngrids, seg = item / ngrids;
+    const int seg_start = seg * g.seg_len, seg_end = min(seg_start + g.seg_len, M);
+    const int i0 = start_g[tile * M + seg_start], i1 = start_g[tile * M + seg_end];
+    if (i0 == i1) return;                                              // no support starts here
+    const int ty = tile / g.NTZ, tz = tile - ty * g.NTZ;
+    const int Y0 = ty * g.TY, Z0 = tz * g.TZ;
+    const int nplanes = seg_end - seg_start + P - 1;
+    const int plane_d = g.WY * g.WZ;                                   // doubles per ring slot
+    const int cw = g.WZL >> 1, nch = g.WY * cw;                        // 16-byte chunks per row, per plane
 
-// Grid: nseg * 2 roles * npatch warps.  Segment s handles the particles whose support starts in planes
-// [s*seg_len, (s+1)*seg_len) and reads planes up to P-1 beyond.
-template <int P>
-__global__ void __launch_bounds__(SWEEP_WARPS * 32, SWEEP_MIN_BLOCKS) k_gather(SeConst c, const double *__restrict__ recs,
-                                                              const int *__restrict__ start_s, const double *__restrict__ Gr,
-                                                              double *__restrict__ moments)
-{
-    extern __shared__ __align__(16) unsigned char sweep_smem[];
-    const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
-    const int wid = blockIdx.x * SWEEP_WARPS + wl;
-    const int npatch = c.NBY * c.NBZ;
-    const int sr = wid / npatch, patch = wid - sr * npatch;
-    if (sr >= 2 * c.nseg) return;
-    const int seg = sr >> 1, role = sr & 1;
-    const int M = c.M, stride = c.rec_stride;
-    const int py = patch / c.NBZ, pz = patch - py * c.NBZ;
-    const int Y0 = py * SE_TILE_Y, Z0 = pz * SE_TILE_Z;
-    const int y = Y0 + (lane >> 3), z = Z0 + (lane & 7);
-    const bool active = (y < M) && (z < M);
-
-    double *slot0 = reinterpret_cast<double *>(sweep_smem) + (size_t)wl * 2 * SWEEP_CAP * stride;
-    double *slot1 = slot0 + (size_t)SWEEP_CAP * stride;
-    const uint32_t bar0 = smem_u32(sweep_smem + (size_t)SWEEP_WARPS * 2 * SWEEP_CAP * stride * 8 + wl * 16), bar1 = bar0 + 8;
-    if (lane == 0) {
-        mbar_init(bar0, 1);
-        mbar_init(bar1, 1);
+    double *ring = reinterpret_cast<double *>(gsm);
+    double *rslots = ring + (size_t)R * plane_d;                       // per consumer warp: one record prefix
+    int2 *table = reinterpret_cast<int2 *>(rslots + GR_WARPS * NR * 32);   // per chunk: (offset in a grid plane, offset in a slot)
+    const uint32_t bars = smem_u32(table + nch);
+    auto full_bar = [&](int sl) { return bars + 16u * (uint32_t)sl; };
+    auto empty_bar = [&](int sl) { return bars + 16u * (uint32_t)sl + 8u; };
+    if (threadIdx.x == 0) {
+        for (int sl = 0; sl < R; ++sl) { mbar_init(full_bar(sl), GR_PROD * 32); mbar_init(empty_bar(sl), GR_WARPS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    __syncwarp();
-
-    const SweepRanges rg = sweep_ranges<P>(c, Y0, Z0, lane);
-    const int seg_start = seg * c.seg_len, seg_end = min(seg_start + c.seg_len, M);
-    const size_t G = (size_t)M * M * M, MM = (size_t)M * M;
-    const double *__restrict__ g0 = Gr + (size_t)(3 * role) * G + (active ? (size_t)y * M + z : 0);
-    auto plane = [&](int q) { return (size_t)(q >= M ? q - M : q) * MM; };
-
-    int p = seg_start;
-    SweepList cur = sweep_scan(sweep_load(rg, start_s, p * npatch, lane), lane);
-    sweep_stage(cur, recs, stride, smem_u32(slot0), bar0, lane);
-    int2 raw = sweep_load(rg, start_s, min(p + 1, seg_end - 1) * npatch, lane);
-
-    double win[P][3], nx[3];
-#pragma unroll
-    for (int k = 0; k < P - 1; ++k) {
-        const size_t o = plane(p + k);
-#pragma unroll
-        for (int g = 0; g < 3; ++g) win[k][g] = active ? g0[g * G + o] : 0.0;
+    for (int ch = threadIdx.x; ch < nch; ch += blockDim.x) {            // periodic wrap along y and z, once per CTA
+        const int r = ch / cw, col = ch - r * cw;
+        table[ch] = make_int2(((Y0 + r) % M) * M + (Z0 + 2 * col) % M, r * g.WZ + 2 * col);
     }
-    {
-        const size_t o = plane(p + P - 1);
-#pragma unroll
-        for (int g = 0; g < 3; ++g) nx[g] = active ? g0[g * G + o] : 0.0;
-    }
-    unsigned parity = 0;
-    for (int buf = 0; p < seg_end; ++p, buf ^= 1) {
-#pragma unroll
-        for (int g = 0; g < 3; ++g) win[P - 1][g] = nx[g];
-        SweepList nxt;
-        nxt.js = 0; nxt.cnt = 0; nxt.off = 0; nxt.n = 0;
-        if (p + 1 < seg_end) {
-            nxt = sweep_scan(raw, lane);
-            sweep_stage(nxt, recs, stride, smem_u32(buf ? slot0 : slot1), buf ? bar0 : bar1, lane);
-            raw = sweep_load(rg, start_s, min(p + 2, seg_end - 1) * npatch, lane);
-            const size_t o = plane(p + P);                    // last plane of the next window
-#pragma unroll
-            for (int g = 0; g < 3; ++g) nx[g] = active ? g0[g * G + o] : 0.0;
-        }
-        if (cur.n > 0) {
-            mbar_wait(buf ? bar1 : bar0, (parity >> buf) & 1u);
-            parity ^= 1u << buf;
-            const double *__restrict__ sl = buf ? slot1 : slot0;
-            const int ns = min(cur.n, SWEEP_CAP);
-            for (int ci = 0; ci < ns; ++ci) gather_hit<P>(c, sl + (size_t)ci * stride, y, z, active, win, role, lane, moments);
-            for (int ci = SWEEP_CAP; ci < cur.n; ++ci) {
-                const int j = sweep_overflow_index(cur, ci);
-                gather_hit<P>(c, recs + (size_t)j * stride, y, z, active, win, role, lane, moments);
+    __syncthreads();
+
+    if (w >= GR_WARPS) {
+        // ---- producers: plane j of the segment goes to slot j % R once every consumer released plane j - R.
+        // 16-byte cp.async per chunk (rows are too short for bulk copies to pay); completion is counted by the
+        // slot's "full" mbarrier, one deferred arrival per producer lane.
+        const double *__restrict__ G0 = Gr + (size_t)grid * M * M * M;
+        const int pl = (w - GR_WARPS) * 32 + lane;
+        const uint32_t ring_a = smem_u32(ring);
+        int sl = 0;
+        uint32_t par = 1;                                              // passes at once in round 0
+        int x = seg_start;
+        for (int j = 0; j < nplanes; ++j) {
+            mbar_wait(empty_bar(sl), par);
+            const double *__restrict__ src = G0 + (size_t)x * M * M;
+            const uint32_t dst = ring_a + 8u * (uint32_t)(sl * plane_d);
+            for (int ch = pl; ch < nch; ch += GR_PROD * 32) {
+                const int2 e = table[ch];
+                cp_async16(dst + 8u * (uint32_t)e.y, src + e.x);
             }
-            __syncwarp();
+            cp_async_arrive(full_bar(sl));
+            if (++sl == R) { sl = 0; par ^= 1u; }
+            if (++x == M) x = 0;
         }
-#pragma unroll
-        for (int k = 0; k < P - 1; ++k) { win[k][0] = win[k + 1][0]; win[k][1] = win[k + 1][1]; win[k][2] = win[k + 1][2]; }
-        cur = nxt;
+        asm volatile("cp.async.wait_all;" ::: "memory");
+        return;
     }
+
+    // ---- consumers: particle i0 + w, i0 + w + 8, ... (non-decreasing starting plane per warp) ----
+    double *rs = rslots + w * NR * 32;
+    // planes [0, jdone) are known loaded (slot/parity of plane jdone: sdone, pdone); planes [0, jrel) released
+    int jdone = 0, sdone = 0, jrel = 0, srel = 0;
+    uint32_t pdone = 0;
+    double pre[NR];
+    auto fetch = [&](int ii) {
+        const double *__restrict__ rec = recs + (size_t)gperm[ii] * stride;
+#pragma unroll
+        for (int q = 0; q < NR; ++q) pre[q] = (q * 32 + lane < NREC) ? rec[q * 32 + lane] : 0.0;
+    };
+    auto observe_next = [&]() {
+        mbar_wait(full_bar(sdone), pdone);
+        ++jdone;
+        if (++sdone == R) { sdone = 0; pdone ^= 1u; }
+    };
+    // Every consumer observes every phase of every slot, in order, and releases a plane only after having
+    // observed it: the parity waits can then never alias, however far apart the starting planes are.
+    auto release_below = [&](int jto) {
+        while (jrel < jto) {
+            if (jrel == jdone) observe_next();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty_bar(srel));
+            ++jrel;
+            if (++srel == R) srel = 0;
+        }
+    };
+    // lane constants: footprint column lane + 32 q -> (ry, rz), its offset in a slot, its distance from the origin
+    int colof[NI], colry[NI], colrz[NI];
+    bool colok[NI];
+    double coldy[NI], coldz[NI];
+#pragma unroll
+    for (int q = 0; q < NI; ++q) {
+        const int cc = lane + 32 * q;
+        colok[q] = cc < PP;
+        const int cl = min(cc, PP - 1);
+        colry[q] = cl / P; colrz[q] = cl - colry[q] * P;
+        colof[q] = colry[q] * g.WZ + colrz[q];
+        coldy[q] = colry[q] * c.Delta; coldz[q] = colrz[q] * c.Delta;
+    }
+    int i = i0 + w;
+    if (i < i1) fetch(i);
+    for (; i < i1; i += GR_WARPS) {
+        __syncwarp();
+#pragma unroll
+        for (int q = 0; q < NR; ++q) rs[q * 32 + lane] = pre[q];
+        __syncwarp();
+        if (i + GR_WARPS < i1) fetch(i + GR_WARPS);                    // next record in flight during the sums
+        const int2 yz = reinterpret_cast<const int2 *>(rs)[0], xo = reinterpret_cast<const int2 *>(rs)[1];
+        const int j0 = xo.x - seg_start;
+        release_below(j0);                                             // now jrel == j0 and srel == j0 % R
+        while (jdone < j0 + P) observe_next();
+
+        const int cb = (yz.x - Y0) * g.WZ + (yz.y - Z0);
+        double m0[NI], m1[NI];
+#pragma unroll
+        for (int q = 0; q < NI; ++q) { m0[q] = 0.0; m1[q] = 0.0; }
+        int sl = srel;
+        const double *__restrict__ X0 = rs + SE_REC_HDR, *__restrict__ X1 = rs + SE_REC_HDR + 3 * P;
+        double gxr[P], gxdr[P];                                        // x tables: loaded before the sums start
+#pragma unroll
+        for (int k = 0; k < P; ++k) { gxr[k] = X0[k]; gxdr[k] = X1[k]; }
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+            const double *__restrict__ pl = ring + sl * plane_d;
+            const double gx = gxr[k], gxd = gxdr[k];
+#pragma unroll
+            for (int q = 0; q < NI; ++q) {
+                const double v = pl[cb + colof[q]];
+                m0[q] = fma(gx, v, m0[q]);
+                m1[q] = fma(gxd, v, m1[q]);
+            }
+            sl = sl + 1 == R ? 0 : sl + 1;
+        }
+        double s0 = 0.0, s1 = 0.0, sy = 0.0, sz = 0.0;
+        const double d0y = rs[REC_D0 + 1], d0z = rs[REC_D0 + 2];
+        const double *__restrict__ GY = rs + SE_REC_HDR + P, *__restrict__ GZ = rs + SE_REC_HDR + 2 * P;
+#pragma unroll
+        for (int q = 0; q < NI; ++q) {
+            const double gyz = colok[q] ? GY[colry[q]] * GZ[colrz[q]] : 0.0;
+            const double a0 = gyz * m0[q];
+            s0 += a0;
+            s1 = fma(gyz, m1[q], s1);
+            sy = fma(d0y + coldy[q], a0, sy);
+            sz = fma(d0z + coldz[q], a0, sz);
+        }
+        // reduce-scatter of the four sums: lane bits (16, 8) select the kind: 00 s0, 01 s1, 10 sy, 11 sz
+        {
+            const bool hi = (lane & 16) != 0;
+            const double a = (hi ? sy : s0) + __shfl_xor_sync(0xffffffffu, hi ? s0 : sy, 16);
+            const double b = (hi ? sz : s1) + __shfl_xor_sync(0xffffffffu, hi ? s1 : sz, 16);
+            const bool h8 = (lane & 8) != 0;
+            double t = (h8 ? b : a) + __shfl_xor_sync(0xffffffffu, h8 ? a : b, 8);
+            t += __shfl_xor_sync(0xffffffffu, t, 4);
+            t += __shfl_xor_sync(0xffffffffu, t, 2);
+            t += __shfl_xor_sync(0xffffffffu, t, 1);
+            if ((lane & 7) == 0) {
+                const int kind = ((lane >> 4) << 1) | ((lane >> 3) & 1);
+                moments[(size_t)xo.y * GATHER_SUMS + (grid / 3) * 12 + kind * 3 + (grid % 3)] = t;
+            }
+        }
+    }
+    __syncwarp();
+    release_below(nplanes);
+}
+
+static inline size_t gather_smem_bytes(const GatherGeom &g, int P)
+{
+    const int NR = (SE_REC_HDR + 4 * P + 31) / 32;
+    return (size_t)g.R * g.WY * g.WZ * 8 + (size_t)GR_WARPS * NR * 32 * 8 + (size_t)g.WY * (g.WZL / 2) * 8 + (size_t)g.R * 16;
 }
 
 // a8: out = real + wave + (one-body - self) * input, in caller order (Eq. 13-15 one-body terms;

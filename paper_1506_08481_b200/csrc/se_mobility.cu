@@ -32,9 +32,11 @@ struct se_plan {
     double *d_radii;
     int *d_key_r, *d_rank_r, *d_cnt_r, *d_start_r;
     int *d_key_s, *d_rank_s, *d_cnt_s, *d_start_s;
+    int *d_key_g, *d_rank_g, *d_cnt_g, *d_start_g, *d_gperm;
     int *d_bsum;
-    int ncell_r, ncell_s;
-    int gseg, gseg_len;            // gather sweep segments (spreading's are in c.nseg, c.seg_len)
+    int ncell_r, ncell_s, ncell_g;
+    GatherGeom gg;                 // ring gather geometry (spreading's segments are in c.nseg, c.seg_len)
+    size_t gather_smem;
     double4 *d_rs_pos;
     double *d_rs_mom;
     int *d_rs_orig;
@@ -128,12 +130,53 @@ static void choose_segments(se_plan *p, int spread_segments, int gather_segments
     int ns = pick(spread_segments, npatch);
     c.seg_len = (M + ns - 1) / ns;
     c.nseg = (M + c.seg_len - 1) / c.seg_len;
-    int ng = pick(gather_segments, 2 * npatch);
-    p->gseg_len = (M + ng - 1) / ng;
-    p->gseg = (M + p->gseg_len - 1) / p->gseg_len;
+    // gather: enough (tile, grid, segment) items for ~8 rounds of one CTA per SM, segments of >= 32 planes
+    GatherGeom &g = p->gg;
+    int ng = gather_segments;
+    if (ng <= 0) {
+        const int items = g.NTY * g.NTZ * 6;
+        ng = (148 * 8 + items - 1) / items;
+        if (ng > maxseg) ng = maxseg;
+    }
+    if (ng > M) ng = M;
+    if (ng < 1) ng = 1;
+    g.seg_len = (M + ng - 1) / ng;
+    g.nseg = (M + g.seg_len - 1) / g.seg_len;
 }
 
-static cudaError_t dispatch_prepare(int P, size_t smem);
+// Ring gather geometry (se_gather.cuh).  Preference: tiles of 16 x 16 support origins with a ring shallow enough
+// for two CTAs per SM (they hide each other's pipeline bubbles; measured best on B200), then one CTA per SM with
+// the largest tile that fits the 227 KB of shared memory; smaller tiles when the grid would otherwise give the
+// 148 SMs too few items.  Rows are padded to WZ = P (mod 16) doubles for even P (P + 1 for odd P: rows must
+// stay 16-byte aligned) so that a half-warp's footprint columns fall in distinct banks.
+static bool choose_gather_geometry(se_plan *p)
+{
+    const int M = p->c.M, P = p->c.P;
+    const size_t one = 227 * 1024 - 1024, two = (228 * 1024) / 2 - 1024;
+    // TY, TZ, ring planes beyond P, CTAs per SM aimed at
+    static const int cand[][4] = { {16, 16, 5, 2}, {16, 16, 3, 2}, {8, 16, 5, 2}, {8, 8, 5, 2}, {16, 32, 7, 1}, {16, 16, 7, 1},
+                                   {8, 16, 7, 1}, {8, 16, 3, 1}, {8, 8, 3, 1}, {4, 8, 2, 1}, {4, 4, 1, 1}, {2, 4, 0, 1}, {2, 2, 0, 1} };
+    for (const auto &cd : cand) {
+        if (cd[3] == 2 && P > GR_P2MAX) continue;
+        GatherGeom g;
+        g.TY = cd[0]; g.TZ = cd[1]; g.R = P + cd[2];
+        g.NTY = (M + g.TY - 1) / g.TY; g.NTZ = (M + g.TZ - 1) / g.TZ;
+        g.WY = g.TY + P - 1;
+        g.WZL = (g.TZ + P - 1 + 1) & ~1;
+        const int want = (P & 1) ? (P + 1) % 16 : P % 16;
+        g.WZ = g.WZL;
+        while (g.WZ % 16 != want) g.WZ += 2;
+        g.nseg = 1; g.seg_len = M;
+        const bool few_items = (long long)g.NTY * g.NTZ * 6 * (M >= 64 ? 2 : 1) < 2 * 148 && g.TY * g.TZ > 64;
+        if (gather_smem_bytes(g, P) <= (cd[3] == 2 ? two : one) && !few_items) {
+            p->gg = g; p->gather_smem = gather_smem_bytes(g, P);
+            return true;
+        }
+    }
+    return false;
+}
+
+static cudaError_t dispatch_prepare(int P, size_t smem, size_t gsmem);
 
 extern "C" const char *se_version(void) { return "se_mobility 0.1 (sm_100a)"; }
 
@@ -145,6 +188,7 @@ extern "C" se_status se_plan_destroy(se_plan *p)
     cudaFree(p->d_radii);
     cudaFree(p->d_key_r); cudaFree(p->d_rank_r); cudaFree(p->d_cnt_r); cudaFree(p->d_start_r);
     cudaFree(p->d_key_s); cudaFree(p->d_rank_s); cudaFree(p->d_cnt_s); cudaFree(p->d_start_s);
+    cudaFree(p->d_key_g); cudaFree(p->d_rank_g); cudaFree(p->d_cnt_g); cudaFree(p->d_start_g); cudaFree(p->d_gperm);
     cudaFree(p->d_bsum);
     cudaFree(p->d_rs_pos); cudaFree(p->d_rs_mom); cudaFree(p->d_rs_orig); cudaFree(p->d_recs);
     cudaFree(p->d_real); cudaFree(p->d_Hk); cudaFree(p->d_Gk);
@@ -188,15 +232,19 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
     c.NBZ = (M + SE_TILE_Z - 1) / SE_TILE_Z;
     p->ncell_s = M * c.NBY * c.NBZ;
     c.rec_stride = (SE_REC_HDR + 6 * P + 1) & ~1;
+    if (!choose_gather_geometry(p)) { free(p); return SE_ERR_UNSUPPORTED; }
+    p->ncell_g = p->gg.NTY * p->gg.NTZ * M;
     choose_segments(p, 0, 0);
 
     se_status st = SE_OK;
     const size_t G = (size_t)M * M * M, Gc = (size_t)M * M * (M / 2 + 1);
-    const int nscan = (p->ncell_s > p->ncell_r ? p->ncell_s : p->ncell_r);
+    int nscan = (p->ncell_s > p->ncell_r ? p->ncell_s : p->ncell_r);
+    if (p->ncell_g > nscan) nscan = p->ncell_g;
 #define ALLOC(ptr, count) if (st == SE_OK) st = dev_alloc(p, &(ptr), (size_t)(count))
     ALLOC(p->d_radii, N);
     ALLOC(p->d_key_r, N); ALLOC(p->d_rank_r, N); ALLOC(p->d_cnt_r, p->ncell_r); ALLOC(p->d_start_r, p->ncell_r + 1);
     ALLOC(p->d_key_s, N); ALLOC(p->d_rank_s, N); ALLOC(p->d_cnt_s, p->ncell_s); ALLOC(p->d_start_s, p->ncell_s + 1);
+    ALLOC(p->d_key_g, N); ALLOC(p->d_rank_g, N); ALLOC(p->d_cnt_g, p->ncell_g); ALLOC(p->d_start_g, p->ncell_g + 1); ALLOC(p->d_gperm, N);
     ALLOC(p->d_bsum, (nscan + SCAN_BLOCK - 1) / SCAN_BLOCK + 1);
     ALLOC(p->d_rs_pos, N); ALLOC(p->d_rs_mom, 12 * (size_t)N); ALLOC(p->d_rs_orig, N);
     ALLOC(p->d_recs, (size_t)N * c.rec_stride);
@@ -225,7 +273,7 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
     for (int k = 0; k <= SE_NUM_STAGES; ++k)
         if (cudaEventCreate(&p->ev[k]) != cudaSuccess) { p->have_events = (k > 0); se_plan_destroy(p); return SE_ERR_CUDA; }
     p->have_events = true;
-    if (dispatch_prepare(P, sweep_smem_bytes(c.rec_stride)) != cudaSuccess) { cudaGetLastError(); se_plan_destroy(p); return SE_ERR_CUDA; }
+    if (dispatch_prepare(P, sweep_smem_bytes(c.rec_stride), p->gather_smem) != cudaSuccess) { cudaGetLastError(); se_plan_destroy(p); return SE_ERR_CUDA; }
     *out = p;
     return SE_OK;
 }
@@ -266,7 +314,7 @@ extern "C" se_status se_plan_get_constants(const se_plan *p, double *out)
 {
     if (!p || !out) return SE_ERR_INVALID_ARG;
     out[0] = p->c.Delta; out[1] = p->c.eta_se; out[2] = p->c.alpha; out[3] = p->m;
-    out[4] = (double)p->c.ncr; out[5] = (double)p->c.nseg; out[6] = (double)p->gseg;
+    out[4] = (double)p->c.ncr; out[5] = (double)p->c.nseg; out[6] = (double)p->gg.nseg;
     return SE_OK;
 }
 
@@ -293,18 +341,18 @@ static void launch_spread(se_plan *p, cudaStream_t s)
 template <int P>
 static void launch_gather(se_plan *p, cudaStream_t s)
 {
-    SeConst c = p->c;
-    c.nseg = p->gseg; c.seg_len = p->gseg_len;
-    const long long warps = (long long)c.NBY * c.NBZ * c.nseg * 2;
-    const int blocks = (int)((warps + SWEEP_WARPS - 1) / SWEEP_WARPS);
-    k_gather<P><<<blocks, SWEEP_WARPS * 32, sweep_smem_bytes(c.rec_stride), s>>>(c, p->d_recs, p->d_start_s, p->d_real, p->d_moments);
+    const GatherGeom &g = p->gg;
+    const int ngrids = 6;
+    const unsigned blocks = (unsigned)(g.NTY * g.NTZ * ngrids * g.nseg);
+    k_gather<P><<<blocks, (GR_WARPS + GR_PROD) * 32, p->gather_smem, s>>>(p->c, g, p->d_recs, p->d_gperm, p->d_start_g, p->d_real, ngrids,
+                                                                   p->d_moments);
 }
 
 template <int P>
-static cudaError_t prepare_sweeps(size_t smem)
+static cudaError_t prepare_sweeps(size_t smem, size_t gsmem)
 {
     cudaError_t e = cudaFuncSetAttribute(k_spread<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gather<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gather<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsmem);
     return e;
 }
 
@@ -320,10 +368,10 @@ static void dispatch_spread(se_plan *p, cudaStream_t s)
     }
 }
 
-static cudaError_t dispatch_prepare(int P, size_t smem)
+static cudaError_t dispatch_prepare(int P, size_t smem, size_t gsmem)
 {
     switch (P) {
-#define X(v) case v: return prepare_sweeps<v>(smem);
+#define X(v) case v: return prepare_sweeps<v>(smem, gsmem);
         FOR_EACH_P(X)
 #undef X
     }
@@ -361,14 +409,18 @@ extern "C" se_status far_mobility_apply(se_plan *p, const double *pos, const dou
     // ---- a1: wrap + counting sorts + packing ----
     CUDA_TRY(p, cudaMemsetAsync(p->d_cnt_r, 0, sizeof(int) * (size_t)p->ncell_r, s));
     CUDA_TRY(p, cudaMemsetAsync(p->d_cnt_s, 0, sizeof(int) * (size_t)p->ncell_s, s));
-    k_keys<<<nbN, TB, 0, s>>>(c, pos, p->d_key_r, p->d_rank_r, p->d_cnt_r, p->d_key_s, p->d_rank_s, p->d_cnt_s);
+    CUDA_TRY(p, cudaMemsetAsync(p->d_cnt_g, 0, sizeof(int) * (size_t)p->ncell_g, s));
+    k_keys<<<nbN, TB, 0, s>>>(c, p->gg, pos, p->d_key_r, p->d_rank_r, p->d_cnt_r, p->d_key_s, p->d_rank_s, p->d_cnt_s,
+                              p->d_key_g, p->d_rank_g, p->d_cnt_g);
     p->last_launches += 1;
     se_status st = scan_cells(p, p->d_cnt_r, p->d_start_r, p->ncell_r, s);
     if (st != SE_OK) return st;
     st = scan_cells(p, p->d_cnt_s, p->d_start_s, p->ncell_s, s);
     if (st != SE_OK) return st;
+    st = scan_cells(p, p->d_cnt_g, p->d_start_g, p->ncell_g, s);
+    if (st != SE_OK) return st;
     k_scatter<<<nbN, TB, 0, s>>>(c, pos, p->d_radii, F, T, S, p->d_key_r, p->d_rank_r, p->d_start_r,
-                                 p->d_key_s, p->d_rank_s, p->d_start_s, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig, p->d_recs);
+                                 p->d_key_s, p->d_rank_s, p->d_start_s, p->d_key_g, p->d_rank_g, p->d_start_g, p->d_gperm, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig, p->d_recs);
     p->last_launches += 1;
     CUDA_TRY(p, cudaGetLastError());
     MARK();
@@ -406,7 +458,6 @@ extern "C" se_status far_mobility_apply(se_plan *p, const double *pos, const dou
     }
     MARK();
     if (on(SE_STAGE_GATHER)) {
-        CUDA_TRY(p, cudaMemsetAsync(p->d_moments, 0, sizeof(double) * GATHER_SUMS * (size_t)c.N, s));
         dispatch_gather(p, s);
         p->last_launches += 1;
         CUDA_TRY(p, cudaGetLastError());

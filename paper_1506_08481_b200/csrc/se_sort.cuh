@@ -4,11 +4,21 @@
 #pragma once
 #include "se_common.cuh"
 
+// Geometry of the ring gather (se_gather.cuh), chosen on the host (choose_gather_geometry).
+struct GatherGeom {
+    int TY, TZ;                    // support origins per tile along y, z
+    int NTY, NTZ;                  // tiles per axis
+    int WY, WZ, WZL;               // haloed tile: rows, padded row length, loaded row length (doubles, even)
+    int R;                         // planes in the ring (>= P)
+    int nseg, seg_len;             // segments of the sweep along x
+};
+
 __device__ __forceinline__ double se_wrap(double x, double L) { return x - L * floor(x / L); }
 
 // One thread per particle: cell keys and the rank inside each cell (atomic counter).
-__global__ void k_keys(SeConst c, const double *__restrict__ pos, int *__restrict__ key_r, int *__restrict__ rank_r,
-                       int *__restrict__ cnt_r, int *__restrict__ key_s, int *__restrict__ rank_s, int *__restrict__ cnt_s)
+__global__ void k_keys(SeConst c, GatherGeom g, const double *__restrict__ pos, int *__restrict__ key_r, int *__restrict__ rank_r,
+                       int *__restrict__ cnt_r, int *__restrict__ key_s, int *__restrict__ rank_s, int *__restrict__ cnt_s,
+                       int *__restrict__ key_g, int *__restrict__ rank_g, int *__restrict__ cnt_g)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= c.N) return;
@@ -25,6 +35,10 @@ __global__ void k_keys(SeConst c, const double *__restrict__ pos, int *__restric
     key_s[i] = ks;
     rank_r[i] = atomicAdd(&cnt_r[kr], 1);
     rank_s[i] = atomicAdd(&cnt_s[ks], 1);
+    // gather order: (y,z) tile of the support origin major, starting plane minor
+    const int kg = ((n0[1] / g.TY) * g.NTZ + n0[2] / g.TZ) * c.M + n0[0];
+    key_g[i] = kg;
+    rank_g[i] = atomicAdd(&cnt_g[kg], 1);
 }
 
 // ---- exclusive prefix sum over n ints (three small kernels; n up to a few million) ----
@@ -103,7 +117,8 @@ __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const doubl
                           const double *__restrict__ F, const double *__restrict__ T, const double *__restrict__ S,
                           const int *__restrict__ key_r, const int *__restrict__ rank_r, const int *__restrict__ start_r,
                           const int *__restrict__ key_s, const int *__restrict__ rank_s, const int *__restrict__ start_s,
-                          double4 *__restrict__ rs_pos, double *__restrict__ rs_mom, int *__restrict__ rs_orig,
+                          const int *__restrict__ key_g, const int *__restrict__ rank_g, const int *__restrict__ start_g,
+                          int *__restrict__ gperm, double4 *__restrict__ rs_pos, double *__restrict__ rs_mom, int *__restrict__ rs_orig,
                           double *__restrict__ recs)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -126,6 +141,7 @@ __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const doubl
 
     // spreading / gather record
     const int ds = start_s[key_s[i]] + rank_s[i];
+    gperm[start_g[key_g[i]] + rank_g[i]] = ds;               // gather order -> record
     double *r = recs + (size_t)ds * c.rec_stride;
     int n0w[3];
     double d0[3];
