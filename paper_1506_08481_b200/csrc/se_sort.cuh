@@ -88,26 +88,29 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_local(const int *__restri
     if (threadIdx.x == 0) bsum[blockIdx.x] = total;
 }
 
-__global__ void __launch_bounds__(SCAN_THREADS) k_scan_sums(int *__restrict__ bsum, int nb)
+// Second pass of the scan.  The three count arrays are concatenated, each followed by one zero pad element:
+//   [cnt_r (n1-1) 0 | cnt_s (n2-n1-1) 0 | cnt_g ... 0],  every array summing to N,
+// so ONE exclusive scan gives all three start tables, each with its sentinel (= N) in the pad slot, after
+// subtracting N (2N) from the second (third) table.  Each block adds the totals of the blocks before it.
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_add(int *__restrict__ out, const int *__restrict__ bsum, int n,
+                                                          int n1, int n2, int N)
 {
-    int carry = 0;
-    for (int b0 = 0; b0 < nb; b0 += SCAN_THREADS) {
-        const int idx = b0 + threadIdx.x;
-        const int v = idx < nb ? bsum[idx] : 0;
-        int total;
-        const int ex = block_exclusive_scan(v, &total);
-        if (idx < nb) bsum[idx] = carry + ex;
-        carry += total;
-    }
-}
-
-__global__ void __launch_bounds__(SCAN_THREADS) k_scan_add(int *__restrict__ out, const int *__restrict__ bsum, int n, int total)
-{
-    const int base = blockIdx.x * SCAN_BLOCK + threadIdx.x * SCAN_ITEMS;
-    const int add = bsum[blockIdx.x];
+    __shared__ int red[SCAN_THREADS / 32];
+    int part = 0;
+    for (int b = threadIdx.x; b < blockIdx.x; b += SCAN_THREADS) part += bsum[b];
 #pragma unroll
-    for (int k = 0; k < SCAN_ITEMS; ++k) if (base + k < n) out[base + k] += add;
-    if (blockIdx.x == 0 && threadIdx.x == 0) out[n] = total;      // sentinel: start[n] = N
+    for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = part;
+    __syncthreads();
+    int add = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_THREADS / 32; ++k) add += red[k];
+    const int base = blockIdx.x * SCAN_BLOCK + threadIdx.x * SCAN_ITEMS;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+        const int q = base + k;
+        if (q < n) out[q] += add - (q >= n1 ? N : 0) - (q >= n2 ? N : 0);
+    }
 }
 
 // One thread per particle: write the real-space packed copy (cell order) and the spreading/gather
