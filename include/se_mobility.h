@@ -98,9 +98,15 @@ se_status far_mobility_apply(se_plan *plan, const double *pos, const double *F, 
                              const double *S, double *U, double *Omega, double *E, void *cuda_stream);
 
 /* Compressible-solvent extension (Sec. 2.3, Eq. 24-34).  As far_mobility_apply with
- *   s_in   [N] DEVICE pressure moments S^H_j (paper's Eq. 25-26 sign), or NULL for none
- *   s_out  [N] DEVICE interaction part 4 pi a_i^3 p'(r_i) of the pressure Faxen law (Eq. 28), or NULL
- * With s_in == NULL the outputs U, Omega, E equal those of far_mobility_apply. */
+ *   s_in   [N] DEVICE pressure moments s_j (paper's Eq. 25-26 sign: s > 0 is a fluid source), or NULL for none.
+ *          Adds the source field grad psi (Eq. 26, split after Eq. 33-34) to U and E: one more spread grid
+ *          and forward FFT, an (i k/k^2) term in the k-space pass, two more couplings in the real-space sum.
+ *   s_out  [N] DEVICE, OVERWRITTEN with the interaction part 4 pi a_i^3 p'(r_i) of the pressure Faxen law
+ *          (Eq. 28-31: pressure from F and S of all particles), or NULL: one more spectrum, inverse FFT and
+ *          plain Gaussian gather, two more couplings in the real-space sum.
+ * With s_in == NULL the outputs U, Omega, E equal those of far_mobility_apply.  The first call that passes
+ * s_in or s_out allocates the extra grids and cuFFT plans (synchronous; later calls only enqueue).
+ * Errors: as far_mobility_apply, plus SE_ERR_ALLOC / SE_ERR_CUFFT from that allocation. */
 se_status far_mobility_apply_compressible(se_plan *plan, const double *pos, const double *F,
                                           const double *T, const double *S, const double *s_in,
                                           double *U, double *Omega, double *E, double *s_out,
@@ -114,7 +120,8 @@ se_status far_mobility_apply_host(se_plan *plan, const double *pos, const double
 
 /* Staged outputs for parity tests (valid after the stream of the last apply has been synchronised).
  * which = 0: the three spread grids H_x,H_y,H_z, [3][M][M][M];  which = 1: the six returned grids
- * u~ (3), w~ (3), [6][M][M][M].  dst is a HOST pointer with room for the whole array.  The spread
+ * u~ (3), w~ (3), [6][M][M][M];  which = 2: the scalar grid of the compressible extension, [M][M][M]
+ * (the spread pressure moments after SE_STAGE_SPREAD, the returned pressure grid p~ after SE_STAGE_FFT_INV).  dst is a HOST pointer with room for the whole array.  The spread
  * grids share storage with the returned grids and are only available from an apply made with flag
  * SE_SKIP_WAVE cleared and read through which = 0 BEFORE a later apply; tests use se_plan_debug_stop. */
 se_status se_plan_copy_grids(se_plan *plan, int which, double *dst);

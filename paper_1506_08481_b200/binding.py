@@ -154,6 +154,17 @@ class SePlan:
                                           _dptr(E, 5 * N, "E"), sp)
         self._check(st, "far_mobility_apply")
 
+    def apply_compressible(self, pos, F, T, S, s_in, U, Omega, E, s_out, stream=None):
+        """far_mobility_apply_compressible; ``s_in`` / ``s_out`` are CUDA float64 tensors of N entries or None."""
+        import torch
+        N = self.N
+        sp = (torch.cuda.current_stream() if stream is None else stream).cuda_stream
+        st = self._lib.far_mobility_apply_compressible(
+            self._h, _dptr(pos, 3 * N, "pos"), _dptr(F, 3 * N, "F"), _dptr(T, 3 * N, "T"), _dptr(S, 5 * N, "S"),
+            None if s_in is None else _dptr(s_in, N, "s_in"), _dptr(U, 3 * N, "U"), _dptr(Omega, 3 * N, "Omega"),
+            _dptr(E, 5 * N, "E"), None if s_out is None else _dptr(s_out, N, "s_out"), sp)
+        self._check(st, "far_mobility_apply_compressible")
+
     def apply_raw(self, pos, F, T, S, U, Omega, E, stream_ptr=0):
         """far_mobility_apply on raw device addresses (ints); used to test NULL handling."""
         return self._lib.far_mobility_apply(self._h, pos, F, T, S, U, Omega, E, stream_ptr)
@@ -169,7 +180,7 @@ class SePlan:
         self._check(st, "far_mobility_apply_host")
 
     def copy_grids(self, which):
-        out = np.empty((3 if which == 0 else 6, self.M, self.M, self.M))
+        out = np.empty(({0: 3, 1: 6, 2: 1}[which], self.M, self.M, self.M))
         self._check(self._lib.se_plan_copy_grids(self._h, int(which), out.ctypes.data), "se_plan_copy_grids")
         return out
 

@@ -30,7 +30,7 @@ struct SeConst {
 //   [2..4]   d0x, d0y, d0z   offset of the first support point from the particle, (n0 - u) Delta
 //   [5..8]   f0, f1, s0, s1  size polynomials: 1-6 al cF, 4 al^2 cF, 2 al (1-10 al cS), 8 al^3 cS
 //   [9..11] F  [12..14] T  [15..20] S (xx,xy,xz,yy,yz,zz)
-//   [21] cF = a^2/6  [22] cS = a^2/10  [23] radius a
+//   [21] cF = a^2/6  [22] cS = a^2/10  [23] pressure moment s (a9; 0 without)
 //   [24..24+P) gx * (al/pi)^{3/2}   [24+P..24+2P) gy   [24+2P..24+3P) gz     per-axis Gaussians
 //   [24+3P..24+6P)  gx dx, gx dx^2, gx dx^3 with dx_k = d0x + k Delta     x-moment tables (P each)
 #define REC_D0 2
@@ -40,7 +40,7 @@ struct SeConst {
 #define REC_S 15
 #define REC_CF 21
 #define REC_CS 22
-#define REC_A 23
+#define REC_SP 23
 
 __host__ __device__ inline int se_support_start(double u, int P)
 {

@@ -47,7 +47,8 @@ __device__ __forceinline__ void cp_async_arrive(uint32_t bar)
 template <int P>
 __global__ void __launch_bounds__((GR_WARPS + GR_PROD) * 32, (P <= GR_P2MAX ? 2 : 1))
 k_gather(SeConst c, GatherGeom g, const double *__restrict__ recs, const int *__restrict__ gperm,
-         const int *__restrict__ start_g, const double *__restrict__ Gr, int ngrids, double *__restrict__ moments)
+         const int *__restrict__ start_g, const double *__restrict__ Gr, int ngrids, double *__restrict__ moments,
+         int mstride)
 {
     extern __shared__ __align__(16) unsigned char gsm[];
     constexpr int PP = P * P, NI = (PP + 31) / 32;
@@ -207,7 +208,7 @@ k_gather(SeConst c, GatherGeom g, const double *__restrict__ recs, const int *__
             t += __shfl_xor_sync(0xffffffffu, t, 1);
             if ((lane & 7) == 0) {
                 const int kind = ((lane >> 4) << 1) | ((lane >> 3) & 1);
-                moments[(size_t)xo.y * GATHER_SUMS + (grid / 3) * 12 + kind * 3 + (grid % 3)] = t;
+                moments[(size_t)xo.y * mstride + (grid / 3) * 12 + kind * 3 + (grid % 3)] = t;
             }
         }
     }
@@ -230,7 +231,9 @@ static inline size_t gather_smem_bytes(const GatherGeom &g, int P)
 __global__ void k_epilogue(SeConst c, unsigned flags, const double *__restrict__ radii,
                            const double *__restrict__ F, const double *__restrict__ T, const double *__restrict__ S,
                            const double *__restrict__ out_real, const double *__restrict__ moments,
-                           double *__restrict__ U, double *__restrict__ W, double *__restrict__ E)
+                           const double *__restrict__ pmom,     // gathered pressure sums [N][12], slot 0 used (a9), or NULL
+                           double *__restrict__ U, double *__restrict__ W, double *__restrict__ E,
+                           double *__restrict__ s_out)           // 4 pi a^3 p'(r_i), Eq. 28 (a9), or NULL
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= c.N) return;
@@ -253,7 +256,7 @@ __global__ void k_epilogue(SeConst c, unsigned flags, const double *__restrict__
 #pragma unroll
     for (int k = 0; k < 11; ++k) v[k] = 0.0;
     if (!(flags & 0x1u)) {                                   // real-space part
-        const double *orl = out_real + 11 * (size_t)i;
+        const double *orl = out_real + 12 * (size_t)i;
 #pragma unroll
         for (int k = 0; k < 11; ++k) v[k] += orl[k];
     }
@@ -287,4 +290,10 @@ __global__ void k_epilogue(SeConst c, unsigned flags, const double *__restrict__
     }
 #pragma unroll
     for (int k = 0; k < 5; ++k) E[5 * (size_t)i + k] = v[6 + k] + cE * S[5 * (size_t)i + k];
+    if (s_out) {
+        double pv = 0.0;
+        if (!(flags & 0x1u)) pv += out_real[12 * (size_t)i + 11];
+        if (!(flags & 0x2u) && pmom) pv += c.D3 * pmom[12 * (size_t)i];
+        s_out[i] = 4.0 * PI * a3 * pv;
+    }
 }

@@ -48,7 +48,13 @@ struct se_plan {
     double *d_real;                // [6][M^3]; the first three double as the spread grids H
     double2 *d_Hk;                 // [3][M][M][M/2+1]
     double2 *d_Gk;                 // [6][M][M][M/2+1]
-    double *d_out_real;            // [N][11] real-space part in caller order
+    double *d_out_real;            // [N][12] real-space part in caller order (slot 11: pressure, a9)
+    // compressible extension (a9): allocated by the first apply that passes s_in or s_out
+    double *d_real_p;              // [M^3]: scalar spread grid Hs, then the returned pressure grid p~
+    double2 *d_Hk_s, *d_Gk_p;      // their spectra
+    double *d_pmom;                // [N][12] gathered pressure sums
+    cufftHandle fft_fwd1, fft_inv1;
+    bool have_comp;
     double *d_moments;             // [N][24] gathered wave-space sums in caller order
     // host-API staging
     double *d_io;                  // pos3 F3 T3 S5 U3 W3 E5 = 25 N doubles
@@ -198,6 +204,10 @@ extern "C" se_status se_plan_destroy(se_plan *p)
     cudaFree(p->d_rs_pos); cudaFree(p->d_rs_mom); cudaFree(p->d_rs_orig); cudaFree(p->d_recs);
     cudaFree(p->d_real); cudaFree(p->d_Hk); cudaFree(p->d_Gk);
     cudaFree(p->d_out_real); cudaFree(p->d_moments); cudaFree(p->d_io);
+    if (p->have_comp) {
+        cudaFree(p->d_real_p); cudaFree(p->d_Hk_s); cudaFree(p->d_Gk_p); cudaFree(p->d_pmom);
+        cufftDestroy(p->fft_fwd1); cufftDestroy(p->fft_inv1);
+    }
     if (p->have_fwd) cufftDestroy(p->fft_fwd);
     if (p->have_inv) cufftDestroy(p->fft_inv);
     if (p->have_events) for (int k = 0; k <= SE_NUM_STAGES; ++k) cudaEventDestroy(p->ev[k]);
@@ -258,12 +268,12 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
     ALLOC(p->d_rs_pos, N); ALLOC(p->d_rs_mom, 12 * (size_t)N); ALLOC(p->d_rs_orig, N);
     ALLOC(p->d_recs, (size_t)N * c.rec_stride);
     ALLOC(p->d_real, 6 * G); ALLOC(p->d_Hk, 3 * Gc); ALLOC(p->d_Gk, 6 * Gc);
-    ALLOC(p->d_out_real, 11 * (size_t)N); ALLOC(p->d_moments, GATHER_SUMS * (size_t)N);
+    ALLOC(p->d_out_real, 12 * (size_t)N); ALLOC(p->d_moments, GATHER_SUMS * (size_t)N);
     ALLOC(p->d_io, 25 * (size_t)N);
 #undef ALLOC
     if (st != SE_OK) { se_plan_destroy(p); return st; }
     if (cudaMemcpy(p->d_radii, radii, sizeof(double) * (size_t)N, cudaMemcpyHostToDevice) != cudaSuccess ||
-        cudaMemset(p->d_out_real, 0, sizeof(double) * 11 * (size_t)N) != cudaSuccess ||
+        cudaMemset(p->d_out_real, 0, sizeof(double) * 12 * (size_t)N) != cudaSuccess ||
         cudaMemset(p->d_moments, 0, sizeof(double) * GATHER_SUMS * (size_t)N) != cudaSuccess) {
         se_plan_destroy(p);
         return SE_ERR_CUDA;
@@ -346,28 +356,33 @@ static se_status scan_cells(se_plan *p, cudaStream_t s)
 }
 
 template <int P>
-static void launch_spread(se_plan *p, cudaStream_t s)
+static void launch_spread(se_plan *p, cudaStream_t s, bool comp_in)
 {
     const SeConst &c = p->c;
     const long long warps = (long long)c.NBY * c.NBZ * c.nseg;
     const int blocks = (int)((warps + SWEEP_WARPS - 1) / SWEEP_WARPS);
-    k_spread<P><<<blocks, SWEEP_WARPS * 32, sweep_smem_bytes(c.rec_stride), s>>>(c, p->d_recs, p->d_start_s, p->d_real);
+    if (comp_in)
+        k_spread<P, 4><<<blocks, SWEEP_WARPS * 32, sweep_smem_bytes(c.rec_stride), s>>>(c, p->d_recs, p->d_start_s, p->d_real, p->d_real_p);
+    else
+        k_spread<P, 3><<<blocks, SWEEP_WARPS * 32, sweep_smem_bytes(c.rec_stride), s>>>(c, p->d_recs, p->d_start_s, p->d_real, nullptr);
 }
 
 template <int P>
-static void launch_gather(se_plan *p, cudaStream_t s)
+static void launch_gather(se_plan *p, cudaStream_t s, bool pressure)
 {
     const GatherGeom &g = p->gg;
-    const int ngrids = 6;
+    const int ngrids = pressure ? 1 : 6;
     const unsigned blocks = (unsigned)(g.NTY * g.NTZ * ngrids * g.nseg);
-    k_gather<P><<<blocks, (GR_WARPS + GR_PROD) * 32, p->gather_smem, s>>>(p->c, g, p->d_recs, p->d_gperm, p->d_start_g, p->d_real, ngrids,
-                                                                   p->d_moments);
+    k_gather<P><<<blocks, (GR_WARPS + GR_PROD) * 32, p->gather_smem, s>>>(p->c, g, p->d_recs, p->d_gperm, p->d_start_g,
+                                                                   pressure ? p->d_real_p : p->d_real, ngrids,
+                                                                   pressure ? p->d_pmom : p->d_moments, pressure ? 12 : GATHER_SUMS);
 }
 
 template <int P>
 static cudaError_t prepare_sweeps(size_t smem, size_t gsmem)
 {
-    cudaError_t e = cudaFuncSetAttribute(k_spread<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(k_spread<P, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_spread<P, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gather<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsmem);
     return e;
 }
@@ -375,10 +390,10 @@ static cudaError_t prepare_sweeps(size_t smem, size_t gsmem)
 #define FOR_EACH_P(X) \
     X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15) X(16) X(17) X(18) X(19) X(20) X(21) X(22) X(23) X(24)
 
-static void dispatch_spread(se_plan *p, cudaStream_t s)
+static void dispatch_spread(se_plan *p, cudaStream_t s, bool comp_in)
 {
     switch (p->c.P) {
-#define X(v) case v: launch_spread<v>(p, s); break;
+#define X(v) case v: launch_spread<v>(p, s, comp_in); break;
         FOR_EACH_P(X)
 #undef X
     }
@@ -394,20 +409,54 @@ static cudaError_t dispatch_prepare(int P, size_t smem, size_t gsmem)
     return cudaErrorInvalidValue;
 }
 
-static void dispatch_gather(se_plan *p, cudaStream_t s)
+static void dispatch_gather(se_plan *p, cudaStream_t s, bool pressure)
 {
     switch (p->c.P) {
-#define X(v) case v: launch_gather<v>(p, s); break;
+#define X(v) case v: launch_gather<v>(p, s, pressure); break;
         FOR_EACH_P(X)
 #undef X
     }
 }
 
-extern "C" se_status far_mobility_apply(se_plan *p, const double *pos, const double *F, const double *T,
-                                        const double *S, double *U, double *Omega, double *E, void *cuda_stream)
+// Buffers and cuFFT plans of the compressible extension (a9), made by the first apply that needs them.
+static se_status ensure_compressible(se_plan *p)
+{
+    if (p->have_comp) return SE_OK;
+    const int M = p->c.M;
+    const size_t G = (size_t)M * M * M, Gc = (size_t)M * M * (M / 2 + 1);
+    se_status st = SE_OK;
+    st = dev_alloc(p, &p->d_real_p, G);
+    if (st == SE_OK) st = dev_alloc(p, &p->d_Hk_s, Gc);
+    if (st == SE_OK) st = dev_alloc(p, &p->d_Gk_p, Gc);
+    if (st == SE_OK) st = dev_alloc(p, &p->d_pmom, 12 * (size_t)p->c.N);
+    cufftResult r = CUFFT_SUCCESS;
+    bool f1 = false, i1 = false;
+    if (st == SE_OK) {
+        r = cufftPlan3d(&p->fft_fwd1, M, M, M, CUFFT_D2Z);
+        f1 = (r == CUFFT_SUCCESS);
+        if (f1) { r = cufftPlan3d(&p->fft_inv1, M, M, M, CUFFT_Z2D); i1 = (r == CUFFT_SUCCESS); }
+        if (r != CUFFT_SUCCESS) st = fail(p, r == CUFFT_ALLOC_FAILED ? SE_ERR_ALLOC : SE_ERR_CUFFT, "cufftPlan3d", "compressible extension");
+    }
+    if (st != SE_OK) {
+        cudaFree(p->d_real_p); cudaFree(p->d_Hk_s); cudaFree(p->d_Gk_p); cudaFree(p->d_pmom);
+        p->d_real_p = nullptr; p->d_Hk_s = nullptr; p->d_Gk_p = nullptr; p->d_pmom = nullptr;
+        if (f1) cufftDestroy(p->fft_fwd1);
+        if (i1) cufftDestroy(p->fft_inv1);
+        cudaGetLastError();
+        return st;
+    }
+    p->have_comp = true;
+    return SE_OK;
+}
+
+static se_status apply_impl(se_plan *p, const double *pos, const double *F, const double *T, const double *S,
+                            const double *s_in, double *U, double *Omega, double *E, double *s_out, void *cuda_stream,
+                            const char *who)
 {
     if (!p) return SE_ERR_INVALID_ARG;
-    if (!pos || !F || !T || !S || !U || !Omega || !E) return fail(p, SE_ERR_INVALID_ARG, "far_mobility_apply", "null pointer");
+    if (!pos || !F || !T || !S || !U || !Omega || !E) return fail(p, SE_ERR_INVALID_ARG, who, "null pointer");
+    const bool comp_in = s_in != nullptr, comp_out = s_out != nullptr, comp = comp_in || comp_out;
+    if (comp) { se_status stc = ensure_compressible(p); if (stc != SE_OK) return stc; }
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const SeConst &c = p->c;
     const unsigned fl = p->flags;
@@ -429,7 +478,7 @@ extern "C" se_status far_mobility_apply(se_plan *p, const double *pos, const dou
     p->last_launches += 1;
     se_status st = scan_cells(p, s);
     if (st != SE_OK) return st;
-    k_scatter<<<nbN, TB, 0, s>>>(c, pos, p->d_radii, F, T, S, p->d_key_r, p->d_rank_r, p->d_start_r,
+    k_scatter<<<nbN, TB, 0, s>>>(c, pos, p->d_radii, F, T, S, s_in, p->d_key_r, p->d_rank_r, p->d_start_r,
                                  p->d_key_s, p->d_rank_s, p->d_start_s, p->d_key_g, p->d_rank_g, p->d_start_g, p->d_gperm, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig, p->d_recs);
     p->last_launches += 1;
     CUDA_TRY(p, cudaGetLastError());
@@ -441,8 +490,9 @@ extern "C" se_status far_mobility_apply(se_plan *p, const double *pos, const dou
     // stream, alone, so that every stage is timed by itself.
     const bool fork = do_real && do_wave && !timing && stop < 0;
     auto launch_real = [&](cudaStream_t sr) {
-        k_real<<<c.ncr > 1 ? p->ncell_r : (c.N + 31) / 32, REAL_WARPS * 32, 0, sr>>>(c, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig,
-                                                                                 p->d_start_r, p->d_out_real);
+        const unsigned nb = (unsigned)(c.ncr > 1 ? p->ncell_r : (c.N + 31) / 32);
+        if (comp) k_real<true><<<nb, REAL_WARPS * 32, 0, sr>>>(c, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig, p->d_start_r, p->d_out_real);
+        else k_real<false><<<nb, REAL_WARPS * 32, 0, sr>>>(c, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig, p->d_start_r, p->d_out_real);
         p->last_launches += 1;
     };
     if (do_real && !fork) {
@@ -460,7 +510,7 @@ extern "C" se_status far_mobility_apply(se_plan *p, const double *pos, const dou
     // ---- a3..a7: Spectral Ewald wave-space sum ----
     bool wave_done = false;
     if (on(SE_STAGE_SPREAD)) {
-        dispatch_spread(p, s);
+        dispatch_spread(p, s, comp_in);
         p->last_launches += 1;
         CUDA_TRY(p, cudaGetLastError());
     }
@@ -468,11 +518,17 @@ extern "C" se_status far_mobility_apply(se_plan *p, const double *pos, const dou
     if (on(SE_STAGE_FFT_FWD)) {
         CUFFT_TRY(p, cufftSetStream(p->fft_fwd, s));
         CUFFT_TRY(p, cufftExecD2Z(p->fft_fwd, p->d_real, (cufftDoubleComplex *)p->d_Hk));
+        if (comp_in) {
+            CUFFT_TRY(p, cufftSetStream(p->fft_fwd1, s));
+            CUFFT_TRY(p, cufftExecD2Z(p->fft_fwd1, p->d_real_p, (cufftDoubleComplex *)p->d_Hk_s));
+        }
     }
     MARK();
     if (on(SE_STAGE_KSPACE)) {
         const size_t Gc = (size_t)c.M * c.M * (c.M / 2 + 1);
-        k_kspace<<<(unsigned)((Gc + KSPACE_THREADS - 1) / KSPACE_THREADS), KSPACE_THREADS, 0, s>>>(c, p->d_Hk, p->d_Gk);
+        k_kspace<<<(unsigned)((Gc + KSPACE_THREADS - 1) / KSPACE_THREADS), KSPACE_THREADS, 0, s>>>(c, p->d_Hk, p->d_Gk,
+                                                                                                   comp_in ? p->d_Hk_s : nullptr,
+                                                                                                   comp_out ? p->d_Gk_p : nullptr);
         p->last_launches += 1;
         CUDA_TRY(p, cudaGetLastError());
     }
@@ -480,18 +536,27 @@ extern "C" se_status far_mobility_apply(se_plan *p, const double *pos, const dou
     if (on(SE_STAGE_FFT_INV)) {
         CUFFT_TRY(p, cufftSetStream(p->fft_inv, s));
         CUFFT_TRY(p, cufftExecZ2D(p->fft_inv, (cufftDoubleComplex *)p->d_Gk, p->d_real));
+        if (comp_out) {
+            CUFFT_TRY(p, cufftSetStream(p->fft_inv1, s));
+            CUFFT_TRY(p, cufftExecZ2D(p->fft_inv1, (cufftDoubleComplex *)p->d_Gk_p, p->d_real_p));
+        }
     }
     MARK();
     if (on(SE_STAGE_GATHER)) {
-        dispatch_gather(p, s);
+        dispatch_gather(p, s, false);
         p->last_launches += 1;
+        if (comp_out) {
+            dispatch_gather(p, s, true);
+            p->last_launches += 1;
+        }
         CUDA_TRY(p, cudaGetLastError());
         wave_done = true;
     }
     MARK();
     // ---- a8: epilogue ----
     if (fork) CUDA_TRY(p, cudaStreamWaitEvent(s, p->ev_join, 0));
-    k_epilogue<<<nbN, TB, 0, s>>>(c, fl | (wave_done ? 0u : SE_SKIP_WAVE), p->d_radii, F, T, S, p->d_out_real, p->d_moments, U, Omega, E);
+    k_epilogue<<<nbN, TB, 0, s>>>(c, fl | (wave_done ? 0u : SE_SKIP_WAVE), p->d_radii, F, T, S, p->d_out_real, p->d_moments,
+                                  comp_out && wave_done ? p->d_pmom : nullptr, U, Omega, E, s_out);
     p->last_launches += 1;
     CUDA_TRY(p, cudaGetLastError());
     MARK();
@@ -500,13 +565,17 @@ extern "C" se_status far_mobility_apply(se_plan *p, const double *pos, const dou
     return SE_OK;
 }
 
+extern "C" se_status far_mobility_apply(se_plan *p, const double *pos, const double *F, const double *T,
+                                        const double *S, double *U, double *Omega, double *E, void *cuda_stream)
+{
+    return apply_impl(p, pos, F, T, S, nullptr, U, Omega, E, nullptr, cuda_stream, "far_mobility_apply");
+}
+
 extern "C" se_status far_mobility_apply_compressible(se_plan *p, const double *pos, const double *F, const double *T,
                                                      const double *S, const double *s_in, double *U, double *Omega,
                                                      double *E, double *s_out, void *cuda_stream)
 {
-    if (!p) return SE_ERR_INVALID_ARG;
-    if (s_in || s_out) return fail(p, SE_ERR_UNSUPPORTED, "far_mobility_apply_compressible", "pressure moments not built yet");
-    return far_mobility_apply(p, pos, F, T, S, U, Omega, E, cuda_stream);
+    return apply_impl(p, pos, F, T, S, s_in, U, Omega, E, s_out, cuda_stream, "far_mobility_apply_compressible");
 }
 
 extern "C" se_status far_mobility_apply_host(se_plan *p, const double *pos, const double *F, const double *T,
@@ -533,8 +602,13 @@ extern "C" se_status far_mobility_apply_host(se_plan *p, const double *pos, cons
 
 extern "C" se_status se_plan_copy_grids(se_plan *p, int which, double *dst)
 {
-    if (!p || !dst || which < 0 || which > 1) return SE_ERR_INVALID_ARG;
+    if (!p || !dst || which < 0 || which > 2) return SE_ERR_INVALID_ARG;
     const size_t G = (size_t)p->c.M * p->c.M * p->c.M;
+    if (which == 2) {
+        if (!p->have_comp) return fail(p, SE_ERR_INVALID_ARG, "se_plan_copy_grids", "no compressible apply was made");
+        CUDA_TRY(p, cudaMemcpy(dst, p->d_real_p, sizeof(double) * G, cudaMemcpyDeviceToHost));
+        return SE_OK;
+    }
     CUDA_TRY(p, cudaMemcpy(dst, p->d_real, sizeof(double) * (which == 0 ? 3 : 6) * G, cudaMemcpyDeviceToHost));
     return SE_OK;
 }

@@ -16,16 +16,23 @@
 //        a2 = L2/4                                                     [ET: (cSi,0)]
 //        a3 = -(L2/2 - 2 Ps3), a4 = -(L1 - 2 Ps2), beta += Ps4 (x.S.x), kappa += Ps3 (x.S.x)   [ES: (cSi,cSj)]
 // with x = r_i - r_j (minimum image), k0 = 1/(8 pi eta0).
+//
+// Compressible extension (a9; Eq. 24-34), template flag COMP: with chi = erfc(xi r)/r (so that
+// chi_n = Phi_{n+1}) and lap chi = 2 xi^2 q g, q_n(c) = chi_n + c (lap chi)_n:
+//   U  += -(k0/2) q_1(cFi) s_j x                                   [U <- s, psi_R = -chi/(16 pi eta0)]
+//   E  += -(k0/2) s_j [ q_2(cSi) x x + q_1(cSi) I ], trace removed  [E <- s]
+//   p   = (1/4pi) [ q_2(cSj) (x.S.x) - q_1(cFj) (x.F) ]            [p <- F, p <- S; Eq. 29-31]
 #pragma once
 #include "se_common.cuh"
 
 #define REAL_WARPS 4
 #define REAL_QCAP 64
 
-// acc[0..2] U, [3..5] Omega, [6..10] E (xx,xy,xz,yy,yz); everything still to be multiplied by k0.
+// acc[0..2] U, [3..5] Omega, [6..10] E (xx,xy,xz,yy,yz), still to be multiplied by k0; acc[11] pressure p (COMP).
+template <bool COMP>
 __device__ __forceinline__ void pair_real(const SeConst &c, double x, double y, double z, double r2,
                                           double cFi, double cSi, double aj, const double *__restrict__ mj,
-                                          double acc[11])
+                                          double acc[12])
 {
     const double cFj = aj * aj * (1.0 / 6.0), cSj = aj * aj * 0.1;
     const double r = sqrt(r2), ir = 1.0 / r, ir2 = ir * ir;
@@ -101,6 +108,21 @@ __device__ __forceinline__ void pair_real(const SeConst &c, double x, double y, 
     acc[8] += x * w2 + z * w0 + a4 * Sxz + beta * x * z;
     acc[9] += 2.0 * y * w1 + a4 * Syy + beta * y * y + kappa;
     acc[10] += y * w2 + z * w1 + a4 * Syz + beta * y * z;
+    if (COMP) {
+        const double sj = mj[11];
+        const double L0c = 2.0 * c.x2 * qg, L1c = -4.0 * c.x4 * qg, L2c = 8.0 * c.x6 * qg;   // (lap chi)_n
+        const double us = -0.5 * (P2 + cFi * L1c) * sj;
+        acc[0] += us * x; acc[1] += us * y; acc[2] += us * z;
+        const double e1 = -0.5 * (P2 + cSi * L1c) * sj, e2 = -0.5 * (P3 + cSi * L2c) * sj;
+        const double tr3 = (3.0 * e1 + e2 * r2) * (1.0 / 3.0);
+        acc[6] += e2 * x * x + e1 - tr3;
+        acc[7] += e2 * x * y;
+        acc[8] += e2 * x * z;
+        acc[9] += e2 * y * y + e1 - tr3;
+        acc[10] += e2 * y * z;
+        acc[11] += 0.07957747154594767 * ((P3 + cSj * L2c) * xSx - (P2 + cFj * L1c) * xF);   // 1/(4 pi)
+        (void)L0c;
+    }
 }
 
 // One CTA per real-space cell (or, when the box holds fewer than 3 cells per axis, per slice of all
@@ -111,6 +133,7 @@ __device__ __forceinline__ void pair_real(const SeConst &c, double x, double y, 
 // Minimum image as in the oracle, x = d - L rint(d/L), with d/L formed as d * (1/L).
 #define REAL_STAGE 1024
 
+template <bool COMP>
 __global__ void __launch_bounds__(REAL_WARPS * 32) k_real(SeConst c, const double4 *__restrict__ rs_pos,
                                                           const double *__restrict__ rs_mom, const int *__restrict__ rs_orig,
                                                           const int *__restrict__ start_r, double *__restrict__ out_real)
@@ -175,9 +198,10 @@ __global__ void __launch_bounds__(REAL_WARPS * 32) k_real(SeConst c, const doubl
             if (i >= t1) break;
             const double4 pi = rs_pos[i];
             const double cFi = pi.w * pi.w * (1.0 / 6.0), cSi = pi.w * pi.w * 0.1;
-            double acc[11];
+            constexpr int NA = COMP ? 12 : 11;
+            double acc[12];
 #pragma unroll
-            for (int k = 0; k < 11; ++k) acc[k] = 0.0;
+            for (int k = 0; k < 12; ++k) acc[k] = 0.0;
             int qn = 0;
             for (int qb = 0; qb < nst; qb += 32) {
                 const int q = qb + lane;
@@ -204,31 +228,32 @@ __global__ void __launch_bounds__(REAL_WARPS * 32) k_real(SeConst c, const doubl
                 if (qn >= 32) {
                     const double4 d = qd[wl][qn - 32 + lane];
                     const int jj = qj[wl][qn - 32 + lane];
-                    pair_real(c, d.x, d.y, d.z, d.x * d.x + d.y * d.y + d.z * d.z, cFi, cSi, d.w, rs_mom + 12 * (size_t)jj, acc);
+                    pair_real<COMP>(c, d.x, d.y, d.z, d.x * d.x + d.y * d.y + d.z * d.z, cFi, cSi, d.w, rs_mom + 12 * (size_t)jj, acc);
                     qn -= 32;
                     __syncwarp();
                 }
             }
             if (lane < qn) {
                 const double4 d = qd[wl][lane];
-                pair_real(c, d.x, d.y, d.z, d.x * d.x + d.y * d.y + d.z * d.z, cFi, cSi, d.w, rs_mom + 12 * (size_t)qj[wl][lane], acc);
+                pair_real<COMP>(c, d.x, d.y, d.z, d.x * d.x + d.y * d.y + d.z * d.z, cFi, cSi, d.w, rs_mom + 12 * (size_t)qj[wl][lane], acc);
             }
             __syncwarp();
 #pragma unroll
-            for (int k = 0; k < 11; ++k) {
+            for (int k = 0; k < NA; ++k) {
                 double v = acc[k];
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
                 acc[k] = v;
             }
             if (lane == 0) {
-                double *o = out_real + 11 * (size_t)rs_orig[i];
+                double *o = out_real + 12 * (size_t)rs_orig[i];
+                if (COMP) acc[11] *= 1.0 / c.k0;                  // p carries its own prefactor
                 if (base == 0) {
 #pragma unroll
-                    for (int k = 0; k < 11; ++k) o[k] = c.k0 * acc[k];
+                    for (int k = 0; k < NA; ++k) o[k] = c.k0 * acc[k];
                 } else {
 #pragma unroll
-                    for (int k = 0; k < 11; ++k) o[k] += c.k0 * acc[k];
+                    for (int k = 0; k < NA; ++k) o[k] += c.k0 * acc[k];
                 }
             }
         }

@@ -118,6 +118,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_add(int *__restrict__ out
 // fast Gaussian gridding, Eq. 47, is replaced by P direct exponentials per axis, done once here).
 __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const double *__restrict__ radii,
                           const double *__restrict__ F, const double *__restrict__ T, const double *__restrict__ S,
+                          const double *__restrict__ s_in,      // pressure moments (a9) or NULL
                           const int *__restrict__ key_r, const int *__restrict__ rank_r, const int *__restrict__ start_r,
                           const int *__restrict__ key_s, const int *__restrict__ rank_s, const int *__restrict__ start_s,
                           const int *__restrict__ key_g, const int *__restrict__ rank_g, const int *__restrict__ start_g,
@@ -139,7 +140,8 @@ __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const doubl
     rs_pos[dr] = make_double4(xw[0], xw[1], xw[2], a);
     double *m = rs_mom + 12 * (size_t)dr;
     m[0] = f[0]; m[1] = f[1]; m[2] = f[2]; m[3] = t[0]; m[4] = t[1]; m[5] = t[2];
-    m[6] = s[0]; m[7] = s[1]; m[8] = s[2]; m[9] = s[3]; m[10] = s[4]; m[11] = 0.0;
+    const double sp = s_in ? s_in[i] : 0.0;
+    m[6] = s[0]; m[7] = s[1]; m[8] = s[2]; m[9] = s[3]; m[10] = s[4]; m[11] = sp;
     rs_orig[dr] = i;
 
     // spreading / gather record
@@ -178,5 +180,5 @@ __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const doubl
     r[REC_T] = t[0]; r[REC_T + 1] = t[1]; r[REC_T + 2] = t[2];
     r[REC_S] = s[0]; r[REC_S + 1] = s[1]; r[REC_S + 2] = s[2]; r[REC_S + 3] = s[3]; r[REC_S + 4] = s[4];
     r[REC_S + 5] = -(s[0] + s[3]);
-    r[REC_CF] = cF; r[REC_CS] = cS; r[REC_A] = a;
+    r[REC_CF] = cF; r[REC_CS] = cS; r[REC_SP] = sp;
 }

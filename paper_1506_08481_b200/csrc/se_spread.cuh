@@ -15,9 +15,11 @@
 #pragma once
 #include "se_sweep.cuh"
 
-template <int P>
+// NC = 3: the three force-density grids; NC = 4: plus the scalar grid of the pressure moments (a9),
+// Hs(x_n) = sum_j gamma(d) s_j, one more FMA per grid point.
+template <int P, int NC>
 __device__ __forceinline__ void spread_hit(const SeConst &c, const double *__restrict__ rec, int y, int z, bool active,
-                                           double (&acc)[P][3])
+                                           double (&acc)[P][NC])
 {
     const int M = c.M;
     const int2 yz = *reinterpret_cast<const int2 *>(rec);
@@ -63,13 +65,15 @@ __device__ __forceinline__ void spread_hit(const SeConst &c, const double *__res
                 t = fma(x2, c2[a], t);
                 acc[k][a] = fma(x3, c3[a], t);
             }
+            if (NC == 4) acc[k][NC - 1] = fma(x0, gyz * rec[REC_SP], acc[k][NC - 1]);
         }
     }
 }
 
-template <int P>
-__global__ void __launch_bounds__(SWEEP_WARPS * 32, SWEEP_MIN_BLOCKS) k_spread(SeConst c, const double *__restrict__ recs,
-                                                              const int *__restrict__ start_s, double *__restrict__ H)
+template <int P, int NC>
+__global__ void __launch_bounds__(SWEEP_WARPS * 32, NC == 3 ? SWEEP_MIN_BLOCKS : 2) k_spread(SeConst c, const double *__restrict__ recs,
+                                                              const int *__restrict__ start_s, double *__restrict__ H,
+                                                              double *__restrict__ Hs)
 {
     extern __shared__ __align__(16) unsigned char sweep_smem[];
     const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
@@ -95,9 +99,11 @@ __global__ void __launch_bounds__(SWEEP_WARPS * 32, SWEEP_MIN_BLOCKS) k_spread(S
 
     const SweepRanges rg = sweep_ranges<P>(c, Y0, Z0, lane);
 
-    double acc[P][3];
+    double acc[P][NC];
 #pragma unroll
-    for (int k = 0; k < P; ++k) { acc[k][0] = 0.0; acc[k][1] = 0.0; acc[k][2] = 0.0; }
+    for (int k = 0; k < P; ++k)
+#pragma unroll
+        for (int a = 0; a < NC; ++a) acc[k][a] = 0.0;
 
     const int seg_start = seg * c.seg_len, seg_end = min(seg_start + c.seg_len, M);
     const size_t G = (size_t)M * M * M;
@@ -120,10 +126,10 @@ __global__ void __launch_bounds__(SWEEP_WARPS * 32, SWEEP_MIN_BLOCKS) k_spread(S
             parity ^= 1u << buf;
             const double *__restrict__ sl = buf ? slot1 : slot0;
             const int ns = min(cur.n, SWEEP_CAP);
-            for (int ci = 0; ci < ns; ++ci) spread_hit<P>(c, sl + (size_t)ci * stride, y, z, active, acc);
+            for (int ci = 0; ci < ns; ++ci) spread_hit<P, NC>(c, sl + (size_t)ci * stride, y, z, active, acc);
             for (int ci = SWEEP_CAP; ci < cur.n; ++ci) {
                 const int j = sweep_overflow_index(cur, ci);
-                spread_hit<P>(c, recs + (size_t)j * stride, y, z, active, acc);
+                spread_hit<P, NC>(c, recs + (size_t)j * stride, y, z, active, acc);
             }
             __syncwarp();                           // slot fully read before it is refilled
         }
@@ -132,10 +138,14 @@ __global__ void __launch_bounds__(SWEEP_WARPS * 32, SWEEP_MIN_BLOCKS) k_spread(S
             H[idx] = acc[0][0];
             H[G + idx] = acc[0][1];
             H[2 * G + idx] = acc[0][2];
+            if (NC == 4) Hs[idx] = acc[0][NC - 1];
         }
 #pragma unroll
-        for (int k = 0; k < P - 1; ++k) { acc[k][0] = acc[k + 1][0]; acc[k][1] = acc[k + 1][1]; acc[k][2] = acc[k + 1][2]; }
-        acc[P - 1][0] = 0.0; acc[P - 1][1] = 0.0; acc[P - 1][2] = 0.0;
+        for (int k = 0; k < P - 1; ++k)
+#pragma unroll
+            for (int a = 0; a < NC; ++a) acc[k][a] = acc[k + 1][a];
+#pragma unroll
+        for (int a = 0; a < NC; ++a) acc[P - 1][a] = 0.0;
         cur = nxt;
     }
 }

@@ -245,3 +245,85 @@ def test_overlapping_and_coincident_particles(pk, oracle, workloads):
     wl.pos[3] = wl.pos[2]                                   # coincident
     r = Runner(pk, wl)
     _check_blocks(r.run(), r.oracle(oracle), TOL)
+
+
+# ------------------------------------------------------------------------------------------------
+# T11: compressible extension (a9): pressure moments in, pressure interaction out
+# ------------------------------------------------------------------------------------------------
+def _pressure_moments(wl, seed=11):
+    return np.random.default_rng([150608481, seed]).standard_normal(wl.N)
+
+
+@pytest.mark.parametrize("name", ["c1", "c2", "c3"])
+def test_compressible_extension_stage_and_full_parity(pk, oracle, workloads, name):
+    import torch
+    wl = workloads.make_workload(name)
+    r = Runner(pk, wl)
+    s_np = _pressure_moments(wl)
+    s_in = torch.tensor(s_np, device=r.pos.device, dtype=torch.float64)
+    s_out = torch.full((wl.N,), float("nan"), device=r.pos.device, dtype=torch.float64)
+
+    def run(flags=0, stop=-1, sin=s_in, sout=s_out):
+        r.plan.set_flags(flags)
+        r.plan.debug_stop(stop)
+        r.plan.apply_compressible(r.pos, r.F, r.T, r.S, sin, r.U, r.W, r.E, sout)
+        torch.cuda.synchronize()
+        return r.U.cpu().numpy(), r.W.cpu().numpy(), r.E.cpu().numpy(), (None if sout is None else sout.cpu().numpy())
+
+    def ref(parts, **kw):
+        return oracle.o2_apply(wl.pos, wl.radii, wl.L, wl.xi, wl.rc, wl.M, wl.P, wl.F, wl.T, wl.S, s=s_np, parts=parts, **kw)
+
+    full = ref(oracle.PART_ALL, want_grids=True)
+    # real-space part alone: U<-s, E<-s, p<-F, p<-S
+    got = run(flags=pk.SE_SKIP_WAVE | pk.SE_SKIP_SELF | pk.SE_SKIP_ONEBODY)
+    rr = ref(oracle.PART_REAL)
+    _check_blocks(got[:3], rr, TOL_STAGE)
+    assert _rel(got[3], rr["s_out"]) <= TOL_STAGE
+    # scalar spread grid, returned pressure grid
+    run(stop=2)
+    assert _rel(r.plan.copy_grids(2)[0], full["gridH"][3]) <= TOL_STAGE
+    assert _rel(r.plan.copy_grids(0), full["gridH"][:3]) <= TOL_STAGE
+    run(stop=5)
+    assert _rel(r.plan.copy_grids(2)[0], full["gridOut"][6]) <= TOL_STAGE
+    Gr = r.plan.copy_grids(1)
+    for g in range(6):
+        assert _rel(Gr[g], full["gridOut"][g]) <= TOL_STAGE, g
+    # wave part alone
+    got = run(flags=pk.SE_SKIP_REAL | pk.SE_SKIP_SELF | pk.SE_SKIP_ONEBODY)
+    rw = ref(oracle.PART_WAVE)
+    _check_blocks(got[:3], rw, TOL_STAGE)
+    assert _rel(got[3], rw["s_out"]) <= TOL_STAGE
+    # full product
+    got = run()
+    _check_blocks(got[:3], full, TOL)
+    assert _rel(got[3], full["s_out"]) <= TOL
+    # the pressure moments really change U and E (the test is not vacuous); Omega only at the SE-error level
+    # (grad psi is curl-free, Eq. 26; the gathered curl of the discretised field is not exactly zero)
+    plain = r.oracle(oracle)
+    assert _rel(got[0], plain["U"]) > 1e-3 and _rel(got[2], plain["E"]) > 1e-3
+    assert _rel(got[1], plain["Omega"]) < 1e-3
+    # s_in only / s_out only / neither
+    got = run(sout=None)
+    _check_blocks(got[:3], full, TOL)
+    got = run(sin=None)
+    _check_blocks(got[:3], plain, TOL)
+    p_only = oracle.o2_apply(wl.pos, wl.radii, wl.L, wl.xi, wl.rc, wl.M, wl.P, wl.F, wl.T, wl.S, s=np.zeros(wl.N))
+    assert _rel(got[3], p_only["s_out"]) <= TOL
+    got = run(sin=None, sout=None)
+    _check_blocks(got[:3], plain, TOL)
+    # the plain entry point still gives the plain product after compressible applies
+    _check_blocks(r.run(), plain, TOL)
+
+
+def test_compressible_extension_full_size_c4(pk, oracle, workloads):
+    import torch
+    wl = workloads.make_workload("c4")
+    r = Runner(pk, wl)
+    s_np = _pressure_moments(wl)
+    s_in = torch.tensor(s_np, device=r.pos.device, dtype=torch.float64)
+    s_out = torch.empty((wl.N,), device=r.pos.device, dtype=torch.float64)
+    r.plan.apply_compressible(r.pos, r.F, r.T, r.S, s_in, r.U, r.W, r.E, s_out)
+    torch.cuda.synchronize()
+    ref = oracle.o2_apply(wl.pos, wl.radii, wl.L, wl.xi, wl.rc, wl.M, wl.P, wl.F, wl.T, wl.S, s=s_np)
+    _check_blocks((r.U.cpu().numpy(), r.W.cpu().numpy(), r.E.cpu().numpy()), ref, TOL)
+    assert _rel(s_out.cpu().numpy(), ref["s_out"]) <= TOL
