@@ -300,7 +300,8 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
         cudaStreamDestroy(p->side); cudaEventDestroy(p->ev_fork); se_plan_destroy(p); return SE_ERR_CUDA;
     }
     p->have_side = true;
-    if (dispatch_prepare(P, sweep_smem_bytes(c.rec_stride), p->gather_smem) != cudaSuccess) { cudaGetLastError(); se_plan_destroy(p); return SE_ERR_CUDA; }
+    if (cudaFuncSetAttribute(k_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)scatter_smem_bytes(c.rec_stride)) != cudaSuccess ||
+        dispatch_prepare(P, sweep_smem_bytes(c.rec_stride), p->gather_smem) != cudaSuccess) { cudaGetLastError(); se_plan_destroy(p); return SE_ERR_CUDA; }
     *out = p;
     return SE_OK;
 }
@@ -478,7 +479,7 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     p->last_launches += 1;
     se_status st = scan_cells(p, s);
     if (st != SE_OK) return st;
-    k_scatter<<<nbN, TB, 0, s>>>(c, pos, p->d_radii, F, T, S, s_in, p->d_key_r, p->d_rank_r, p->d_start_r,
+    k_scatter<<<(c.N + SCATTER_THREADS - 1) / SCATTER_THREADS, SCATTER_THREADS, scatter_smem_bytes(c.rec_stride), s>>>(c, pos, p->d_radii, F, T, S, s_in, p->d_key_r, p->d_rank_r, p->d_start_r,
                                  p->d_key_s, p->d_rank_s, p->d_start_s, p->d_key_g, p->d_rank_g, p->d_start_g, p->d_gperm, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig, p->d_recs);
     p->last_launches += 1;
     CUDA_TRY(p, cudaGetLastError());

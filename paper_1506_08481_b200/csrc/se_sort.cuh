@@ -113,6 +113,9 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_add(int *__restrict__ out
     }
 }
 
+#define SCATTER_THREADS 64
+// Records are built in shared memory (one row per thread, odd row pitch) and copied out by whole warps,
+// rec_stride contiguous doubles at a time: per-thread stores of 480-byte records were the whole cost of a1.
 // One thread per particle: write the real-space packed copy (cell order) and the spreading/gather
 // record (tile order) with the per-axis Gaussian tables (Eq. 41 in physical coordinates; the paper's
 // fast Gaussian gridding, Eq. 47, is replaced by P direct exponentials per axis, done once here).
@@ -125,8 +128,12 @@ __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const doubl
                           int *__restrict__ gperm, double4 *__restrict__ rs_pos, double *__restrict__ rs_mom, int *__restrict__ rs_orig,
                           double *__restrict__ recs)
 {
+    extern __shared__ __align__(16) double sc_rows[];          // [SCATTER_THREADS][rec_stride + 1] then int dst[]
+    const int pitch = c.rec_stride + 1;
+    int *sc_dst = reinterpret_cast<int *>(sc_rows + SCATTER_THREADS * pitch);
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= c.N) return;
+    sc_dst[threadIdx.x] = -1;
+    if (i < c.N) {
     const size_t i3 = 3 * (size_t)i, i5 = 5 * (size_t)i;
     const double a = radii[i];
     double xw[3];
@@ -147,7 +154,8 @@ __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const doubl
     // spreading / gather record
     const int ds = start_s[key_s[i]] + rank_s[i];
     gperm[start_g[key_g[i]] + rank_g[i]] = ds;               // gather order -> record
-    double *r = recs + (size_t)ds * c.rec_stride;
+    double *r = sc_rows + threadIdx.x * pitch;
+    sc_dst[threadIdx.x] = ds;
     int n0w[3];
     double d0[3];
     const double cF = a * a / 6.0, cS = a * a / 10.0, al = c.alpha;
@@ -169,8 +177,8 @@ __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const doubl
             }
         }
     }
-    reinterpret_cast<int2 *>(r)[0] = make_int2(n0w[1], n0w[2]);
-    reinterpret_cast<int2 *>(r)[1] = make_int2(n0w[0], i);
+    r[0] = __longlong_as_double(((long long)(unsigned)n0w[2] << 32) | (unsigned)n0w[1]);     // int2 (y0w, z0w)
+    r[1] = __longlong_as_double(((long long)(unsigned)i << 32) | (unsigned)n0w[0]);          // int2 (x0w, orig)
     r[REC_D0] = d0[0]; r[REC_D0 + 1] = d0[1]; r[REC_D0 + 2] = d0[2];
     r[REC_POLY] = 1.0 - 6.0 * al * cF;
     r[REC_POLY + 1] = 4.0 * al * al * cF;
@@ -181,4 +189,19 @@ __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const doubl
     r[REC_S] = s[0]; r[REC_S + 1] = s[1]; r[REC_S + 2] = s[2]; r[REC_S + 3] = s[3]; r[REC_S + 4] = s[4];
     r[REC_S + 5] = -(s[0] + s[3]);
     r[REC_CF] = cF; r[REC_CS] = cS; r[REC_SP] = sp;
+    }
+    __syncthreads();
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    for (int rr = w; rr < SCATTER_THREADS; rr += SCATTER_THREADS / 32) {
+        const int ds = sc_dst[rr];
+        if (ds < 0) continue;
+        const double *__restrict__ src = sc_rows + rr * pitch;
+        double *__restrict__ dst = recs + (size_t)ds * c.rec_stride;
+        for (int q = lane; q < c.rec_stride; q += 32) dst[q] = src[q];
+    }
+}
+
+static inline size_t scatter_smem_bytes(int rec_stride)
+{
+    return (size_t)SCATTER_THREADS * (rec_stride + 1) * 8 + SCATTER_THREADS * 4;
 }
