@@ -45,15 +45,20 @@ typedef enum {
 #define SE_SKIP_SELF     0x4u         /* do not subtract the wave-space self terms (Eq. 37)           */
 #define SE_SKIP_ONEBODY  0x8u         /* do not add the one-body Faxen terms (Eq. 13-15)              */
 #define SE_TIMING        0x10u        /* record CUDA events between stages (se_plan_get_timings)      */
+#define SE_FUSED_X       0x20u        /* opt-in variant of a4-a6 for power-of-two 32 <= M <= 512 (ignored otherwise and
+                                         by the compressible entry point): batched 2-D (y,z) cuFFT transforms and ONE
+                                         kernel doing the x transform, the k-space pass and the inverse x transform in a
+                                         single pass over HBM, instead of 3-D cuFFT + k-space kernel + 3-D cuFFT.  Same
+                                         results to FFT round-off; measured slower on B200 so far       */
 
 /* stage indices of se_plan_get_timings */
 enum {
     SE_STAGE_SORT = 0,                /* a1: wrap, counting sorts by real-space cell and grid tile, packing */
     SE_STAGE_REAL = 1,                /* a2: real-space pair sum                                      */
     SE_STAGE_SPREAD = 2,              /* a3: Gaussian spreading onto the grid                         */
-    SE_STAGE_FFT_FWD = 3,             /* a4: forward FFTs (cuFFT)                                     */
-    SE_STAGE_KSPACE = 4,              /* a5: fused k-space scaling                                    */
-    SE_STAGE_FFT_INV = 5,             /* a6: inverse FFTs (cuFFT)                                     */
+    SE_STAGE_FFT_FWD = 3,             /* a4: forward FFTs (cuFFT; on the fused path the 2-D (y,z) part) */
+    SE_STAGE_KSPACE = 4,              /* a5: fused k-space scaling (on the fused path with both x transforms) */
+    SE_STAGE_FFT_INV = 5,             /* a6: inverse FFTs (cuFFT; on the fused path the 2-D (y,z) part) */
     SE_STAGE_GATHER = 6,              /* a7: Gaussian gather                                          */
     SE_STAGE_EPILOGUE = 7,            /* a8: self / one-body terms, sum, un-permute                   */
     SE_NUM_STAGES = 8

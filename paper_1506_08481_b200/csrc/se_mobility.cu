@@ -14,6 +14,7 @@
 #include "se_real.cuh"
 #include "se_spread.cuh"
 #include "se_kspace.cuh"
+#include "se_xfft.cuh"
 #include "se_gather.cuh"
 
 #ifndef M_PI
@@ -58,8 +59,12 @@ struct se_plan {
     double *d_moments;             // [N][24] gathered wave-space sums in caller order
     // host-API staging
     double *d_io;                  // pos3 F3 T3 S5 U3 W3 E5 = 25 N doubles
-    cufftHandle fft_fwd, fft_inv;
+    cufftHandle fft_fwd, fft_inv;  // 3-D batched plans (unfused path), made when first needed
     bool have_fwd, have_inv;
+    cufftHandle fft2_fwd, fft2_inv; // 2-D batched plans of the fused path (se_xfft.cuh)
+    bool have_xf;
+    int lM;
+    double2 *d_wtab;               // exp(-2 pi i q / M), q < M
     size_t fft_bytes;
     cudaEvent_t ev[SE_NUM_STAGES + 1];
     bool have_events, timed;
@@ -208,11 +213,79 @@ extern "C" se_status se_plan_destroy(se_plan *p)
         cudaFree(p->d_real_p); cudaFree(p->d_Hk_s); cudaFree(p->d_Gk_p); cudaFree(p->d_pmom);
         cufftDestroy(p->fft_fwd1); cufftDestroy(p->fft_inv1);
     }
+    if (p->have_xf) { cufftDestroy(p->fft2_fwd); cufftDestroy(p->fft2_inv); }
+    cudaFree(p->d_wtab);
     if (p->have_fwd) cufftDestroy(p->fft_fwd);
     if (p->have_inv) cufftDestroy(p->fft_inv);
     if (p->have_events) for (int k = 0; k <= SE_NUM_STAGES; ++k) cudaEventDestroy(p->ev[k]);
     cudaGetLastError();
     free(p);
+    return SE_OK;
+}
+
+// Batched 3-D cuFFT plans of the unfused path: D2Z (3 grids) and Z2D (6 grids), out of place, contiguous batches.
+static se_status ensure_fft3d(se_plan *p)
+{
+    if (p->have_fwd && p->have_inv) return SE_OK;
+    const int M = p->c.M;
+    int n3[3] = { M, M, M };
+    size_t ws = 0, tot = 0;
+    cufftResult r = CUFFT_SUCCESS;
+    if (!p->have_fwd) {
+        r = cufftCreate(&p->fft_fwd);
+        if (r == CUFFT_SUCCESS) { p->have_fwd = true; r = cufftMakePlanMany(p->fft_fwd, 3, n3, NULL, 1, 0, NULL, 1, 0, CUFFT_D2Z, 3, &ws); tot += ws; }
+    }
+    if (r == CUFFT_SUCCESS && !p->have_inv) {
+        r = cufftCreate(&p->fft_inv);
+        if (r == CUFFT_SUCCESS) { p->have_inv = true; r = cufftMakePlanMany(p->fft_inv, 3, n3, NULL, 1, 0, NULL, 1, 0, CUFFT_Z2D, 6, &ws); tot += ws; }
+    }
+    if (r != CUFFT_SUCCESS) {
+        if (p->have_fwd) { cufftDestroy(p->fft_fwd); p->have_fwd = false; }
+        if (p->have_inv) { cufftDestroy(p->fft_inv); p->have_inv = false; }
+        return fail(p, r == CUFFT_ALLOC_FAILED ? SE_ERR_ALLOC : SE_ERR_CUFFT, "cufftMakePlanMany", "3-D plans");
+    }
+    p->fft_bytes += tot;
+    p->bytes += tot;
+    return SE_OK;
+}
+
+// Plans and twiddle table of the fused path (se_xfft.cuh): batched 2-D (y,z) transforms, 3M forward and 6M inverse
+// planes; the x transforms run inside k_xfused.
+static se_status ensure_xf(se_plan *p)
+{
+    if (p->have_xf) return SE_OK;
+    const int M = p->c.M;
+    int n2[2] = { M, M };
+    size_t ws = 0, tot = 0;
+    cufftResult r = cufftCreate(&p->fft2_fwd);
+    bool c1 = (r == CUFFT_SUCCESS), c2 = false;
+    if (c1) { r = cufftMakePlanMany(p->fft2_fwd, 2, n2, NULL, 1, 0, NULL, 1, 0, CUFFT_D2Z, 3 * M, &ws); tot += ws; }
+    if (r == CUFFT_SUCCESS) { r = cufftCreate(&p->fft2_inv); c2 = (r == CUFFT_SUCCESS); }
+    if (r == CUFFT_SUCCESS) { r = cufftMakePlanMany(p->fft2_inv, 2, n2, NULL, 1, 0, NULL, 1, 0, CUFFT_Z2D, 6 * M, &ws); tot += ws; }
+    double2 *wt = (double2 *)malloc(sizeof(double2) * (size_t)M);
+    se_status st = SE_OK;
+    if (r != CUFFT_SUCCESS) st = fail(p, r == CUFFT_ALLOC_FAILED ? SE_ERR_ALLOC : SE_ERR_CUFFT, "cufftMakePlanMany", "2-D plans");
+    if (st == SE_OK && !wt) st = fail(p, SE_ERR_ALLOC, "malloc", "twiddle table");
+    if (st == SE_OK && !p->d_wtab) st = dev_alloc(p, &p->d_wtab, (size_t)M);
+    if (st == SE_OK) {
+        for (int q = 0; q < M; ++q) { const double a = 2.0 * M_PI * q / M; wt[q].x = cos(a); wt[q].y = -sin(a); }
+        if (cudaMemcpy(p->d_wtab, wt, sizeof(double2) * (size_t)M, cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaFuncSetAttribute(k_xfused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)xf_smem_bytes(M)) != cudaSuccess) {
+            cudaGetLastError();
+            st = fail(p, SE_ERR_CUDA, "ensure_xf", "twiddle table / shared-memory attribute");
+        }
+    }
+    free(wt);
+    if (st != SE_OK) {
+        if (c1) cufftDestroy(p->fft2_fwd);
+        if (c2) cufftDestroy(p->fft2_inv);
+        return st;
+    }
+    p->have_xf = true;
+    p->lM = 0;
+    while ((1 << p->lM) < M) ++p->lM;
+    p->fft_bytes += tot;
+    p->bytes += tot;
     return SE_OK;
 }
 
@@ -279,15 +352,12 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
         return SE_ERR_CUDA;
     }
 
-    // cuFFT: batched D2Z (3 grids) and Z2D (6 grids), out of place, contiguous batches
-    int n3[3] = { M, M, M };
-    size_t ws = 0;
-    cufftResult r = cufftCreate(&p->fft_fwd);
-    if (r == CUFFT_SUCCESS) { p->have_fwd = true; r = cufftMakePlanMany(p->fft_fwd, 3, n3, NULL, 1, 0, NULL, 1, 0, CUFFT_D2Z, 3, &ws); p->fft_bytes += ws; }
-    if (r == CUFFT_SUCCESS) r = cufftCreate(&p->fft_inv);
-    if (r == CUFFT_SUCCESS) { p->have_inv = true; r = cufftMakePlanMany(p->fft_inv, 3, n3, NULL, 1, 0, NULL, 1, 0, CUFFT_Z2D, 6, &ws); p->fft_bytes += ws; }
-    if (r != CUFFT_SUCCESS) { se_plan_destroy(p); return r == CUFFT_ALLOC_FAILED ? SE_ERR_ALLOC : SE_ERR_CUFFT; }
-    p->bytes += p->fft_bytes;
+    // cuFFT: batched 3-D transforms (the default a4 / a6).  The plans of the opt-in fused path (SE_FUSED_X) are
+    // made by the first apply that asks for it.
+    {
+        const se_status stf = ensure_fft3d(p);
+        if (stf != SE_OK) { se_plan_destroy(p); return stf; }
+    }
 
     for (int k = 0; k <= SE_NUM_STAGES; ++k)
         if (cudaEventCreate(&p->ev[k]) != cudaSuccess) { p->have_events = (k > 0); se_plan_destroy(p); return SE_ERR_CUDA; }
@@ -323,7 +393,7 @@ extern "C" se_status se_plan_set_tuning(se_plan *p, int spread_segments, int gat
 
 extern "C" se_status se_plan_set_flags(se_plan *p, unsigned flags)
 {
-    if (!p || (flags & ~0x1fu)) return SE_ERR_INVALID_ARG;
+    if (!p || (flags & ~0x3fu)) return SE_ERR_INVALID_ARG;
     p->flags = flags;
     return SE_OK;
 }
@@ -458,6 +528,9 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     if (!pos || !F || !T || !S || !U || !Omega || !E) return fail(p, SE_ERR_INVALID_ARG, who, "null pointer");
     const bool comp_in = s_in != nullptr, comp_out = s_out != nullptr, comp = comp_in || comp_out;
     if (comp) { se_status stc = ensure_compressible(p); if (stc != SE_OK) return stc; }
+    // opt-in: 2-D cuFFT + fused x-transform / k-space / x-transform kernel (se_xfft.cuh)
+    const bool use_xf = (p->flags & SE_FUSED_X) && xf_supported(p->c.M) && !comp;
+    if (use_xf) { se_status stf = ensure_xf(p); if (stf != SE_OK) return stf; }
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const SeConst &c = p->c;
     const unsigned fl = p->flags;
@@ -516,7 +589,10 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
         CUDA_TRY(p, cudaGetLastError());
     }
     MARK();
-    if (on(SE_STAGE_FFT_FWD)) {
+    if (on(SE_STAGE_FFT_FWD) && use_xf) {
+        CUFFT_TRY(p, cufftSetStream(p->fft2_fwd, s));
+        CUFFT_TRY(p, cufftExecD2Z(p->fft2_fwd, p->d_real, (cufftDoubleComplex *)p->d_Hk));
+    } else if (on(SE_STAGE_FFT_FWD)) {
         CUFFT_TRY(p, cufftSetStream(p->fft_fwd, s));
         CUFFT_TRY(p, cufftExecD2Z(p->fft_fwd, p->d_real, (cufftDoubleComplex *)p->d_Hk));
         if (comp_in) {
@@ -525,7 +601,12 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
         }
     }
     MARK();
-    if (on(SE_STAGE_KSPACE)) {
+    if (on(SE_STAGE_KSPACE) && use_xf) {
+        const unsigned nb = (unsigned)((size_t)c.M * (c.M / 2 + 1) / (XF_ELEMS / c.M));
+        k_xfused<<<nb, XF_THREADS, xf_smem_bytes(c.M), s>>>(c, p->lM, p->d_Hk, p->d_Gk, p->d_wtab);
+        p->last_launches += 1;
+        CUDA_TRY(p, cudaGetLastError());
+    } else if (on(SE_STAGE_KSPACE)) {
         const size_t Gc = (size_t)c.M * c.M * (c.M / 2 + 1);
         k_kspace<<<(unsigned)((Gc + KSPACE_THREADS - 1) / KSPACE_THREADS), KSPACE_THREADS, 0, s>>>(c, p->d_Hk, p->d_Gk,
                                                                                                    comp_in ? p->d_Hk_s : nullptr,
@@ -534,7 +615,10 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
         CUDA_TRY(p, cudaGetLastError());
     }
     MARK();
-    if (on(SE_STAGE_FFT_INV)) {
+    if (on(SE_STAGE_FFT_INV) && use_xf) {
+        CUFFT_TRY(p, cufftSetStream(p->fft2_inv, s));
+        CUFFT_TRY(p, cufftExecZ2D(p->fft2_inv, (cufftDoubleComplex *)p->d_Gk, p->d_real));
+    } else if (on(SE_STAGE_FFT_INV)) {
         CUFFT_TRY(p, cufftSetStream(p->fft_inv, s));
         CUFFT_TRY(p, cufftExecZ2D(p->fft_inv, (cufftDoubleComplex *)p->d_Gk, p->d_real));
         if (comp_out) {

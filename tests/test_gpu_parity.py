@@ -327,3 +327,18 @@ def test_compressible_extension_full_size_c4(pk, oracle, workloads):
     ref = oracle.o2_apply(wl.pos, wl.radii, wl.L, wl.xi, wl.rc, wl.M, wl.P, wl.F, wl.T, wl.S, s=s_np)
     _check_blocks((r.U.cpu().numpy(), r.W.cpu().numpy(), r.E.cpu().numpy()), ref, TOL)
     assert _rel(s_out.cpu().numpy(), ref["s_out"]) <= TOL
+
+
+@pytest.mark.parametrize("name", ["c1", "c2", "c3"])
+def test_fused_x_transform_kspace_path_agrees(pk, oracle, workloads, name):
+    """SE_FUSED_X: 2-D cuFFT + one kernel for the x transform, the k-space pass and the inverse x transform,
+    instead of 3-D cuFFT + k_kspace.  Both must give the oracle's returned grids and the same product."""
+    wl = workloads.make_workload(name)
+    r = Runner(pk, wl)
+    ref = r.oracle(oracle, want_grids=True)
+    for flags in (0, pk.SE_FUSED_X):
+        r.run(flags=flags, stop=5)
+        Gr = r.plan.copy_grids(1)
+        for g in range(6):
+            assert _rel(Gr[g], ref["gridOut"][g]) <= TOL_STAGE, (flags, g)
+        _check_blocks(r.run(flags=flags), ref, TOL)
