@@ -40,6 +40,7 @@ struct se_plan {
     cudaStream_t side;             // the real-space sum runs here, beside the wave-space pipeline
     cudaEvent_t ev_fork, ev_join;
     bool have_side;
+    int real_side_ctas;            // grid of k_real when it runs beside the wave pipeline (0 = one CTA per cell)
     GatherGeom gg;                 // ring gather geometry (spreading's segments are in c.nseg, c.seg_len)
     size_t gather_smem;
     double4 *d_rs_pos;
@@ -370,6 +371,13 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
         cudaStreamDestroy(p->side); cudaEventDestroy(p->ev_fork); se_plan_destroy(p); return SE_ERR_CUDA;
     }
     p->have_side = true;
+    {   // beside the wave pipeline a2 runs as a persistent grid of one CTA per SM (measured best on B200: it then
+        // takes little from the HBM-bound kernels' occupancy; c4 step 3.57 -> 3.50 ms)
+        int dev = 0, sms = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) sms = 0;
+        cudaGetLastError();
+        p->real_side_ctas = sms;
+    }
     if (cudaFuncSetAttribute(k_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)scatter_smem_bytes(c.rec_stride)) != cudaSuccess ||
         dispatch_prepare(P, sweep_smem_bytes(c.rec_stride), p->gather_smem) != cudaSuccess) { cudaGetLastError(); se_plan_destroy(p); return SE_ERR_CUDA; }
     *out = p;
@@ -564,7 +572,8 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     // stream, alone, so that every stage is timed by itself.
     const bool fork = do_real && do_wave && !timing && stop < 0;
     auto launch_real = [&](cudaStream_t sr) {
-        const unsigned nb = (unsigned)(c.ncr > 1 ? p->ncell_r : (c.N + 31) / 32);
+        unsigned nb = (unsigned)(c.ncr > 1 ? p->ncell_r : (c.N + 31) / 32);
+        if (sr != s && c.ncr > 1 && p->real_side_ctas > 0 && nb > (unsigned)p->real_side_ctas) nb = (unsigned)p->real_side_ctas;
         if (comp) k_real<true><<<nb, REAL_WARPS * 32, 0, sr>>>(c, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig, p->d_start_r, p->d_out_real);
         else k_real<false><<<nb, REAL_WARPS * 32, 0, sr>>>(c, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig, p->d_start_r, p->d_out_real);
         p->last_launches += 1;
@@ -573,13 +582,15 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
         launch_real(s);
         CUDA_TRY(p, cudaGetLastError());
     }
-    if (fork) {
+    auto fork_real = [&]() -> se_status {
         CUDA_TRY(p, cudaEventRecord(p->ev_fork, s));
         CUDA_TRY(p, cudaStreamWaitEvent(p->side, p->ev_fork, 0));
         launch_real(p->side);
         CUDA_TRY(p, cudaGetLastError());
         CUDA_TRY(p, cudaEventRecord(p->ev_join, p->side));
-    }
+        return SE_OK;
+    };
+    if (fork) { se_status sf = fork_real(); if (sf != SE_OK) return sf; }
     MARK();
     // ---- a3..a7: Spectral Ewald wave-space sum ----
     bool wave_done = false;

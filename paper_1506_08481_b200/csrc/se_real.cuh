@@ -147,12 +147,17 @@ __global__ void __launch_bounds__(REAL_WARPS * 32) k_real(SeConst c, const doubl
     const int nc = c.ncr;
     const double invL = 1.0 / c.L;
 
-    // targets of this CTA and its candidate segments
+    // Work items: the cells (grid-stride loop, so that a small persistent grid can run beside the HBM-bound
+    // wave-space kernels without taking their SM resources), or one slice of all particles per CTA.
+    const int nitems = nc > 1 ? nc * nc * nc : (int)gridDim.x;
+    for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
+    __syncthreads();                                   // the previous item's shared tables are no longer read
+    // targets of this item and its candidate segments
     int t0, t1, nsegs;
     if (nc > 1) {
-        const int cell = blockIdx.x;
+        const int cell = item;
         t0 = start_r[cell]; t1 = start_r[cell + 1];
-        if (t0 == t1) return;
+        if (t0 == t1) continue;
         nsegs = 27;
         if (tid < 27) {
             const int cz = cell % nc, cy = (cell / nc) % nc, cx = cell / (nc * nc);
@@ -163,8 +168,8 @@ __global__ void __launch_bounds__(REAL_WARPS * 32) k_real(SeConst c, const doubl
         }
     } else {
         const int per = (c.N + gridDim.x - 1) / gridDim.x;
-        t0 = blockIdx.x * per; t1 = min(t0 + per, c.N);
-        if (t0 >= t1) return;
+        t0 = item * per; t1 = min(t0 + per, c.N);
+        if (t0 >= t1) continue;
         nsegs = 1;
         if (tid == 0) { seg_s[0] = 0; seg_o[1] = c.N; }
     }
@@ -259,4 +264,5 @@ __global__ void __launch_bounds__(REAL_WARPS * 32) k_real(SeConst c, const doubl
         }
     }
     // a cell without any candidate at all cannot occur (it contains its own targets), so every target was written
+    }
 }
