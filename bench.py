@@ -246,10 +246,26 @@ def main():
     own = {k: stage[k] for k in ("sort", "real", "spread", "kspace", "gather", "epilogue")}
     dom = max(("spread", "kspace", "gather"), key=lambda k: stage[k])
     achieved = alg_bytes[dom] / (stage[dom] * 1e-3) / 1e9
+    # dram__bytes_read.sum + dram__bytes_write.sum per launch, from the ncu --set full capture summarised in
+    # profiles/r01c_summary.md (c4 only; other configs have no capture)
+    traffic_c4 = {"spread": 0.0895e9 + 351.5e6, "kspace": 0.4027e9 + 754.8e6, "gather": 1.2960e9 + 55.6e6}
+    traffic = traffic_c4.get(dom) if args.config == "c4" else None
+    # spreading and gather are FP64-issue bound before they are HBM bound: 12 N P^3 DFMA each
+    try:
+        fp64_peak = pk.measure_fp64_peak()
+    except Exception:
+        fp64_peak = None
+    sg_flops = 2.0 * 12.0 * wl.N * float(wl.P) ** 3
+    per_kernel = {}
+    for k in alg_bytes:
+        gbs = alg_bytes[k] / (stage[k] * 1e-3) / 1e9
+        per_kernel[k] = {"ms": stage[k], "GB/s": gbs, "frac": gbs / peak}
+        if k in ("spread", "gather"):
+            tf = sg_flops / (stage[k] * 1e-3) / 1e12
+            per_kernel[k]["fp64_TFLOP/s"] = tf
+            per_kernel[k]["fp64_frac"] = tf / fp64_peak if fp64_peak else None
     roofline = {"kernel": dom, "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "peak_source": peak_src,
-                "all": {k: {"ms": stage[k], "GB/s": alg_bytes[k] / (stage[k] * 1e-3) / 1e9,
-                            "frac": alg_bytes[k] / (stage[k] * 1e-3) / 1e9 / peak} for k in alg_bytes}}
+                "traffic": traffic, "peak_source": peak_src, "fp64_peak_TFLOP/s": fp64_peak, "all": per_kernel}
 
     cpu = None
     if not args.no_cpu_baseline:

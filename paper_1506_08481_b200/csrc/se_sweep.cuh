@@ -31,16 +31,20 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
+// suspend-time hint of try_wait: the waiting warp sleeps in hardware instead of polling shared memory
+#ifndef SE_WAIT_HINT_NS
+#define SE_WAIT_HINT_NS 20000u
+#endif
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
     asm volatile("{\n"
                  ".reg .pred P1;\n"
                  "LAB_WAIT:\n"
-                 "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+                 "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1, %2;\n"
                  "@P1 bra DONE;\n"
                  "bra LAB_WAIT;\n"
                  "DONE:\n"
-                 "}" ::"r"(bar), "r"(parity) : "memory");
+                 "}" ::"r"(bar), "r"(parity), "r"(SE_WAIT_HINT_NS) : "memory");
 }
 
 // Per-lane description of the candidate ranges of a patch: lane r < nr owns the bins
