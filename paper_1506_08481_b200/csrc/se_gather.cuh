@@ -8,9 +8,14 @@
 //
 // Design ("plane ring"): a CTA owns one returned grid, one (y,z) tile of TY x TZ support origins and one
 // segment of x.  It streams the planes of its haloed tile, (TY+P-1) x (TZ+P-1) columns, through a ring of R
-// planes in shared memory: two producer warps copy it with 16-byte cp.async (completion counted by the slot's
-// mbarrier), R-P planes ahead of the consumers, so every grid value crosses L2->SM once per tile and is then
-// read from shared memory.  The particles whose support starts in the tile are sorted by starting plane (a1,
+// planes in shared memory, R-P planes ahead of the consumers, so every grid value crosses L2->SM once per tile
+// and is then read from shared memory.  The fill has two paths with the same slot layout.  A tile whose halo
+// stays inside the grid takes ONE TMA tensor-box copy per plane (cp.async.bulk.tensor.3d issued by one elected
+// thread, completion counted in bytes by the slot's mbarrier).  A tile whose halo crosses the periodic seam (the
+// last tile row and column) copies the plane with 16-byte cp.async through a table that wraps the coordinates
+// (two producer warps, completion counted by deferred mbarrier arrivals).  Measured on B200: the cp.async path
+// sustains only ~10 B/clk/SM and bounded the whole kernel when every tile used it; a box copy per plane is
+// ~6 times faster, and per-row bulk copies were slower than either.  The particles whose support starts in the tile are sorted by starting plane (a1,
 // second counting sort); the eight consumer warps take them round-robin, ONE WARP PER PARTICLE: the lanes
 // own the P^2 columns of the footprint (all lanes busy), reduce along x in registers,
 //     m0 = sum_k gx(k) g(x0+k),   m1 = sum_k gx(k) dx_k g(x0+k),
@@ -20,6 +25,7 @@
 // distinct shared-memory banks.  Planes are released through per-slot "empty" mbarriers (one arrival per
 // consumer warp), so warps run up to R-P planes apart without CTA-wide barriers.
 #pragma once
+#include <cuda.h>                  // CUtensorMap (type only; the encoder is fetched through the runtime)
 #include "se_sweep.cuh"
 #include "se_sort.cuh"
 
@@ -44,28 +50,43 @@ __device__ __forceinline__ void cp_async_arrive(uint32_t bar)
     asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
 }
 
+// One box of the tensor `tmap` at element coordinates (c0 fastest, c1, c2) into shared memory at `dst`.
+__device__ __forceinline__ void tma_box3(uint32_t dst, const CUtensorMap *tmap, int c0, int c1, int c2, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                 ::"r"(dst), "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
+}
+
 template <int P>
 __global__ void __launch_bounds__((GR_WARPS + GR_PROD) * 32, (P <= GR_P2MAX ? 2 : 1))
 k_gather(SeConst c, GatherGeom g, const double *__restrict__ recs, const int *__restrict__ gperm,
-         const int *__restrict__ start_g, const double *__restrict__ Gr, int ngrids, double *__restrict__ moments,
-         int mstride)
+         const int *__restrict__ start_g, const double *__restrict__ Gr, const __grid_constant__ CUtensorMap tmap, int ngrids,
+         double *__restrict__ moments, int mstride)
 {
-    extern __shared__ __align__(16) unsigned char gsm[];
+    extern __shared__ __align__(128) unsigned char gsm[];
     constexpr int PP = P * P, NI = (PP + 31) / 32;
     constexpr int NREC = SE_REC_HDR + 4 * P, NR = (NREC + 31) / 32;      // record prefix the gather needs
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int M = c.M, stride = c.rec_stride, R = g.R;
-    const int ntile = g.NTY * g.NTZ;
-    int item = blockIdx.x;
-    const int tile = item % ntile; item /= ntile;
-    const int grid = item % ngrids, seg = item / ngrids;
+    // Work items in launch order: tile slowest, and the seam tiles (last tile row and column: the slow cp.async
+    // fill, see below) first, so that they do not form the tail of the launch.
+    const int per_tile = ngrids * g.nseg;
+    const int q = blockIdx.x / per_tile, rest = blockIdx.x - q * per_tile;
+    const int grid = rest % ngrids, seg = rest / ngrids;
+    const int nseam = g.NTY + g.NTZ - 1;
+    int ty, tz;
+    if (q < g.NTZ) { ty = g.NTY - 1; tz = q; }
+    else if (q < nseam) { ty = q - g.NTZ; tz = g.NTZ - 1; }
+    else { const int r = q - nseam; ty = r / (g.NTZ - 1); tz = r - ty * (g.NTZ - 1); }
+    const int tile = ty * g.NTZ + tz;
     const int seg_start = seg * g.seg_len, seg_end = min(seg_start + g.seg_len, M);
     const int i0 = start_g[tile * M + seg_start], i1 = start_g[tile * M + seg_end];
     if (i0 == i1) return;                                              // no support starts here
-    const int ty = tile / g.NTZ, tz = tile - ty * g.NTZ;
     const int Y0 = ty * g.TY, Z0 = tz * g.TZ;
     const int nplanes = seg_end - seg_start + P - 1;
-    const int plane_d = g.WY * g.WZ;                                   // doubles per ring slot
+    const int plane_d = g.slot_d;                                      // doubles per ring slot (a multiple of 128 bytes)
+    // the box [Y0, Y0+WY) x [Z0, Z0+WZ) may reach beyond the grid only in its unused pad columns (zero-filled)
+    const bool use_tma = (Y0 + g.TY + P - 1 <= M) && (Z0 + g.TZ + P - 1 <= M);
     const int cw = g.WZL >> 1, nch = g.WY * cw;                        // 16-byte chunks per row, per plane
 
     double *ring = reinterpret_cast<double *>(gsm);
@@ -75,17 +96,35 @@ k_gather(SeConst c, GatherGeom g, const double *__restrict__ recs, const int *__
     auto full_bar = [&](int sl) { return bars + 16u * (uint32_t)sl; };
     auto empty_bar = [&](int sl) { return bars + 16u * (uint32_t)sl + 8u; };
     if (threadIdx.x == 0) {
-        for (int sl = 0; sl < R; ++sl) { mbar_init(full_bar(sl), GR_PROD * 32); mbar_init(empty_bar(sl), GR_WARPS); }
+        for (int sl = 0; sl < R; ++sl) { mbar_init(full_bar(sl), use_tma ? 1 : GR_PROD * 32); mbar_init(empty_bar(sl), GR_WARPS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
-    for (int ch = threadIdx.x; ch < nch; ch += blockDim.x) {            // periodic wrap along y and z, once per CTA
+    if (!use_tma) for (int ch = threadIdx.x; ch < nch; ch += blockDim.x) {   // periodic wrap along y and z, once per CTA
         const int r = ch / cw, col = ch - r * cw;
         table[ch] = make_int2(((Y0 + r) % M) * M + (Z0 + 2 * col) % M, r * g.WZ + 2 * col);
     }
     __syncthreads();
 
+    if (w >= GR_WARPS && use_tma) {
+        // ---- producer, interior tile (one elected thread): plane j of the segment goes to slot j % R once every
+        // consumer has released plane j - R; one tensor-box copy per plane.
+        if (w == GR_WARPS && lane == 0) {
+            const uint32_t ring_a = smem_u32(ring), box_bytes = (uint32_t)(g.WY * g.WZ * 8);
+            int sl = 0, x = seg_start;
+            uint32_t par = 1;                                          // passes at once in round 0
+            for (int j = 0; j < nplanes; ++j) {
+                mbar_wait(empty_bar(sl), par);
+                mbar_expect_tx(full_bar(sl), box_bytes);
+                tma_box3(ring_a + 8u * (uint32_t)(sl * plane_d), &tmap, Z0, Y0, grid * M + x, full_bar(sl));
+                if (++sl == R) { sl = 0; par ^= 1u; }
+                if (++x == M) x = 0;
+            }
+        }
+        return;
+    }
     if (w >= GR_WARPS) {
-        // ---- producers: plane j of the segment goes to slot j % R once every consumer released plane j - R.
+        // ---- producers, seam tile: as above, with the periodic wrap done by the chunk table.
         // 16-byte cp.async per chunk (rows are too short for bulk copies to pay); completion is counted by the
         // slot's "full" mbarrier, one deferred arrival per producer lane.
         const double *__restrict__ G0 = Gr + (size_t)grid * M * M * M;
@@ -219,7 +258,7 @@ k_gather(SeConst c, GatherGeom g, const double *__restrict__ recs, const int *__
 static inline size_t gather_smem_bytes(const GatherGeom &g, int P)
 {
     const int NR = (SE_REC_HDR + 4 * P + 31) / 32;
-    return (size_t)g.R * g.WY * g.WZ * 8 + (size_t)GR_WARPS * NR * 32 * 8 + (size_t)g.WY * (g.WZL / 2) * 8 + (size_t)g.R * 16;
+    return (size_t)g.R * g.slot_d * 8 + (size_t)GR_WARPS * NR * 32 * 8 + (size_t)g.WY * (g.WZL / 2) * 8 + (size_t)g.R * 16;
 }
 
 // a8: out = real + wave + (one-body - self) * input, in caller order (Eq. 13-15 one-body terms;

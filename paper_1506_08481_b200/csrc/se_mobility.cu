@@ -42,6 +42,7 @@ struct se_plan {
     bool have_side;
     int real_side_ctas;            // grid of k_real when it runs beside the wave pipeline (0 = one CTA per cell)
     GatherGeom gg;                 // ring gather geometry (spreading's segments are in c.nseg, c.seg_len)
+    CUtensorMap tmap, tmap_p;      // TMA descriptors of the six returned grids / of the pressure grid (se_gather.cuh)
     size_t gather_smem;
     double4 *d_rs_pos;
     double *d_rs_mom;
@@ -152,6 +153,7 @@ static void choose_segments(se_plan *p, int spread_segments, int gather_segments
     if (ng <= 0) {
         const int items = g.NTY * g.NTZ * 6;
         ng = (148 * 8 + items - 1) / items;
+        if (ng < 2) ng = 2;                            // two segments measured best at c4 (more items, small warm-up cost)
         if (ng > maxseg) ng = maxseg;
     }
     if (ng > M) ng = M;
@@ -182,6 +184,8 @@ static bool choose_gather_geometry(se_plan *p)
         const int want = (P & 1) ? (P + 1) % 16 : P % 16;
         g.WZ = g.WZL;
         while (g.WZ % 16 != want) g.WZ += 2;
+        g.slot_d = (g.WY * g.WZ + 15) & ~15;
+        if (g.WY > 256 || g.WZ > 256) continue;          // TMA box limits
         g.nseg = 1; g.seg_len = M;
         const bool few_items = (long long)g.NTY * g.NTZ * 6 * (M >= 64 ? 2 : 1) < 2 * 148 && g.TY * g.TZ > 64;
         if (gather_smem_bytes(g, P) <= (cd[3] == 2 ? two : one) && !few_items) {
@@ -221,6 +225,36 @@ extern "C" se_status se_plan_destroy(se_plan *p)
     if (p->have_events) for (int k = 0; k <= SE_NUM_STAGES; ++k) cudaEventDestroy(p->ev[k]);
     cudaGetLastError();
     free(p);
+    return SE_OK;
+}
+
+// TMA descriptor of nplanes grid planes [M][M] at `base`: 3-D tensor (z, y, plane), box = one haloed tile.
+// The encoder lives in the driver; it is fetched through the runtime so that the library links against cudart only.
+static se_status make_tensor_map(se_plan *p, CUtensorMap *map, double *base, int nplanes)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || !fn ||
+        qr != cudaDriverEntryPointSuccess) {
+        cudaGetLastError();
+        return fail(p, SE_ERR_CUDA, "cudaGetDriverEntryPoint", "cuTensorMapEncodeTiled");
+    }
+    const GatherGeom &g = p->gg;
+    const int M = p->c.M;
+    const cuuint64_t dims[3] = { (cuuint64_t)M, (cuuint64_t)M, (cuuint64_t)nplanes };
+    const cuuint64_t strides[2] = { (cuuint64_t)M * 8, (cuuint64_t)M * M * 8 };
+    const cuuint32_t box[3] = { (cuuint32_t)g.WZ, (cuuint32_t)g.WY, 1 };
+    const cuuint32_t estr[3] = { 1, 1, 1 };
+    const CUresult cr = ((encode_fn)fn)(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, base, dims, strides, box, estr,
+                                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                        CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (cr != CUDA_SUCCESS) {
+        char b[32]; snprintf(b, sizeof(b), "CUresult %d", (int)cr);
+        return fail(p, SE_ERR_CUDA, "cuTensorMapEncodeTiled", b);
+    }
     return SE_OK;
 }
 
@@ -301,8 +335,9 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
     if (P > SE_PMAX) return SE_ERR_UNSUPPORTED;
     for (int64_t i = 0; i < N; ++i) if (!(radii[i] > 0.0)) return SE_ERR_INVALID_ARG;
 
-    se_plan *p = (se_plan *)calloc(1, sizeof(se_plan));
+    se_plan *p = (se_plan *)aligned_alloc(64, (sizeof(se_plan) + 63) & ~(size_t)63);     // CUtensorMap members: 64-byte aligned
     if (!p) return SE_ERR_ALLOC;
+    memset(p, 0, sizeof(se_plan));
     p->debug_stop = -1;
     SeConst &c = p->c;
     c.N = (int)N; c.M = M; c.P = P; c.L = L; c.xi = xi; c.rc2 = r_c * r_c; c.eta0 = eta0;
@@ -356,7 +391,8 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
     // cuFFT: batched 3-D transforms (the default a4 / a6).  The plans of the opt-in fused path (SE_FUSED_X) are
     // made by the first apply that asks for it.
     {
-        const se_status stf = ensure_fft3d(p);
+        se_status stf = ensure_fft3d(p);
+        if (stf == SE_OK) stf = make_tensor_map(p, &p->tmap, p->d_real, 6 * M);
         if (stf != SE_OK) { se_plan_destroy(p); return stf; }
     }
 
@@ -453,7 +489,7 @@ static void launch_gather(se_plan *p, cudaStream_t s, bool pressure)
     const int ngrids = pressure ? 1 : 6;
     const unsigned blocks = (unsigned)(g.NTY * g.NTZ * ngrids * g.nseg);
     k_gather<P><<<blocks, (GR_WARPS + GR_PROD) * 32, p->gather_smem, s>>>(p->c, g, p->d_recs, p->d_gperm, p->d_start_g,
-                                                                   pressure ? p->d_real_p : p->d_real, ngrids,
+                                                                   pressure ? p->d_real_p : p->d_real, pressure ? p->tmap_p : p->tmap, ngrids,
                                                                    pressure ? p->d_pmom : p->d_moments, pressure ? 12 : GATHER_SUMS);
 }
 
@@ -522,6 +558,13 @@ static se_status ensure_compressible(se_plan *p)
         if (f1) cufftDestroy(p->fft_fwd1);
         if (i1) cufftDestroy(p->fft_inv1);
         cudaGetLastError();
+        return st;
+    }
+    st = make_tensor_map(p, &p->tmap_p, p->d_real_p, M);
+    if (st != SE_OK) {
+        cudaFree(p->d_real_p); cudaFree(p->d_Hk_s); cudaFree(p->d_Gk_p); cudaFree(p->d_pmom);
+        p->d_real_p = nullptr; p->d_Hk_s = nullptr; p->d_Gk_p = nullptr; p->d_pmom = nullptr;
+        cufftDestroy(p->fft_fwd1); cufftDestroy(p->fft_inv1);
         return st;
     }
     p->have_comp = true;

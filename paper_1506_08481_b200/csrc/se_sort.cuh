@@ -8,7 +8,8 @@
 struct GatherGeom {
     int TY, TZ;                    // support origins per tile along y, z
     int NTY, NTZ;                  // tiles per axis
-    int WY, WZ, WZL;               // haloed tile: rows, padded row length, loaded row length (doubles, even)
+    int WY, WZ, WZL;               // haloed tile: rows, padded row length (= TMA box), loaded row length (doubles, even)
+    int slot_d;                    // doubles per ring slot: WY * WZ rounded up to a multiple of 16 (128 bytes)
     int R;                         // planes in the ring (>= P)
     int nseg, seg_len;             // segments of the sweep along x
 };
