@@ -30,9 +30,13 @@
 #include "se_sort.cuh"
 
 #define GATHER_SUMS 24             // per particle: slot (g/3)*12 + kind*3 + g%3, kind = 0 (1), 1 (dx), 2 (dy), 3 (dz)
+#ifndef GR_WARPS
 #define GR_WARPS 8                 // consumer warps
+#endif
 // Two CTAs per SM hide each other's pipeline bubbles; supports up to GR_P2MAX keep the register budget for it.
+#ifndef GR_P2MAX
 #define GR_P2MAX 14
+#endif
 #define GR_PROD 2                  // producer warps (GR_WARPS, GR_WARPS + 1)
 
 __device__ __forceinline__ void mbar_arrive(uint32_t bar)
