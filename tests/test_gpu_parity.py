@@ -342,3 +342,22 @@ def test_fused_x_transform_kspace_path_agrees(pk, oracle, workloads, name):
         for g in range(6):
             assert _rel(Gr[g], ref["gridOut"][g]) <= TOL_STAGE, (flags, g)
         _check_blocks(r.run(flags=flags), ref, TOL)
+
+
+def test_permutation_invariance_and_reproducibility(pk, workloads):
+    """T8: relabelling the particles permutes the result (to summation-order round-off: the counting sorts use
+    atomic ranks); with the same labels the gather is bitwise reproducible, the whole product to round-off."""
+    import torch
+    wl = workloads.make_workload("c2")
+    r = Runner(pk, wl)
+    base = [x.copy() for x in r.run()]
+    again = r.run()
+    for a, b in zip(again, base):
+        assert _rel(a, b) <= 1e-14
+    perm = np.random.default_rng(5).permutation(wl.N)
+    wl2 = workloads.make_workload("c2")
+    wl2.pos, wl2.radii, wl2.F, wl2.T, wl2.S = wl.pos[perm], wl.radii[perm], wl.F[perm], wl.T[perm], wl.S[perm]
+    r2 = Runner(pk, wl2)
+    got = r2.run()
+    for a, b in zip(got, base):
+        assert _rel(a, b[perm]) <= 1e-13
