@@ -361,3 +361,25 @@ def test_permutation_invariance_and_reproducibility(pk, workloads):
     got = r2.run()
     for a, b in zip(got, base):
         assert _rel(a, b[perm]) <= 1e-13
+
+
+def test_apply_is_capturable_in_a_cuda_graph(pk, oracle, workloads):
+    """The product is a fixed sequence of kernels, cuFFT calls and an event fork/join on plan-owned streams: it can
+    be captured once and replayed (launch-bound small systems).  Replays with new inputs in the same buffers."""
+    import torch
+    wl = workloads.make_workload("c2")
+    r = Runner(pk, wl)
+    r.run()                                             # warm-up outside the capture (lazy initialisation)
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        r.plan.apply(r.pos, r.F, r.T, r.S, r.U, r.W, r.E)
+    r.U.fill_(float("nan")); r.W.fill_(float("nan")); r.E.fill_(float("nan"))
+    g.replay()
+    torch.cuda.synchronize()
+    ref = r.oracle(oracle)
+    _check_blocks((r.U.cpu().numpy(), r.W.cpu().numpy(), r.E.cpu().numpy()), ref, TOL)
+    r.F.mul_(-2.0)                                      # new right-hand side in place, same graph
+    g.replay()
+    torch.cuda.synchronize()
+    ref2 = oracle.o2_apply(wl.pos, wl.radii, wl.L, wl.xi, wl.rc, wl.M, wl.P, -2.0 * wl.F, wl.T, wl.S)
+    _check_blocks((r.U.cpu().numpy(), r.W.cpu().numpy(), r.E.cpu().numpy()), ref2, TOL)
