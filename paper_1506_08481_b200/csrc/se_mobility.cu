@@ -603,15 +603,16 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     p->last_launches += 1;
     se_status st = scan_cells(p, s);
     if (st != SE_OK) return st;
-    k_scatter<<<(c.N + SCATTER_THREADS - 1) / SCATTER_THREADS, SCATTER_THREADS, scatter_smem_bytes(c.rec_stride), s>>>(c, pos, p->d_radii, F, T, S, s_in, p->d_key_r, p->d_rank_r, p->d_start_r,
-                                 p->d_key_s, p->d_rank_s, p->d_start_s, p->d_key_g, p->d_rank_g, p->d_start_g, p->d_gperm, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig, p->d_recs);
+    k_scatter<<<(c.N + SCATTER_THREADS - 1) / SCATTER_THREADS, SCATTER_THREADS, scatter_smem_bytes(c.rec_stride), s>>>(
+        c, pos, p->d_radii, F, T, S, s_in, p->d_key_r, p->d_rank_r, p->d_start_r, p->d_key_s, p->d_rank_s, p->d_start_s,
+        p->d_key_g, p->d_rank_g, p->d_start_g, p->d_gperm, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig, p->d_recs);
     p->last_launches += 1;
     CUDA_TRY(p, cudaGetLastError());
     MARK();
     // ---- a2: real-space pair sum ----
     // a2 is independent of the wave pipeline: it runs on the plan's (low-priority) side stream, forked here and
     // joined before the epilogue, and fills what the wave-space kernels leave idle (tails, the HBM-bound stages).
-    // Measured gain on B200 is small (c4: 2 %).  When stage timings are asked for it runs on the caller's
+    // Measured gain on B200 is small (c4: 4 %).  When stage timings are asked for it runs on the caller's
     // stream, alone, so that every stage is timed by itself.
     const bool fork = do_real && do_wave && !timing && stop < 0;
     auto launch_real = [&](cudaStream_t sr) {
