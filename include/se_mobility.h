@@ -91,14 +91,25 @@ se_status se_plan_set_tuning(se_plan *plan, int spread_segments, int gather_segm
 /* Bitwise OR of the SE_* flags above. */
 se_status se_plan_set_flags(se_plan *plan, unsigned flags);
 
+/* Fix the particle configuration for the following products (the iterative solver applies the
+ * operator many times per configuration).  Runs a1 once (wrap, counting sorts, per-particle
+ * Gaussian tables and indices) on cuda_stream; afterwards far_mobility_apply / far_mobility_apply_compressible
+ * may be called with pos == NULL and then only refresh the moments (F, T, S, s) of the packed records.
+ *   pos    [N][3] DEVICE, as in far_mobility_apply; NULL forgets the cached configuration
+ * The cache is dropped by se_plan_set_shape and by any apply that passes pos != NULL.  With a cached configuration
+ * the summation order is fixed, so repeated products are bitwise reproducible. */
+se_status se_plan_set_positions(se_plan *plan, const double *pos, void *cuda_stream);
+
 /* The product.  All pointers are DEVICE pointers to arrays the caller owns:
- *   pos    [N][3] row-major particle centres, any real value (wrapped into the box internally)
+ *   pos    [N][3] row-major particle centres, any real value (wrapped into the box internally);
+ *          NULL = the configuration given to se_plan_set_positions
  *   F, T   [N][3] force and torque on the fluid
  *   S      [N][5] stresslet on the fluid, (xx,xy,xz,yy,yz)
  *   U, Omega [N][3], E [N][5]  outputs, OVERWRITTEN (never accumulated into)
  *   cuda_stream   a cudaStream_t (NULL = default stream); the work is enqueued and the call returns
  *                 without synchronising.  Inputs must stay valid until the stream reaches the end.
- * Errors: SE_ERR_INVALID_ARG for NULL pointers; SE_ERR_CUDA / SE_ERR_CUFFT on launch failure. */
+ * Errors: SE_ERR_INVALID_ARG for NULL pointers (pos == NULL without se_plan_set_positions included);
+ * SE_ERR_CUDA / SE_ERR_CUFFT on launch failure. */
 se_status far_mobility_apply(se_plan *plan, const double *pos, const double *F, const double *T,
                              const double *S, double *U, double *Omega, double *E, void *cuda_stream);
 

@@ -51,6 +51,8 @@ def load_library(build_if_missing: bool = True):
     L.se_plan_set_shape.argtypes = [P, D]
     L.se_plan_set_tuning.restype = INT
     L.se_plan_set_tuning.argtypes = [P, INT, INT]
+    L.se_plan_set_positions.restype = INT
+    L.se_plan_set_positions.argtypes = [P, P, P]
     L.se_plan_set_flags.restype = INT
     L.se_plan_set_flags.argtypes = [P, U]
     L.far_mobility_apply.restype = INT
@@ -141,6 +143,13 @@ class SePlan:
     def set_flags(self, flags):
         self._check(self._lib.se_plan_set_flags(self._h, int(flags)), "se_plan_set_flags")
 
+    def set_positions(self, pos, stream=None):
+        """se_plan_set_positions: run a1 once for ``pos`` (CUDA float64 [N,3]); later applies may pass pos=None."""
+        import torch
+        sp = (torch.cuda.current_stream() if stream is None else stream).cuda_stream
+        ptr = None if pos is None else _dptr(pos, 3 * self.N, "pos")
+        self._check(self._lib.se_plan_set_positions(self._h, ptr, sp), "se_plan_set_positions")
+
     def debug_stop(self, stage):
         self._check(self._lib.se_plan_debug_stop(self._h, int(stage)), "se_plan_debug_stop")
 
@@ -149,7 +158,7 @@ class SePlan:
         import torch
         N = self.N
         sp = (torch.cuda.current_stream() if stream is None else stream).cuda_stream
-        st = self._lib.far_mobility_apply(self._h, _dptr(pos, 3 * N, "pos"), _dptr(F, 3 * N, "F"), _dptr(T, 3 * N, "T"),
+        st = self._lib.far_mobility_apply(self._h, None if pos is None else _dptr(pos, 3 * N, "pos"), _dptr(F, 3 * N, "F"), _dptr(T, 3 * N, "T"),
                                           _dptr(S, 5 * N, "S"), _dptr(U, 3 * N, "U"), _dptr(Omega, 3 * N, "Omega"),
                                           _dptr(E, 5 * N, "E"), sp)
         self._check(st, "far_mobility_apply")
@@ -160,7 +169,7 @@ class SePlan:
         N = self.N
         sp = (torch.cuda.current_stream() if stream is None else stream).cuda_stream
         st = self._lib.far_mobility_apply_compressible(
-            self._h, _dptr(pos, 3 * N, "pos"), _dptr(F, 3 * N, "F"), _dptr(T, 3 * N, "T"), _dptr(S, 5 * N, "S"),
+            self._h, None if pos is None else _dptr(pos, 3 * N, "pos"), _dptr(F, 3 * N, "F"), _dptr(T, 3 * N, "T"), _dptr(S, 5 * N, "S"),
             None if s_in is None else _dptr(s_in, N, "s_in"), _dptr(U, 3 * N, "U"), _dptr(Omega, 3 * N, "Omega"),
             _dptr(E, 5 * N, "E"), None if s_out is None else _dptr(s_out, N, "s_out"), sp)
         self._check(st, "far_mobility_apply_compressible")

@@ -34,6 +34,8 @@ struct se_plan {
     int *d_key_r, *d_rank_r, *d_cnt_r, *d_start_r;
     int *d_key_s, *d_rank_s, *d_cnt_s, *d_start_s;
     int *d_key_g, *d_rank_g, *d_cnt_g, *d_start_g, *d_gperm;
+    int2 *d_dst_rs;                // per particle (caller order): index in cell order, record index
+    bool have_positions;           // a1 was run by se_plan_set_positions and is reused while pos == NULL
     int *d_cnt_all, *d_start_all;  // the three count / start tables, concatenated (one pad element after each)
     int *d_bsum;
     int ncell_r, ncell_s, ncell_g, ncell_all;
@@ -208,7 +210,7 @@ extern "C" se_status se_plan_destroy(se_plan *p)
     cudaFree(p->d_radii);
     cudaFree(p->d_key_r); cudaFree(p->d_rank_r); cudaFree(p->d_key_s); cudaFree(p->d_rank_s);
     cudaFree(p->d_key_g); cudaFree(p->d_rank_g); cudaFree(p->d_gperm);
-    cudaFree(p->d_cnt_all); cudaFree(p->d_start_all);
+    cudaFree(p->d_cnt_all); cudaFree(p->d_start_all); cudaFree(p->d_dst_rs);
     if (p->have_side) { cudaStreamDestroy(p->side); cudaEventDestroy(p->ev_fork); cudaEventDestroy(p->ev_join); }
     cudaFree(p->d_bsum);
     cudaFree(p->d_rs_pos); cudaFree(p->d_rs_mom); cudaFree(p->d_rs_orig); cudaFree(p->d_recs);
@@ -368,7 +370,7 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
     ALLOC(p->d_radii, N);
     ALLOC(p->d_key_r, N); ALLOC(p->d_rank_r, N); ALLOC(p->d_key_s, N); ALLOC(p->d_rank_s, N);
     ALLOC(p->d_key_g, N); ALLOC(p->d_rank_g, N); ALLOC(p->d_gperm, N);
-    ALLOC(p->d_cnt_all, p->ncell_all); ALLOC(p->d_start_all, p->ncell_all);
+    ALLOC(p->d_cnt_all, p->ncell_all); ALLOC(p->d_start_all, p->ncell_all); ALLOC(p->d_dst_rs, N);
     if (st == SE_OK) {
         p->d_cnt_r = p->d_cnt_all; p->d_cnt_s = p->d_cnt_r + p->ncell_r + 1; p->d_cnt_g = p->d_cnt_s + p->ncell_s + 1;
         p->d_start_r = p->d_start_all; p->d_start_s = p->d_start_r + p->ncell_r + 1; p->d_start_g = p->d_start_s + p->ncell_s + 1;
@@ -425,6 +427,7 @@ extern "C" se_status se_plan_set_shape(se_plan *p, double m)
     if (!p || !(m > 0.0)) return SE_ERR_INVALID_ARG;
     p->m = m;
     derive_constants(p);
+    p->have_positions = false;          // the cached Gaussian tables depend on the shape
     return SE_OK;
 }
 
@@ -571,12 +574,45 @@ static se_status ensure_compressible(se_plan *p)
     return SE_OK;
 }
 
+// a1: wrap, the three counting sorts, packed records and real-space copies (F == NULL: zero moments).
+static se_status sort_and_pack(se_plan *p, const double *pos, const double *F, const double *T, const double *S,
+                               const double *s_in, cudaStream_t s)
+{
+    const SeConst &c = p->c;
+    const int TB = 128, nbN = (c.N + TB - 1) / TB;
+    CUDA_TRY(p, cudaMemsetAsync(p->d_cnt_all, 0, sizeof(int) * (size_t)p->ncell_all, s));
+    k_keys<<<nbN, TB, 0, s>>>(c, p->gg, pos, p->d_key_r, p->d_rank_r, p->d_cnt_r, p->d_key_s, p->d_rank_s, p->d_cnt_s,
+                              p->d_key_g, p->d_rank_g, p->d_cnt_g);
+    p->last_launches += 1;
+    const se_status st = scan_cells(p, s);
+    if (st != SE_OK) return st;
+    k_scatter<<<(c.N + SCATTER_THREADS - 1) / SCATTER_THREADS, SCATTER_THREADS, scatter_smem_bytes(c.rec_stride), s>>>(
+        c, pos, p->d_radii, F, T, S, s_in, p->d_key_r, p->d_rank_r, p->d_start_r, p->d_key_s, p->d_rank_s, p->d_start_s,
+        p->d_key_g, p->d_rank_g, p->d_start_g, p->d_gperm, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig, p->d_recs, p->d_dst_rs);
+    p->last_launches += 1;
+    CUDA_TRY(p, cudaGetLastError());
+    return SE_OK;
+}
+
+extern "C" se_status se_plan_set_positions(se_plan *p, const double *pos, void *cuda_stream)
+{
+    if (!p) return SE_ERR_INVALID_ARG;
+    if (!pos) { p->have_positions = false; return SE_OK; }            // forget the cached configuration
+    p->last_launches = 0;
+    p->have_positions = false;
+    const se_status st = sort_and_pack(p, pos, nullptr, nullptr, nullptr, nullptr, (cudaStream_t)cuda_stream);
+    if (st != SE_OK) return st;
+    p->have_positions = true;
+    return SE_OK;
+}
+
 static se_status apply_impl(se_plan *p, const double *pos, const double *F, const double *T, const double *S,
                             const double *s_in, double *U, double *Omega, double *E, double *s_out, void *cuda_stream,
                             const char *who)
 {
     if (!p) return SE_ERR_INVALID_ARG;
-    if (!pos || !F || !T || !S || !U || !Omega || !E) return fail(p, SE_ERR_INVALID_ARG, who, "null pointer");
+    if (!F || !T || !S || !U || !Omega || !E) return fail(p, SE_ERR_INVALID_ARG, who, "null pointer");
+    if (!pos && !p->have_positions) return fail(p, SE_ERR_INVALID_ARG, who, "pos is NULL and no positions were set (se_plan_set_positions)");
     const bool comp_in = s_in != nullptr, comp_out = s_out != nullptr, comp = comp_in || comp_out;
     if (comp) { se_status stc = ensure_compressible(p); if (stc != SE_OK) return stc; }
     // opt-in: 2-D cuFFT + fused x-transform / k-space / x-transform kernel (se_xfft.cuh)
@@ -596,18 +632,16 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     int evi = 0;
 #define MARK() do { if (timing) CUDA_TRY(p, cudaEventRecord(p->ev[evi], s)); ++evi; } while (0)
     MARK();
-    // ---- a1: wrap + counting sorts + packing ----
-    CUDA_TRY(p, cudaMemsetAsync(p->d_cnt_all, 0, sizeof(int) * (size_t)p->ncell_all, s));
-    k_keys<<<nbN, TB, 0, s>>>(c, p->gg, pos, p->d_key_r, p->d_rank_r, p->d_cnt_r, p->d_key_s, p->d_rank_s, p->d_cnt_s,
-                              p->d_key_g, p->d_rank_g, p->d_cnt_g);
-    p->last_launches += 1;
-    se_status st = scan_cells(p, s);
-    if (st != SE_OK) return st;
-    k_scatter<<<(c.N + SCATTER_THREADS - 1) / SCATTER_THREADS, SCATTER_THREADS, scatter_smem_bytes(c.rec_stride), s>>>(
-        c, pos, p->d_radii, F, T, S, s_in, p->d_key_r, p->d_rank_r, p->d_start_r, p->d_key_s, p->d_rank_s, p->d_start_s,
-        p->d_key_g, p->d_rank_g, p->d_start_g, p->d_gperm, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig, p->d_recs);
-    p->last_launches += 1;
-    CUDA_TRY(p, cudaGetLastError());
+    // ---- a1: wrap + counting sorts + packing; with cached positions (pos == NULL) only the moments are refreshed ----
+    if (pos) {
+        p->have_positions = false;
+        const se_status st = sort_and_pack(p, pos, F, T, S, s_in, s);
+        if (st != SE_OK) return st;
+    } else {
+        k_moments<<<nbN, TB, 0, s>>>(c, F, T, S, s_in, p->d_dst_rs, p->d_rs_mom, p->d_recs);
+        p->last_launches += 1;
+        CUDA_TRY(p, cudaGetLastError());
+    }
     MARK();
     // ---- a2: real-space pair sum ----
     // a2 is independent of the wave pipeline: it runs on the plan's (low-priority) side stream, forked here and

@@ -127,7 +127,7 @@ __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const doubl
                           const int *__restrict__ key_s, const int *__restrict__ rank_s, const int *__restrict__ start_s,
                           const int *__restrict__ key_g, const int *__restrict__ rank_g, const int *__restrict__ start_g,
                           int *__restrict__ gperm, double4 *__restrict__ rs_pos, double *__restrict__ rs_mom, int *__restrict__ rs_orig,
-                          double *__restrict__ recs)
+                          double *__restrict__ recs, int2 *__restrict__ dst_rs)   // dst_rs[i] = (cell-order index, record index)
 {
     extern __shared__ __align__(16) double sc_rows[];          // [SCATTER_THREADS][rec_stride + 1] then int dst[]
     const int pitch = c.rec_stride + 1;
@@ -140,8 +140,12 @@ __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const doubl
     double xw[3];
 #pragma unroll
     for (int d = 0; d < 3; ++d) xw[d] = se_wrap(pos[i3 + d], c.L);
-    const double f[3] = { F[i3], F[i3 + 1], F[i3 + 2] }, t[3] = { T[i3], T[i3 + 1], T[i3 + 2] };
-    const double s[5] = { S[i5], S[i5 + 1], S[i5 + 2], S[i5 + 3], S[i5 + 4] };
+    // F == NULL: positions only (se_plan_set_positions); the moments are filled in later by k_moments
+    double f[3] = { 0.0, 0.0, 0.0 }, t[3] = { 0.0, 0.0, 0.0 }, s[5] = { 0.0, 0.0, 0.0, 0.0, 0.0 };
+    if (F) {
+        f[0] = F[i3]; f[1] = F[i3 + 1]; f[2] = F[i3 + 2]; t[0] = T[i3]; t[1] = T[i3 + 1]; t[2] = T[i3 + 2];
+        s[0] = S[i5]; s[1] = S[i5 + 1]; s[2] = S[i5 + 2]; s[3] = S[i5 + 3]; s[4] = S[i5 + 4];
+    }
 
     // real-space copy
     const int dr = start_r[key_r[i]] + rank_r[i];
@@ -155,6 +159,7 @@ __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const doubl
     // spreading / gather record
     const int ds = start_s[key_s[i]] + rank_s[i];
     gperm[start_g[key_g[i]] + rank_g[i]] = ds;               // gather order -> record
+    dst_rs[i] = make_int2(dr, ds);
     double *r = sc_rows + threadIdx.x * pitch;
     sc_dst[threadIdx.x] = ds;
     int n0w[3];
@@ -200,6 +205,28 @@ __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const doubl
         double *__restrict__ dst = recs + (size_t)ds * c.rec_stride;
         for (int q = lane; q < c.rec_stride; q += 32) dst[q] = src[q];
     }
+}
+
+// Positions unchanged since se_plan_set_positions: only the moments of the records and of the real-space copy
+// are refreshed (the sorts, indices and Gaussian tables are reused).
+__global__ void k_moments(SeConst c, const double *__restrict__ F, const double *__restrict__ T, const double *__restrict__ S,
+                          const double *__restrict__ s_in, const int2 *__restrict__ dst_rs, double *__restrict__ rs_mom,
+                          double *__restrict__ recs)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= c.N) return;
+    const size_t i3 = 3 * (size_t)i, i5 = 5 * (size_t)i;
+    const int2 d = dst_rs[i];
+    const double sp = s_in ? s_in[i] : 0.0;
+    double *m = rs_mom + 12 * (size_t)d.x, *r = recs + (size_t)d.y * c.rec_stride;
+    const double f0 = F[i3], f1 = F[i3 + 1], f2 = F[i3 + 2], t0 = T[i3], t1 = T[i3 + 1], t2 = T[i3 + 2];
+    const double s0 = S[i5], s1 = S[i5 + 1], s2 = S[i5 + 2], s3 = S[i5 + 3], s4 = S[i5 + 4];
+    m[0] = f0; m[1] = f1; m[2] = f2; m[3] = t0; m[4] = t1; m[5] = t2;
+    m[6] = s0; m[7] = s1; m[8] = s2; m[9] = s3; m[10] = s4; m[11] = sp;
+    r[REC_F] = f0; r[REC_F + 1] = f1; r[REC_F + 2] = f2;
+    r[REC_T] = t0; r[REC_T + 1] = t1; r[REC_T + 2] = t2;
+    r[REC_S] = s0; r[REC_S + 1] = s1; r[REC_S + 2] = s2; r[REC_S + 3] = s3; r[REC_S + 4] = s4; r[REC_S + 5] = -(s0 + s3);
+    r[REC_SP] = sp;
 }
 
 static inline size_t scatter_smem_bytes(int rec_stride)

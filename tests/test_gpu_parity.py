@@ -383,3 +383,44 @@ def test_apply_is_capturable_in_a_cuda_graph(pk, oracle, workloads):
     torch.cuda.synchronize()
     ref2 = oracle.o2_apply(wl.pos, wl.radii, wl.L, wl.xi, wl.rc, wl.M, wl.P, -2.0 * wl.F, wl.T, wl.S)
     _check_blocks((r.U.cpu().numpy(), r.W.cpu().numpy(), r.E.cpu().numpy()), ref2, TOL)
+
+
+def test_cached_positions_many_right_hand_sides(pk, oracle, workloads):
+    """se_plan_set_positions: a1 runs once, later products pass pos=None and only refresh the moments."""
+    import torch
+    wl = workloads.make_workload("c2")
+    r = Runner(pk, wl)
+    assert r.plan.apply_raw(None, *[t.data_ptr() for t in (r.F, r.T, r.S, r.U, r.W, r.E)]) == 1     # nothing cached yet
+    base = [x.copy() for x in r.run()]
+    r.plan.set_positions(r.pos)
+    r.plan.set_flags(0); r.plan.debug_stop(-1)
+
+    def cached(F, T, S):
+        r.plan.apply(None, F, T, S, r.U, r.W, r.E)
+        torch.cuda.synchronize()
+        return r.U.cpu().numpy().copy(), r.W.cpu().numpy().copy(), r.E.cpu().numpy().copy()
+
+    got = cached(r.F, r.T, r.S)
+    _check_blocks(got, r.oracle(oracle), TOL)
+    for a, b in zip(got, base):
+        assert _rel(a, b) <= 1e-13
+    assert r.plan.last_launch_count() == 6              # a1 is one kernel instead of four
+    again = cached(r.F, r.T, r.S)
+    for a, b in zip(again, got):
+        assert np.array_equal(a, b)                     # fixed summation order: bitwise reproducible
+    rng = np.random.default_rng(9)
+    F2, T2, S2 = rng.standard_normal((wl.N, 3)), rng.standard_normal((wl.N, 3)), rng.standard_normal((wl.N, 5))
+    t = lambda a: torch.tensor(a, device=r.pos.device, dtype=torch.float64)
+    got2 = cached(t(F2), t(T2), t(S2))
+    _check_blocks(got2, oracle.o2_apply(wl.pos, wl.radii, wl.L, wl.xi, wl.rc, wl.M, wl.P, F2, T2, S2), TOL)
+    # compressible entry point with the cached configuration
+    s_np = rng.standard_normal(wl.N)
+    s_out = torch.empty((wl.N,), device=r.pos.device, dtype=torch.float64)
+    r.plan.apply_compressible(None, t(F2), t(T2), t(S2), t(s_np), r.U, r.W, r.E, s_out)
+    torch.cuda.synchronize()
+    refc = oracle.o2_apply(wl.pos, wl.radii, wl.L, wl.xi, wl.rc, wl.M, wl.P, F2, T2, S2, s=s_np)
+    _check_blocks((r.U.cpu().numpy(), r.W.cpu().numpy(), r.E.cpu().numpy()), refc, TOL)
+    assert _rel(s_out.cpu().numpy(), refc["s_out"]) <= TOL
+    # a new configuration through the normal entry point drops the cache; so does set_shape
+    _check_blocks(r.run(), r.oracle(oracle), TOL)
+    assert r.plan.apply_raw(None, *[t_.data_ptr() for t_ in (r.F, r.T, r.S, r.U, r.W, r.E)]) == 1
