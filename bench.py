@@ -101,6 +101,48 @@ def cpu_oracle_seconds(wl, repeats=1):
     return best, O.num_threads()
 
 
+def measure_config(name, dev, peak, steps):
+    """Cold-path product of one more configuration (north_star: every config reported at 1 GPU): device-timed
+    ms per product, stage times, algorithmic HBM fractions of the three grid kernels."""
+    import torch
+    import workloads as W
+    import paper_1506_08481_b200 as pk
+    wl = W.make_workload(name)
+    plan = pk.SePlan(wl.N, wl.L, wl.radii, wl.xi, wl.rc, wl.M, wl.P, wl.eta0)
+    t = lambda a: torch.tensor(np.ascontiguousarray(a), device=dev, dtype=torch.float64)
+    pos, F, T, S = t(wl.pos), t(wl.F), t(wl.T), t(wl.S)
+    U = torch.empty((wl.N, 3), device=dev, dtype=torch.float64)
+    Om = torch.empty_like(U)
+    E = torch.empty((wl.N, 5), device=dev, dtype=torch.float64)
+    stream = torch.cuda.current_stream()
+    for _ in range(3):
+        plan.apply(pos, F, T, S, U, Om, E)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(steps):
+        plan.apply(pos, F, T, S, U, Om, E)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    plan.set_flags(pk.SE_TIMING)
+    stage = {k: 0.0 for k in pk.STAGE_NAMES}
+    for _ in range(steps):
+        plan.apply(pos, F, T, S, U, Om, E)
+        for k, v in plan.timings().items():
+            stage[k] += v / steps
+    G = float(wl.M) ** 3
+    Gc = float(wl.M) ** 2 * (wl.M // 2 + 1)
+    alg = {"spread": 24.0 * G + 120.0 * wl.N, "kspace": 144.0 * Gc, "gather": 48.0 * G + 120.0 * wl.N}
+    out = {"N": wl.N, "M": wl.M, "P": wl.P, "ms_per_step": ms, "products_per_s": 1e3 / ms, "ns_per_particle": 1e6 * ms / wl.N,
+           "stages_ms": {k: round(v, 4) for k, v in stage.items()},
+           "hbm_frac": {k: alg[k] / (stage[k] * 1e-3) / 1e9 / peak for k in alg}}
+    plan.destroy()
+    del pos, F, T, S, U, Om, E
+    torch.cuda.empty_cache()
+    return out
+
+
 def run_reference(args, rank, world):
     """--impl reference: the CPU oracle timed on the host cores, rank 0 only."""
     if rank != 0:
@@ -138,6 +180,7 @@ def main():
     ap.add_argument("--config", default="c4", choices=["c1", "c2", "c3", "c4", "c5"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the c1-c3, c5 lines of 'all_configs'")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -288,6 +331,15 @@ def main():
         cpu = {"value": 1.0 / sec, "unit": UNIT, "cores": threads, "kind": "oracle",
                "sample": f"one full {args.config} product (oracle O2 as it stands, gcc -O2 -fopenmp), {sec:.2f} s"}
 
+    others = {}
+    if world == 1 and not args.no_other_configs and not args.no_cpu_baseline:
+        for name in ("c1", "c2", "c3", "c5"):
+            if name != args.config:
+                try:
+                    others[name] = measure_config(name, dev, peak, 5 if name == "c5" else args.steps)
+                except Exception as exc:           # e.g. not enough memory on a shared device: reported, not fatal
+                    others[name] = {"error": str(exc)[:200]}
+
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
@@ -303,6 +355,7 @@ def main():
         "gpu_launches": launches,
         "roofline": roofline,
         "cpu_baseline": cpu,
+        "all_configs": others,
     }
     print(json.dumps(line), flush=True)
     if dist is not None:
