@@ -307,7 +307,8 @@ static se_status ensure_xf(se_plan *p)
     if (st == SE_OK) {
         for (int q = 0; q < M; ++q) { const double a = 2.0 * M_PI * q / M; wt[q].x = cos(a); wt[q].y = -sin(a); }
         if (cudaMemcpy(p->d_wtab, wt, sizeof(double2) * (size_t)M, cudaMemcpyHostToDevice) != cudaSuccess ||
-            cudaFuncSetAttribute(k_xfused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)xf_smem_bytes(M)) != cudaSuccess) {
+            cudaFuncSetAttribute(k_xfused<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)xf_smem_bytes(M)) != cudaSuccess ||
+            cudaFuncSetAttribute(k_xfused<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)xf_smem_bytes(M)) != cudaSuccess) {
             cudaGetLastError();
             st = fail(p, SE_ERR_CUDA, "ensure_xf", "twiddle table / shared-memory attribute");
         }
@@ -692,7 +693,8 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     MARK();
     if (on(SE_STAGE_KSPACE) && use_xf) {
         const unsigned nb = (unsigned)((size_t)c.M * (c.M / 2 + 1) / (XF_ELEMS / c.M));
-        k_xfused<<<nb, XF_THREADS, xf_smem_bytes(c.M), s>>>(c, p->lM, p->d_Hk, p->d_Gk, p->d_wtab);
+        if (xf_lv(c.M) == 4) k_xfused<4><<<nb, XF_THREADS(4), xf_smem_bytes(c.M), s>>>(c, p->lM, p->d_Hk, p->d_Gk, p->d_wtab);
+        else k_xfused<3><<<nb, XF_THREADS(3), xf_smem_bytes(c.M), s>>>(c, p->lM, p->d_Hk, p->d_Gk, p->d_wtab);
         p->last_launches += 1;
         CUDA_TRY(p, cudaGetLastError());
     } else if (on(SE_STAGE_KSPACE)) {
