@@ -15,6 +15,7 @@
 #include "se_spread.cuh"
 #include "se_kspace.cuh"
 #include "se_xfft.cuh"
+#include "se_zfft.cuh"
 #include "se_gather.cuh"
 
 #ifndef M_PI
@@ -67,6 +68,8 @@ struct se_plan {
     bool have_fwd, have_inv;
     cufftHandle fft2_fwd, fft2_inv; // 2-D batched plans of the fused path (se_xfft.cuh)
     bool have_xf;
+    cufftHandle fftz_fwd, fftz_inv; // contiguous batched 2-D complex plans (x,y) of the own-z-transform path (se_zfft.cuh)
+    bool have_zt;
     int lM;
     double2 *d_wtab;               // exp(-2 pi i q / M), q < M
     size_t fft_bytes;
@@ -221,6 +224,7 @@ extern "C" se_status se_plan_destroy(se_plan *p)
         cufftDestroy(p->fft_fwd1); cufftDestroy(p->fft_inv1);
     }
     if (p->have_xf) { cufftDestroy(p->fft2_fwd); cufftDestroy(p->fft2_inv); }
+    if (p->have_zt) { cufftDestroy(p->fftz_fwd); cufftDestroy(p->fftz_inv); }
     cudaFree(p->d_wtab);
     if (p->have_fwd) cufftDestroy(p->fft_fwd);
     if (p->have_inv) cufftDestroy(p->fft_inv);
@@ -286,6 +290,8 @@ static se_status ensure_fft3d(se_plan *p)
     return SE_OK;
 }
 
+static se_status ensure_wtab(se_plan *p);
+
 // Plans and twiddle table of the fused path (se_xfft.cuh): batched 2-D (y,z) transforms, 3M forward and 6M inverse
 // planes; the x transforms run inside k_xfused.
 static se_status ensure_xf(se_plan *p)
@@ -299,27 +305,74 @@ static se_status ensure_xf(se_plan *p)
     if (c1) { r = cufftMakePlanMany(p->fft2_fwd, 2, n2, NULL, 1, 0, NULL, 1, 0, CUFFT_D2Z, 3 * M, &ws); tot += ws; }
     if (r == CUFFT_SUCCESS) { r = cufftCreate(&p->fft2_inv); c2 = (r == CUFFT_SUCCESS); }
     if (r == CUFFT_SUCCESS) { r = cufftMakePlanMany(p->fft2_inv, 2, n2, NULL, 1, 0, NULL, 1, 0, CUFFT_Z2D, 6 * M, &ws); tot += ws; }
-    double2 *wt = (double2 *)malloc(sizeof(double2) * (size_t)M);
     se_status st = SE_OK;
     if (r != CUFFT_SUCCESS) st = fail(p, r == CUFFT_ALLOC_FAILED ? SE_ERR_ALLOC : SE_ERR_CUFFT, "cufftMakePlanMany", "2-D plans");
-    if (st == SE_OK && !wt) st = fail(p, SE_ERR_ALLOC, "malloc", "twiddle table");
-    if (st == SE_OK && !p->d_wtab) st = dev_alloc(p, &p->d_wtab, (size_t)M);
-    if (st == SE_OK) {
-        for (int q = 0; q < M; ++q) { const double a = 2.0 * M_PI * q / M; wt[q].x = cos(a); wt[q].y = -sin(a); }
-        if (cudaMemcpy(p->d_wtab, wt, sizeof(double2) * (size_t)M, cudaMemcpyHostToDevice) != cudaSuccess ||
-            cudaFuncSetAttribute(k_xfused<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)xf_smem_bytes(M)) != cudaSuccess ||
-            cudaFuncSetAttribute(k_xfused<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)xf_smem_bytes(M)) != cudaSuccess) {
-            cudaGetLastError();
-            st = fail(p, SE_ERR_CUDA, "ensure_xf", "twiddle table / shared-memory attribute");
-        }
+    if (st == SE_OK) st = ensure_wtab(p);
+    if (st == SE_OK &&
+        (cudaFuncSetAttribute(k_xfused<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)xf_smem_bytes(M)) != cudaSuccess ||
+         cudaFuncSetAttribute(k_xfused<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)xf_smem_bytes(M)) != cudaSuccess)) {
+        cudaGetLastError();
+        st = fail(p, SE_ERR_CUDA, "ensure_xf", "shared-memory attribute");
     }
-    free(wt);
     if (st != SE_OK) {
         if (c1) cufftDestroy(p->fft2_fwd);
         if (c2) cufftDestroy(p->fft2_inv);
         return st;
     }
     p->have_xf = true;
+    p->lM = 0;
+    while ((1 << p->lM) < M) ++p->lM;
+    p->fft_bytes += tot;
+    p->bytes += tot;
+    return SE_OK;
+}
+
+// Twiddle table exp(-2 pi i q / M), q < M (fused x path and own z transforms).
+static se_status ensure_wtab(se_plan *p)
+{
+    if (p->d_wtab) return SE_OK;
+    const int M = p->c.M;
+    double2 *wt = (double2 *)malloc(sizeof(double2) * (size_t)M);
+    if (!wt) return fail(p, SE_ERR_ALLOC, "malloc", "twiddle table");
+    se_status st = dev_alloc(p, &p->d_wtab, (size_t)M);
+    if (st == SE_OK) {
+        for (int q = 0; q < M; ++q) { const double a = 2.0 * M_PI * q / M; wt[q].x = cos(a); wt[q].y = -sin(a); }
+        if (cudaMemcpy(p->d_wtab, wt, sizeof(double2) * (size_t)M, cudaMemcpyHostToDevice) != cudaSuccess) {
+            cudaGetLastError(); cudaFree(p->d_wtab); p->d_wtab = nullptr;
+            st = fail(p, SE_ERR_CUDA, "cudaMemcpy", "twiddle table");
+        }
+    }
+    free(wt);
+    return st;
+}
+
+// Plans of the own-z-transform path (se_zfft.cuh): contiguous batched 2-D complex transforms over (x,y), 3 (M/2+1)
+// planes forward and 6 (M/2+1) inverse, in place.
+static se_status ensure_zt(se_plan *p)
+{
+    if (p->have_zt) return SE_OK;
+    const int M = p->c.M, Zc = M / 2 + 1;
+    se_status st = ensure_wtab(p);
+    if (st != SE_OK) return st;
+    int n2[2] = { M, M };
+    size_t ws = 0, tot = 0;
+    cufftResult r = cufftCreate(&p->fftz_fwd);
+    bool c1 = (r == CUFFT_SUCCESS), c2 = false;
+    if (c1) { r = cufftMakePlanMany(p->fftz_fwd, 2, n2, NULL, 1, 0, NULL, 1, 0, CUFFT_Z2Z, 3 * Zc, &ws); tot += ws; }
+    if (r == CUFFT_SUCCESS) { r = cufftCreate(&p->fftz_inv); c2 = (r == CUFFT_SUCCESS); }
+    if (r == CUFFT_SUCCESS) { r = cufftMakePlanMany(p->fftz_inv, 2, n2, NULL, 1, 0, NULL, 1, 0, CUFFT_Z2Z, 6 * Zc, &ws); tot += ws; }
+    if (r == CUFFT_SUCCESS &&
+        (cudaFuncSetAttribute(k_zfft_r2c, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zt_smem_bytes(M)) != cudaSuccess ||
+         cudaFuncSetAttribute(k_zfft_c2r, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zt_smem_bytes(M)) != cudaSuccess)) {
+        cudaGetLastError();
+        r = CUFFT_INTERNAL_ERROR;
+    }
+    if (r != CUFFT_SUCCESS) {
+        if (c1) cufftDestroy(p->fftz_fwd);
+        if (c2) cufftDestroy(p->fftz_inv);
+        return fail(p, r == CUFFT_ALLOC_FAILED ? SE_ERR_ALLOC : SE_ERR_CUFFT, "ensure_zt", "2-D complex plans");
+    }
+    p->have_zt = true;
     p->lM = 0;
     while ((1 << p->lM) < M) ++p->lM;
     p->fft_bytes += tot;
@@ -391,10 +444,10 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
         return SE_ERR_CUDA;
     }
 
-    // cuFFT: batched 3-D transforms (the default a4 / a6).  The plans of the opt-in fused path (SE_FUSED_X) are
-    // made by the first apply that asks for it.
+    // cuFFT: power-of-two grids use the own-z-transform path (2-D complex plans, made here); the batched 3-D real plans
+    // and the plans of the fused path (SE_FUSED_X) are made by the first apply that needs them.
     {
-        se_status stf = ensure_fft3d(p);
+        se_status stf = xf_supported(M) ? ensure_zt(p) : ensure_fft3d(p);
         if (stf == SE_OK) stf = make_tensor_map(p, &p->tmap, p->d_real, 6 * M);
         if (stf != SE_OK) { se_plan_destroy(p); return stf; }
     }
@@ -441,7 +494,7 @@ extern "C" se_status se_plan_set_tuning(se_plan *p, int spread_segments, int gat
 
 extern "C" se_status se_plan_set_flags(se_plan *p, unsigned flags)
 {
-    if (!p || (flags & ~0x3fu)) return SE_ERR_INVALID_ARG;
+    if (!p || (flags & ~0x7fu)) return SE_ERR_INVALID_ARG;
     p->flags = flags;
     return SE_OK;
 }
@@ -619,6 +672,11 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     // opt-in: 2-D cuFFT + fused x-transform / k-space / x-transform kernel (se_xfft.cuh)
     const bool use_xf = (p->flags & SE_FUSED_X) && xf_supported(p->c.M) && !comp;
     if (use_xf) { se_status stf = ensure_xf(p); if (stf != SE_OK) return stf; }
+    // default for power-of-two grids: own z transforms with transposed spectra + contiguous 2-D complex cuFFT plans
+    // (se_zfft.cuh); otherwise, and with SE_CUFFT3D, cuFFT's 3-D real transforms
+    const bool use_zt = !use_xf && !(p->flags & SE_CUFFT3D) && xf_supported(p->c.M) && !comp;
+    if (use_zt) { se_status stf = ensure_zt(p); if (stf != SE_OK) return stf; }
+    if (!use_zt && !use_xf) { se_status stf = ensure_fft3d(p); if (stf != SE_OK) return stf; }
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const SeConst &c = p->c;
     const unsigned fl = p->flags;
@@ -682,6 +740,13 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     if (on(SE_STAGE_FFT_FWD) && use_xf) {
         CUFFT_TRY(p, cufftSetStream(p->fft2_fwd, s));
         CUFFT_TRY(p, cufftExecD2Z(p->fft2_fwd, p->d_real, (cufftDoubleComplex *)p->d_Hk));
+    } else if (on(SE_STAGE_FFT_FWD) && use_zt) {
+        const int M = c.M;
+        k_zfft_r2c<<<3 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_real, p->d_Hk, p->d_wtab);
+        p->last_launches += 1;
+        CUDA_TRY(p, cudaGetLastError());
+        CUFFT_TRY(p, cufftSetStream(p->fftz_fwd, s));
+        CUFFT_TRY(p, cufftExecZ2Z(p->fftz_fwd, (cufftDoubleComplex *)p->d_Hk, (cufftDoubleComplex *)p->d_Hk, CUFFT_FORWARD));
     } else if (on(SE_STAGE_FFT_FWD)) {
         CUFFT_TRY(p, cufftSetStream(p->fft_fwd, s));
         CUFFT_TRY(p, cufftExecD2Z(p->fft_fwd, p->d_real, (cufftDoubleComplex *)p->d_Hk));
@@ -699,9 +764,10 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
         CUDA_TRY(p, cudaGetLastError());
     } else if (on(SE_STAGE_KSPACE)) {
         const size_t Gc = (size_t)c.M * c.M * (c.M / 2 + 1);
-        k_kspace<<<(unsigned)((Gc + KSPACE_THREADS - 1) / KSPACE_THREADS), KSPACE_THREADS, 0, s>>>(c, p->d_Hk, p->d_Gk,
-                                                                                                   comp_in ? p->d_Hk_s : nullptr,
-                                                                                                   comp_out ? p->d_Gk_p : nullptr);
+        const unsigned nbk = (unsigned)((Gc + KSPACE_THREADS - 1) / KSPACE_THREADS);
+        if (use_zt) k_kspace<true><<<nbk, KSPACE_THREADS, 0, s>>>(c, p->d_Hk, p->d_Gk, nullptr, nullptr);
+        else k_kspace<false><<<nbk, KSPACE_THREADS, 0, s>>>(c, p->d_Hk, p->d_Gk, comp_in ? p->d_Hk_s : nullptr,
+                                                            comp_out ? p->d_Gk_p : nullptr);
         p->last_launches += 1;
         CUDA_TRY(p, cudaGetLastError());
     }
@@ -709,6 +775,13 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     if (on(SE_STAGE_FFT_INV) && use_xf) {
         CUFFT_TRY(p, cufftSetStream(p->fft2_inv, s));
         CUFFT_TRY(p, cufftExecZ2D(p->fft2_inv, (cufftDoubleComplex *)p->d_Gk, p->d_real));
+    } else if (on(SE_STAGE_FFT_INV) && use_zt) {
+        const int M = c.M;
+        CUFFT_TRY(p, cufftSetStream(p->fftz_inv, s));
+        CUFFT_TRY(p, cufftExecZ2Z(p->fftz_inv, (cufftDoubleComplex *)p->d_Gk, (cufftDoubleComplex *)p->d_Gk, CUFFT_INVERSE));
+        k_zfft_c2r<<<6 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk, p->d_real, p->d_wtab);
+        p->last_launches += 1;
+        CUDA_TRY(p, cudaGetLastError());
     } else if (on(SE_STAGE_FFT_INV)) {
         CUFFT_TRY(p, cufftSetStream(p->fft_inv, s));
         CUFFT_TRY(p, cufftExecZ2D(p->fft_inv, (cufftDoubleComplex *)p->d_Gk, p->d_real));

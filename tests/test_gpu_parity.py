@@ -200,7 +200,7 @@ def test_host_entry_point_and_stage_timings(pk, oracle, workloads):
     _check_blocks((U, W, E), ref, TOL)
     tm = r.plan.timings()
     assert set(tm) == set(pk.STAGE_NAMES) and all(v >= 0 for v in tm.values()) and sum(tm.values()) > 0
-    assert r.plan.last_launch_count() == 9
+    assert r.plan.last_launch_count() == 11             # a1: 4, real, spread, z r2c, k-space, z c2r, gather, epilogue
     assert r.plan.workspace_bytes() > 6 * 8 * wl.M ** 3
 
 
@@ -332,11 +332,12 @@ def test_compressible_extension_full_size_c4(pk, oracle, workloads):
 @pytest.mark.parametrize("name", ["c1", "c2", "c3"])
 def test_fused_x_transform_kspace_path_agrees(pk, oracle, workloads, name):
     """SE_FUSED_X: 2-D cuFFT + one kernel for the x transform, the k-space pass and the inverse x transform,
-    instead of 3-D cuFFT + k_kspace.  Both must give the oracle's returned grids and the same product."""
+    instead of the default (own z transforms with transposed spectra + contiguous 2-D complex cuFFT + k_kspace).
+    SE_CUFFT3D: cuFFT's batched 3-D real transforms.  All must give the oracle's returned grids and the same product."""
     wl = workloads.make_workload(name)
     r = Runner(pk, wl)
     ref = r.oracle(oracle, want_grids=True)
-    for flags in (0, pk.SE_FUSED_X):
+    for flags in (0, pk.SE_FUSED_X, pk.SE_CUFFT3D):
         r.run(flags=flags, stop=5)
         Gr = r.plan.copy_grids(1)
         for g in range(6):
@@ -404,7 +405,7 @@ def test_cached_positions_many_right_hand_sides(pk, oracle, workloads):
     _check_blocks(got, r.oracle(oracle), TOL)
     for a, b in zip(got, base):
         assert _rel(a, b) <= 1e-13
-    assert r.plan.last_launch_count() == 6              # a1 is one kernel instead of four
+    assert r.plan.last_launch_count() == 8              # a1 is one kernel instead of four
     again = cached(r.F, r.T, r.S)
     for a, b in zip(again, got):
         assert np.array_equal(a, b)                     # fixed summation order: bitwise reproducible
