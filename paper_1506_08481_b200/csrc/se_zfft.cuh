@@ -25,6 +25,66 @@ __host__ __device__ inline int zt_pitch(int Nh) { return (xf_sk<4>(Nh) + 1) | 1;
 static inline size_t zt_smem_bytes(int M) { return (size_t)(ZT_LINES * zt_pitch(M / 2) + M / 2 + M / 2 + 1) * 16; }
 static inline int zt_threads(int M) { return ZT_LINES * (M / 2) / 16; }
 
+// One Stockham stage on one line as xf_stage<4, R, INV> (se_xfft.cuh), with the line's input taken straight from
+// global memory (GIN: the first stage of the forward transform reads the real row as Nh complex values) or its
+// output written straight to global memory (GOUT: the last stage of the inverse transform writes the real row):
+// two shared-memory passes fewer per transform.
+template <int R, bool INV, bool GIN, bool GOUT>
+__device__ __forceinline__ void zt_stage(cplx *__restrict__ line, const double2 *__restrict__ gin, double2 *__restrict__ gout,
+                                         const cplx *__restrict__ W, int M, int lNs, int jj)
+{
+    constexpr int V = 16, NB = V / R;
+    const int M16 = M >> 4, Ns = 1 << lNs;
+    cplx v[V];
+#pragma unroll
+    for (int q = 0; q < V; ++q) {
+        if (GIN) { const double2 t = __ldcs(gin + jj + q * M16); v[q] = { t.x, t.y }; }
+        else v[q] = line[xf_sk<4>(jj + q * M16)];
+    }
+    if (!GIN) __syncwarp();
+    const int twstep = M >> (lNs + (R == 16 ? 4 : R == 8 ? 3 : R == 4 ? 2 : 1));
+#pragma unroll
+    for (int u = 0; u < NB; ++u) {
+        const int j = jj + u * M16, k = j & (Ns - 1);
+        if (lNs > 0) {
+#pragma unroll
+            for (int r = 1; r < R; ++r) {
+                cplx w = W[r * k * twstep];
+                if (INV) w.y = -w.y;
+                v[u + r * NB] = cmul(v[u + r * NB], w);
+            }
+        }
+        RegFft<R, NB, INV>::run(v + u);
+        const int base = ((j >> lNs) << lNs) * R + k;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            if (GOUT) __stcs(gout + base + r * Ns, make_double2(v[u + r * NB].x, v[u + r * NB].y));
+            else line[xf_sk<4>(base + r * Ns)] = v[u + r * NB];
+        }
+    }
+    if (!GOUT) __syncwarp();
+}
+
+// Length-Nh transform of one line (Nh = 2^lNh >= 16): radix-16 stages, then one stage of the remaining radix.
+template <bool INV, bool GIN, bool GOUT>
+__device__ __forceinline__ void zt_fft(cplx *__restrict__ line, const double2 *__restrict__ gin, double2 *__restrict__ gout,
+                                       const cplx *__restrict__ W, int Nh, int lNh, int jj)
+{
+    int lNs = 0;
+    while (lNh - lNs >= 4) {
+        const bool first = lNs == 0, last = lNs + 4 == lNh;
+        if (GIN && first && GOUT && last) zt_stage<16, INV, true, true>(line, gin, gout, W, Nh, lNs, jj);
+        else if (GIN && first) zt_stage<16, INV, true, false>(line, gin, gout, W, Nh, lNs, jj);
+        else if (GOUT && last) zt_stage<16, INV, false, true>(line, gin, gout, W, Nh, lNs, jj);
+        else zt_stage<16, INV, false, false>(line, gin, gout, W, Nh, lNs, jj);
+        lNs += 4;
+    }
+    const int rem = lNh - lNs;                     // 0 .. 3: the last stage, never the first (Nh >= 16)
+    if (rem == 3) { if (GOUT) zt_stage<8, INV, false, true>(line, gin, gout, W, Nh, lNs, jj); else zt_stage<8, INV, false, false>(line, gin, gout, W, Nh, lNs, jj); }
+    else if (rem == 2) { if (GOUT) zt_stage<4, INV, false, true>(line, gin, gout, W, Nh, lNs, jj); else zt_stage<4, INV, false, false>(line, gin, gout, W, Nh, lNs, jj); }
+    else if (rem == 1) { if (GOUT) zt_stage<2, INV, false, true>(line, gin, gout, W, Nh, lNs, jj); else zt_stage<2, INV, false, false>(line, gin, gout, W, Nh, lNs, jj); }
+}
+
 // H: [ng][M][M][M] real -> spec: [ng][M/2+1][M][M] complex.  Wtab: [M] complex, exp(-2 pi i q / M).
 // Grid: ng * M * (M / ZT_LINES) CTAs of ZT_LINES * Nh / 16 threads.
 __global__ void __launch_bounds__(ZT_LINES * 16) k_zfft_r2c(int M, int lNh, const double *__restrict__ H, double2 *__restrict__ spec,
@@ -39,33 +99,24 @@ __global__ void __launch_bounds__(ZT_LINES * 16) k_zfft_r2c(int M, int lNh, cons
     for (int q = tid; q < Nh; q += nt) { const double2 w = Wtab[2 * q]; WN[q] = { w.x, w.y }; }
     for (int q = tid; q <= Nh; q += nt) { const double2 w = q < M ? Wtab[q] : make_double2(1.0, 0.0); WP[q] = { w.x, w.y }; }
     const double2 *__restrict__ rows = reinterpret_cast<const double2 *>(H + ((size_t)gx * M + y0) * M);
-    {   // ZT_LINES * Nh = 16 nt values: all sixteen loads of a thread in flight before the first is stored
-        double2 v[16];
-#pragma unroll
-        for (int q = 0; q < 16; ++q) v[q] = __ldcs(rows + tid + q * nt);          // the block's rows are contiguous
-#pragma unroll
-        for (int q = 0; q < 16; ++q) {
-            const int e = tid + q * nt, r = e >> lNh, n = e & (Nh - 1);
-            L[r * LP + xf_sk<4>(n)] = { v[q].x, v[q].y };
-        }
-    }
-    __syncthreads();
-    {
+    __syncthreads();                                   // twiddle tables
+    {   // the first stage reads the real rows straight from global memory (sixteen loads per thread in flight)
         const int tpl = Nh >> 4, line = tid / tpl, jj = tid - line * tpl;
-        xf_fft<4, false>(L + line * LP, WN, Nh, lNh, jj);
+        zt_fft<false, true, false>(L + line * LP, rows + (size_t)line * Nh, nullptr, WN, Nh, lNh, jj);
     }
     __syncthreads();
     double2 *__restrict__ out = spec + (((size_t)g * Zc) * M + x) * M + y0;
     const size_t kstride = (size_t)M * M;
-    for (int e = tid; e < Zc * ZT_LINES; e += nt) {
-        const int k = e / ZT_LINES, r = e - k * ZT_LINES;
-        const cplx zk = L[r * LP + xf_sk<4>(k & (Nh - 1))], zm = L[r * LP + xf_sk<4>((Nh - k) & (Nh - 1))];
-        const cplx w = WP[k];
-        const double sr = zk.x + zm.x, si = zk.y - zm.y;          // Z_k + conj Z_{Nh-k}
-        const double dr = zk.x - zm.x, di = zk.y + zm.y;          // Z_k - conj Z_{Nh-k}
-        // -i w d = -i (wr + i wi)(dr + i di) = (wr di + wi dr) - i (wr dr - wi di)
-        const double tr = w.x * di + w.y * dr, ti = -(w.x * dr - w.y * di);
-        __stcs(out + (size_t)k * kstride + r, make_double2(0.5 * (sr + tr), 0.5 * (si + ti)));
+    // split step on the fly, the pair (k, Nh - k) from one read of Z_k and Z_{Nh-k}: k = 0 also gives X_Nh
+    for (int e = tid; e < (Nh / 2 + 1) * ZT_LINES; e += nt) {
+        const int k = e / ZT_LINES, r = e - k * ZT_LINES, km = Nh - k;
+        const cplx zk = L[r * LP + xf_sk<4>(k)], zm = L[r * LP + xf_sk<4>(km & (Nh - 1))];
+        auto xfrom = [&](cplx a, cplx b, cplx w) {                // 1/2 [ (a + conj b) - i w (a - conj b) ]
+            const double sr = a.x + b.x, si = a.y - b.y, dr = a.x - b.x, di = a.y + b.y;
+            return make_double2(0.5 * (sr + (w.x * di + w.y * dr)), 0.5 * (si - (w.x * dr - w.y * di)));
+        };
+        __stcs(out + (size_t)k * kstride + r, xfrom(zk, zm, WP[k]));
+        if (km != k) __stcs(out + (size_t)km * kstride + r, xfrom(zm, zk, WP[km]));
     }
 }
 
@@ -83,47 +134,40 @@ __global__ void __launch_bounds__(ZT_LINES * 16) k_zfft_c2r(int M, int lNh, cons
     for (int q = tid; q <= Nh; q += nt) { const double2 w = q < M ? Wtab[q] : make_double2(1.0, 0.0); WP[q] = { w.x, -w.y }; }   // w^{-k}
     const double2 *__restrict__ in = spec + (((size_t)g * Zc) * M + x) * M + y0;
     const size_t kstride = (size_t)M * M;
-    // X_k of the ZT_LINES lines, k = 0 .. Nh (position Nh sits one past the skewed Nh - 1)
-    {   // Zc * ZT_LINES = 16 nt + ZT_LINES values: sixteen batched loads per thread, then the k = Nh row
-        double2 v[16];
-#pragma unroll
-        for (int q = 0; q < 16; ++q) { const int e = tid + q * nt; v[q] = __ldcs(in + (size_t)(e / ZT_LINES) * kstride + (e % ZT_LINES)); }
-#pragma unroll
-        for (int q = 0; q < 16; ++q) {
-            const int e = tid + q * nt, k = e / ZT_LINES, r = e - k * ZT_LINES;
-            L[r * LP + xf_sk<4>(k)] = { v[q].x, v[q].y };
-        }
-        if (tid < ZT_LINES) {
-            const double2 w = __ldcs(in + (size_t)Nh * kstride + tid);
-            L[tid * LP + xf_sk<4>(Nh - 1) + 1] = { w.x, w.y };
-        }
-    }
-    __syncthreads();
-    // split step in place: the pair (k, Nh - k) is read and written by one thread
-    for (int e = tid; e < (Nh / 2 + 1) * ZT_LINES; e += nt) {
-        const int k = e / ZT_LINES, r = e - k * ZT_LINES, km = Nh - k;
-        cplx *ln = L + r * LP;
-        const int pk = xf_sk<4>(k), pm = km < Nh ? xf_sk<4>(km) : xf_sk<4>(Nh - 1) + 1;
-        const cplx xk = ln[pk], xm = ln[pm];
-        auto zfrom = [&](cplx a, cplx b, cplx w) {                // (a + conj b) + i w (a - conj b)
-            const double sr = a.x + b.x, si = a.y - b.y, dr = a.x - b.x, di = a.y + b.y;
-            return cplx{ sr - (w.x * di + w.y * dr), si + (w.x * dr - w.y * di) };
-        };
-        const cplx zk = zfrom(xk, xm, WP[k]);
-        const cplx zm = zfrom(xm, xk, WP[km]);
-        ln[pk] = zk;
-        if (km < Nh && km != k) ln[pm] = zm;
-    }
-    __syncthreads();
+    __syncthreads();                                   // twiddle tables
+    // load with the split step fused: the pair (X_k, X_{Nh-k}) gives Z_k and Z_{Nh-k}; nine pairs per thread in flight
     {
-        const int tpl = Nh >> 4, line = tid / tpl, jj = tid - line * tpl;
-        xf_fft<4, true>(L + line * LP, WN, Nh, lNh, jj);
+        constexpr int NPQ = 9;                             // (Nh/2 + 1) ZT_LINES = 8 nt + ZT_LINES pairs
+        double2 a[NPQ], b[NPQ];
+        const int npair = (Nh / 2 + 1) * ZT_LINES;
+#pragma unroll
+        for (int q = 0; q < NPQ; ++q) {
+            const int e = tid + q * nt;
+            if (e < npair) {
+                const int k = e / ZT_LINES, r = e - k * ZT_LINES;
+                a[q] = __ldcs(in + (size_t)k * kstride + r);
+                b[q] = __ldcs(in + (size_t)(Nh - k) * kstride + r);
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < NPQ; ++q) {
+            const int e = tid + q * nt;
+            if (e < npair) {
+                const int k = e / ZT_LINES, r = e - k * ZT_LINES, km = Nh - k;
+                auto zfrom = [&](double2 x, double2 y, cplx w) {      // (x + conj y) + i w (x - conj y)
+                    const double sr = x.x + y.x, si = x.y - y.y, dr = x.x - y.x, di = x.y + y.y;
+                    return cplx{ sr - (w.x * di + w.y * dr), si + (w.x * dr - w.y * di) };
+                };
+                cplx *ln = L + r * LP;
+                ln[xf_sk<4>(k)] = zfrom(a[q], b[q], WP[k]);
+                if (km < Nh && km != k) ln[xf_sk<4>(km)] = zfrom(b[q], a[q], WP[km]);
+            }
+        }
     }
     __syncthreads();
-    double2 *__restrict__ rows = reinterpret_cast<double2 *>(R + ((size_t)gx * M + y0) * M);
-    for (int e = tid; e < ZT_LINES * Nh; e += nt) {
-        const int r = e >> lNh, n = e & (Nh - 1);
-        const cplx v = L[r * LP + xf_sk<4>(n)];
-        __stcs(rows + (size_t)r * Nh + n, make_double2(v.x, v.y));
+    {   // the last stage writes the real rows straight to global memory
+        double2 *__restrict__ rows = reinterpret_cast<double2 *>(R + ((size_t)gx * M + y0) * M);
+        const int tpl = Nh >> 4, line = tid / tpl, jj = tid - line * tpl;
+        zt_fft<true, false, true>(L + line * LP, nullptr, rows + (size_t)line * Nh, WN, Nh, lNh, jj);
     }
 }
