@@ -305,7 +305,7 @@ def main():
     dom = max(("spread", "kspace", "gather"), key=lambda k: stage[k])
     achieved = alg_bytes[dom] / (stage[dom] * 1e-3) / 1e9
     # dram__bytes_read.sum + dram__bytes_write.sum per launch, from the ncu --set full capture summarised in
-    # profiles/r01e_summary.md (c4 only; other configs have no capture)
+    # profiles/r01g_summary.md (c4 only; other configs have no capture)
     traffic_c4 = {"spread": 0.0895e9 + 352.0e6, "kspace": 0.4028e9 + 754.1e6, "gather": 1.4570e9 + 21.9e6}
     traffic = traffic_c4.get(dom) if args.config == "c4" else None
     # spreading and gather are FP64-issue bound before they are HBM bound: 12 N P^3 DFMA each
