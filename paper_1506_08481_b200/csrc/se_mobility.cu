@@ -362,8 +362,10 @@ static se_status ensure_zt(se_plan *p)
     if (r == CUFFT_SUCCESS) { r = cufftCreate(&p->fftz_inv); c2 = (r == CUFFT_SUCCESS); }
     if (r == CUFFT_SUCCESS) { r = cufftMakePlanMany(p->fftz_inv, 2, n2, NULL, 1, 0, NULL, 1, 0, CUFFT_Z2Z, 6 * Zc, &ws); tot += ws; }
     if (r == CUFFT_SUCCESS &&
-        (cudaFuncSetAttribute(k_zfft_r2c, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zt_smem_bytes(M)) != cudaSuccess ||
-         cudaFuncSetAttribute(k_zfft_c2r, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zt_smem_bytes(M)) != cudaSuccess)) {
+        (cudaFuncSetAttribute(k_zfft_r2c<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zt_smem_bytes(M)) != cudaSuccess ||
+         cudaFuncSetAttribute(k_zfft_c2r<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zt_smem_bytes(M)) != cudaSuccess ||
+         cudaFuncSetAttribute(k_zfft_r2c<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zt_smem_bytes(M)) != cudaSuccess ||
+         cudaFuncSetAttribute(k_zfft_c2r<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zt_smem_bytes(M)) != cudaSuccess)) {
         cudaGetLastError();
         r = CUFFT_INTERNAL_ERROR;
     }
@@ -742,7 +744,8 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
         CUFFT_TRY(p, cufftExecD2Z(p->fft2_fwd, p->d_real, (cufftDoubleComplex *)p->d_Hk));
     } else if (on(SE_STAGE_FFT_FWD) && use_zt) {
         const int M = c.M;
-        k_zfft_r2c<<<3 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_real, p->d_Hk, p->d_wtab);
+        if (zt_threads(M) <= 128) k_zfft_r2c<128><<<3 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_real, p->d_Hk, p->d_wtab);
+        else k_zfft_r2c<256><<<3 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_real, p->d_Hk, p->d_wtab);
         p->last_launches += 1;
         CUDA_TRY(p, cudaGetLastError());
         CUFFT_TRY(p, cufftSetStream(p->fftz_fwd, s));
@@ -779,7 +782,8 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
         const int M = c.M;
         CUFFT_TRY(p, cufftSetStream(p->fftz_inv, s));
         CUFFT_TRY(p, cufftExecZ2Z(p->fftz_inv, (cufftDoubleComplex *)p->d_Gk, (cufftDoubleComplex *)p->d_Gk, CUFFT_INVERSE));
-        k_zfft_c2r<<<6 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk, p->d_real, p->d_wtab);
+        if (zt_threads(M) <= 128) k_zfft_c2r<128><<<6 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk, p->d_real, p->d_wtab);
+        else k_zfft_c2r<256><<<6 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk, p->d_real, p->d_wtab);
         p->last_launches += 1;
         CUDA_TRY(p, cudaGetLastError());
     } else if (on(SE_STAGE_FFT_INV)) {

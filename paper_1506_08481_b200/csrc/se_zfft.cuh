@@ -18,6 +18,9 @@
 
 #ifndef ZT_LINES
 #define ZT_LINES 16
+#ifndef ZT_MINB
+#define ZT_MINB 4               // resident CTAs per SM aimed at for blocks of <= 128 threads (M <= 256); 5 spills and is slower
+#endif
 #endif
 
 // pitch of a line in shared memory (complex values): skewed positions of Nh + 1 values, made odd
@@ -87,7 +90,8 @@ __device__ __forceinline__ void zt_fft(cplx *__restrict__ line, const double2 *_
 
 // H: [ng][M][M][M] real -> spec: [ng][M/2+1][M][M] complex.  Wtab: [M] complex, exp(-2 pi i q / M).
 // Grid: ng * M * (M / ZT_LINES) CTAs of ZT_LINES * Nh / 16 threads.
-__global__ void __launch_bounds__(ZT_LINES * 16) k_zfft_r2c(int M, int lNh, const double *__restrict__ H, double2 *__restrict__ spec,
+template <int NT>
+__global__ void __launch_bounds__(NT, NT <= 128 ? ZT_MINB : 2) k_zfft_r2c(int M, int lNh, const double *__restrict__ H, double2 *__restrict__ spec,
                                                            const double2 *__restrict__ Wtab)
 {
     extern __shared__ __align__(16) unsigned char zt_smem[];
@@ -121,7 +125,8 @@ __global__ void __launch_bounds__(ZT_LINES * 16) k_zfft_r2c(int M, int lNh, cons
 }
 
 // spec: [ng][M/2+1][M][M] complex -> R: [ng][M][M][M] real (unnormalised inverse).
-__global__ void __launch_bounds__(ZT_LINES * 16) k_zfft_c2r(int M, int lNh, const double2 *__restrict__ spec, double *__restrict__ R,
+template <int NT>
+__global__ void __launch_bounds__(NT, NT <= 128 ? ZT_MINB : 2) k_zfft_c2r(int M, int lNh, const double2 *__restrict__ spec, double *__restrict__ R,
                                                            const double2 *__restrict__ Wtab)
 {
     extern __shared__ __align__(16) unsigned char zt_smem[];
