@@ -55,7 +55,7 @@ typedef enum {
                                          grids 32 <= M <= 512 take the faster default: the z transforms (real <->
                                          half-complex) by own kernels that keep the spectra transposed, [kz][x][y], so
                                          that cuFFT only runs contiguous batched 2-D complex plans over (x,y).  Other
-                                         M and the compressible entry point always use the 3-D transforms.          */
+                                         M always use the 3-D transforms.                                           */
 
 /* stage indices of se_plan_get_timings */
 enum {

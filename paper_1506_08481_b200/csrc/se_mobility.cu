@@ -60,6 +60,8 @@ struct se_plan {
     double2 *d_Hk_s, *d_Gk_p;      // their spectra
     double *d_pmom;                // [N][12] gathered pressure sums
     cufftHandle fft_fwd1, fft_inv1;
+    cufftHandle fftz_1;            // 2-D complex plan over (x,y), M/2+1 planes: the scalar / pressure grid on the own-z path
+    bool have_fftz1;
     bool have_comp;
     double *d_moments;             // [N][24] gathered wave-space sums in caller order
     // host-API staging
@@ -222,6 +224,7 @@ extern "C" se_status se_plan_destroy(se_plan *p)
     if (p->have_comp) {
         cudaFree(p->d_real_p); cudaFree(p->d_Hk_s); cudaFree(p->d_Gk_p); cudaFree(p->d_pmom);
         cufftDestroy(p->fft_fwd1); cufftDestroy(p->fft_inv1);
+        if (p->have_fftz1) cufftDestroy(p->fftz_1);
     }
     if (p->have_xf) { cufftDestroy(p->fft2_fwd); cufftDestroy(p->fft2_inv); }
     if (p->have_zt) { cufftDestroy(p->fftz_fwd); cufftDestroy(p->fftz_inv); }
@@ -619,6 +622,14 @@ static se_status ensure_compressible(se_plan *p)
         cudaGetLastError();
         return st;
     }
+    if (xf_supported(M)) {
+        int n2[2] = { M, M };
+        size_t ws = 0;
+        if (cufftCreate(&p->fftz_1) == CUFFT_SUCCESS) {
+            if (cufftMakePlanMany(p->fftz_1, 2, n2, NULL, 1, 0, NULL, 1, 0, CUFFT_Z2Z, M / 2 + 1, &ws) == CUFFT_SUCCESS) p->have_fftz1 = true;
+            else cufftDestroy(p->fftz_1);
+        }
+    }
     st = make_tensor_map(p, &p->tmap_p, p->d_real_p, M);
     if (st != SE_OK) {
         cudaFree(p->d_real_p); cudaFree(p->d_Hk_s); cudaFree(p->d_Gk_p); cudaFree(p->d_pmom);
@@ -676,7 +687,7 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     if (use_xf) { se_status stf = ensure_xf(p); if (stf != SE_OK) return stf; }
     // default for power-of-two grids: own z transforms with transposed spectra + contiguous 2-D complex cuFFT plans
     // (se_zfft.cuh); otherwise, and with SE_CUFFT3D, cuFFT's 3-D real transforms
-    const bool use_zt = !use_xf && !(p->flags & SE_CUFFT3D) && xf_supported(p->c.M) && !comp;
+    const bool use_zt = !use_xf && !(p->flags & SE_CUFFT3D) && xf_supported(p->c.M) && (!comp || p->have_fftz1);
     if (use_zt) { se_status stf = ensure_zt(p); if (stf != SE_OK) return stf; }
     if (!use_zt && !use_xf) { se_status stf = ensure_fft3d(p); if (stf != SE_OK) return stf; }
     cudaStream_t s = (cudaStream_t)cuda_stream;
@@ -750,6 +761,14 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
         CUDA_TRY(p, cudaGetLastError());
         CUFFT_TRY(p, cufftSetStream(p->fftz_fwd, s));
         CUFFT_TRY(p, cufftExecZ2Z(p->fftz_fwd, (cufftDoubleComplex *)p->d_Hk, (cufftDoubleComplex *)p->d_Hk, CUFFT_FORWARD));
+        if (comp_in) {
+            if (zt_threads(M) <= 128) k_zfft_r2c<128><<<M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_real_p, p->d_Hk_s, p->d_wtab);
+            else k_zfft_r2c<256><<<M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_real_p, p->d_Hk_s, p->d_wtab);
+            p->last_launches += 1;
+            CUDA_TRY(p, cudaGetLastError());
+            CUFFT_TRY(p, cufftSetStream(p->fftz_1, s));
+            CUFFT_TRY(p, cufftExecZ2Z(p->fftz_1, (cufftDoubleComplex *)p->d_Hk_s, (cufftDoubleComplex *)p->d_Hk_s, CUFFT_FORWARD));
+        }
     } else if (on(SE_STAGE_FFT_FWD)) {
         CUFFT_TRY(p, cufftSetStream(p->fft_fwd, s));
         CUFFT_TRY(p, cufftExecD2Z(p->fft_fwd, p->d_real, (cufftDoubleComplex *)p->d_Hk));
@@ -768,7 +787,8 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     } else if (on(SE_STAGE_KSPACE)) {
         const size_t Gc = (size_t)c.M * c.M * (c.M / 2 + 1);
         const unsigned nbk = (unsigned)((Gc + KSPACE_THREADS - 1) / KSPACE_THREADS);
-        if (use_zt) k_kspace<true><<<nbk, KSPACE_THREADS, 0, s>>>(c, p->d_Hk, p->d_Gk, nullptr, nullptr);
+        if (use_zt) k_kspace<true><<<nbk, KSPACE_THREADS, 0, s>>>(c, p->d_Hk, p->d_Gk, comp_in ? p->d_Hk_s : nullptr,
+                                                                  comp_out ? p->d_Gk_p : nullptr);
         else k_kspace<false><<<nbk, KSPACE_THREADS, 0, s>>>(c, p->d_Hk, p->d_Gk, comp_in ? p->d_Hk_s : nullptr,
                                                             comp_out ? p->d_Gk_p : nullptr);
         p->last_launches += 1;
@@ -786,6 +806,14 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
         else k_zfft_c2r<256><<<6 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk, p->d_real, p->d_wtab);
         p->last_launches += 1;
         CUDA_TRY(p, cudaGetLastError());
+        if (comp_out) {
+            CUFFT_TRY(p, cufftSetStream(p->fftz_1, s));
+            CUFFT_TRY(p, cufftExecZ2Z(p->fftz_1, (cufftDoubleComplex *)p->d_Gk_p, (cufftDoubleComplex *)p->d_Gk_p, CUFFT_INVERSE));
+            if (zt_threads(M) <= 128) k_zfft_c2r<128><<<M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk_p, p->d_real_p, p->d_wtab);
+            else k_zfft_c2r<256><<<M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk_p, p->d_real_p, p->d_wtab);
+            p->last_launches += 1;
+            CUDA_TRY(p, cudaGetLastError());
+        }
     } else if (on(SE_STAGE_FFT_INV)) {
         CUFFT_TRY(p, cufftSetStream(p->fft_inv, s));
         CUFFT_TRY(p, cufftExecZ2D(p->fft_inv, (cufftDoubleComplex *)p->d_Gk, p->d_real));
