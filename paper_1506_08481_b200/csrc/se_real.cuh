@@ -35,7 +35,7 @@ __device__ __forceinline__ void pair_real(const SeConst &c, double x, double y, 
                                           double acc[12])
 {
     const double cFj = aj * aj * (1.0 / 6.0), cSj = aj * aj * 0.1;
-    const double r = sqrt(r2), ir = 1.0 / r, ir2 = ir * ir;
+    const double ir = rsqrt(r2), r = r2 * ir, ir2 = ir * ir;      // one reciprocal square root instead of a root and a division
     const double xr = c.xi * r;
     const double Ec = erfc(xr), qg = c.q * exp(-xr * xr);
     const double ir3 = ir2 * ir, ir4 = ir2 * ir2, ir5 = ir4 * ir, ir6 = ir4 * ir2, ir7 = ir6 * ir, ir8 = ir4 * ir4, ir9 = ir8 * ir;
