@@ -14,7 +14,7 @@
 // positions), twiddles from a table made on the host.  u_k overwrites H_k, w_k goes to a second buffer; CTA-wide
 // barriers only around the load, the k-space pass and the store.
 // Opt-in (flag SE_FUSED_X), for power-of-two 32 <= M <= 512 and without the compressible extension; the default is
-// the 3-D cuFFT + k_kspace path (se_kspace.cuh).  Results agree with that path to FFT round-off.  On B200 the
+// own z transforms + 2-D cuFFT + k_kspace (se_zfft.cuh, se_kspace.cuh).  Results agree to FFT round-off.  On B200 the
 // kernel is bound by shared memory and registers (103 KB and 168 registers per CTA: 12 warps per SM), not by HBM:
 // 0.65 ms at M = 256 against the 0.18 ms HBM floor, which does not yet pay for cuFFT's slower 2-D plans.
 #pragma once
