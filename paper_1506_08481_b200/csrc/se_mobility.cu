@@ -44,6 +44,7 @@ struct se_plan {
     cudaEvent_t ev_fork, ev_join;
     bool have_side;
     int real_side_ctas;            // grid of k_real when it runs beside the wave pipeline (0 = one CTA per cell)
+    int sms;                       // multiprocessors of the plan's device (grid sizing)
     GatherGeom gg;                 // ring gather geometry (spreading's segments are in c.nseg, c.seg_len)
     CUtensorMap tmap, tmap_p;      // TMA descriptors of the six returned grids / of the pressure grid (se_gather.cuh)
     size_t gather_smem;
@@ -138,14 +139,14 @@ static void derive_constants(se_plan *p)
 
 // Sweep segments along x.  Spreading re-processes the particles of the P-1 planes before a segment, the
 // gather re-reads P-1 planes per segment, so segments are long; they exist only to fill the machine:
-// aim at >= 148 SMs x 16 resident warps, segments no shorter than 32 planes.
+// aim at >= 16 resident warps per SM, segments no shorter than 32 planes.
 static void choose_segments(se_plan *p, int spread_segments, int gather_segments)
 {
     SeConst &c = p->c;
     const int npatch = c.NBY * c.NBZ, M = c.M;
     const int maxseg = M / 32 > 1 ? M / 32 : 1;
     auto pick = [&](int want, int warps_per_seg) {
-        int nseg = want > 0 ? want : (148 * 16 + warps_per_seg - 1) / warps_per_seg;
+        int nseg = want > 0 ? want : (p->sms * 16 + warps_per_seg - 1) / warps_per_seg;
         if (nseg > maxseg && want <= 0) nseg = maxseg;
         if (nseg > M) nseg = M;
         if (nseg < 1) nseg = 1;
@@ -159,7 +160,7 @@ static void choose_segments(se_plan *p, int spread_segments, int gather_segments
     int ng = gather_segments;
     if (ng <= 0) {
         const int items = g.NTY * g.NTZ * 6;
-        ng = (148 * 8 + items - 1) / items;
+        ng = (p->sms * 8 + items - 1) / items;
         if (ng < 2) ng = 2;                            // two segments measured best at c4 (more items, small warm-up cost)
         if (ng > maxseg) ng = maxseg;
     }
@@ -194,7 +195,7 @@ static bool choose_gather_geometry(se_plan *p)
         g.slot_d = (g.WY * g.WZ + 15) & ~15;
         if (g.WY > 256 || g.WZ > 256) continue;          // TMA box limits
         g.nseg = 1; g.seg_len = M;
-        const bool few_items = (long long)g.NTY * g.NTZ * 6 * (M >= 64 ? 2 : 1) < 2 * 148 && g.TY * g.TZ > 64;
+        const bool few_items = (long long)g.NTY * g.NTZ * 6 * (M >= 64 ? 2 : 1) < 2 * p->sms && g.TY * g.TZ > 64;
         if (gather_smem_bytes(g, P) <= (cd[3] == 2 ? two : one) && !few_items) {
             p->gg = g; p->gather_smem = gather_smem_bytes(g, P);
             return true;
@@ -203,7 +204,22 @@ static bool choose_gather_geometry(se_plan *p)
     return false;
 }
 
-static cudaError_t dispatch_prepare(int P, size_t smem, size_t gsmem);
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-kernel, process-wide limit: it is set to the device's opt-in
+// maximum (minus the kernel's static shared memory), never to one plan's own need, so that a later plan with a smaller
+// requirement cannot lower the limit an earlier plan still relies on.
+template <typename K>
+static cudaError_t raise_smem_limit(K kernel)
+{
+    int dev = 0, optin = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    cudaFuncAttributes fa;
+    if (e == cudaSuccess) e = cudaFuncGetAttributes(&fa, kernel);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, optin - (int)fa.sharedSizeBytes);
+    return e;
+}
+
+static cudaError_t dispatch_prepare(int P);
 
 extern "C" const char *se_version(void) { return "se_mobility 0.1 (sm_100a)"; }
 
@@ -311,9 +327,7 @@ static se_status ensure_xf(se_plan *p)
     se_status st = SE_OK;
     if (r != CUFFT_SUCCESS) st = fail(p, r == CUFFT_ALLOC_FAILED ? SE_ERR_ALLOC : SE_ERR_CUFFT, "cufftMakePlanMany", "2-D plans");
     if (st == SE_OK) st = ensure_wtab(p);
-    if (st == SE_OK &&
-        (cudaFuncSetAttribute(k_xfused<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)xf_smem_bytes(M)) != cudaSuccess ||
-         cudaFuncSetAttribute(k_xfused<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)xf_smem_bytes(M)) != cudaSuccess)) {
+    if (st == SE_OK && (raise_smem_limit(k_xfused<3>) != cudaSuccess || raise_smem_limit(k_xfused<4>) != cudaSuccess)) {
         cudaGetLastError();
         st = fail(p, SE_ERR_CUDA, "ensure_xf", "shared-memory attribute");
     }
@@ -365,10 +379,8 @@ static se_status ensure_zt(se_plan *p)
     if (r == CUFFT_SUCCESS) { r = cufftCreate(&p->fftz_inv); c2 = (r == CUFFT_SUCCESS); }
     if (r == CUFFT_SUCCESS) { r = cufftMakePlanMany(p->fftz_inv, 2, n2, NULL, 1, 0, NULL, 1, 0, CUFFT_Z2Z, 6 * Zc, &ws); tot += ws; }
     if (r == CUFFT_SUCCESS &&
-        (cudaFuncSetAttribute(k_zfft_r2c<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zt_smem_bytes(M)) != cudaSuccess ||
-         cudaFuncSetAttribute(k_zfft_c2r<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zt_smem_bytes(M)) != cudaSuccess ||
-         cudaFuncSetAttribute(k_zfft_r2c<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zt_smem_bytes(M)) != cudaSuccess ||
-         cudaFuncSetAttribute(k_zfft_c2r<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zt_smem_bytes(M)) != cudaSuccess)) {
+        (raise_smem_limit(k_zfft_r2c<128>) != cudaSuccess || raise_smem_limit(k_zfft_c2r<128>) != cudaSuccess ||
+         raise_smem_limit(k_zfft_r2c<256>) != cudaSuccess || raise_smem_limit(k_zfft_c2r<256>) != cudaSuccess)) {
         cudaGetLastError();
         r = CUFFT_INTERNAL_ERROR;
     }
@@ -404,6 +416,12 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
     c.N = (int)N; c.M = M; c.P = P; c.L = L; c.xi = xi; c.rc2 = r_c * r_c; c.eta0 = eta0;
     p->m = sqrt(M_PI * P);
     derive_constants(p);
+    {
+        int dev = 0, sms = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) sms = 0;
+        cudaGetLastError();
+        p->sms = sms > 0 ? sms : 148;                  // without a device the allocations below fail anyway
+    }
 
     // real-space cell grid: edge >= r_c, at least 3 cells per axis, else all pairs (one cell)
     int ncr = (int)floor(L / r_c);
@@ -470,13 +488,9 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
     p->have_side = true;
     {   // beside the wave pipeline a2 runs as a persistent grid of one CTA per SM (measured best on B200: it then
         // takes little from the HBM-bound kernels' occupancy; c4 step 3.57 -> 3.50 ms)
-        int dev = 0, sms = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) sms = 0;
-        cudaGetLastError();
-        p->real_side_ctas = sms;
+        p->real_side_ctas = p->sms;
     }
-    if (cudaFuncSetAttribute(k_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)scatter_smem_bytes(c.rec_stride)) != cudaSuccess ||
-        dispatch_prepare(P, sweep_smem_bytes(c.rec_stride), p->gather_smem) != cudaSuccess) { cudaGetLastError(); se_plan_destroy(p); return SE_ERR_CUDA; }
+    if (raise_smem_limit(k_scatter) != cudaSuccess || dispatch_prepare(P) != cudaSuccess) { cudaGetLastError(); se_plan_destroy(p); return SE_ERR_CUDA; }
     *out = p;
     return SE_OK;
 }
@@ -556,11 +570,11 @@ static void launch_gather(se_plan *p, cudaStream_t s, bool pressure)
 }
 
 template <int P>
-static cudaError_t prepare_sweeps(size_t smem, size_t gsmem)
+static cudaError_t prepare_sweeps()
 {
-    cudaError_t e = cudaFuncSetAttribute(k_spread<P, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_spread<P, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_gather<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsmem);
+    cudaError_t e = raise_smem_limit(k_spread<P, 3>);
+    if (e == cudaSuccess) e = raise_smem_limit(k_spread<P, 4>);
+    if (e == cudaSuccess) e = raise_smem_limit(k_gather<P>);
     return e;
 }
 
@@ -576,10 +590,10 @@ static void dispatch_spread(se_plan *p, cudaStream_t s, bool comp_in)
     }
 }
 
-static cudaError_t dispatch_prepare(int P, size_t smem, size_t gsmem)
+static cudaError_t dispatch_prepare(int P)
 {
     switch (P) {
-#define X(v) case v: return prepare_sweeps<v>(smem, gsmem);
+#define X(v) case v: return prepare_sweeps<v>();
         FOR_EACH_P(X)
 #undef X
     }

@@ -248,6 +248,62 @@ def test_overlapping_and_coincident_particles(pk, oracle, workloads):
 
 
 # ------------------------------------------------------------------------------------------------
+# Dense / degenerate branches of the kernels (round-1 review: never reached by c1-c5)
+# ------------------------------------------------------------------------------------------------
+def test_real_space_many_candidates_per_cell_and_all_pairs(pk, oracle, workloads):
+    """(a) 3 cells per axis, so the 27 neighbour cells hold all 3000 particles: the staged-candidate chunks of the
+    real-space kernel beyond the first (accumulating branch).  (b) fewer than 3 cells per axis with N = 3000: the
+    all-pairs path with several chunks and more than one target slice per CTA."""
+    wl = workloads.make_uniform_system(1, 3000, 0.3, 64, 12, 1.0 / 3.001)
+    r = Runner(pk, wl)
+    assert r.plan.constants()["real_cells"] == 3
+    ref_real = r.oracle(oracle, parts=oracle.PART_REAL)
+    _check_blocks(r.run(flags=pk.SE_SKIP_WAVE | pk.SE_SKIP_SELF | pk.SE_SKIP_ONEBODY), ref_real, TOL_STAGE)
+    _check_blocks(r.run(), r.oracle(oracle), TOL)
+    wl2 = workloads.make_uniform_system(1, 3000, 0.3, 64, 12, 0.45)
+    r2 = Runner(pk, wl2)
+    assert r2.plan.constants()["real_cells"] == 1
+    ref_real2 = r2.oracle(oracle, parts=oracle.PART_REAL)
+    _check_blocks(r2.run(flags=pk.SE_SKIP_WAVE | pk.SE_SKIP_SELF | pk.SE_SKIP_ONEBODY), ref_real2, TOL_STAGE)
+    _check_blocks(r2.run(), r2.oracle(oracle), TOL)
+
+
+@pytest.mark.parametrize("M,P", [(48, 12), (64, 10)])
+def test_clustered_particles_overflow_the_spreading_bins(pk, oracle, workloads, M, P):
+    """300 of 400 particles have their support origin in ONE plane-thin spreading bin (1 x 4 x 8 grid cells) and in
+    one gather tile: the bin-overflow path of the spreading kernel and a maximally dense gather tile, per stage."""
+    wl = workloads.make_clustered_system(1, 400, 300, 20.0, M, P, 6.0)
+    r = Runner(pk, wl)
+    ref = r.oracle(oracle, want_grids=True)
+    r.run(stop=2)
+    assert _rel(r.plan.copy_grids(0), ref["gridH"]) <= TOL_STAGE
+    r.run(stop=5)
+    Gr = r.plan.copy_grids(1)
+    for g in range(6):
+        assert _rel(Gr[g], ref["gridOut"][g]) <= TOL_STAGE, g
+    ref_wave = r.oracle(oracle, parts=oracle.PART_WAVE)
+    _check_blocks(r.run(flags=pk.SE_SKIP_REAL | pk.SE_SKIP_SELF | pk.SE_SKIP_ONEBODY), ref_wave, TOL_STAGE)
+    ref_real = r.oracle(oracle, parts=oracle.PART_REAL)
+    _check_blocks(r.run(flags=pk.SE_SKIP_WAVE | pk.SE_SKIP_SELF | pk.SE_SKIP_ONEBODY), ref_real, TOL_STAGE)
+    _check_blocks(r.run(), ref, TOL)
+
+
+def test_plans_of_different_sizes_interleaved(pk, oracle, workloads):
+    """A later, smaller plan must not shrink what an earlier plan's kernels may use (dynamic shared-memory limits
+    are per kernel and process-wide): c3-sized plan, then c1, then the first one again; different P likewise."""
+    wl_big = workloads.make_workload("c3")
+    big = Runner(pk, wl_big)
+    ref_big = big.oracle(oracle)
+    _check_blocks(big.run(), ref_big, TOL)
+    small = Runner(pk, workloads.make_workload("c1"))
+    _check_blocks(small.run(), small.oracle(oracle), TOL)
+    other = Runner(pk, workloads.make_workload("c1"), M=32, P=6)
+    _check_blocks(other.run(), other.oracle(oracle), TOL)
+    _check_blocks(big.run(), ref_big, TOL)
+    _check_blocks(small.run(), small.oracle(oracle), TOL)
+
+
+# ------------------------------------------------------------------------------------------------
 # T11: compressible extension (a9): pressure moments in, pressure interaction out
 # ------------------------------------------------------------------------------------------------
 def _pressure_moments(wl, seed=11):

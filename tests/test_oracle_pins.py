@@ -59,6 +59,31 @@ def test_self_terms_equal_the_k_integral(oracle):
         assert got[2] == pytest.approx(es, rel=1e-11)
 
 
+def test_one_body_faxen_terms_printed_denominators(oracle, workloads):
+    """Eq. 13-15: with every interaction switched off (parts = PART_ONEBODY) both oracles must
+    return F/(6 pi eta0 a), T/(8 pi eta0 a^3), S/((20/3) pi eta0 a^3) with the PRINTED denominators, for a
+    polydisperse system and a viscosity that is not 1 (on-fluid moments, reading 1: plus signs)."""
+    dU, dW, num, den = _gold("faxen_onebody.txt")
+    sysm = workloads.random_small_system(5, 6, 9.0)
+    rad, eta0 = sysm["radii"], 0.37
+    F, T, S = sysm["F"], sysm["T"], sysm["S"]
+    assert len(set(np.round(rad, 6))) > 1                      # really polydisperse
+    want_U = F / (dU * math.pi * eta0 * rad[:, None])
+    want_W = T / (dW * math.pi * eta0 * rad[:, None] ** 3)
+    want_E = S / ((num / den) * math.pi * eta0 * rad[:, None] ** 3)
+    U, W, E, _ = oracle.o1_apply(sysm["pos"], rad, sysm["L"], 0.6, F, T, S, eta0=eta0, nimg=1, kmax=1,
+                                 parts=oracle.PART_ONEBODY)
+    assert _rel(U, want_U) < 1e-15 and _rel(W, want_W) < 1e-15 and _rel(E, want_E) < 1e-15
+    o2 = oracle.o2_apply(sysm["pos"], rad, sysm["L"], 0.6, 4.0, 16, 8, F, T, S, eta0=eta0, parts=oracle.PART_ONEBODY)
+    assert _rel(o2["U"], want_U) < 1e-15 and _rel(o2["Omega"], want_W) < 1e-15 and _rel(o2["E"], want_E) < 1e-15
+    # the full product contains exactly this term: (all parts) - (all but one-body) = the printed one-body part
+    nimg, kmax = _ewald_cut(0.6, sysm["L"])
+    full = oracle.o1_apply(sysm["pos"], rad, sysm["L"], 0.6, F, T, S, eta0=eta0, nimg=nimg, kmax=kmax)
+    rest = oracle.o1_apply(sysm["pos"], rad, sysm["L"], 0.6, F, T, S, eta0=eta0, nimg=nimg, kmax=kmax,
+                           parts=oracle.PART_ALL & ~oracle.PART_ONEBODY)
+    assert _rel(full[2] - rest[2], want_E) < 1e-12 and _rel(full[0] - rest[0], want_U) < 1e-12
+
+
 # ------------------------------------------------------------------------------------------------
 # Eq. 22 and everything generated from it, against brute-force numerical differentiation
 # ------------------------------------------------------------------------------------------------

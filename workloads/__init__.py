@@ -236,3 +236,44 @@ def shard_range(n_units: int, rank: int, world: int) -> range:
     base, rem = divmod(n_units, world)
     lo = rank * base + min(rank, rem)
     return range(lo, lo + base + (1 if rank < rem else 0))
+
+
+def make_uniform_system(seed: int, N: int, phi: float, M: int, P: int, rc_over_L: float) -> Workload:
+    """Monodisperse (a = 1) RSA suspension with the real-space cutoff given as a fraction of the box edge --
+    parity cases that reach the dense branches of the real-space kernel (many candidates per cell; all pairs)."""
+    rng = np.random.Generator(np.random.PCG64(np.random.SeedSequence([_BASE_SEED, 3000 + seed])))
+    radii = np.ones(N)
+    L = box_edge(radii, phi)
+    pos = rsa_positions(radii, L, int(rng.integers(0, 2 ** 63 - 1)))
+    F, T, S = make_moments(N, rng)
+    xi, _ = resolve_split(L, M)
+    return Workload(name=f"uniform{seed}", N=N, L=L, radii=radii, pos=pos, F=F, T=T, S=S, xi=xi, rc=rc_over_L * L,
+                    M=M, P=P, m=math.sqrt(math.pi * P), eta0=1.0, phi=phi, meta=dict(radii="mono", positions="rsa"))
+
+
+def make_clustered_system(seed: int, N: int, n_cluster: int, L: float, M: int, P: int, rc: float) -> Workload:
+    """Polydisperse point cloud (overlaps allowed: the formulas are regular for r > 0) in which ``n_cluster`` particles
+    sit inside ONE grid cell column of 1 x 4 x 8 grid spacings, so that their P^3 supports all start in the same
+    plane-thin tile bin -- the degenerate case of the particle<->grid kernels (bin overflow, one dense tile).  The
+    cluster members keep a minimum mutual distance of 0.05 so that the pair terms stay well conditioned."""
+    rng = np.random.Generator(np.random.PCG64(np.random.SeedSequence([_BASE_SEED, 4000 + seed])))
+    radii = 0.6 + 0.9 * rng.random(N)
+    pos = L * rng.random((N, 3))
+    D = L / M
+    # support origin n0 = floor(x / D) - P/2 + 1 (even P): choose the cell column so that n0_y is a multiple of 4 and
+    # n0_z a multiple of 8, the bin edges of the spreading sort
+    assert P % 2 == 0
+    corner = np.array([M // 2 + 1, 4 * (M // 8) + P // 2 - 1, 8 * (M // 16) + P // 2 - 1], dtype=np.float64) * D
+    ext = np.array([0.98 * D, 3.98 * D, 7.98 * D])
+    pts = []
+    while len(pts) < n_cluster:
+        c = corner + 0.01 * D + ext * rng.random(3)
+        if all(np.linalg.norm(c - q) >= 0.05 for q in pts):
+            pts.append(c)
+    pos[:n_cluster] = np.array(pts)
+    perm = rng.permutation(N)
+    radii, pos = np.ascontiguousarray(radii[perm]), np.ascontiguousarray(pos[perm])
+    F, T, S = make_moments(N, rng)
+    xi, _ = resolve_split(L, M)
+    return Workload(name=f"cluster{seed}", N=N, L=L, radii=radii, pos=pos, F=F, T=T, S=S, xi=xi, rc=rc,
+                    M=M, P=P, m=math.sqrt(math.pi * P), eta0=1.0, phi=0.0, meta=dict(radii="uniform[0.6,1.5]", positions="clustered"))
