@@ -45,12 +45,6 @@ typedef enum {
 #define SE_SKIP_SELF     0x4u         /* do not subtract the wave-space self terms (Eq. 37)           */
 #define SE_SKIP_ONEBODY  0x8u         /* do not add the one-body Faxen terms (Eq. 13-15)              */
 #define SE_TIMING        0x10u        /* record CUDA events between stages (se_plan_get_timings)      */
-#define SE_FUSED_X       0x20u        /* opt-in variant of a4-a6 for power-of-two 32 <= M <= 512 (ignored otherwise and
-                                         by the compressible entry point): batched 2-D (y,z) cuFFT transforms and ONE
-                                         kernel doing the x transform, the k-space pass and the inverse x transform in a
-                                         single pass over HBM, instead of 3-D cuFFT + k-space kernel + 3-D cuFFT.  Same
-                                         results to FFT round-off; measured slower on B200 so far       */
-
 #define SE_CUFFT3D       0x40u        /* a4/a6 by cuFFT's batched 3-D real transforms.  Without this flag, power-of-two
                                          grids 32 <= M <= 512 take the faster default: the z transforms (real <->
                                          half-complex) by own kernels that keep the spectra transposed, [kz][x][y], so
@@ -62,9 +56,9 @@ enum {
     SE_STAGE_SORT = 0,                /* a1: wrap, counting sorts by real-space cell and grid tile, packing */
     SE_STAGE_REAL = 1,                /* a2: real-space pair sum                                      */
     SE_STAGE_SPREAD = 2,              /* a3: Gaussian spreading onto the grid                         */
-    SE_STAGE_FFT_FWD = 3,             /* a4: forward FFTs (own z kernel + cuFFT 2-D, or cuFFT 3-D; with SE_FUSED_X the 2-D (y,z) part) */
-    SE_STAGE_KSPACE = 4,              /* a5: fused k-space scaling (on the fused path with both x transforms) */
-    SE_STAGE_FFT_INV = 5,             /* a6: inverse FFTs (cuFFT 2-D + own z kernel, or cuFFT 3-D; with SE_FUSED_X the 2-D (y,z) part) */
+    SE_STAGE_FFT_FWD = 3,             /* a4: forward FFTs (own z kernel + cuFFT 2-D, or cuFFT 3-D)    */
+    SE_STAGE_KSPACE = 4,              /* a5: fused k-space scaling                                    */
+    SE_STAGE_FFT_INV = 5,             /* a6: inverse FFTs (cuFFT 2-D + own z kernel, or cuFFT 3-D)    */
     SE_STAGE_GATHER = 6,              /* a7: Gaussian gather                                          */
     SE_STAGE_EPILOGUE = 7,            /* a8: self / one-body terms, sum, un-permute                   */
     SE_NUM_STAGES = 8

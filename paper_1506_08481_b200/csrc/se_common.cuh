@@ -13,7 +13,8 @@ struct SeConst {
     int N, M, P;
     int ncr;                       // real-space cells per axis (1 = all pairs)
     int NBY, NBZ;                  // spreading tile bins per plane: ceil(M/4), ceil(M/8)
-    int rec_stride;                // doubles per particle record
+    int rec_stride;                // doubles per spreading record
+    int grec_stride;               // doubles per gather record
     int nseg, seg_len;             // sweep segments of the spreading kernel
     double L, MoverL, Delta, alpha, gnorm, eta_se;
     double xi, rc2, eta0, hr;      // hr = real-space cell edge L/ncr
@@ -24,23 +25,36 @@ struct SeConst {
     double D3;                     // Delta^3 (gather quadrature weight)
 };
 
-// Particle record (AoS, rec_stride doubles, 16-byte aligned), in spreading-tile order:
+// Spreading record (AoS, rec_stride doubles, 32-byte aligned), in spreading-tile order:
 //   [0]  int2 (y0w, z0w)   wrapped first support index along y, z
 //   [1]  int2 (x0w, orig)  wrapped first support plane along x (the sweep axis), caller index
-//   [2..4]   d0x, d0y, d0z   offset of the first support point from the particle, (n0 - u) Delta
-//   [5..8]   f0, f1, s0, s1  size polynomials: 1-6 al cF, 4 al^2 cF, 2 al (1-10 al cS), 8 al^3 cS
-//   [9..11] F  [12..14] T  [15..20] S (xx,xy,xz,yy,yz,zz)
-//   [21] cF = a^2/6  [22] cS = a^2/10  [23] pressure moment s (a9; 0 without)
-//   [24..24+P) gx * (al/pi)^{3/2}   [24+P..24+2P) gy   [24+2P..24+3P) gz     per-axis Gaussians
-//   [24+3P..24+6P)  gx dx, gx dx^2, gx dx^3 with dx_k = d0x + k Delta     x-moment tables (P each)
-#define REC_D0 2
-#define REC_POLY 5
-#define REC_F 9
-#define REC_T 12
-#define REC_S 15
+//   [2..3]   d0y, d0z      offset of the first support point from the particle, (n0 - u) Delta
+//   [4..7]   f0, f1, s0, s1  size polynomials: 1-6 al cF, 4 al^2 cF, 2 al (1-10 al cS), 8 al^3 cS
+//   [8..10] F  [11..13] T  [14..19] S (xx,xy,xz,yy,yz,zz)
+//   [20] d0x  [21] cF = a^2/6  [22] cS = a^2/10  [23] pressure moment s (a9; 0 without)
+//   [24..24+P) gy   [24+P..24+2P) gz                      per-axis Gaussians
+//   [XOFF .. XOFF + 8P)  X[j] = (gx, gx dx, gx dx^2, gx dx^3)(j mod P), j < 2P, gx with the factor (al/pi)^{3/2},
+//                        dx_k = d0x + k Delta: the x tables interleaved per support plane and stored TWICE, so
+//                        that the spreading kernel can address them through a rotating register window.
+#define REC_D0Y 2
+#define REC_D0Z 3
+#define REC_POLY 4
+#define REC_F 8
+#define REC_T 11
+#define REC_S 14
+#define REC_D0X 20
 #define REC_CF 21
 #define REC_CS 22
 #define REC_SP 23
+__host__ __device__ inline int se_rec_xoff(int P) { return (SE_REC_HDR + 2 * P + 3) & ~3; }
+__host__ __device__ inline int se_rec_stride(int P) { return se_rec_xoff(P) + 8 * P; }
+
+// Gather record (grec_stride doubles, 16-byte aligned), in gather order (tile major, starting plane minor):
+//   [0] int2 (y0w, z0w)  [1] int2 (x0w, orig)  [2] d0y  [3] d0z
+//   [4 .. 4+PP) gy, [4+PP .. 4+2PP) gz, zero beyond P (PP = P rounded up to a multiple of 8)
+//   [4+2PP .. 4+2PP+2P)  (gx, gx dx)(k) interleaved, gx with the factor (al/pi)^{3/2}
+__host__ __device__ inline int se_grec_pp(int P) { return (P + 7) & ~7; }
+__host__ __device__ inline int se_grec_stride(int P) { return 4 + 2 * se_grec_pp(P) + 2 * P; }
 
 __host__ __device__ inline int se_support_start(double u, int P)
 {

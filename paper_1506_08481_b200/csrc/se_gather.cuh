@@ -6,24 +6,22 @@
 //     A0[g] = sum gamma g,  A1[g] = sum gamma dx g,  Ay[g] = sum gamma dy g,  Az[g] = sum gamma dz g,
 // which this kernel writes to moments[N][24] (caller order); a8 combines them per particle.
 //
-// Design ("plane ring"): a CTA owns one returned grid, one (y,z) tile of TY x TZ support origins and one
-// segment of x.  It streams the planes of its haloed tile, (TY+P-1) x (TZ+P-1) columns, through a ring of R
-// planes in shared memory, R-P planes ahead of the consumers, so every grid value crosses L2->SM once per tile
-// and is then read from shared memory.  The fill has two paths with the same slot layout.  A tile whose halo
-// stays inside the grid takes ONE TMA tensor-box copy per plane (cp.async.bulk.tensor.3d issued by one elected
-// thread, completion counted in bytes by the slot's mbarrier).  A tile whose halo crosses the periodic seam (the
-// last tile row and column) copies the plane with 16-byte cp.async through a table that wraps the coordinates
-// (two producer warps, completion counted by deferred mbarrier arrivals).  Measured on B200: the cp.async path
-// sustains only ~10 B/clk/SM and bounded the whole kernel when every tile used it; a box copy per plane is
-// ~6 times faster, and per-row bulk copies were slower than either.  The particles whose support starts in the tile are sorted by starting plane (a1,
-// second counting sort); the eight consumer warps take them round-robin, ONE WARP PER PARTICLE: the lanes
-// own the P^2 columns of the footprint (all lanes busy), reduce along x in registers,
-//     m0 = sum_k gx(k) g(x0+k),   m1 = sum_k gx(k) dx_k g(x0+k),
-// weight with the (y,z) Gaussian and reduce over the warp once per particle.  Every (particle, grid) pair
-// is produced by exactly one warp in a fixed order: no atomics, no zero-fill, bitwise reproducible.
-// Rows are padded to WZ = P (mod 16) doubles so that the footprint columns of a half-warp fall in
-// distinct shared-memory banks.  Planes are released through per-slot "empty" mbarriers (one arrival per
-// consumer warp), so warps run up to R-P planes apart without CTA-wide barriers.
+// Design ("plane ring", persistent): one CTA per SM walks over work items (returned grid, x segment, (y,z) tile of
+// TY x TZ support origins).  The planes of the item's haloed tile, WY x WZ columns, stream through a ring of R planes
+// in shared memory, filled by ONE TMA tensor-box copy per plane (cp.async.bulk.tensor.3d issued by one elected
+// thread, completion counted in bytes by the slot's "full" mbarrier).  The returned grids are stored with P-1
+// periodic halo rows and columns (written by the inverse z transform itself), so every box lies inside the padded
+// plane: there is no seam path.  The producer runs across item boundaries, so the ring never drains between items.
+// Consumers: the particles whose support starts in the tile are sorted by starting plane (a1); a consumer warp takes
+// TWO particles at a time for P <= 16, one per half-warp (one per warp for larger P).  The 16 lanes of a particle
+// form a 4 x 4 grid (by, bz) and own the footprint columns (by + 4a, bz + 4b): with rows padded to WZ = 4 (mod 8)
+// doubles the sixteen columns of one load fall in sixteen different banks, all other addresses of a lane differ
+// from its first by compile-time constants, and for P = 12 every lane owns exactly nine columns.  A lane reduces
+// along x in registers,   m0 = sum_k gx(k) g(x0+k),   m1 = sum_k gx(k) dx_k g(x0+k),
+// weights with the (y,z) Gaussians and the four sums are reduced over the 16 (32) lanes once per particle.  Every
+// (particle, grid) pair is produced by exactly one half-warp in a fixed order: no atomics, bitwise reproducible.
+// Planes are released through per-slot "empty" mbarriers (one arrival per consumer warp), so warps run up to R-P
+// planes apart without CTA-wide barriers.  Gather records (se_common.cuh) arrive by bulk copies, double-buffered.
 #pragma once
 #include <cuda.h>                  // CUtensorMap (type only; the encoder is fetched through the runtime)
 #include "se_sweep.cuh"
@@ -31,27 +29,39 @@
 
 #define GATHER_SUMS 24             // per particle: slot (g/3)*12 + kind*3 + g%3, kind = 0 (1), 1 (dx), 2 (dy), 3 (dz)
 #ifndef GR_WARPS
-#define GR_WARPS 8                 // consumer warps
+#define GR_WARPS 8                 // consumer warps; warp GR_WARPS is the producer
 #endif
-// Two CTAs per SM hide each other's pipeline bubbles; supports up to GR_P2MAX keep the register budget for it.
-#ifndef GR_P2MAX
-#define GR_P2MAX 14
-#endif
-#define GR_PROD 2                  // producer warps (GR_WARPS, GR_WARPS + 1)
+
+// Compile-time geometry of the gather for support P.
+template <int P> struct GatherTraits {
+    static constexpr bool HALF = P <= 16;                       // two particles per warp
+    static constexpr int LP = HALF ? 16 : 32;                   // lanes per particle
+    static constexpr int LZ = LP / 4;                           // lane grid 4 x LZ
+    static constexpr int CY = (P + 3) / 4, CZ = (P + LZ - 1) / LZ;   // footprint columns per lane: CY x CZ
+    static constexpr int TY = P <= 16 ? 16 : (P <= 20 ? 8 : 2);
+    static constexpr int TZ = P <= 12 ? 32 : (P <= 16 ? 16 : 8);
+    static constexpr int R = P <= 12 ? P + 5 : (P <= 16 ? P + 4 : (P <= 20 ? P + 3 : P + 1));
+    static constexpr int WY = TY + 4 * CY - 1;                  // rows of the haloed tile (>= TY + P - 1)
+    static constexpr int WZ0 = TZ + LZ * CZ - 1;
+    // row pitch = 4 (mod 8) [half-warp particles] or 8 (mod 16) [warp particles]: conflict-free column loads
+    static constexpr int WZ = HALF ? ((WZ0 + 3) / 8) * 8 + 4 : ((WZ0 + 7) / 16) * 16 + 8;
+    static constexpr int SLOT = (WY * WZ + 15) & ~15;           // doubles per ring slot (a multiple of 128 bytes)
+    static constexpr int PP = (P + 7) & ~7;
+    static constexpr int GSTRIDE = 4 + 2 * PP + 2 * P;          // = se_grec_stride(P)
+    static constexpr int NPW = HALF ? 2 : 1;                    // particles per warp pass
+    static constexpr size_t SMEM = (size_t)R * SLOT * 8 + (size_t)GR_WARPS * 2 * NPW * GSTRIDE * 8 + (size_t)R * 16 + GR_WARPS * 16;
+};
 
 __device__ __forceinline__ void mbar_arrive(uint32_t bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void *src)
+__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity)
 {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
-}
-// Arrive on `bar` once all cp.async of this thread issued so far have landed (counted in the barrier's init count).
-__device__ __forceinline__ void cp_async_arrive(uint32_t bar)
-{
-    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
+    uint32_t ok;
+    asm volatile("{\n.reg .pred P1;\nmbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\nselp.u32 %0, 1, 0, P1;\n}"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
 }
 
 // One box of the tensor `tmap` at element coordinates (c0 fastest, c1, c2) into shared memory at `dst`.
@@ -61,208 +71,206 @@ __device__ __forceinline__ void tma_box3(uint32_t dst, const CUtensorMap *tmap, 
                  ::"r"(dst), "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
 }
 
-template <int P>
-__global__ void __launch_bounds__((GR_WARPS + GR_PROD) * 32, (P <= GR_P2MAX ? 2 : 1))
-k_gather(SeConst c, GatherGeom g, const double *__restrict__ recs, const int *__restrict__ gperm,
-         const int *__restrict__ start_g, const double *__restrict__ Gr, const __grid_constant__ CUtensorMap tmap, int ngrids,
-         double *__restrict__ moments, int mstride)
+// Work item `it` of the launch: all tiles of one (grid, segment) are consecutive, so that the CTAs of one round work
+// on neighbouring tiles of the same planes and the halo re-reads hit L2.
+struct GatherItem { int grid, seg_start, nplanes, Y0, Z0, i0, i1; };
+__device__ __forceinline__ GatherItem gather_item(int it, const SeConst &c, const GatherGeom &g, int ngrids, const int *__restrict__ start_g)
 {
+    const int ntile = g.NTY * g.NTZ;
+    const int gs = it / ntile, tile = it - gs * ntile;
+    GatherItem r;
+    r.grid = gs % ngrids;
+    const int seg = gs / ngrids;
+    r.seg_start = seg * g.seg_len;
+    const int seg_end = min(r.seg_start + g.seg_len, c.M);
+    r.nplanes = seg_end - r.seg_start + c.P - 1;
+    const int ty = tile / g.NTZ, tz = tile - ty * g.NTZ;
+    r.Y0 = ty * g.TY; r.Z0 = tz * g.TZ;
+    r.i0 = start_g[tile * c.M + r.seg_start];
+    r.i1 = start_g[tile * c.M + seg_end];
+    return r;
+}
+
+template <int P>
+__global__ void __launch_bounds__((GR_WARPS + 1) * 32, 1)
+k_gather(SeConst c, GatherGeom g, const double *__restrict__ grecs, const int *__restrict__ start_g,
+         const __grid_constant__ CUtensorMap tmap, int ngrids, double *__restrict__ moments, int mstride)
+{
+    using GT = GatherTraits<P>;
+    constexpr int R = GT::R, SLOT = GT::SLOT, WZ = GT::WZ, CY = GT::CY, CZ = GT::CZ, LZ = GT::LZ, LP = GT::LP, NPW = GT::NPW;
+    constexpr int GS = GT::GSTRIDE, PP = GT::PP;
     extern __shared__ __align__(128) unsigned char gsm[];
-    constexpr int PP = P * P, NI = (PP + 31) / 32;
-    constexpr int NREC = SE_REC_HDR + 4 * P, NR = (NREC + 31) / 32;      // record prefix the gather needs
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int M = c.M, stride = c.rec_stride, R = g.R;
-    // Work items in launch order: tile slowest, and the seam tiles (last tile row and column: the slow cp.async
-    // fill, see below) first, so that they do not form the tail of the launch.
-    const int per_tile = ngrids * g.nseg;
-    const int q = blockIdx.x / per_tile, rest = blockIdx.x - q * per_tile;
-    const int grid = rest % ngrids, seg = rest / ngrids;
-    const int nseam = g.NTY + g.NTZ - 1;
-    int ty, tz;
-    if (q < g.NTZ) { ty = g.NTY - 1; tz = q; }
-    else if (q < nseam) { ty = q - g.NTZ; tz = g.NTZ - 1; }
-    else { const int r = q - nseam; ty = r / (g.NTZ - 1); tz = r - ty * (g.NTZ - 1); }
-    const int tile = ty * g.NTZ + tz;
-    const int seg_start = seg * g.seg_len, seg_end = min(seg_start + g.seg_len, M);
-    const int i0 = start_g[tile * M + seg_start], i1 = start_g[tile * M + seg_end];
-    if (i0 == i1) return;                                              // no support starts here
-    const int Y0 = ty * g.TY, Z0 = tz * g.TZ;
-    const int nplanes = seg_end - seg_start + P - 1;
-    const int plane_d = g.slot_d;                                      // doubles per ring slot (a multiple of 128 bytes)
-    // the box [Y0, Y0+WY) x [Z0, Z0+WZ) may reach beyond the grid only in its unused pad columns (zero-filled)
-    const bool use_tma = (Y0 + g.TY + P - 1 <= M) && (Z0 + g.TZ + P - 1 <= M);
-    const int cw = g.WZL >> 1, nch = g.WY * cw;                        // 16-byte chunks per row, per plane
+    const int M = c.M;
+    const int nitems = g.NTY * g.NTZ * ngrids * g.nseg;
 
     double *ring = reinterpret_cast<double *>(gsm);
-    double *rslots = ring + (size_t)R * plane_d;                       // per consumer warp: one record prefix
-    int2 *table = reinterpret_cast<int2 *>(rslots + GR_WARPS * NR * 32);   // per chunk: (offset in a grid plane, offset in a slot)
-    const uint32_t bars = smem_u32(table + nch);
+    double *rbuf = ring + (size_t)R * SLOT;                            // [GR_WARPS][2][NPW][GS] record buffers
+    const uint32_t bars = smem_u32(rbuf + GR_WARPS * 2 * NPW * GS);
     auto full_bar = [&](int sl) { return bars + 16u * (uint32_t)sl; };
     auto empty_bar = [&](int sl) { return bars + 16u * (uint32_t)sl + 8u; };
+    const uint32_t rbars = bars + 16u * R;                             // per consumer warp: two record barriers
     if (threadIdx.x == 0) {
-        for (int sl = 0; sl < R; ++sl) { mbar_init(full_bar(sl), use_tma ? 1 : GR_PROD * 32); mbar_init(empty_bar(sl), GR_WARPS); }
+        for (int sl = 0; sl < R; ++sl) { mbar_init(full_bar(sl), 1); mbar_init(empty_bar(sl), GR_WARPS); }
+        for (int q = 0; q < 2 * GR_WARPS; ++q) mbar_init(rbars + 8u * q, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
-    if (!use_tma) for (int ch = threadIdx.x; ch < nch; ch += blockDim.x) {   // periodic wrap along y and z, once per CTA
-        const int r = ch / cw, col = ch - r * cw;
-        table[ch] = make_int2(((Y0 + r) % M) * M + (Z0 + 2 * col) % M, r * g.WZ + 2 * col);
-    }
     __syncthreads();
 
-    if (w >= GR_WARPS && use_tma) {
-        // ---- producer, interior tile (one elected thread): plane j of the segment goes to slot j % R once every
-        // consumer has released plane j - R; one tensor-box copy per plane.
-        if (w == GR_WARPS && lane == 0) {
-            const uint32_t ring_a = smem_u32(ring), box_bytes = (uint32_t)(g.WY * g.WZ * 8);
-            int sl = 0, x = seg_start;
+    if (w == GR_WARPS) {
+        // ---- producer (one elected thread): plane after plane of item after item; global plane n goes to slot n % R
+        // once every consumer has released plane n - R; one tensor-box copy per plane.
+        if (lane == 0) {
+            const uint32_t ring_a = smem_u32(ring);
+            constexpr uint32_t box_bytes = (uint32_t)(GT::WY * WZ * 8);
+            int sl = 0;
             uint32_t par = 1;                                          // passes at once in round 0
-            for (int j = 0; j < nplanes; ++j) {
-                mbar_wait(empty_bar(sl), par);
-                mbar_expect_tx(full_bar(sl), box_bytes);
-                tma_box3(ring_a + 8u * (uint32_t)(sl * plane_d), &tmap, Z0, Y0, grid * M + x, full_bar(sl));
-                if (++sl == R) { sl = 0; par ^= 1u; }
-                if (++x == M) x = 0;
+            for (int it = blockIdx.x; it < nitems; it += gridDim.x) {
+                const GatherItem I = gather_item(it, c, g, ngrids, start_g);
+                if (I.i0 == I.i1) continue;                            // no support starts here: skipped by everybody
+                int x = I.seg_start;
+                for (int j = 0; j < I.nplanes; ++j) {
+                    mbar_wait(empty_bar(sl), par);
+                    mbar_expect_tx(full_bar(sl), box_bytes);
+                    tma_box3(ring_a + 8u * (uint32_t)(sl * SLOT), &tmap, I.Z0, I.Y0, I.grid * M + x, full_bar(sl));
+                    if (++sl == R) { sl = 0; par ^= 1u; }
+                    if (++x == M) x = 0;
+                }
             }
         }
-        return;
-    }
-    if (w >= GR_WARPS) {
-        // ---- producers, seam tile: as above, with the periodic wrap done by the chunk table.
-        // 16-byte cp.async per chunk (rows are too short for bulk copies to pay); completion is counted by the
-        // slot's "full" mbarrier, one deferred arrival per producer lane.
-        const double *__restrict__ G0 = Gr + (size_t)grid * M * M * M;
-        const int pl = (w - GR_WARPS) * 32 + lane;
-        const uint32_t ring_a = smem_u32(ring);
-        int sl = 0;
-        uint32_t par = 1;                                              // passes at once in round 0
-        int x = seg_start;
-        for (int j = 0; j < nplanes; ++j) {
-            mbar_wait(empty_bar(sl), par);
-            const double *__restrict__ src = G0 + (size_t)x * M * M;
-            const uint32_t dst = ring_a + 8u * (uint32_t)(sl * plane_d);
-            for (int ch = pl; ch < nch; ch += GR_PROD * 32) {
-                const int2 e = table[ch];
-                cp_async16(dst + 8u * (uint32_t)e.y, src + e.x);
-            }
-            cp_async_arrive(full_bar(sl));
-            if (++sl == R) { sl = 0; par ^= 1u; }
-            if (++x == M) x = 0;
-        }
-        asm volatile("cp.async.wait_all;" ::: "memory");
         return;
     }
 
-    // ---- consumers: particle i0 + w, i0 + w + 8, ... (non-decreasing starting plane per warp) ----
-    double *rs = rslots + w * NR * 32;
-    // planes [0, jdone) are known loaded (slot/parity of plane jdone: sdone, pdone); planes [0, jrel) released
-    int jdone = 0, sdone = 0, jrel = 0, srel = 0;
+    // ---- consumers ----
+    // ring state: planes of the current item below jdone are known loaded (slot / parity of plane jdone: sdone, pdone),
+    // planes below jrel are released by this warp (slot of plane jrel: srel).  Every consumer observes every phase of
+    // every slot in order and releases a plane only after having observed it: the parity waits can never alias.
+    int sdone = 0, srel = 0;
     uint32_t pdone = 0;
-    double pre[NR];
-    auto fetch = [&](int ii) {
-        const double *__restrict__ rec = recs + (size_t)gperm[ii] * stride;
-#pragma unroll
-        for (int q = 0; q < NR; ++q) pre[q] = (q * 32 + lane < NREC) ? rec[q * 32 + lane] : 0.0;
-    };
-    auto observe_next = [&]() {
-        mbar_wait(full_bar(sdone), pdone);
-        ++jdone;
-        if (++sdone == R) { sdone = 0; pdone ^= 1u; }
-    };
-    // Every consumer observes every phase of every slot, in order, and releases a plane only after having
-    // observed it: the parity waits can then never alias, however far apart the starting planes are.
-    auto release_below = [&](int jto) {
-        while (jrel < jto) {
-            if (jrel == jdone) observe_next();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(empty_bar(srel));
-            ++jrel;
-            if (++srel == R) srel = 0;
-        }
-    };
-    // lane constants: footprint column lane + 32 q -> (ry, rz), its offset in a slot, its distance from the origin
-    int colof[NI], colry[NI], colrz[NI];
-    bool colok[NI];
-    double coldy[NI], coldz[NI];
-#pragma unroll
-    for (int q = 0; q < NI; ++q) {
-        const int cc = lane + 32 * q;
-        colok[q] = cc < PP;
-        const int cl = min(cc, PP - 1);
-        colry[q] = cl / P; colrz[q] = cl - colry[q] * P;
-        colof[q] = colry[q] * g.WZ + colrz[q];
-        coldy[q] = colry[q] * c.Delta; coldz[q] = colrz[q] * c.Delta;
-    }
-    int i = i0 + w;
-    if (i < i1) fetch(i);
-    for (; i < i1; i += GR_WARPS) {
-        __syncwarp();
-#pragma unroll
-        for (int q = 0; q < NR; ++q) rs[q * 32 + lane] = pre[q];
-        __syncwarp();
-        if (i + GR_WARPS < i1) fetch(i + GR_WARPS);                    // next record in flight during the sums
-        const int2 yz = reinterpret_cast<const int2 *>(rs)[0], xo = reinterpret_cast<const int2 *>(rs)[1];
-        const int j0 = xo.x - seg_start;
-        release_below(j0);                                             // now jrel == j0 and srel == j0 % R
-        while (jdone < j0 + P) observe_next();
+    const int half = NPW == 2 ? lane >> 4 : 0, hl = lane & (LP - 1);
+    const int by = hl / LZ, bz = hl - by * LZ;
+    double *rb = rbuf + (size_t)w * 2 * NPW * GS;
+    const uint32_t rbar0 = rbars + 16u * (uint32_t)w;
+    uint32_t rpar = 0;                                                 // bit b: parity of record buffer b
+    const double Delta = c.Delta;
 
-        const int cb = (yz.x - Y0) * g.WZ + (yz.y - Z0);
-        double m0[NI], m1[NI];
-#pragma unroll
-        for (int q = 0; q < NI; ++q) { m0[q] = 0.0; m1[q] = 0.0; }
-        int sl = srel;
-        const double *__restrict__ X0 = rs + SE_REC_HDR, *__restrict__ X1 = rs + SE_REC_HDR + 3 * P;
-        double gxr[P], gxdr[P];                                        // x tables: loaded before the sums start
-#pragma unroll
-        for (int k = 0; k < P; ++k) { gxr[k] = X0[k]; gxdr[k] = X1[k]; }
-#pragma unroll
-        for (int k = 0; k < P; ++k) {
-            const double *__restrict__ pl = ring + sl * plane_d;
-            const double gx = gxr[k], gxd = gxdr[k];
-#pragma unroll
-            for (int q = 0; q < NI; ++q) {
-                const double v = pl[cb + colof[q]];
-                m0[q] = fma(gx, v, m0[q]);
-                m1[q] = fma(gxd, v, m1[q]);
+    for (int it = blockIdx.x; it < nitems; it += gridDim.x) {
+        const GatherItem I = gather_item(it, c, g, ngrids, start_g);
+        if (I.i0 == I.i1) continue;
+        int jdone = 0, jrel = 0;
+        auto observe_next = [&]() {
+            mbar_wait(full_bar(sdone), pdone);
+            ++jdone;
+            if (++sdone == R) { sdone = 0; pdone ^= 1u; }
+        };
+        auto release_below = [&](int jto) {
+            while (jrel < jto) {
+                if (jrel == jdone) observe_next();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty_bar(srel));
+                ++jrel;
+                if (++srel == R) srel = 0;
             }
-            sl = sl + 1 == R ? 0 : sl + 1;
-        }
-        double s0 = 0.0, s1 = 0.0, sy = 0.0, sz = 0.0;
-        const double d0y = rs[REC_D0 + 1], d0z = rs[REC_D0 + 2];
-        const double *__restrict__ GY = rs + SE_REC_HDR + P, *__restrict__ GZ = rs + SE_REC_HDR + 2 * P;
+        };
+        // passes of this warp: particles i0 + NPW (w + GR_WARPS t) [+ 1]
+        const int npass = (I.i1 - I.i0 + NPW - 1) / NPW;
+        auto stage = [&](int t, int b) {                               // records of pass t into buffer b
+            if (lane == 0) {
+                const int i = I.i0 + NPW * t, n = min(NPW, I.i1 - i);
+                const uint32_t bytes = (uint32_t)(n * GS * 8);
+                mbar_expect_tx(rbar0 + 8u * b, bytes);
+                bulk_g2s(smem_u32(rb + (size_t)b * NPW * GS), grecs + (size_t)i * GS, bytes, rbar0 + 8u * b);
+            }
+        };
+        int b = 0;
+        if (w < npass) stage(w, 0);
+        for (int t = w; t < npass; t += GR_WARPS, b ^= 1) {
+            __syncwarp();                                              // buffer b^1 no longer read by any lane
+            if (t + GR_WARPS < npass) stage(t + GR_WARPS, b ^ 1);
+            mbar_wait(rbar0 + 8u * b, (rpar >> b) & 1u);
+            rpar ^= 1u << b;
+            const bool valid = NPW == 1 || I.i0 + NPW * t + half < I.i1;       // the odd particle out has no partner
+            const double *__restrict__ rs = rb + (size_t)(b * NPW + (valid ? half : 0)) * GS;
+            const int2 yz = reinterpret_cast<const int2 *>(rs)[0], xo = reinterpret_cast<const int2 *>(rs)[1];
+            const int j0 = xo.x - I.seg_start;
+            int jlo = j0, jhi = j0;
+            if (NPW == 2) {
+                const int o = __shfl_xor_sync(0xffffffffu, j0, 16);
+                jlo = min(j0, o); jhi = max(j0, o);
+            }
+            // Two particles whose windows do not fit the ring together take one turn each (then jlo < jhi strictly).
+            const int nturn = (NPW == 2 && jhi - jlo + P > R) ? 2 : 1;
+            for (int turn = 0; turn < nturn; ++turn) {
+                const bool mine = nturn == 1 || j0 == (turn == 0 ? jlo : jhi);
+                const int ja = (nturn == 2 && turn == 1) ? jhi : jlo, jb = (nturn == 2 && turn == 0) ? jlo : jhi;
+                release_below(ja);                                     // now jrel == ja, srel = slot of plane ja
+                while (jdone < jb + P) observe_next();
+                int sl = srel + (mine ? j0 - ja : 0);                  // slot of my first plane (idle lanes: any loaded one)
+                if (sl >= R) sl -= R;
+                const double *__restrict__ col = ring + ((yz.x - I.Y0 + by) * WZ + (yz.y - I.Z0 + bz));
+                double m0[CY][CZ], m1[CY][CZ];
 #pragma unroll
-        for (int q = 0; q < NI; ++q) {
-            const double gyz = colok[q] ? GY[colry[q]] * GZ[colrz[q]] : 0.0;
-            const double a0 = gyz * m0[q];
-            s0 += a0;
-            s1 = fma(gyz, m1[q], s1);
-            sy = fma(d0y + coldy[q], a0, sy);
-            sz = fma(d0z + coldz[q], a0, sz);
-        }
-        // reduce-scatter of the four sums: lane bits (16, 8) select the kind: 00 s0, 01 s1, 10 sy, 11 sz
-        {
-            const bool hi = (lane & 16) != 0;
-            const double a = (hi ? sy : s0) + __shfl_xor_sync(0xffffffffu, hi ? s0 : sy, 16);
-            const double b = (hi ? sz : s1) + __shfl_xor_sync(0xffffffffu, hi ? s1 : sz, 16);
-            const bool h8 = (lane & 8) != 0;
-            double t = (h8 ? b : a) + __shfl_xor_sync(0xffffffffu, h8 ? a : b, 8);
-            t += __shfl_xor_sync(0xffffffffu, t, 4);
-            t += __shfl_xor_sync(0xffffffffu, t, 2);
-            t += __shfl_xor_sync(0xffffffffu, t, 1);
-            if ((lane & 7) == 0) {
-                const int kind = ((lane >> 4) << 1) | ((lane >> 3) & 1);
-                moments[(size_t)xo.y * mstride + (grid / 3) * 12 + kind * 3 + (grid % 3)] = t;
+                for (int a = 0; a < CY; ++a)
+#pragma unroll
+                    for (int q = 0; q < CZ; ++q) { m0[a][q] = 0.0; m1[a][q] = 0.0; }
+                const double2 *__restrict__ GX = reinterpret_cast<const double2 *>(rs + 4 + 2 * PP);
+#pragma unroll
+                for (int k = 0; k < P; ++k) {
+                    const double *__restrict__ pl = col + sl * SLOT;
+                    const double2 gx = GX[k];
+#pragma unroll
+                    for (int a = 0; a < CY; ++a)
+#pragma unroll
+                        for (int q = 0; q < CZ; ++q) {
+                            const double v = pl[4 * a * WZ + LZ * q];
+                            m0[a][q] = fma(gx.x, v, m0[a][q]);
+                            m1[a][q] = fma(gx.y, v, m1[a][q]);
+                        }
+                    sl = sl + 1 == R ? 0 : sl + 1;
+                }
+                // weights: sums over this lane's columns of gy gz {m0, m1, dy m0, dz m0}; gy, gz are zero beyond P
+                const double d0y = rs[2] + by * Delta, d0z = rs[3] + bz * Delta;
+                double gz[CZ], gzd[CZ];
+#pragma unroll
+                for (int q = 0; q < CZ; ++q) { gz[q] = rs[4 + PP + bz + LZ * q]; gzd[q] = gz[q] * (d0z + (LZ * q) * Delta); }
+                double s0 = 0.0, s1 = 0.0, sy = 0.0, sz = 0.0;
+#pragma unroll
+                for (int a = 0; a < CY; ++a) {
+                    double r0 = 0.0, r1 = 0.0, rz = 0.0;
+#pragma unroll
+                    for (int q = 0; q < CZ; ++q) {
+                        r0 = fma(gz[q], m0[a][q], r0);
+                        r1 = fma(gz[q], m1[a][q], r1);
+                        rz = fma(gzd[q], m0[a][q], rz);
+                    }
+                    const double gy = rs[4 + by + 4 * a], gr0 = gy * r0;
+                    s0 += gr0;
+                    s1 = fma(gy, r1, s1);
+                    sy = fma(d0y + (4 * a) * Delta, gr0, sy);
+                    sz = fma(gy, rz, sz);
+                }
+                // reduce-scatter of the four sums over the LP lanes of the particle: the two highest lane bits select
+                // the kind (00 s0, 01 s1, 10 sy, 11 sz), the remaining bits are summed
+                {
+                    constexpr int B1 = LP / 2, B2 = LP / 4;
+                    const bool hi = (hl & B1) != 0;
+                    const double a = (hi ? sy : s0) + __shfl_xor_sync(0xffffffffu, hi ? s0 : sy, B1);
+                    const double bb = (hi ? sz : s1) + __shfl_xor_sync(0xffffffffu, hi ? s1 : sz, B1);
+                    const bool h2 = (hl & B2) != 0;
+                    double tt = (h2 ? bb : a) + __shfl_xor_sync(0xffffffffu, h2 ? a : bb, B2);
+#pragma unroll
+                    for (int o = B2 / 2; o > 0; o >>= 1) tt += __shfl_xor_sync(0xffffffffu, tt, o);
+                    if ((hl & (B2 - 1)) == 0 && valid && mine) {
+                        const int kind = (hi ? 2 : 0) | (h2 ? 1 : 0);
+                        moments[(size_t)xo.y * mstride + (I.grid / 3) * 12 + kind * 3 + (I.grid % 3)] = tt;
+                    }
+                }
             }
         }
+        __syncwarp();
+        release_below(I.nplanes);
     }
-    __syncwarp();
-    release_below(nplanes);
-}
-
-static inline size_t gather_smem_bytes(const GatherGeom &g, int P)
-{
-    const int NR = (SE_REC_HDR + 4 * P + 31) / 32;
-    return (size_t)g.R * g.slot_d * 8 + (size_t)GR_WARPS * NR * 32 * 8 + (size_t)g.WY * (g.WZL / 2) * 8 + (size_t)g.R * 16;
 }
 
 // a8: out = real + wave + (one-body - self) * input, in caller order (Eq. 13-15 one-body terms;

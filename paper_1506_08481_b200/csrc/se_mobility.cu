@@ -34,7 +34,8 @@ struct se_plan {
     double *d_radii;
     int *d_key_r, *d_rank_r, *d_cnt_r, *d_start_r;
     int *d_key_s, *d_rank_s, *d_cnt_s, *d_start_s;
-    int *d_key_g, *d_rank_g, *d_cnt_g, *d_start_g, *d_gperm;
+    int *d_key_g, *d_rank_g, *d_cnt_g, *d_start_g;
+    double *d_grecs;               // gather records [N][grec_stride], gather order
     int2 *d_dst_rs;                // per particle (caller order): index in cell order, record index
     bool have_positions;           // a1 was run by se_plan_set_positions and is reused while pos == NULL
     int *d_cnt_all, *d_start_all;  // the three count / start tables, concatenated (one pad element after each)
@@ -48,16 +49,19 @@ struct se_plan {
     GatherGeom gg;                 // ring gather geometry (spreading's segments are in c.nseg, c.seg_len)
     CUtensorMap tmap, tmap_p;      // TMA descriptors of the six returned grids / of the pressure grid (se_gather.cuh)
     size_t gather_smem;
+    int gWY, gWZ;                  // TMA box of the gather: rows, columns of the haloed tile
+    size_t Gp;                     // doubles per padded returned grid: M * MYp * MZp
+    bool real_p_padded;            // d_real_p currently holds the returned pressure grid (padded layout)
     double4 *d_rs_pos;
     double *d_rs_mom;
     int *d_rs_orig;
     double *d_recs;
-    double *d_real;                // [6][M^3]; the first three double as the spread grids H
+    double *d_real;                // [6][M][MYp][MZp] returned grids with periodic halo; the first 3 M^3 doubles double as the spread grids H
     double2 *d_Hk;                 // [3][M][M][M/2+1]
     double2 *d_Gk;                 // [6][M][M][M/2+1]
     double *d_out_real;            // [N][12] real-space part in caller order (slot 11: pressure, a9)
     // compressible extension (a9): allocated by the first apply that passes s_in or s_out
-    double *d_real_p;              // [M^3]: scalar spread grid Hs, then the returned pressure grid p~
+    double *d_real_p;              // [M][MYp][MZp]: scalar spread grid Hs (first M^3 doubles), then the returned pressure grid p~ (padded)
     double2 *d_Hk_s, *d_Gk_p;      // their spectra
     double *d_pmom;                // [N][12] gathered pressure sums
     cufftHandle fft_fwd1, fft_inv1;
@@ -68,9 +72,7 @@ struct se_plan {
     // host-API staging
     double *d_io;                  // pos3 F3 T3 S5 U3 W3 E5 = 25 N doubles
     cufftHandle fft_fwd, fft_inv;  // 3-D batched plans (unfused path), made when first needed
-    bool have_fwd, have_inv;
-    cufftHandle fft2_fwd, fft2_inv; // 2-D batched plans of the fused path (se_xfft.cuh)
-    bool have_xf;
+    bool have_fwd, have_inv, have_fft1;
     cufftHandle fftz_fwd, fftz_inv; // contiguous batched 2-D complex plans (x,y) of the own-z-transform path (se_zfft.cuh)
     bool have_zt;
     int lM;
@@ -155,13 +157,12 @@ static void choose_segments(se_plan *p, int spread_segments, int gather_segments
     int ns = pick(spread_segments, npatch);
     c.seg_len = (M + ns - 1) / ns;
     c.nseg = (M + c.seg_len - 1) / c.seg_len;
-    // gather: enough (tile, grid, segment) items for ~8 rounds of one CTA per SM, segments of >= 32 planes
+    // gather (persistent, one CTA per SM): enough (tile, grid, segment) items for ~8 rounds, segments of >= 32 planes
     GatherGeom &g = p->gg;
     int ng = gather_segments;
     if (ng <= 0) {
         const int items = g.NTY * g.NTZ * 6;
         ng = (p->sms * 8 + items - 1) / items;
-        if (ng < 2) ng = 2;                            // two segments measured best at c4 (more items, small warm-up cost)
         if (ng > maxseg) ng = maxseg;
     }
     if (ng > M) ng = M;
@@ -170,38 +171,30 @@ static void choose_segments(se_plan *p, int spread_segments, int gather_segments
     g.nseg = (M + g.seg_len - 1) / g.seg_len;
 }
 
-// Ring gather geometry (se_gather.cuh).  Preference: tiles of 16 x 16 support origins with a ring shallow enough
-// for two CTAs per SM (they hide each other's pipeline bubbles; measured best on B200), then one CTA per SM with
-// the largest tile that fits the 227 KB of shared memory; smaller tiles when the grid would otherwise give the
-// 148 SMs too few items.  Rows are padded to WZ = P (mod 16) doubles for even P (P + 1 for odd P: rows must
-// stay 16-byte aligned) so that a half-warp's footprint columns fall in distinct banks.
+#ifndef FOR_EACH_P                 // a development build may define a shorter list on the command line
+#define FOR_EACH_P(X) \
+    X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15) X(16) X(17) X(18) X(19) X(20) X(21) X(22) X(23) X(24)
+#endif
+
+// Ring gather geometry (se_gather.cuh): tile, ring and box are compile-time functions of P (GatherTraits); the padded
+// extents of the returned grids follow from M and P.
 static bool choose_gather_geometry(se_plan *p)
 {
     const int M = p->c.M, P = p->c.P;
-    const size_t one = 227 * 1024 - 1024, two = (228 * 1024) / 2 - 1024;
-    // TY, TZ, ring planes beyond P, CTAs per SM aimed at
-    static const int cand[][4] = { {16, 16, 5, 2}, {16, 16, 3, 2}, {8, 16, 5, 2}, {8, 8, 5, 2}, {16, 32, 7, 1}, {16, 16, 7, 1},
-                                   {8, 16, 7, 1}, {8, 16, 3, 1}, {8, 8, 3, 1}, {4, 8, 2, 1}, {4, 4, 1, 1}, {2, 4, 0, 1}, {2, 2, 0, 1} };
-    for (const auto &cd : cand) {
-        if (cd[3] == 2 && P > GR_P2MAX) continue;
-        GatherGeom g;
-        g.TY = cd[0]; g.TZ = cd[1]; g.R = P + cd[2];
-        g.NTY = (M + g.TY - 1) / g.TY; g.NTZ = (M + g.TZ - 1) / g.TZ;
-        g.WY = g.TY + P - 1;
-        g.WZL = (g.TZ + P - 1 + 1) & ~1;
-        const int want = (P & 1) ? (P + 1) % 16 : P % 16;
-        g.WZ = g.WZL;
-        while (g.WZ % 16 != want) g.WZ += 2;
-        g.slot_d = (g.WY * g.WZ + 15) & ~15;
-        if (g.WY > 256 || g.WZ > 256) continue;          // TMA box limits
-        g.nseg = 1; g.seg_len = M;
-        const bool few_items = (long long)g.NTY * g.NTZ * 6 * (M >= 64 ? 2 : 1) < 2 * p->sms && g.TY * g.TZ > 64;
-        if (gather_smem_bytes(g, P) <= (cd[3] == 2 ? two : one) && !few_items) {
-            p->gg = g; p->gather_smem = gather_smem_bytes(g, P);
-            return true;
-        }
+    GatherGeom &g = p->gg;
+    switch (P) {
+#define X(v) case v: g.TY = GatherTraits<v>::TY; g.TZ = GatherTraits<v>::TZ; p->gWY = GatherTraits<v>::WY; p->gWZ = GatherTraits<v>::WZ; \
+                     p->gather_smem = GatherTraits<v>::SMEM; break;
+        FOR_EACH_P(X)
+#undef X
+        default: return false;
     }
-    return false;
+    g.NTY = (M + g.TY - 1) / g.TY; g.NTZ = (M + g.TZ - 1) / g.TZ;
+    g.MYp = M + P - 1;
+    g.MZp = (M + P + 3) & ~3;                          // >= M + P, rows start on 32-byte boundaries
+    g.nseg = 1; g.seg_len = M;
+    p->Gp = (size_t)M * g.MYp * g.MZp;
+    return p->gather_smem <= 227 * 1024;
 }
 
 // cudaFuncAttributeMaxDynamicSharedMemorySize is a per-kernel, process-wide limit: it is set to the device's opt-in
@@ -230,7 +223,7 @@ extern "C" se_status se_plan_destroy(se_plan *p)
     if (!p) return SE_OK;
     cudaFree(p->d_radii);
     cudaFree(p->d_key_r); cudaFree(p->d_rank_r); cudaFree(p->d_key_s); cudaFree(p->d_rank_s);
-    cudaFree(p->d_key_g); cudaFree(p->d_rank_g); cudaFree(p->d_gperm);
+    cudaFree(p->d_key_g); cudaFree(p->d_rank_g); cudaFree(p->d_grecs);
     cudaFree(p->d_cnt_all); cudaFree(p->d_start_all); cudaFree(p->d_dst_rs);
     if (p->have_side) { cudaStreamDestroy(p->side); cudaEventDestroy(p->ev_fork); cudaEventDestroy(p->ev_join); }
     cudaFree(p->d_bsum);
@@ -239,10 +232,9 @@ extern "C" se_status se_plan_destroy(se_plan *p)
     cudaFree(p->d_out_real); cudaFree(p->d_moments); cudaFree(p->d_io);
     if (p->have_comp) {
         cudaFree(p->d_real_p); cudaFree(p->d_Hk_s); cudaFree(p->d_Gk_p); cudaFree(p->d_pmom);
-        cufftDestroy(p->fft_fwd1); cufftDestroy(p->fft_inv1);
+        if (p->have_fft1) { cufftDestroy(p->fft_fwd1); cufftDestroy(p->fft_inv1); }
         if (p->have_fftz1) cufftDestroy(p->fftz_1);
     }
-    if (p->have_xf) { cufftDestroy(p->fft2_fwd); cufftDestroy(p->fft2_inv); }
     if (p->have_zt) { cufftDestroy(p->fftz_fwd); cufftDestroy(p->fftz_inv); }
     cudaFree(p->d_wtab);
     if (p->have_fwd) cufftDestroy(p->fft_fwd);
@@ -253,7 +245,8 @@ extern "C" se_status se_plan_destroy(se_plan *p)
     return SE_OK;
 }
 
-// TMA descriptor of nplanes grid planes [M][M] at `base`: 3-D tensor (z, y, plane), box = one haloed tile.
+// TMA descriptor of nplanes padded grid planes [MYp][MZp] at `base`: 3-D tensor (z, y, plane), box = one haloed tile
+// (parts of a box beyond the padded plane are zero-filled; they lie beyond every support).
 // The encoder lives in the driver; it is fetched through the runtime so that the library links against cudart only.
 static se_status make_tensor_map(se_plan *p, CUtensorMap *map, double *base, int nplanes)
 {
@@ -268,10 +261,9 @@ static se_status make_tensor_map(se_plan *p, CUtensorMap *map, double *base, int
         return fail(p, SE_ERR_CUDA, "cudaGetDriverEntryPoint", "cuTensorMapEncodeTiled");
     }
     const GatherGeom &g = p->gg;
-    const int M = p->c.M;
-    const cuuint64_t dims[3] = { (cuuint64_t)M, (cuuint64_t)M, (cuuint64_t)nplanes };
-    const cuuint64_t strides[2] = { (cuuint64_t)M * 8, (cuuint64_t)M * M * 8 };
-    const cuuint32_t box[3] = { (cuuint32_t)g.WZ, (cuuint32_t)g.WY, 1 };
+    const cuuint64_t dims[3] = { (cuuint64_t)g.MZp, (cuuint64_t)g.MYp, (cuuint64_t)nplanes };
+    const cuuint64_t strides[2] = { (cuuint64_t)g.MZp * 8, (cuuint64_t)g.MYp * g.MZp * 8 };
+    const cuuint32_t box[3] = { (cuuint32_t)p->gWZ, (cuuint32_t)p->gWY, 1 };
     const cuuint32_t estr[3] = { 1, 1, 1 };
     const CUresult cr = ((encode_fn)fn)(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, base, dims, strides, box, estr,
                                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
@@ -283,27 +275,43 @@ static se_status make_tensor_map(se_plan *p, CUtensorMap *map, double *base, int
     return SE_OK;
 }
 
-// Batched 3-D cuFFT plans of the unfused path: D2Z (3 grids) and Z2D (6 grids), out of place, contiguous batches.
-static se_status ensure_fft3d(se_plan *p)
+// Periodic halo of the padded returned grids after cuFFT's 3-D inverse transforms (which fill the M^3 interior only):
+// rows / columns M .. M+P-2 repeat 0 .. P-2.  The own z transform (se_zfft.cuh) writes its halo itself.
+__global__ void k_halo_fill(double *__restrict__ Rg, int M, int MYp, int MZp, int halo, size_t nplanes)
 {
-    if (p->have_fwd && p->have_inv) return SE_OK;
+    const size_t per = (size_t)MYp * MZp;
+    const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= nplanes * per) return;
+    const size_t pl = q / per;
+    const int r = (int)(q - pl * per), y = r / MZp, z = r - y * MZp;
+    if ((y < M && z < M) || y >= M + halo || z >= M + halo + 1) return;
+    Rg[q] = Rg[pl * per + (size_t)(y % M) * MZp + (z % M)];
+}
+
+// Batched 3-D cuFFT plans (other grid sizes than powers of two, or flag SE_CUFFT3D): D2Z (3 grids, contiguous) and
+// Z2D (6 grids) into the padded layout of the returned grids; `single`: the one-grid plans of the compressible extension.
+static se_status ensure_fft3d(se_plan *p, bool single)
+{
+    if (single ? p->have_fft1 : (p->have_fwd && p->have_inv)) return SE_OK;
     const int M = p->c.M;
-    int n3[3] = { M, M, M };
+    int n3[3] = { M, M, M }, ic[3] = { M, M, M / 2 + 1 }, orl[3] = { M, p->gg.MYp, p->gg.MZp };
+    const int idist = M * M * (M / 2 + 1);
+    const long long odist = (long long)p->Gp;
+    if (odist > 0x7fffffffLL) return fail(p, SE_ERR_UNSUPPORTED, "ensure_fft3d", "grid too large for cuFFT's int distances");
     size_t ws = 0, tot = 0;
-    cufftResult r = CUFFT_SUCCESS;
-    if (!p->have_fwd) {
-        r = cufftCreate(&p->fft_fwd);
-        if (r == CUFFT_SUCCESS) { p->have_fwd = true; r = cufftMakePlanMany(p->fft_fwd, 3, n3, NULL, 1, 0, NULL, 1, 0, CUFFT_D2Z, 3, &ws); tot += ws; }
-    }
-    if (r == CUFFT_SUCCESS && !p->have_inv) {
-        r = cufftCreate(&p->fft_inv);
-        if (r == CUFFT_SUCCESS) { p->have_inv = true; r = cufftMakePlanMany(p->fft_inv, 3, n3, NULL, 1, 0, NULL, 1, 0, CUFFT_Z2D, 6, &ws); tot += ws; }
-    }
+    cufftHandle *fw = single ? &p->fft_fwd1 : &p->fft_fwd, *iv = single ? &p->fft_inv1 : &p->fft_inv;
+    const int nf = single ? 1 : 3, ni = single ? 1 : 6;
+    cufftResult r = cufftCreate(fw);
+    bool c1 = (r == CUFFT_SUCCESS), c2 = false;
+    if (c1) { r = cufftMakePlanMany(*fw, 3, n3, NULL, 1, 0, NULL, 1, 0, CUFFT_D2Z, nf, &ws); tot += ws; }
+    if (r == CUFFT_SUCCESS) { r = cufftCreate(iv); c2 = (r == CUFFT_SUCCESS); }
+    if (r == CUFFT_SUCCESS) { r = cufftMakePlanMany(*iv, 3, n3, ic, 1, idist, orl, 1, (int)odist, CUFFT_Z2D, ni, &ws); tot += ws; }
     if (r != CUFFT_SUCCESS) {
-        if (p->have_fwd) { cufftDestroy(p->fft_fwd); p->have_fwd = false; }
-        if (p->have_inv) { cufftDestroy(p->fft_inv); p->have_inv = false; }
+        if (c1) cufftDestroy(*fw);
+        if (c2) cufftDestroy(*iv);
         return fail(p, r == CUFFT_ALLOC_FAILED ? SE_ERR_ALLOC : SE_ERR_CUFFT, "cufftMakePlanMany", "3-D plans");
     }
+    if (single) p->have_fft1 = true; else { p->have_fwd = true; p->have_inv = true; }
     p->fft_bytes += tot;
     p->bytes += tot;
     return SE_OK;
@@ -311,40 +319,7 @@ static se_status ensure_fft3d(se_plan *p)
 
 static se_status ensure_wtab(se_plan *p);
 
-// Plans and twiddle table of the fused path (se_xfft.cuh): batched 2-D (y,z) transforms, 3M forward and 6M inverse
-// planes; the x transforms run inside k_xfused.
-static se_status ensure_xf(se_plan *p)
-{
-    if (p->have_xf) return SE_OK;
-    const int M = p->c.M;
-    int n2[2] = { M, M };
-    size_t ws = 0, tot = 0;
-    cufftResult r = cufftCreate(&p->fft2_fwd);
-    bool c1 = (r == CUFFT_SUCCESS), c2 = false;
-    if (c1) { r = cufftMakePlanMany(p->fft2_fwd, 2, n2, NULL, 1, 0, NULL, 1, 0, CUFFT_D2Z, 3 * M, &ws); tot += ws; }
-    if (r == CUFFT_SUCCESS) { r = cufftCreate(&p->fft2_inv); c2 = (r == CUFFT_SUCCESS); }
-    if (r == CUFFT_SUCCESS) { r = cufftMakePlanMany(p->fft2_inv, 2, n2, NULL, 1, 0, NULL, 1, 0, CUFFT_Z2D, 6 * M, &ws); tot += ws; }
-    se_status st = SE_OK;
-    if (r != CUFFT_SUCCESS) st = fail(p, r == CUFFT_ALLOC_FAILED ? SE_ERR_ALLOC : SE_ERR_CUFFT, "cufftMakePlanMany", "2-D plans");
-    if (st == SE_OK) st = ensure_wtab(p);
-    if (st == SE_OK && (raise_smem_limit(k_xfused<3>) != cudaSuccess || raise_smem_limit(k_xfused<4>) != cudaSuccess)) {
-        cudaGetLastError();
-        st = fail(p, SE_ERR_CUDA, "ensure_xf", "shared-memory attribute");
-    }
-    if (st != SE_OK) {
-        if (c1) cufftDestroy(p->fft2_fwd);
-        if (c2) cufftDestroy(p->fft2_inv);
-        return st;
-    }
-    p->have_xf = true;
-    p->lM = 0;
-    while ((1 << p->lM) < M) ++p->lM;
-    p->fft_bytes += tot;
-    p->bytes += tot;
-    return SE_OK;
-}
-
-// Twiddle table exp(-2 pi i q / M), q < M (fused x path and own z transforms).
+// Twiddle table exp(-2 pi i q / M), q < M (own z transforms).
 static se_status ensure_wtab(se_plan *p)
 {
     if (p->d_wtab) return SE_OK;
@@ -434,19 +409,20 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
     c.NBY = (M + SE_TILE_Y - 1) / SE_TILE_Y;
     c.NBZ = (M + SE_TILE_Z - 1) / SE_TILE_Z;
     p->ncell_s = M * c.NBY * c.NBZ;
-    c.rec_stride = (SE_REC_HDR + 6 * P + 1) & ~1;
+    c.rec_stride = se_rec_stride(P);
+    c.grec_stride = se_grec_stride(P);
     if (!choose_gather_geometry(p)) { free(p); return SE_ERR_UNSUPPORTED; }
     p->ncell_g = p->gg.NTY * p->gg.NTZ * M;
     choose_segments(p, 0, 0);
 
     se_status st = SE_OK;
-    const size_t G = (size_t)M * M * M, Gc = (size_t)M * M * (M / 2 + 1);
+    const size_t Gc = (size_t)M * M * (M / 2 + 1);
     p->ncell_all = p->ncell_r + p->ncell_s + p->ncell_g + 3;
     const int nscan = p->ncell_all;
 #define ALLOC(ptr, count) if (st == SE_OK) st = dev_alloc(p, &(ptr), (size_t)(count))
     ALLOC(p->d_radii, N);
     ALLOC(p->d_key_r, N); ALLOC(p->d_rank_r, N); ALLOC(p->d_key_s, N); ALLOC(p->d_rank_s, N);
-    ALLOC(p->d_key_g, N); ALLOC(p->d_rank_g, N); ALLOC(p->d_gperm, N);
+    ALLOC(p->d_key_g, N); ALLOC(p->d_rank_g, N); ALLOC(p->d_grecs, (size_t)N * c.grec_stride);
     ALLOC(p->d_cnt_all, p->ncell_all); ALLOC(p->d_start_all, p->ncell_all); ALLOC(p->d_dst_rs, N);
     if (st == SE_OK) {
         p->d_cnt_r = p->d_cnt_all; p->d_cnt_s = p->d_cnt_r + p->ncell_r + 1; p->d_cnt_g = p->d_cnt_s + p->ncell_s + 1;
@@ -455,22 +431,24 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
     ALLOC(p->d_bsum, (nscan + SCAN_BLOCK - 1) / SCAN_BLOCK + 1);
     ALLOC(p->d_rs_pos, N); ALLOC(p->d_rs_mom, 12 * (size_t)N); ALLOC(p->d_rs_orig, N);
     ALLOC(p->d_recs, (size_t)N * c.rec_stride);
-    ALLOC(p->d_real, 6 * G); ALLOC(p->d_Hk, 3 * Gc); ALLOC(p->d_Gk, 6 * Gc);
+    ALLOC(p->d_real, 6 * p->Gp); ALLOC(p->d_Hk, 3 * Gc); ALLOC(p->d_Gk, 6 * Gc);
     ALLOC(p->d_out_real, 12 * (size_t)N); ALLOC(p->d_moments, GATHER_SUMS * (size_t)N);
     ALLOC(p->d_io, 25 * (size_t)N);
 #undef ALLOC
     if (st != SE_OK) { se_plan_destroy(p); return st; }
     if (cudaMemcpy(p->d_radii, radii, sizeof(double) * (size_t)N, cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMemset(p->d_out_real, 0, sizeof(double) * 12 * (size_t)N) != cudaSuccess ||
+        cudaMemset(p->d_real, 0, sizeof(double) * 6 * p->Gp) != cudaSuccess ||       // alignment padding is read (with zero weight): keep it finite
+
         cudaMemset(p->d_moments, 0, sizeof(double) * GATHER_SUMS * (size_t)N) != cudaSuccess) {
         se_plan_destroy(p);
         return SE_ERR_CUDA;
     }
 
     // cuFFT: power-of-two grids use the own-z-transform path (2-D complex plans, made here); the batched 3-D real plans
-    // and the plans of the fused path (SE_FUSED_X) are made by the first apply that needs them.
+    // are made by the first apply that needs them.
     {
-        se_status stf = xf_supported(M) ? ensure_zt(p) : ensure_fft3d(p);
+        se_status stf = xf_supported(M) ? ensure_zt(p) : ensure_fft3d(p, false);
         if (stf == SE_OK) stf = make_tensor_map(p, &p->tmap, p->d_real, 6 * M);
         if (stf != SE_OK) { se_plan_destroy(p); return stf; }
     }
@@ -513,7 +491,7 @@ extern "C" se_status se_plan_set_tuning(se_plan *p, int spread_segments, int gat
 
 extern "C" se_status se_plan_set_flags(se_plan *p, unsigned flags)
 {
-    if (!p || (flags & ~0x7fu)) return SE_ERR_INVALID_ARG;
+    if (!p || (flags & ~0x5fu)) return SE_ERR_INVALID_ARG;
     p->flags = flags;
     return SE_OK;
 }
@@ -563,10 +541,10 @@ static void launch_gather(se_plan *p, cudaStream_t s, bool pressure)
 {
     const GatherGeom &g = p->gg;
     const int ngrids = pressure ? 1 : 6;
-    const unsigned blocks = (unsigned)(g.NTY * g.NTZ * ngrids * g.nseg);
-    k_gather<P><<<blocks, (GR_WARPS + GR_PROD) * 32, p->gather_smem, s>>>(p->c, g, p->d_recs, p->d_gperm, p->d_start_g,
-                                                                   pressure ? p->d_real_p : p->d_real, pressure ? p->tmap_p : p->tmap, ngrids,
-                                                                   pressure ? p->d_pmom : p->d_moments, pressure ? 12 : GATHER_SUMS);
+    const int items = g.NTY * g.NTZ * ngrids * g.nseg;
+    const unsigned blocks = (unsigned)(items < p->sms ? items : p->sms);          // persistent: one CTA per SM
+    k_gather<P><<<blocks, (GR_WARPS + 1) * 32, p->gather_smem, s>>>(p->c, g, p->d_grecs, p->d_start_g, pressure ? p->tmap_p : p->tmap, ngrids,
+                                                             pressure ? p->d_pmom : p->d_moments, pressure ? 12 : GATHER_SUMS);
 }
 
 template <int P>
@@ -577,9 +555,6 @@ static cudaError_t prepare_sweeps()
     if (e == cudaSuccess) e = raise_smem_limit(k_gather<P>);
     return e;
 }
-
-#define FOR_EACH_P(X) \
-    X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15) X(16) X(17) X(18) X(19) X(20) X(21) X(22) X(23) X(24)
 
 static void dispatch_spread(se_plan *p, cudaStream_t s, bool comp_in)
 {
@@ -609,49 +584,46 @@ static void dispatch_gather(se_plan *p, cudaStream_t s, bool pressure)
     }
 }
 
-// Buffers and cuFFT plans of the compressible extension (a9), made by the first apply that needs them.
+// Buffers of the compressible extension (a9), made by the first apply that needs them; its cuFFT plans are made by
+// ensure_comp_plans for the transform path actually taken.
 static se_status ensure_compressible(se_plan *p)
 {
     if (p->have_comp) return SE_OK;
     const int M = p->c.M;
-    const size_t G = (size_t)M * M * M, Gc = (size_t)M * M * (M / 2 + 1);
-    se_status st = SE_OK;
-    st = dev_alloc(p, &p->d_real_p, G);
+    const size_t Gc = (size_t)M * M * (M / 2 + 1);
+    se_status st = dev_alloc(p, &p->d_real_p, p->Gp);
     if (st == SE_OK) st = dev_alloc(p, &p->d_Hk_s, Gc);
     if (st == SE_OK) st = dev_alloc(p, &p->d_Gk_p, Gc);
     if (st == SE_OK) st = dev_alloc(p, &p->d_pmom, 12 * (size_t)p->c.N);
-    cufftResult r = CUFFT_SUCCESS;
-    bool f1 = false, i1 = false;
-    if (st == SE_OK) {
-        r = cufftPlan3d(&p->fft_fwd1, M, M, M, CUFFT_D2Z);
-        f1 = (r == CUFFT_SUCCESS);
-        if (f1) { r = cufftPlan3d(&p->fft_inv1, M, M, M, CUFFT_Z2D); i1 = (r == CUFFT_SUCCESS); }
-        if (r != CUFFT_SUCCESS) st = fail(p, r == CUFFT_ALLOC_FAILED ? SE_ERR_ALLOC : SE_ERR_CUFFT, "cufftPlan3d", "compressible extension");
-    }
+    if (st == SE_OK && cudaMemset(p->d_real_p, 0, sizeof(double) * p->Gp) != cudaSuccess) st = fail(p, SE_ERR_CUDA, "cudaMemset", "pressure grid");
+    if (st == SE_OK) st = make_tensor_map(p, &p->tmap_p, p->d_real_p, M);
     if (st != SE_OK) {
         cudaFree(p->d_real_p); cudaFree(p->d_Hk_s); cudaFree(p->d_Gk_p); cudaFree(p->d_pmom);
         p->d_real_p = nullptr; p->d_Hk_s = nullptr; p->d_Gk_p = nullptr; p->d_pmom = nullptr;
-        if (f1) cufftDestroy(p->fft_fwd1);
-        if (i1) cufftDestroy(p->fft_inv1);
         cudaGetLastError();
         return st;
     }
-    if (xf_supported(M)) {
-        int n2[2] = { M, M };
-        size_t ws = 0;
-        if (cufftCreate(&p->fftz_1) == CUFFT_SUCCESS) {
-            if (cufftMakePlanMany(p->fftz_1, 2, n2, NULL, 1, 0, NULL, 1, 0, CUFFT_Z2Z, M / 2 + 1, &ws) == CUFFT_SUCCESS) p->have_fftz1 = true;
-            else cufftDestroy(p->fftz_1);
-        }
-    }
-    st = make_tensor_map(p, &p->tmap_p, p->d_real_p, M);
-    if (st != SE_OK) {
-        cudaFree(p->d_real_p); cudaFree(p->d_Hk_s); cudaFree(p->d_Gk_p); cudaFree(p->d_pmom);
-        p->d_real_p = nullptr; p->d_Hk_s = nullptr; p->d_Gk_p = nullptr; p->d_pmom = nullptr;
-        cufftDestroy(p->fft_fwd1); cufftDestroy(p->fft_inv1);
-        return st;
-    }
     p->have_comp = true;
+    return SE_OK;
+}
+
+// Single-grid cuFFT plans of the compressible extension: the 2-D complex plan of the own-z-transform path, or the 3-D pair.
+static se_status ensure_comp_plans(se_plan *p, bool zt)
+{
+    if (!zt) return ensure_fft3d(p, true);
+    if (p->have_fftz1) return SE_OK;
+    const int M = p->c.M;
+    int n2[2] = { M, M };
+    size_t ws = 0;
+    cufftResult r = cufftCreate(&p->fftz_1);
+    if (r == CUFFT_SUCCESS) {
+        r = cufftMakePlanMany(p->fftz_1, 2, n2, NULL, 1, 0, NULL, 1, 0, CUFFT_Z2Z, M / 2 + 1, &ws);
+        if (r != CUFFT_SUCCESS) cufftDestroy(p->fftz_1);
+    }
+    if (r != CUFFT_SUCCESS) return fail(p, r == CUFFT_ALLOC_FAILED ? SE_ERR_ALLOC : SE_ERR_CUFFT, "cufftMakePlanMany", "2-D plan of the compressible extension");
+    p->have_fftz1 = true;
+    p->fft_bytes += ws;
+    p->bytes += ws;
     return SE_OK;
 }
 
@@ -667,9 +639,9 @@ static se_status sort_and_pack(se_plan *p, const double *pos, const double *F, c
     p->last_launches += 1;
     const se_status st = scan_cells(p, s);
     if (st != SE_OK) return st;
-    k_scatter<<<(c.N + SCATTER_THREADS - 1) / SCATTER_THREADS, SCATTER_THREADS, scatter_smem_bytes(c.rec_stride), s>>>(
+    k_scatter<<<(c.N + SCATTER_THREADS - 1) / SCATTER_THREADS, SCATTER_THREADS, scatter_smem_bytes(c.P), s>>>(
         c, pos, p->d_radii, F, T, S, s_in, p->d_key_r, p->d_rank_r, p->d_start_r, p->d_key_s, p->d_rank_s, p->d_start_s,
-        p->d_key_g, p->d_rank_g, p->d_start_g, p->d_gperm, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig, p->d_recs, p->d_dst_rs);
+        p->d_key_g, p->d_rank_g, p->d_start_g, p->d_grecs, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig, p->d_recs, p->d_dst_rs);
     p->last_launches += 1;
     CUDA_TRY(p, cudaGetLastError());
     return SE_OK;
@@ -696,14 +668,12 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     if (!pos && !p->have_positions) return fail(p, SE_ERR_INVALID_ARG, who, "pos is NULL and no positions were set (se_plan_set_positions)");
     const bool comp_in = s_in != nullptr, comp_out = s_out != nullptr, comp = comp_in || comp_out;
     if (comp) { se_status stc = ensure_compressible(p); if (stc != SE_OK) return stc; }
-    // opt-in: 2-D cuFFT + fused x-transform / k-space / x-transform kernel (se_xfft.cuh)
-    const bool use_xf = (p->flags & SE_FUSED_X) && xf_supported(p->c.M) && !comp;
-    if (use_xf) { se_status stf = ensure_xf(p); if (stf != SE_OK) return stf; }
     // default for power-of-two grids: own z transforms with transposed spectra + contiguous 2-D complex cuFFT plans
     // (se_zfft.cuh); otherwise, and with SE_CUFFT3D, cuFFT's 3-D real transforms
-    const bool use_zt = !use_xf && !(p->flags & SE_CUFFT3D) && xf_supported(p->c.M) && (!comp || p->have_fftz1);
+    const bool use_zt = !(p->flags & SE_CUFFT3D) && xf_supported(p->c.M);
     if (use_zt) { se_status stf = ensure_zt(p); if (stf != SE_OK) return stf; }
-    if (!use_zt && !use_xf) { se_status stf = ensure_fft3d(p); if (stf != SE_OK) return stf; }
+    if (!use_zt) { se_status stf = ensure_fft3d(p, false); if (stf != SE_OK) return stf; }
+    if (comp) { se_status stf = ensure_comp_plans(p, use_zt); if (stf != SE_OK) return stf; }
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const SeConst &c = p->c;
     const unsigned fl = p->flags;
@@ -759,15 +729,13 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     // ---- a3..a7: Spectral Ewald wave-space sum ----
     bool wave_done = false;
     if (on(SE_STAGE_SPREAD)) {
+        if (comp_in) p->real_p_padded = false;
         dispatch_spread(p, s, comp_in);
         p->last_launches += 1;
         CUDA_TRY(p, cudaGetLastError());
     }
     MARK();
-    if (on(SE_STAGE_FFT_FWD) && use_xf) {
-        CUFFT_TRY(p, cufftSetStream(p->fft2_fwd, s));
-        CUFFT_TRY(p, cufftExecD2Z(p->fft2_fwd, p->d_real, (cufftDoubleComplex *)p->d_Hk));
-    } else if (on(SE_STAGE_FFT_FWD) && use_zt) {
+    if (on(SE_STAGE_FFT_FWD) && use_zt) {
         const int M = c.M;
         if (zt_threads(M) <= 128) k_zfft_r2c<128><<<3 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_real, p->d_Hk, p->d_wtab);
         else k_zfft_r2c<256><<<3 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_real, p->d_Hk, p->d_wtab);
@@ -792,13 +760,7 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
         }
     }
     MARK();
-    if (on(SE_STAGE_KSPACE) && use_xf) {
-        const unsigned nb = (unsigned)((size_t)c.M * (c.M / 2 + 1) / (XF_ELEMS / c.M));
-        if (xf_lv(c.M) == 4) k_xfused<4><<<nb, XF_THREADS(4), xf_smem_bytes(c.M), s>>>(c, p->lM, p->d_Hk, p->d_Gk, p->d_wtab);
-        else k_xfused<3><<<nb, XF_THREADS(3), xf_smem_bytes(c.M), s>>>(c, p->lM, p->d_Hk, p->d_Gk, p->d_wtab);
-        p->last_launches += 1;
-        CUDA_TRY(p, cudaGetLastError());
-    } else if (on(SE_STAGE_KSPACE)) {
+    if (on(SE_STAGE_KSPACE)) {
         const size_t Gc = (size_t)c.M * c.M * (c.M / 2 + 1);
         const unsigned nbk = (unsigned)((Gc + KSPACE_THREADS - 1) / KSPACE_THREADS);
         if (use_zt) k_kspace<true><<<nbk, KSPACE_THREADS, 0, s>>>(c, p->d_Hk, p->d_Gk, comp_in ? p->d_Hk_s : nullptr,
@@ -809,32 +771,38 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
         CUDA_TRY(p, cudaGetLastError());
     }
     MARK();
-    if (on(SE_STAGE_FFT_INV) && use_xf) {
-        CUFFT_TRY(p, cufftSetStream(p->fft2_inv, s));
-        CUFFT_TRY(p, cufftExecZ2D(p->fft2_inv, (cufftDoubleComplex *)p->d_Gk, p->d_real));
-    } else if (on(SE_STAGE_FFT_INV) && use_zt) {
-        const int M = c.M;
+    if (on(SE_STAGE_FFT_INV) && use_zt) {
+        const int M = c.M, MYp = p->gg.MYp, MZp = p->gg.MZp, halo = c.P - 1;
         CUFFT_TRY(p, cufftSetStream(p->fftz_inv, s));
         CUFFT_TRY(p, cufftExecZ2Z(p->fftz_inv, (cufftDoubleComplex *)p->d_Gk, (cufftDoubleComplex *)p->d_Gk, CUFFT_INVERSE));
-        if (zt_threads(M) <= 128) k_zfft_c2r<128><<<6 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk, p->d_real, p->d_wtab);
-        else k_zfft_c2r<256><<<6 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk, p->d_real, p->d_wtab);
+        if (zt_threads(M) <= 128) k_zfft_c2r<128><<<6 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk, p->d_real, p->d_wtab, MYp, MZp, halo);
+        else k_zfft_c2r<256><<<6 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk, p->d_real, p->d_wtab, MYp, MZp, halo);
         p->last_launches += 1;
         CUDA_TRY(p, cudaGetLastError());
         if (comp_out) {
             CUFFT_TRY(p, cufftSetStream(p->fftz_1, s));
             CUFFT_TRY(p, cufftExecZ2Z(p->fftz_1, (cufftDoubleComplex *)p->d_Gk_p, (cufftDoubleComplex *)p->d_Gk_p, CUFFT_INVERSE));
-            if (zt_threads(M) <= 128) k_zfft_c2r<128><<<M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk_p, p->d_real_p, p->d_wtab);
-            else k_zfft_c2r<256><<<M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk_p, p->d_real_p, p->d_wtab);
+            if (zt_threads(M) <= 128) k_zfft_c2r<128><<<M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk_p, p->d_real_p, p->d_wtab, MYp, MZp, halo);
+            else k_zfft_c2r<256><<<M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk_p, p->d_real_p, p->d_wtab, MYp, MZp, halo);
             p->last_launches += 1;
             CUDA_TRY(p, cudaGetLastError());
+            p->real_p_padded = true;
         }
     } else if (on(SE_STAGE_FFT_INV)) {
+        const int M = c.M, MYp = p->gg.MYp, MZp = p->gg.MZp, halo = c.P - 1;
+        const size_t per = (size_t)MYp * MZp;
         CUFFT_TRY(p, cufftSetStream(p->fft_inv, s));
         CUFFT_TRY(p, cufftExecZ2D(p->fft_inv, (cufftDoubleComplex *)p->d_Gk, p->d_real));
+        k_halo_fill<<<(unsigned)((6 * M * per + 255) / 256), 256, 0, s>>>(p->d_real, M, MYp, MZp, halo, (size_t)6 * M);
+        p->last_launches += 1;
         if (comp_out) {
             CUFFT_TRY(p, cufftSetStream(p->fft_inv1, s));
             CUFFT_TRY(p, cufftExecZ2D(p->fft_inv1, (cufftDoubleComplex *)p->d_Gk_p, p->d_real_p));
+            k_halo_fill<<<(unsigned)((M * per + 255) / 256), 256, 0, s>>>(p->d_real_p, M, MYp, MZp, halo, (size_t)M);
+            p->last_launches += 1;
+            p->real_p_padded = true;
         }
+        CUDA_TRY(p, cudaGetLastError());
     }
     MARK();
     if (on(SE_STAGE_GATHER)) {
@@ -898,13 +866,20 @@ extern "C" se_status far_mobility_apply_host(se_plan *p, const double *pos, cons
 extern "C" se_status se_plan_copy_grids(se_plan *p, int which, double *dst)
 {
     if (!p || !dst || which < 0 || which > 2) return SE_ERR_INVALID_ARG;
-    const size_t G = (size_t)p->c.M * p->c.M * p->c.M;
-    if (which == 2) {
-        if (!p->have_comp) return fail(p, SE_ERR_INVALID_ARG, "se_plan_copy_grids", "no compressible apply was made");
-        CUDA_TRY(p, cudaMemcpy(dst, p->d_real_p, sizeof(double) * G, cudaMemcpyDeviceToHost));
+    const int M = p->c.M;
+    const size_t G = (size_t)M * M * M, per = (size_t)p->gg.MYp * p->gg.MZp;
+    if (which == 2 && !p->have_comp) return fail(p, SE_ERR_INVALID_ARG, "se_plan_copy_grids", "no compressible apply was made");
+    CUDA_TRY(p, cudaDeviceSynchronize());
+    if (which == 0 || (which == 2 && !p->real_p_padded)) {              // spread grids: plain [M][M][M]
+        CUDA_TRY(p, cudaMemcpy(dst, which == 0 ? p->d_real : p->d_real_p, sizeof(double) * (which == 0 ? 3 : 1) * G, cudaMemcpyDeviceToHost));
         return SE_OK;
     }
-    CUDA_TRY(p, cudaMemcpy(dst, p->d_real, sizeof(double) * (which == 0 ? 3 : 6) * G, cudaMemcpyDeviceToHost));
+    // returned grids: strip the periodic halo of the padded layout, plane by plane
+    const double *src = which == 1 ? p->d_real : p->d_real_p;
+    const size_t nplanes = (size_t)(which == 1 ? 6 : 1) * M;
+    for (size_t pl = 0; pl < nplanes; ++pl)
+        CUDA_TRY(p, cudaMemcpy2D(dst + pl * M * M, sizeof(double) * M, src + pl * per, sizeof(double) * p->gg.MZp, sizeof(double) * M, M,
+                                 cudaMemcpyDeviceToHost));
     return SE_OK;
 }
 

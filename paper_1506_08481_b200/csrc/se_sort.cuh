@@ -4,14 +4,13 @@
 #pragma once
 #include "se_common.cuh"
 
-// Geometry of the ring gather (se_gather.cuh), chosen on the host (choose_gather_geometry).
+// Geometry of the ring gather (se_gather.cuh).  The tile shape, ring depth and slot layout are compile-time functions
+// of P (GatherTraits); this struct carries them, and the run-time tile / segment counts, to the kernels.
 struct GatherGeom {
     int TY, TZ;                    // support origins per tile along y, z
     int NTY, NTZ;                  // tiles per axis
-    int WY, WZ, WZL;               // haloed tile: rows, padded row length (= TMA box), loaded row length (doubles, even)
-    int slot_d;                    // doubles per ring slot: WY * WZ rounded up to a multiple of 16 (128 bytes)
-    int R;                         // planes in the ring (>= P)
     int nseg, seg_len;             // segments of the sweep along x
+    int MYp, MZp;                  // padded extents of the returned real grids: rows M + P - 1, row pitch >= M + P - 1
 };
 
 __device__ __forceinline__ double se_wrap(double x, double L) { return x - L * floor(x / L); }
@@ -115,23 +114,23 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_add(int *__restrict__ out
 }
 
 #define SCATTER_THREADS 64
-// Records are built in shared memory (one row per thread, odd row pitch) and copied out by whole warps,
-// rec_stride contiguous doubles at a time: per-thread stores of 480-byte records were the whole cost of a1.
-// One thread per particle: write the real-space packed copy (cell order) and the spreading/gather
-// record (tile order) with the per-axis Gaussian tables (Eq. 41 in physical coordinates; the paper's
+// One thread per particle: write the real-space packed copy (cell order), the spreading record (tile order) and the
+// gather record (gather order) with the per-axis Gaussian tables (Eq. 41 in physical coordinates; the paper's
 // fast Gaussian gridding, Eq. 47, is replaced by P direct exponentials per axis, done once here).
+// The record is built in shared memory (one row per thread, odd row pitch: header, gy, gz, one copy of the x tables)
+// and copied out by whole warps, contiguous doubles at a time: per-thread stores of whole records were the whole cost of a1.
 __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const double *__restrict__ radii,
                           const double *__restrict__ F, const double *__restrict__ T, const double *__restrict__ S,
                           const double *__restrict__ s_in,      // pressure moments (a9) or NULL
                           const int *__restrict__ key_r, const int *__restrict__ rank_r, const int *__restrict__ start_r,
                           const int *__restrict__ key_s, const int *__restrict__ rank_s, const int *__restrict__ start_s,
                           const int *__restrict__ key_g, const int *__restrict__ rank_g, const int *__restrict__ start_g,
-                          int *__restrict__ gperm, double4 *__restrict__ rs_pos, double *__restrict__ rs_mom, int *__restrict__ rs_orig,
+                          double *__restrict__ grecs, double4 *__restrict__ rs_pos, double *__restrict__ rs_mom, int *__restrict__ rs_orig,
                           double *__restrict__ recs, int2 *__restrict__ dst_rs)   // dst_rs[i] = (cell-order index, record index)
 {
-    extern __shared__ __align__(16) double sc_rows[];          // [SCATTER_THREADS][rec_stride + 1] then int dst[]
-    const int pitch = c.rec_stride + 1;
-    int *sc_dst = reinterpret_cast<int *>(sc_rows + SCATTER_THREADS * pitch);
+    extern __shared__ __align__(16) double sc_rows[];          // [SCATTER_THREADS][row + 1] then int dst[2][SCATTER_THREADS]
+    const int P = c.P, XOFF = se_rec_xoff(P), row = XOFF + 4 * P, pitch = row + 1;
+    int *sc_dst = reinterpret_cast<int *>(sc_rows + SCATTER_THREADS * pitch), *sc_dg = sc_dst + SCATTER_THREADS;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     sc_dst[threadIdx.x] = -1;
     if (i < c.N) {
@@ -156,36 +155,37 @@ __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const doubl
     m[6] = s[0]; m[7] = s[1]; m[8] = s[2]; m[9] = s[3]; m[10] = s[4]; m[11] = sp;
     rs_orig[dr] = i;
 
-    // spreading / gather record
+    // spreading / gather records
     const int ds = start_s[key_s[i]] + rank_s[i];
-    gperm[start_g[key_g[i]] + rank_g[i]] = ds;               // gather order -> record
     dst_rs[i] = make_int2(dr, ds);
     double *r = sc_rows + threadIdx.x * pitch;
     sc_dst[threadIdx.x] = ds;
+    sc_dg[threadIdx.x] = start_g[key_g[i]] + rank_g[i];
     int n0w[3];
     double d0[3];
     const double cF = a * a / 6.0, cS = a * a / 10.0, al = c.alpha;
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
         const double u = xw[d] * c.MoverL;
-        const int n0 = se_support_start(u, c.P);
+        const int n0 = se_support_start(u, P);
         n0w[d] = se_mod(n0, c.M);
         d0[d] = ((double)n0 - u) * c.Delta;
-        double *g = r + SE_REC_HDR + d * c.P;
-        for (int k = 0; k < c.P; ++k) {
+        for (int k = 0; k < P; ++k) {
             const double dk = ((double)(n0 + k) - u) * c.Delta;
             const double e = exp(-al * dk * dk);
-            g[k] = d == 0 ? c.gnorm * e : e;
-            if (d == 0) {                                   // x-moment tables gx dx^n, n = 1..3
-                double *xm = r + SE_REC_HDR + 3 * c.P;
-                const double g1 = g[k] * dk, g2 = g1 * dk;
-                xm[k] = g1; xm[c.P + k] = g2; xm[2 * c.P + k] = g2 * dk;
+            if (d == 0) {                                   // x tables (gx, gx dx, gx dx^2, gx dx^3)(k)
+                double *xm = r + XOFF + 4 * k;
+                const double g0 = c.gnorm * e, g1 = g0 * dk, g2 = g1 * dk;
+                xm[0] = g0; xm[1] = g1; xm[2] = g2; xm[3] = g2 * dk;
+            } else {
+                r[SE_REC_HDR + (d - 1) * P + k] = e;
             }
         }
     }
+    for (int q = SE_REC_HDR + 2 * P; q < XOFF; ++q) r[q] = 0.0;
     r[0] = __longlong_as_double(((long long)(unsigned)n0w[2] << 32) | (unsigned)n0w[1]);     // int2 (y0w, z0w)
     r[1] = __longlong_as_double(((long long)(unsigned)i << 32) | (unsigned)n0w[0]);          // int2 (x0w, orig)
-    r[REC_D0] = d0[0]; r[REC_D0 + 1] = d0[1]; r[REC_D0 + 2] = d0[2];
+    r[REC_D0Y] = d0[1]; r[REC_D0Z] = d0[2]; r[REC_D0X] = d0[0];
     r[REC_POLY] = 1.0 - 6.0 * al * cF;
     r[REC_POLY + 1] = 4.0 * al * al * cF;
     r[REC_POLY + 2] = 2.0 * al * (1.0 - 10.0 * al * cS);
@@ -198,17 +198,27 @@ __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const doubl
     }
     __syncthreads();
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int PP = se_grec_pp(P), gstride = c.grec_stride;
     for (int rr = w; rr < SCATTER_THREADS; rr += SCATTER_THREADS / 32) {
         const int ds = sc_dst[rr];
         if (ds < 0) continue;
         const double *__restrict__ src = sc_rows + rr * pitch;
         double *__restrict__ dst = recs + (size_t)ds * c.rec_stride;
-        for (int q = lane; q < c.rec_stride; q += 32) dst[q] = src[q];
+        for (int q = lane; q < c.rec_stride; q += 32) dst[q] = src[q < row ? q : q - 4 * P];      // x tables stored twice
+        double *__restrict__ dg = grecs + (size_t)sc_dg[rr] * gstride;
+        for (int q = lane; q < gstride; q += 32) {
+            double v;
+            if (q < 2) v = src[q];
+            else if (q < 4) v = src[REC_D0Y + q - 2];
+            else if (q < 4 + 2 * PP) { const int ax = (q - 4) / PP, k = (q - 4) - ax * PP; v = k < P ? src[SE_REC_HDR + ax * P + k] : 0.0; }
+            else { const int e = q - 4 - 2 * PP; v = src[XOFF + 4 * (e >> 1) + (e & 1)]; }
+            dg[q] = v;
+        }
     }
 }
 
-// Positions unchanged since se_plan_set_positions: only the moments of the records and of the real-space copy
-// are refreshed (the sorts, indices and Gaussian tables are reused).
+// Positions unchanged since se_plan_set_positions: only the moments of the spreading records and of the real-space
+// copy are refreshed (the sorts, indices and Gaussian tables, and the gather records, are reused).
 __global__ void k_moments(SeConst c, const double *__restrict__ F, const double *__restrict__ T, const double *__restrict__ S,
                           const double *__restrict__ s_in, const int2 *__restrict__ dst_rs, double *__restrict__ rs_mom,
                           double *__restrict__ recs)
@@ -229,7 +239,7 @@ __global__ void k_moments(SeConst c, const double *__restrict__ F, const double 
     r[REC_SP] = sp;
 }
 
-static inline size_t scatter_smem_bytes(int rec_stride)
+static inline size_t scatter_smem_bytes(int P)
 {
-    return (size_t)SCATTER_THREADS * (rec_stride + 1) * 8 + SCATTER_THREADS * 4;
+    return (size_t)SCATTER_THREADS * (se_rec_xoff(P) + 4 * P + 1) * 8 + 2 * SCATTER_THREADS * 4;
 }

@@ -33,9 +33,11 @@ static inline int zt_threads(int M) { return ZT_LINES * (M / 2) / 16; }
 // global memory (GIN: the first stage of the forward transform reads the real row as Nh complex values) or its
 // output written straight to global memory (GOUT: the last stage of the inverse transform writes the real row):
 // two shared-memory passes fewer per transform.
+// GOUT rows may carry a periodic halo (the padded layout of the returned grids, se_gather.cuh): the first hz values are
+// stored again M further on, and the whole row a second time at gout2 (the halo row y + M) when gout2 is not NULL.
 template <int R, bool INV, bool GIN, bool GOUT>
 __device__ __forceinline__ void zt_stage(cplx *__restrict__ line, const double2 *__restrict__ gin, double2 *__restrict__ gout,
-                                         const cplx *__restrict__ W, int M, int lNs, int jj)
+                                         const cplx *__restrict__ W, int M, int lNs, int jj, int hz = 0, double2 *__restrict__ gout2 = nullptr)
 {
     constexpr int V = 16, NB = V / R;
     const int M16 = M >> 4, Ns = 1 << lNs;
@@ -62,8 +64,13 @@ __device__ __forceinline__ void zt_stage(cplx *__restrict__ line, const double2 
         const int base = ((j >> lNs) << lNs) * R + k;
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            if (GOUT) __stcs(gout + base + r * Ns, make_double2(v[u + r * NB].x, v[u + r * NB].y));
-            else line[xf_sk<4>(base + r * Ns)] = v[u + r * NB];
+            if (GOUT) {
+                const int e = base + r * Ns;
+                const double2 val = make_double2(v[u + r * NB].x, v[u + r * NB].y);
+                __stcs(gout + e, val);
+                if (e < hz) __stcs(gout + e + M, val);                 // M complex pairs = one period of the real row
+                if (gout2) { __stcs(gout2 + e, val); if (e < hz) __stcs(gout2 + e + M, val); }
+            } else line[xf_sk<4>(base + r * Ns)] = v[u + r * NB];
         }
     }
     if (!GOUT) __syncwarp();
@@ -72,21 +79,21 @@ __device__ __forceinline__ void zt_stage(cplx *__restrict__ line, const double2 
 // Length-Nh transform of one line (Nh = 2^lNh >= 16): radix-16 stages, then one stage of the remaining radix.
 template <bool INV, bool GIN, bool GOUT>
 __device__ __forceinline__ void zt_fft(cplx *__restrict__ line, const double2 *__restrict__ gin, double2 *__restrict__ gout,
-                                       const cplx *__restrict__ W, int Nh, int lNh, int jj)
+                                       const cplx *__restrict__ W, int Nh, int lNh, int jj, int hz = 0, double2 *__restrict__ gout2 = nullptr)
 {
     int lNs = 0;
     while (lNh - lNs >= 4) {
         const bool first = lNs == 0, last = lNs + 4 == lNh;
-        if (GIN && first && GOUT && last) zt_stage<16, INV, true, true>(line, gin, gout, W, Nh, lNs, jj);
+        if (GIN && first && GOUT && last) zt_stage<16, INV, true, true>(line, gin, gout, W, Nh, lNs, jj, hz, gout2);
         else if (GIN && first) zt_stage<16, INV, true, false>(line, gin, gout, W, Nh, lNs, jj);
-        else if (GOUT && last) zt_stage<16, INV, false, true>(line, gin, gout, W, Nh, lNs, jj);
+        else if (GOUT && last) zt_stage<16, INV, false, true>(line, gin, gout, W, Nh, lNs, jj, hz, gout2);
         else zt_stage<16, INV, false, false>(line, gin, gout, W, Nh, lNs, jj);
         lNs += 4;
     }
     const int rem = lNh - lNs;                     // 0 .. 3: the last stage, never the first (Nh >= 16)
-    if (rem == 3) { if (GOUT) zt_stage<8, INV, false, true>(line, gin, gout, W, Nh, lNs, jj); else zt_stage<8, INV, false, false>(line, gin, gout, W, Nh, lNs, jj); }
-    else if (rem == 2) { if (GOUT) zt_stage<4, INV, false, true>(line, gin, gout, W, Nh, lNs, jj); else zt_stage<4, INV, false, false>(line, gin, gout, W, Nh, lNs, jj); }
-    else if (rem == 1) { if (GOUT) zt_stage<2, INV, false, true>(line, gin, gout, W, Nh, lNs, jj); else zt_stage<2, INV, false, false>(line, gin, gout, W, Nh, lNs, jj); }
+    if (rem == 3) { if (GOUT) zt_stage<8, INV, false, true>(line, gin, gout, W, Nh, lNs, jj, hz, gout2); else zt_stage<8, INV, false, false>(line, gin, gout, W, Nh, lNs, jj); }
+    else if (rem == 2) { if (GOUT) zt_stage<4, INV, false, true>(line, gin, gout, W, Nh, lNs, jj, hz, gout2); else zt_stage<4, INV, false, false>(line, gin, gout, W, Nh, lNs, jj); }
+    else if (rem == 1) { if (GOUT) zt_stage<2, INV, false, true>(line, gin, gout, W, Nh, lNs, jj, hz, gout2); else zt_stage<2, INV, false, false>(line, gin, gout, W, Nh, lNs, jj); }
 }
 
 // H: [ng][M][M][M] real -> spec: [ng][M/2+1][M][M] complex.  Wtab: [M] complex, exp(-2 pi i q / M).
@@ -125,10 +132,12 @@ __global__ void __launch_bounds__(NT, NT <= 128 ? ZT_MINB : 2) k_zfft_r2c(int M,
     }
 }
 
-// spec: [ng][M/2+1][M][M] complex -> R: [ng][M][M][M] real (unnormalised inverse).
+// spec: [ng][M/2+1][M][M] complex -> R: [ng][M][MYp][MZp] real (unnormalised inverse), rows and columns M .. M+halo-1
+// repeating 0 .. halo-1 (the periodic halo the gather's tensor boxes read; halo = P - 1, MYp >= M + halo,
+// MZp >= M + halo + 1 and even).
 template <int NT>
 __global__ void __launch_bounds__(NT, NT <= 128 ? ZT_MINB : 2) k_zfft_c2r(int M, int lNh, const double2 *__restrict__ spec, double *__restrict__ R,
-                                                           const double2 *__restrict__ Wtab)
+                                                           const double2 *__restrict__ Wtab, int MYp, int MZp, int halo)
 {
     extern __shared__ __align__(16) unsigned char zt_smem[];
     const int Nh = M >> 1, Zc = Nh + 1, LP = zt_pitch(Nh), nt = blockDim.x, tid = threadIdx.x;
@@ -172,8 +181,9 @@ __global__ void __launch_bounds__(NT, NT <= 128 ? ZT_MINB : 2) k_zfft_c2r(int M,
     }
     __syncthreads();
     {   // the last stage writes the real rows straight to global memory
-        double2 *__restrict__ rows = reinterpret_cast<double2 *>(R + ((size_t)gx * M + y0) * M);
         const int tpl = Nh >> 4, line = tid / tpl, jj = tid - line * tpl;
-        zt_fft<true, false, true>(L + line * LP, nullptr, rows + (size_t)line * Nh, WN, Nh, lNh, jj);
+        double2 *__restrict__ row = reinterpret_cast<double2 *>(R + ((size_t)gx * MYp + y0 + line) * MZp);
+        double2 *__restrict__ row2 = y0 + line < halo ? row + (size_t)M * (MZp >> 1) : nullptr;      // halo row y + M
+        zt_fft<true, false, true>(L + line * LP, nullptr, row, WN, Nh, lNh, jj, (halo + 1) >> 1, row2);
     }
 }

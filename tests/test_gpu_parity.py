@@ -386,14 +386,14 @@ def test_compressible_extension_full_size_c4(pk, oracle, workloads):
 
 
 @pytest.mark.parametrize("name", ["c1", "c2", "c3"])
-def test_fused_x_transform_kspace_path_agrees(pk, oracle, workloads, name):
-    """SE_FUSED_X: 2-D cuFFT + one kernel for the x transform, the k-space pass and the inverse x transform,
-    instead of the default (own z transforms with transposed spectra + contiguous 2-D complex cuFFT + k_kspace).
-    SE_CUFFT3D: cuFFT's batched 3-D real transforms.  All must give the oracle's returned grids and the same product."""
+def test_both_transform_paths_agree(pk, oracle, workloads, name):
+    """Default for power-of-two grids: own z transforms with transposed spectra + contiguous 2-D complex cuFFT + k_kspace,
+    the inverse z transform writing the periodic halo of the returned grids itself.  SE_CUFFT3D: cuFFT's batched 3-D
+    real transforms into the same padded layout + halo-fill kernel.  Both must give the oracle's returned grids."""
     wl = workloads.make_workload(name)
     r = Runner(pk, wl)
     ref = r.oracle(oracle, want_grids=True)
-    for flags in (0, pk.SE_FUSED_X, pk.SE_CUFFT3D):
+    for flags in (0, pk.SE_CUFFT3D):
         r.run(flags=flags, stop=5)
         Gr = r.plan.copy_grids(1)
         for g in range(6):
