@@ -88,6 +88,16 @@ se_status se_plan_set_shape(se_plan *plan, double m);
  * (0 = the plan's own choice).  Results do not depend on it beyond summation order. */
 se_status se_plan_set_tuning(se_plan *plan, int spread_segments, int gather_segments);
 
+/* Further performance knobs, one integer each (results do not depend on them beyond summation order):
+ *   SE_OPT_REAL_OVERLAP  where the real-space sum (a2), which is independent of the wave-space pipeline, runs:
+ *                        0 = on the caller's stream before the spreading; 1 = on a plan-owned low-priority stream
+ *                        beside the whole wave pipeline; 2 = on that stream, started after the spreading (beside the
+ *                        HBM-bound transforms).  Joined before the epilogue in every case.
+ *   SE_OPT_REAL_CTAS     CTAs of the real-space kernel when it runs beside the wave pipeline (0 = one per cell).
+ * Errors: SE_ERR_INVALID_ARG for an unknown key or a value out of range. */
+enum { SE_OPT_REAL_OVERLAP = 0, SE_OPT_REAL_CTAS = 1, SE_NUM_OPTS = 2 };
+se_status se_plan_set_option(se_plan *plan, int key, int value);
+
 /* Bitwise OR of the SE_* flags above. */
 se_status se_plan_set_flags(se_plan *plan, unsigned flags);
 

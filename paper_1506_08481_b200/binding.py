@@ -10,6 +10,7 @@ import numpy as np
 from . import build as _build
 
 SE_SKIP_REAL, SE_SKIP_WAVE, SE_SKIP_SELF, SE_SKIP_ONEBODY, SE_TIMING, SE_CUFFT3D = 0x1, 0x2, 0x4, 0x8, 0x10, 0x40
+SE_OPT_REAL_OVERLAP, SE_OPT_REAL_CTAS = 0, 1
 SE_NUM_STAGES = 8
 STAGE_NAMES = ("sort", "real", "spread", "fft_fwd", "kspace", "fft_inv", "gather", "epilogue")
 _STATUS = {0: "SE_OK", 1: "SE_ERR_INVALID_ARG", 2: "SE_ERR_UNSUPPORTED", 3: "SE_ERR_ALLOC", 4: "SE_ERR_CUDA",
@@ -51,6 +52,8 @@ def load_library(build_if_missing: bool = True):
     L.se_plan_set_shape.argtypes = [P, D]
     L.se_plan_set_tuning.restype = INT
     L.se_plan_set_tuning.argtypes = [P, INT, INT]
+    L.se_plan_set_option.restype = INT
+    L.se_plan_set_option.argtypes = [P, INT, INT]
     L.se_plan_set_positions.restype = INT
     L.se_plan_set_positions.argtypes = [P, P, P]
     L.se_plan_set_flags.restype = INT
@@ -139,6 +142,9 @@ class SePlan:
 
     def set_tuning(self, spread_segments=0, gather_segments=0):
         self._check(self._lib.se_plan_set_tuning(self._h, int(spread_segments), int(gather_segments)), "se_plan_set_tuning")
+
+    def set_option(self, key, value):
+        self._check(self._lib.se_plan_set_option(self._h, int(key), int(value)), "se_plan_set_option")
 
     def set_flags(self, flags):
         self._check(self._lib.se_plan_set_flags(self._h, int(flags)), "se_plan_set_flags")

@@ -25,29 +25,24 @@ struct SeConst {
     double D3;                     // Delta^3 (gather quadrature weight)
 };
 
-// Spreading record (AoS, rec_stride doubles, 32-byte aligned), in spreading-tile order:
+// Spreading record (AoS, rec_stride doubles, 16-byte aligned), in spreading-tile order:
 //   [0]  int2 (y0w, z0w)   wrapped first support index along y, z
 //   [1]  int2 (x0w, orig)  wrapped first support plane along x (the sweep axis), caller index
-//   [2..3]   d0y, d0z      offset of the first support point from the particle, (n0 - u) Delta
-//   [4..7]   f0, f1, s0, s1  size polynomials: 1-6 al cF, 4 al^2 cF, 2 al (1-10 al cS), 8 al^3 cS
-//   [8..10] F  [11..13] T  [14..19] S (xx,xy,xz,yy,yz,zz)
-//   [20] d0x  [21] cF = a^2/6  [22] cS = a^2/10  [23] pressure moment s (a9; 0 without)
-//   [24..24+P) gy   [24+P..24+2P) gz                      per-axis Gaussians
-//   [XOFF .. XOFF + 8P)  X[j] = (gx, gx dx, gx dx^2, gx dx^3)(j mod P), j < 2P, gx with the factor (al/pi)^{3/2},
-//                        dx_k = d0x + k Delta: the x tables interleaved per support plane and stored TWICE, so
-//                        that the spreading kernel can address them through a rotating register window.
-#define REC_D0Y 2
-#define REC_D0Z 3
-#define REC_POLY 4
-#define REC_F 8
-#define REC_T 11
-#define REC_S 14
-#define REC_D0X 20
+//   [2..4]   d0x, d0y, d0z   offset of the first support point from the particle, (n0 - u) Delta
+//   [5..8]   f0, f1, s0, s1  size polynomials: 1-6 al cF, 4 al^2 cF, 2 al (1-10 al cS), 8 al^3 cS
+//   [9..11] F  [12..14] T  [15..20] S (xx,xy,xz,yy,yz,zz)
+//   [21] cF = a^2/6  [22] cS = a^2/10  [23] pressure moment s (a9; 0 without)
+//   [24..24+P) gx * (al/pi)^{3/2}   [24+P..24+2P) gy   [24+2P..24+3P) gz     per-axis Gaussians
+//   [24+3P..24+6P)  gx dx, gx dx^2, gx dx^3 with dx_k = d0x + k Delta     x-moment tables (P each)
+#define REC_D0 2
+#define REC_POLY 5
+#define REC_F 9
+#define REC_T 12
+#define REC_S 15
 #define REC_CF 21
 #define REC_CS 22
 #define REC_SP 23
-__host__ __device__ inline int se_rec_xoff(int P) { return (SE_REC_HDR + 2 * P + 3) & ~3; }
-__host__ __device__ inline int se_rec_stride(int P) { return se_rec_xoff(P) + 8 * P; }
+__host__ __device__ inline int se_rec_stride(int P) { return (SE_REC_HDR + 6 * P + 1) & ~1; }
 
 // Gather record (grec_stride doubles, 16-byte aligned), in gather order (tile major, starting plane minor):
 //   [0] int2 (y0w, z0w)  [1] int2 (x0w, orig)  [2] d0y  [3] d0z

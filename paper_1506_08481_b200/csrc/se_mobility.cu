@@ -45,6 +45,7 @@ struct se_plan {
     cudaEvent_t ev_fork, ev_join;
     bool have_side;
     int real_side_ctas;            // grid of k_real when it runs beside the wave pipeline (0 = one CTA per cell)
+    int real_overlap;              // SE_OPT_REAL_OVERLAP
     int sms;                       // multiprocessors of the plan's device (grid sizing)
     GatherGeom gg;                 // ring gather geometry (spreading's segments are in c.nseg, c.seg_len)
     CUtensorMap tmap, tmap_p;      // TMA descriptors of the six returned grids / of the pressure grid (se_gather.cuh)
@@ -467,6 +468,7 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
     {   // beside the wave pipeline a2 runs as a persistent grid of one CTA per SM (measured best on B200: it then
         // takes little from the HBM-bound kernels' occupancy; c4 step 3.57 -> 3.50 ms)
         p->real_side_ctas = p->sms;
+        p->real_overlap = 1;
     }
     if (raise_smem_limit(k_scatter) != cudaSuccess || dispatch_prepare(P) != cudaSuccess) { cudaGetLastError(); se_plan_destroy(p); return SE_ERR_CUDA; }
     *out = p;
@@ -486,6 +488,17 @@ extern "C" se_status se_plan_set_tuning(se_plan *p, int spread_segments, int gat
 {
     if (!p || spread_segments < 0 || gather_segments < 0) return SE_ERR_INVALID_ARG;
     choose_segments(p, spread_segments, gather_segments);
+    return SE_OK;
+}
+
+extern "C" se_status se_plan_set_option(se_plan *p, int key, int value)
+{
+    if (!p || value < 0) return SE_ERR_INVALID_ARG;
+    switch (key) {
+    case SE_OPT_REAL_OVERLAP: if (value > 2) return SE_ERR_INVALID_ARG; p->real_overlap = value; break;
+    case SE_OPT_REAL_CTAS: p->real_side_ctas = value; break;
+    default: return SE_ERR_INVALID_ARG;
+    }
     return SE_OK;
 }
 
@@ -704,7 +717,7 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     // joined before the epilogue, and fills what the wave-space kernels leave idle (tails, the HBM-bound stages).
     // Measured gain on B200 is small (c4: 4 %).  When stage timings are asked for it runs on the caller's
     // stream, alone, so that every stage is timed by itself.
-    const bool fork = do_real && do_wave && !timing && stop < 0;
+    const bool fork = do_real && do_wave && !timing && stop < 0 && p->real_overlap > 0;
     auto launch_real = [&](cudaStream_t sr) {
         unsigned nb = (unsigned)(c.ncr > 1 ? p->ncell_r : (c.N + 31) / 32);
         if (sr != s && c.ncr > 1 && p->real_side_ctas > 0 && nb > (unsigned)p->real_side_ctas) nb = (unsigned)p->real_side_ctas;
@@ -724,7 +737,7 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
         CUDA_TRY(p, cudaEventRecord(p->ev_join, p->side));
         return SE_OK;
     };
-    if (fork) { se_status sf = fork_real(); if (sf != SE_OK) return sf; }
+    if (fork && p->real_overlap == 1) { se_status sf = fork_real(); if (sf != SE_OK) return sf; }
     MARK();
     // ---- a3..a7: Spectral Ewald wave-space sum ----
     bool wave_done = false;
@@ -734,6 +747,7 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
         p->last_launches += 1;
         CUDA_TRY(p, cudaGetLastError());
     }
+    if (fork && p->real_overlap == 2) { se_status sf = fork_real(); if (sf != SE_OK) return sf; }
     MARK();
     if (on(SE_STAGE_FFT_FWD) && use_zt) {
         const int M = c.M;

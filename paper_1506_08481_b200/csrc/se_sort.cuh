@@ -117,8 +117,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_add(int *__restrict__ out
 // One thread per particle: write the real-space packed copy (cell order), the spreading record (tile order) and the
 // gather record (gather order) with the per-axis Gaussian tables (Eq. 41 in physical coordinates; the paper's
 // fast Gaussian gridding, Eq. 47, is replaced by P direct exponentials per axis, done once here).
-// The record is built in shared memory (one row per thread, odd row pitch: header, gy, gz, one copy of the x tables)
-// and copied out by whole warps, contiguous doubles at a time: per-thread stores of whole records were the whole cost of a1.
+// The record is built in shared memory (one row per thread, odd row pitch) and copied out by whole warps, contiguous doubles at a time: per-thread stores of whole records were the whole cost of a1.
 __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const double *__restrict__ radii,
                           const double *__restrict__ F, const double *__restrict__ T, const double *__restrict__ S,
                           const double *__restrict__ s_in,      // pressure moments (a9) or NULL
@@ -128,8 +127,8 @@ __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const doubl
                           double *__restrict__ grecs, double4 *__restrict__ rs_pos, double *__restrict__ rs_mom, int *__restrict__ rs_orig,
                           double *__restrict__ recs, int2 *__restrict__ dst_rs)   // dst_rs[i] = (cell-order index, record index)
 {
-    extern __shared__ __align__(16) double sc_rows[];          // [SCATTER_THREADS][row + 1] then int dst[2][SCATTER_THREADS]
-    const int P = c.P, XOFF = se_rec_xoff(P), row = XOFF + 4 * P, pitch = row + 1;
+    extern __shared__ __align__(16) double sc_rows[];          // [SCATTER_THREADS][rec_stride + 1] then int dst[2][SCATTER_THREADS]
+    const int P = c.P, pitch = c.rec_stride + 1;
     int *sc_dst = reinterpret_cast<int *>(sc_rows + SCATTER_THREADS * pitch), *sc_dg = sc_dst + SCATTER_THREADS;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     sc_dst[threadIdx.x] = -1;
@@ -170,22 +169,22 @@ __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const doubl
         const int n0 = se_support_start(u, P);
         n0w[d] = se_mod(n0, c.M);
         d0[d] = ((double)n0 - u) * c.Delta;
+        double *g = r + SE_REC_HDR + d * P;
         for (int k = 0; k < P; ++k) {
             const double dk = ((double)(n0 + k) - u) * c.Delta;
             const double e = exp(-al * dk * dk);
-            if (d == 0) {                                   // x tables (gx, gx dx, gx dx^2, gx dx^3)(k)
-                double *xm = r + XOFF + 4 * k;
-                const double g0 = c.gnorm * e, g1 = g0 * dk, g2 = g1 * dk;
-                xm[0] = g0; xm[1] = g1; xm[2] = g2; xm[3] = g2 * dk;
-            } else {
-                r[SE_REC_HDR + (d - 1) * P + k] = e;
+            g[k] = d == 0 ? c.gnorm * e : e;
+            if (d == 0) {                                   // x-moment tables gx dx^n, n = 1..3
+                double *xm = r + SE_REC_HDR + 3 * P;
+                const double g1 = g[k] * dk, g2 = g1 * dk;
+                xm[k] = g1; xm[P + k] = g2; xm[2 * P + k] = g2 * dk;
             }
         }
     }
-    for (int q = SE_REC_HDR + 2 * P; q < XOFF; ++q) r[q] = 0.0;
+    if (c.rec_stride > SE_REC_HDR + 6 * P) r[SE_REC_HDR + 6 * P] = 0.0;
     r[0] = __longlong_as_double(((long long)(unsigned)n0w[2] << 32) | (unsigned)n0w[1]);     // int2 (y0w, z0w)
     r[1] = __longlong_as_double(((long long)(unsigned)i << 32) | (unsigned)n0w[0]);          // int2 (x0w, orig)
-    r[REC_D0Y] = d0[1]; r[REC_D0Z] = d0[2]; r[REC_D0X] = d0[0];
+    r[REC_D0] = d0[0]; r[REC_D0 + 1] = d0[1]; r[REC_D0 + 2] = d0[2];
     r[REC_POLY] = 1.0 - 6.0 * al * cF;
     r[REC_POLY + 1] = 4.0 * al * al * cF;
     r[REC_POLY + 2] = 2.0 * al * (1.0 - 10.0 * al * cS);
@@ -204,14 +203,14 @@ __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const doubl
         if (ds < 0) continue;
         const double *__restrict__ src = sc_rows + rr * pitch;
         double *__restrict__ dst = recs + (size_t)ds * c.rec_stride;
-        for (int q = lane; q < c.rec_stride; q += 32) dst[q] = src[q < row ? q : q - 4 * P];      // x tables stored twice
+        for (int q = lane; q < c.rec_stride; q += 32) dst[q] = src[q];
         double *__restrict__ dg = grecs + (size_t)sc_dg[rr] * gstride;
         for (int q = lane; q < gstride; q += 32) {
             double v;
             if (q < 2) v = src[q];
-            else if (q < 4) v = src[REC_D0Y + q - 2];
-            else if (q < 4 + 2 * PP) { const int ax = (q - 4) / PP, k = (q - 4) - ax * PP; v = k < P ? src[SE_REC_HDR + ax * P + k] : 0.0; }
-            else { const int e = q - 4 - 2 * PP; v = src[XOFF + 4 * (e >> 1) + (e & 1)]; }
+            else if (q < 4) v = src[REC_D0 + q - 1];
+            else if (q < 4 + 2 * PP) { const int ax = (q - 4) / PP, k = (q - 4) - ax * PP; v = k < P ? src[SE_REC_HDR + (ax + 1) * P + k] : 0.0; }
+            else { const int e = q - 4 - 2 * PP; v = src[SE_REC_HDR + ((e & 1) ? 3 * P : 0) + (e >> 1)]; }
             dg[q] = v;
         }
     }
@@ -241,5 +240,5 @@ __global__ void k_moments(SeConst c, const double *__restrict__ F, const double 
 
 static inline size_t scatter_smem_bytes(int P)
 {
-    return (size_t)SCATTER_THREADS * (se_rec_xoff(P) + 4 * P + 1) * 8 + 2 * SCATTER_THREADS * 4;
+    return (size_t)SCATTER_THREADS * (se_rec_stride(P) + 1) * 8 + 2 * SCATTER_THREADS * 4;
 }

@@ -5,10 +5,9 @@
 //
 // Design ("register sweep", se_sweep.cuh; no atomics, every grid point written exactly once, zeros included):
 // a thread owns one grid column (y,z) and sweeps along x.  It keeps a window of P partial sums per component
-// in registers: window slot s is the plane q = s (mod P).  At plane p it adds, for every particle whose support
-// STARTS at plane p and covers the column, that particle's contribution to all P slots (statically indexed; the
-// rotation is taken by the address of the doubled x tables), then stores and clears slot p mod P (plane p is
-// now final) and moves on -- the window is never shifted.  For a fixed column the summand is
+// in registers: window slot k is plane p+k.  At plane p it adds, for every particle whose support STARTS at
+// plane p and covers the column, that particle's contribution to all P slots (statically indexed), then
+// stores slot 0 (plane p is now final), shifts the window and moves on.  For a fixed column the summand is
 // a cubic in dx = x_n - x_j times the x-Gaussian:
 //   H_c = gx(k) [ c0 + dx c1 + dx^2 c2 + dx^3 c3 ]_c      -> 4 FMA per component and grid point,
 // with the (y,z) Gaussian folded into the four coefficients and gx dx^n tabulated per particle (a1).  The sweep is cut into segments along x for
@@ -18,11 +17,8 @@
 
 // NC = 3: the three force-density grids; NC = 4: plus the scalar grid of the pressure moments (a9),
 // Hs(x_n) = sum_j gamma(d) s_j, one more FMA per grid point.
-// The register window is ROTATING: slot s holds the plane q with q = s (mod P); a particle whose support starts at
-// plane p (p0 = p mod P) adds its k-th support plane to slot (p0 + k) mod P, i.e. slot s takes entry s + P - p0 of the
-// x tables, which the record stores twice (se_common.cuh) -- X points at entry P - p0, the slot index is static.
 template <int P, int NC>
-__device__ __forceinline__ void spread_hit(const SeConst &c, const double *__restrict__ rec, int xrot, int y, int z, bool active,
+__device__ __forceinline__ void spread_hit(const SeConst &c, const double *__restrict__ rec, int y, int z, bool active,
                                            double (&acc)[P][NC])
 {
     const int M = c.M;
@@ -31,75 +27,47 @@ __device__ __forceinline__ void spread_hit(const SeConst &c, const double *__res
     ry += ry < 0 ? M : 0;
     rz += rz < 0 ? M : 0;
     if (active && ry < P && rz < P) {
-        const double Delta = c.Delta;
-        const double dy = rec[REC_D0Y] + ry * Delta, dz = rec[REC_D0Z] + rz * Delta;
-        const double g = rec[SE_REC_HDR + ry] * rec[SE_REC_HDR + P + rz];
+        const double Delta = c.Delta, al = c.alpha;
+        const double dy = rec[REC_D0 + 1] + ry * Delta, dz = rec[REC_D0 + 2] + rz * Delta;
+        const double gyz = rec[SE_REC_HDR + P + ry] * rec[SE_REC_HDR + 2 * P + rz];
         const double rho2 = dy * dy + dz * dz;
-        const double2 pf = *reinterpret_cast<const double2 *>(rec + REC_POLY), ps = *reinterpret_cast<const double2 *>(rec + REC_POLY + 2);
-        // the (y,z) Gaussian folded into the five scalars the coefficients are made of
-        const double gfa = g * (pf.x + pf.y * rho2);           // g [(1 - 6 al cF) + 4 al^2 cF rho^2]
-        const double gsa = g * (ps.x + ps.y * rho2);           // g [2 al (1 - 10 al cS) + 8 al^3 cS rho^2]
-        const double gal = g * c.alpha, gf1 = g * pf.y, gs1 = g * ps.y;
-        const double2 m0 = *reinterpret_cast<const double2 *>(rec + REC_F), m1 = *reinterpret_cast<const double2 *>(rec + REC_F + 2),
-                      m2 = *reinterpret_cast<const double2 *>(rec + REC_F + 4), m3 = *reinterpret_cast<const double2 *>(rec + REC_F + 6),
-                      m4 = *reinterpret_cast<const double2 *>(rec + REC_F + 8), m5 = *reinterpret_cast<const double2 *>(rec + REC_F + 10);
-        const double Fx = m0.x, Fy = m0.y, Fz = m1.x, Tx = m1.y, Ty = m2.x, Tz = m2.y;
-        const double Sxx = m3.x, Sxy = m3.y, Sxz = m4.x, Syy = m4.y, Syz = m5.x, Szz = m5.y;
+        const double f1 = rec[REC_POLY + 1], s1 = rec[REC_POLY + 3];
+        const double fa = rec[REC_POLY] + f1 * rho2;          // (1 - 6 al cF) + 4 al^2 cF rho^2
+        const double sa = rec[REC_POLY + 2] + s1 * rho2;      // 2 al (1 - 10 al cS) + 8 al^3 cS rho^2
+        const double Fx = rec[REC_F], Fy = rec[REC_F + 1], Fz = rec[REC_F + 2];
+        const double Tx = rec[REC_T], Ty = rec[REC_T + 1], Tz = rec[REC_T + 2];
+        const double Sxx = rec[REC_S], Sxy = rec[REC_S + 1], Sxz = rec[REC_S + 2];
+        const double Syy = rec[REC_S + 3], Syz = rec[REC_S + 4], Szz = rec[REC_S + 5];
         // S.d = S_cx dx + sig_c;  d x T = tau0 + dx tau1 with tau1 = (0, -Tz, Ty)
         const double sg0 = Sxy * dy + Sxz * dz, sg1 = Syy * dy + Syz * dz, sg2 = Syz * dy + Szz * dz;
         const double t00 = dy * Tz - dz * Ty, t01 = dz * Tx, t02 = -dy * Tx;
         double c0[3], c1[3], c2[3], c3[3];
-        c0[0] = gfa * Fx - gal * t00 + gsa * sg0;
-        c0[1] = gfa * Fy - gal * t01 + gsa * sg1;
-        c0[2] = gfa * Fz - gal * t02 + gsa * sg2;
-        c1[0] = gsa * Sxx;
-        c1[1] = gsa * Sxy + gal * Tz;
-        c1[2] = gsa * Sxz - gal * Ty;
-        c2[0] = gf1 * Fx + gs1 * sg0;
-        c2[1] = gf1 * Fy + gs1 * sg1;
-        c2[2] = gf1 * Fz + gs1 * sg2;
-        c3[0] = gs1 * Sxx; c3[1] = gs1 * Sxy; c3[2] = gs1 * Sxz;
-        const double gsp = NC == 4 ? g * rec[REC_SP] : 0.0;
-        // acc[s][a] += sum_n X[s][n] c_n[a]: 3P independent chains of four FMAs
-        const double2 *__restrict__ X = reinterpret_cast<const double2 *>(rec + xrot);
+        c0[0] = gyz * (fa * Fx - al * t00 + sa * sg0);
+        c0[1] = gyz * (fa * Fy - al * t01 + sa * sg1);
+        c0[2] = gyz * (fa * Fz - al * t02 + sa * sg2);
+        c1[0] = gyz * (sa * Sxx);
+        c1[1] = gyz * (sa * Sxy + al * Tz);
+        c1[2] = gyz * (sa * Sxz - al * Ty);
+        c2[0] = gyz * (f1 * Fx + s1 * sg0);
+        c2[1] = gyz * (f1 * Fy + s1 * sg1);
+        c2[2] = gyz * (f1 * Fz + s1 * sg2);
+        c3[0] = gyz * s1 * Sxx; c3[1] = gyz * s1 * Sxy; c3[2] = gyz * s1 * Sxz;
+        // acc[k][a] += sum_n (gx dx^n)(k) c_n[a]: four passes of 3P independent FMAs, accumulated in place
+        const double *__restrict__ X0 = rec + SE_REC_HDR, *__restrict__ X1 = rec + SE_REC_HDR + 3 * P;
 #pragma unroll
-        for (int s = 0; s < P; ++s) {
-            const double2 x01 = X[2 * s], x23 = X[2 * s + 1];
+        for (int k = 0; k < P; ++k) {
+            const double x0 = X0[k], x1 = X1[k], x2 = X1[P + k], x3 = X1[2 * P + k];
 #pragma unroll
             for (int a = 0; a < 3; ++a) {
-                double t = acc[s][a];
-                t = fma(x01.x, c0[a], t);
-                t = fma(x01.y, c1[a], t);
-                t = fma(x23.x, c2[a], t);
-                acc[s][a] = fma(x23.y, c3[a], t);
+                double t = acc[k][a];
+                t = fma(x0, c0[a], t);
+                t = fma(x1, c1[a], t);
+                t = fma(x2, c2[a], t);
+                acc[k][a] = fma(x3, c3[a], t);
             }
-            if (NC == 4) acc[s][NC - 1] = fma(x01.x, gsp, acc[s][NC - 1]);
+            if (NC == 4) acc[k][NC - 1] = fma(x0, gyz * rec[REC_SP], acc[k][NC - 1]);
         }
     }
-}
-
-// Store window slot p0 (now final: the plane whose index is p0 mod P) if `st`, and clear it for the plane P further on.
-template <int P, int NC>
-__device__ __forceinline__ void spread_flush(int p0, bool st, size_t idx, size_t G, double *__restrict__ H, double *__restrict__ Hs,
-                                             double (&acc)[P][NC])
-{
-#define SE_SLOT(S)                                                                  \
-    case S:                                                                         \
-        if (S < P) {                                                                \
-            constexpr int s_ = S < P ? S : 0;                                       \
-            if (st) {                                                               \
-                H[idx] = acc[s_][0]; H[G + idx] = acc[s_][1]; H[2 * G + idx] = acc[s_][2]; \
-                if (NC == 4) Hs[idx] = acc[s_][NC - 1];                             \
-            }                                                                       \
-            _Pragma("unroll") for (int a = 0; a < NC; ++a) acc[s_][a] = 0.0;        \
-        }                                                                           \
-        break;
-    switch (p0) {
-        SE_SLOT(0) SE_SLOT(1) SE_SLOT(2) SE_SLOT(3) SE_SLOT(4) SE_SLOT(5) SE_SLOT(6) SE_SLOT(7)
-        SE_SLOT(8) SE_SLOT(9) SE_SLOT(10) SE_SLOT(11) SE_SLOT(12) SE_SLOT(13) SE_SLOT(14) SE_SLOT(15)
-        SE_SLOT(16) SE_SLOT(17) SE_SLOT(18) SE_SLOT(19) SE_SLOT(20) SE_SLOT(21) SE_SLOT(22) SE_SLOT(23)
-    }
-#undef SE_SLOT
 }
 
 template <int P, int NC>
@@ -107,7 +75,7 @@ __global__ void __launch_bounds__(SWEEP_WARPS * 32, NC == 3 ? SWEEP_MIN_BLOCKS :
                                                               const int *__restrict__ start_s, double *__restrict__ H,
                                                               double *__restrict__ Hs)
 {
-    extern __shared__ __align__(32) unsigned char sweep_smem[];
+    extern __shared__ __align__(16) unsigned char sweep_smem[];
     const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
     const int wid = blockIdx.x * SWEEP_WARPS + wl;
     const int npatch = c.NBY * c.NBZ;
@@ -139,9 +107,7 @@ __global__ void __launch_bounds__(SWEEP_WARPS * 32, NC == 3 ? SWEEP_MIN_BLOCKS :
 
     const int seg_start = seg * c.seg_len, seg_end = min(seg_start + c.seg_len, M);
     const size_t G = (size_t)M * M * M;
-    constexpr int XOFF = (SE_REC_HDR + 2 * P + 3) & ~3;
     int p = seg_start - (P - 1);
-    int p0 = (p % P + P) % P;                            // window slot of plane p
     auto binbase = [&](int q) { return (q < 0 ? q + M : q) * npatch; };
     SweepList cur = sweep_scan(sweep_load(rg, start_s, binbase(p), lane), lane);
     sweep_stage(cur, recs, stride, smem_u32(slot0), bar0, lane);
@@ -160,17 +126,26 @@ __global__ void __launch_bounds__(SWEEP_WARPS * 32, NC == 3 ? SWEEP_MIN_BLOCKS :
             parity ^= 1u << buf;
             const double *__restrict__ sl = buf ? slot1 : slot0;
             const int ns = min(cur.n, SWEEP_CAP);
-            const int xrot = XOFF + 4 * (P - p0);
-            for (int ci = 0; ci < ns; ++ci) spread_hit<P, NC>(c, sl + (size_t)ci * stride, xrot, y, z, active, acc);
+            for (int ci = 0; ci < ns; ++ci) spread_hit<P, NC>(c, sl + (size_t)ci * stride, y, z, active, acc);
             for (int ci = SWEEP_CAP; ci < cur.n; ++ci) {
                 const int j = sweep_overflow_index(cur, ci);
-                spread_hit<P, NC>(c, recs + (size_t)j * stride, xrot, y, z, active, acc);
+                spread_hit<P, NC>(c, recs + (size_t)j * stride, y, z, active, acc);
             }
             __syncwarp();                           // slot fully read before it is refilled
         }
-        // plane p is final: no later particle of this sweep reaches it
-        spread_flush<P, NC>(p0, p >= seg_start && active, ((size_t)max(p, 0) * M + y) * M + z, G, H, Hs, acc);
-        p0 = p0 + 1 == P ? 0 : p0 + 1;
+        if (p >= seg_start && active) {
+            const size_t idx = ((size_t)p * M + y) * M + z;
+            H[idx] = acc[0][0];
+            H[G + idx] = acc[0][1];
+            H[2 * G + idx] = acc[0][2];
+            if (NC == 4) Hs[idx] = acc[0][NC - 1];
+        }
+#pragma unroll
+        for (int k = 0; k < P - 1; ++k)
+#pragma unroll
+            for (int a = 0; a < NC; ++a) acc[k][a] = acc[k + 1][a];
+#pragma unroll
+        for (int a = 0; a < NC; ++a) acc[P - 1][a] = 0.0;
         cur = nxt;
     }
 }
