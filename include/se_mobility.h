@@ -94,8 +94,11 @@ se_status se_plan_set_tuning(se_plan *plan, int spread_segments, int gather_segm
  *                        beside the whole wave pipeline; 2 = on that stream, started after the spreading (beside the
  *                        HBM-bound transforms).  Joined before the epilogue in every case.
  *   SE_OPT_REAL_CTAS     CTAs of the real-space kernel when it runs beside the wave pipeline (0 = one per cell).
+ *   SE_OPT_XY_PATH       (x,y) transforms of power-of-two grids: 0 = own kernels, the y transforms and ONE kernel that
+ *                        fuses the x transforms with the k-space scaling (default); 1 = cuFFT's batched 2-D complex plans
+ *                        and a separate k-space kernel.
  * Errors: SE_ERR_INVALID_ARG for an unknown key or a value out of range. */
-enum { SE_OPT_REAL_OVERLAP = 0, SE_OPT_REAL_CTAS = 1, SE_NUM_OPTS = 2 };
+enum { SE_OPT_REAL_OVERLAP = 0, SE_OPT_REAL_CTAS = 1, SE_OPT_XY_PATH = 2, SE_NUM_OPTS = 3 };
 se_status se_plan_set_option(se_plan *plan, int key, int value);
 
 /* Bitwise OR of the SE_* flags above. */

@@ -16,6 +16,7 @@
 #include "se_kspace.cuh"
 #include "se_xfft.cuh"
 #include "se_zfft.cuh"
+#include "se_xyfft.cuh"
 #include "se_gather.cuh"
 
 #ifndef M_PI
@@ -78,6 +79,8 @@ struct se_plan {
     bool have_zt;
     int lM;
     double2 *d_wtab;               // exp(-2 pi i q / M), q < M
+    double *d_etab;                // exp(-(1 - eta_se) k_q^2 / 4 xi^2), q < M (k-space pass of se_xyfft.cuh)
+    int xy_path;                   // SE_OPT_XY_PATH: 0 = own y / fused x kernels, 1 = cuFFT 2-D plans + k_kspace
     size_t fft_bytes;
     cudaEvent_t ev[SE_NUM_STAGES + 1];
     bool have_events, timed;
@@ -237,7 +240,7 @@ extern "C" se_status se_plan_destroy(se_plan *p)
         if (p->have_fftz1) cufftDestroy(p->fftz_1);
     }
     if (p->have_zt) { cufftDestroy(p->fftz_fwd); cufftDestroy(p->fftz_inv); }
-    cudaFree(p->d_wtab);
+    cudaFree(p->d_wtab); cudaFree(p->d_etab);
     if (p->have_fwd) cufftDestroy(p->fft_fwd);
     if (p->have_inv) cufftDestroy(p->fft_inv);
     if (p->have_events) for (int k = 0; k <= SE_NUM_STAGES; ++k) cudaEventDestroy(p->ev[k]);
@@ -339,6 +342,84 @@ static se_status ensure_wtab(se_plan *p)
     return st;
 }
 
+// Per-axis table of the separable Gaussian factor of the k-space pass; depends on the shape parameter m.
+static se_status upload_etab(se_plan *p)
+{
+    const int M = p->c.M;
+    if (!p->d_etab) { se_status st = dev_alloc(p, &p->d_etab, (size_t)M); if (st != SE_OK) return st; }
+    double *et = (double *)malloc(sizeof(double) * (size_t)M);
+    if (!et) return fail(p, SE_ERR_ALLOC, "malloc", "exp table");
+    for (int q = 0; q < M; ++q) { const double k = p->c.twopiL * (q < M / 2 ? q : q - M); et[q] = exp(-p->c.dec * k * k); }
+    const cudaError_t e = cudaMemcpy(p->d_etab, et, sizeof(double) * (size_t)M, cudaMemcpyHostToDevice);
+    free(et);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(p, SE_ERR_CUDA, "cudaMemcpy", "exp table"); }
+    return SE_OK;
+}
+
+// y-batch of k_xmid: 4 columns (64-byte runs), 2 where the compressible variant would not fit the register file
+template <int LM, bool COMP> struct XmChoice { static constexpr int YB = (COMP && LM == 9) ? 2 : 4; };
+
+template <int LM>
+static cudaError_t prepare_xy()
+{
+    cudaError_t e = raise_smem_limit(k_yfft<LM, false>);
+    if (e == cudaSuccess) e = raise_smem_limit(k_yfft<LM, true>);
+    if (e == cudaSuccess) e = raise_smem_limit(k_xmid<LM, XmChoice<LM, false>::YB, false>);
+    if (e == cudaSuccess) e = raise_smem_limit(k_xmid<LM, XmChoice<LM, true>::YB, true>);
+    return e;
+}
+
+template <int LM>
+static void launch_yfft(cudaStream_t s, double2 *spec, const double2 *wtab, int ngrids, bool inv)
+{
+    using TR = YfTraits<LM>;
+    const size_t nlines = (size_t)ngrids * (TR::M / 2) * TR::M;
+    const unsigned nb = (unsigned)((nlines + TR::LPC - 1) / TR::LPC);
+    if (inv) k_yfft<LM, true><<<nb, YF_THREADS, TR::SMEM, s>>>(spec, wtab, ngrids);
+    else k_yfft<LM, false><<<nb, YF_THREADS, TR::SMEM, s>>>(spec, wtab, ngrids);
+}
+
+template <int LM, bool COMP>
+static void launch_xmid(const SeConst &c, cudaStream_t s, const double2 *Hk, const double2 *Hsk, double2 *Gk, double2 *Pk,
+                        const double2 *wtab, const double *etab)
+{
+    constexpr int YB = XmChoice<LM, COMP>::YB;
+    using TR = XmTraits<LM, YB, COMP>;
+    const unsigned nb = (unsigned)((TR::M / 2 + 1) * (TR::M / YB));
+    k_xmid<LM, YB, COMP><<<nb, TR::NT, TR::SMEM, s>>>(c, Hk, Hsk, Gk, Pk, wtab, etab);
+}
+
+#define FOR_EACH_LM(X) X(5) X(6) X(7) X(8) X(9)
+
+static cudaError_t dispatch_prepare_xy(int lM)
+{
+    switch (lM) {
+#define X(v) case v: return prepare_xy<v>();
+        FOR_EACH_LM(X)
+#undef X
+    }
+    return cudaErrorInvalidValue;
+}
+
+static void dispatch_yfft(int lM, cudaStream_t s, double2 *spec, const double2 *wtab, int ngrids, bool inv)
+{
+    switch (lM) {
+#define X(v) case v: launch_yfft<v>(s, spec, wtab, ngrids, inv); break;
+        FOR_EACH_LM(X)
+#undef X
+    }
+}
+
+static void dispatch_xmid(int lM, bool comp, const SeConst &c, cudaStream_t s, const double2 *Hk, const double2 *Hsk, double2 *Gk,
+                          double2 *Pk, const double2 *wtab, const double *etab)
+{
+    switch (lM) {
+#define X(v) case v: if (comp) launch_xmid<v, true>(c, s, Hk, Hsk, Gk, Pk, wtab, etab); else launch_xmid<v, false>(c, s, Hk, Hsk, Gk, Pk, wtab, etab); break;
+        FOR_EACH_LM(X)
+#undef X
+    }
+}
+
 // Plans of the own-z-transform path (se_zfft.cuh): contiguous batched 2-D complex transforms over (x,y), 3 (M/2+1)
 // planes forward and 6 (M/2+1) inverse, in place.
 static se_status ensure_zt(se_plan *p)
@@ -365,9 +446,14 @@ static se_status ensure_zt(se_plan *p)
         if (c2) cufftDestroy(p->fftz_inv);
         return fail(p, r == CUFFT_ALLOC_FAILED ? SE_ERR_ALLOC : SE_ERR_CUFFT, "ensure_zt", "2-D complex plans");
     }
-    p->have_zt = true;
     p->lM = 0;
     while ((1 << p->lM) < M) ++p->lM;
+    {
+        se_status ste = upload_etab(p);
+        if (ste == SE_OK && dispatch_prepare_xy(p->lM) != cudaSuccess) { cudaGetLastError(); ste = fail(p, SE_ERR_CUDA, "ensure_zt", "shared-memory limit"); }
+        if (ste != SE_OK) { cufftDestroy(p->fftz_fwd); cufftDestroy(p->fftz_inv); return ste; }
+    }
+    p->have_zt = true;
     p->fft_bytes += tot;
     p->bytes += tot;
     return SE_OK;
@@ -481,6 +567,7 @@ extern "C" se_status se_plan_set_shape(se_plan *p, double m)
     p->m = m;
     derive_constants(p);
     p->have_positions = false;          // the cached Gaussian tables depend on the shape
+    if (p->d_etab) return upload_etab(p);
     return SE_OK;
 }
 
@@ -497,6 +584,7 @@ extern "C" se_status se_plan_set_option(se_plan *p, int key, int value)
     switch (key) {
     case SE_OPT_REAL_OVERLAP: if (value > 2) return SE_ERR_INVALID_ARG; p->real_overlap = value; break;
     case SE_OPT_REAL_CTAS: p->real_side_ctas = value; break;
+    case SE_OPT_XY_PATH: if (value > 1) return SE_ERR_INVALID_ARG; p->xy_path = value; break;
     default: return SE_ERR_INVALID_ARG;
     }
     return SE_OK;
@@ -686,7 +774,7 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     const bool use_zt = !(p->flags & SE_CUFFT3D) && xf_supported(p->c.M);
     if (use_zt) { se_status stf = ensure_zt(p); if (stf != SE_OK) return stf; }
     if (!use_zt) { se_status stf = ensure_fft3d(p, false); if (stf != SE_OK) return stf; }
-    if (comp) { se_status stf = ensure_comp_plans(p, use_zt); if (stf != SE_OK) return stf; }
+    if (comp && !(use_zt && p->xy_path == 0)) { se_status stf = ensure_comp_plans(p, use_zt); if (stf != SE_OK) return stf; }
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const SeConst &c = p->c;
     const unsigned fl = p->flags;
@@ -755,15 +843,27 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
         else k_zfft_r2c<256><<<3 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_real, p->d_Hk, p->d_wtab);
         p->last_launches += 1;
         CUDA_TRY(p, cudaGetLastError());
-        CUFFT_TRY(p, cufftSetStream(p->fftz_fwd, s));
-        CUFFT_TRY(p, cufftExecZ2Z(p->fftz_fwd, (cufftDoubleComplex *)p->d_Hk, (cufftDoubleComplex *)p->d_Hk, CUFFT_FORWARD));
+        if (p->xy_path == 0) {
+            dispatch_yfft(p->lM, s, p->d_Hk, p->d_wtab, 3, false);
+            p->last_launches += 1;
+            CUDA_TRY(p, cudaGetLastError());
+        } else {
+            CUFFT_TRY(p, cufftSetStream(p->fftz_fwd, s));
+            CUFFT_TRY(p, cufftExecZ2Z(p->fftz_fwd, (cufftDoubleComplex *)p->d_Hk, (cufftDoubleComplex *)p->d_Hk, CUFFT_FORWARD));
+        }
         if (comp_in) {
             if (zt_threads(M) <= 128) k_zfft_r2c<128><<<M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_real_p, p->d_Hk_s, p->d_wtab);
             else k_zfft_r2c<256><<<M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_real_p, p->d_Hk_s, p->d_wtab);
             p->last_launches += 1;
             CUDA_TRY(p, cudaGetLastError());
-            CUFFT_TRY(p, cufftSetStream(p->fftz_1, s));
-            CUFFT_TRY(p, cufftExecZ2Z(p->fftz_1, (cufftDoubleComplex *)p->d_Hk_s, (cufftDoubleComplex *)p->d_Hk_s, CUFFT_FORWARD));
+            if (p->xy_path == 0) {
+                dispatch_yfft(p->lM, s, p->d_Hk_s, p->d_wtab, 1, false);
+                p->last_launches += 1;
+                CUDA_TRY(p, cudaGetLastError());
+            } else {
+                CUFFT_TRY(p, cufftSetStream(p->fftz_1, s));
+                CUFFT_TRY(p, cufftExecZ2Z(p->fftz_1, (cufftDoubleComplex *)p->d_Hk_s, (cufftDoubleComplex *)p->d_Hk_s, CUFFT_FORWARD));
+            }
         }
     } else if (on(SE_STAGE_FFT_FWD)) {
         CUFFT_TRY(p, cufftSetStream(p->fft_fwd, s));
@@ -777,7 +877,9 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     if (on(SE_STAGE_KSPACE)) {
         const size_t Gc = (size_t)c.M * c.M * (c.M / 2 + 1);
         const unsigned nbk = (unsigned)((Gc + KSPACE_THREADS - 1) / KSPACE_THREADS);
-        if (use_zt) k_kspace<true><<<nbk, KSPACE_THREADS, 0, s>>>(c, p->d_Hk, p->d_Gk, comp_in ? p->d_Hk_s : nullptr,
+        if (use_zt && p->xy_path == 0) dispatch_xmid(p->lM, comp, c, s, p->d_Hk, comp_in ? p->d_Hk_s : nullptr, p->d_Gk, comp_out ? p->d_Gk_p : nullptr,
+                                                      p->d_wtab, p->d_etab);
+        else if (use_zt) k_kspace<true><<<nbk, KSPACE_THREADS, 0, s>>>(c, p->d_Hk, p->d_Gk, comp_in ? p->d_Hk_s : nullptr,
                                                                   comp_out ? p->d_Gk_p : nullptr);
         else k_kspace<false><<<nbk, KSPACE_THREADS, 0, s>>>(c, p->d_Hk, p->d_Gk, comp_in ? p->d_Hk_s : nullptr,
                                                             comp_out ? p->d_Gk_p : nullptr);
@@ -787,15 +889,27 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     MARK();
     if (on(SE_STAGE_FFT_INV) && use_zt) {
         const int M = c.M, MYp = p->gg.MYp, MZp = p->gg.MZp, halo = c.P - 1;
-        CUFFT_TRY(p, cufftSetStream(p->fftz_inv, s));
-        CUFFT_TRY(p, cufftExecZ2Z(p->fftz_inv, (cufftDoubleComplex *)p->d_Gk, (cufftDoubleComplex *)p->d_Gk, CUFFT_INVERSE));
+        if (p->xy_path == 0) {
+            dispatch_yfft(p->lM, s, p->d_Gk, p->d_wtab, 6, true);
+            p->last_launches += 1;
+            CUDA_TRY(p, cudaGetLastError());
+        } else {
+            CUFFT_TRY(p, cufftSetStream(p->fftz_inv, s));
+            CUFFT_TRY(p, cufftExecZ2Z(p->fftz_inv, (cufftDoubleComplex *)p->d_Gk, (cufftDoubleComplex *)p->d_Gk, CUFFT_INVERSE));
+        }
         if (zt_threads(M) <= 128) k_zfft_c2r<128><<<6 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk, p->d_real, p->d_wtab, MYp, MZp, halo);
         else k_zfft_c2r<256><<<6 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk, p->d_real, p->d_wtab, MYp, MZp, halo);
         p->last_launches += 1;
         CUDA_TRY(p, cudaGetLastError());
         if (comp_out) {
-            CUFFT_TRY(p, cufftSetStream(p->fftz_1, s));
-            CUFFT_TRY(p, cufftExecZ2Z(p->fftz_1, (cufftDoubleComplex *)p->d_Gk_p, (cufftDoubleComplex *)p->d_Gk_p, CUFFT_INVERSE));
+            if (p->xy_path == 0) {
+                dispatch_yfft(p->lM, s, p->d_Gk_p, p->d_wtab, 1, true);
+                p->last_launches += 1;
+                CUDA_TRY(p, cudaGetLastError());
+            } else {
+                CUFFT_TRY(p, cufftSetStream(p->fftz_1, s));
+                CUFFT_TRY(p, cufftExecZ2Z(p->fftz_1, (cufftDoubleComplex *)p->d_Gk_p, (cufftDoubleComplex *)p->d_Gk_p, CUFFT_INVERSE));
+            }
             if (zt_threads(M) <= 128) k_zfft_c2r<128><<<M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk_p, p->d_real_p, p->d_wtab, MYp, MZp, halo);
             else k_zfft_c2r<256><<<M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk_p, p->d_real_p, p->d_wtab, MYp, MZp, halo);
             p->last_launches += 1;
