@@ -97,8 +97,11 @@ se_status se_plan_set_tuning(se_plan *plan, int spread_segments, int gather_segm
  *   SE_OPT_XY_PATH       (x,y) transforms of power-of-two grids: 0 = own kernels, the y transforms and ONE kernel that
  *                        fuses the x transforms with the k-space scaling (default); 1 = cuFFT's batched 2-D complex plans
  *                        and a separate k-space kernel.
+ *   SE_OPT_YZ_FUSED      with SE_OPT_XY_PATH = 0: 1 = the y and z transforms of a direction in ONE kernel (thread-block
+ *                        clusters exchanging through distributed shared memory; default for M <= 128), 0 = separate
+ *                        z and y kernels.
  * Errors: SE_ERR_INVALID_ARG for an unknown key or a value out of range. */
-enum { SE_OPT_REAL_OVERLAP = 0, SE_OPT_REAL_CTAS = 1, SE_OPT_XY_PATH = 2, SE_NUM_OPTS = 3 };
+enum { SE_OPT_REAL_OVERLAP = 0, SE_OPT_REAL_CTAS = 1, SE_OPT_XY_PATH = 2, SE_OPT_YZ_FUSED = 3, SE_NUM_OPTS = 4 };
 se_status se_plan_set_option(se_plan *plan, int key, int value);
 
 /* Bitwise OR of the SE_* flags above. */

@@ -29,9 +29,18 @@
 
 #define GATHER_SUMS 24             // per particle: slot (g/3)*12 + kind*3 + g%3, kind = 0 (1), 1 (dx), 2 (dy), 3 (dz)
 #ifndef GR_WARPS
-#define GR_WARPS 8                 // consumer warps; warp GR_WARPS is the producer
+#define GR_WARPS 12                // consumer warps; warp GR_WARPS is the producer
 #endif
 
+#ifndef GR_PREFETCH
+#define GR_PREFETCH 16             // planes the producer's L2 prefetch cursor runs ahead of its loads
+#endif
+#ifndef GT_TZ12
+#define GT_TZ12 32                 // tile width along z for P <= 12
+#endif
+#ifndef GT_RS12
+#define GT_RS12 7                  // ring slack for P <= 12: R = P + GT_RS12 planes
+#endif
 // Compile-time geometry of the gather for support P.
 template <int P> struct GatherTraits {
     static constexpr bool HALF = P <= 16;                       // two particles per warp
@@ -39,8 +48,8 @@ template <int P> struct GatherTraits {
     static constexpr int LZ = LP / 4;                           // lane grid 4 x LZ
     static constexpr int CY = (P + 3) / 4, CZ = (P + LZ - 1) / LZ;   // footprint columns per lane: CY x CZ
     static constexpr int TY = P <= 16 ? 16 : (P <= 20 ? 8 : 2);
-    static constexpr int TZ = P <= 12 ? 32 : (P <= 16 ? 16 : 8);
-    static constexpr int R = P <= 12 ? P + 5 : (P <= 16 ? P + 4 : (P <= 20 ? P + 3 : P + 1));
+    static constexpr int TZ = P <= 12 ? GT_TZ12 : (P <= 16 ? 16 : 8);
+    static constexpr int R = P <= 12 ? P + GT_RS12 : (P <= 16 ? P + 4 : (P <= 20 ? P + 3 : P + 1));
     static constexpr int WY = TY + 4 * CY - 1;                  // rows of the haloed tile (>= TY + P - 1)
     static constexpr int WZ0 = TZ + LZ * CZ - 1;
     // row pitch = 4 (mod 8) [half-warp particles] or 8 (mod 16) [warp particles]: conflict-free column loads
@@ -69,6 +78,12 @@ __device__ __forceinline__ void tma_box3(uint32_t dst, const CUtensorMap *tmap, 
 {
     asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
                  ::"r"(dst), "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
+}
+
+// Ask for the same box to be brought into L2 (no shared-memory destination, no completion to wait for).
+__device__ __forceinline__ void tma_prefetch3(const CUtensorMap *tmap, int c0, int c1, int c2)
+{
+    asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];" ::"l"(tmap), "r"(c0), "r"(c1), "r"(c2) : "memory");
 }
 
 // Work item `it` of the launch: all tiles of one (grid, segment) are consecutive, so that the CTAs of one round work
@@ -126,14 +141,32 @@ k_gather(SeConst c, GatherGeom g, const double *__restrict__ grecs, const int *_
             constexpr uint32_t box_bytes = (uint32_t)(GT::WY * WZ * 8);
             int sl = 0;
             uint32_t par = 1;                                          // passes at once in round 0
+            // A second cursor runs GR_PREFETCH planes ahead of the loads (across item boundaries) and asks for the boxes
+            // to be brought into L2, so that the ring fill itself sees L2 latency only: the ring's slack of R - P planes
+            // is too short to cover a DRAM miss under load.
+            int pit = blockIdx.x, pj = 0, ahead = 0;
+            GatherItem PI = pit < nitems ? gather_item(pit, c, g, ngrids, start_g) : GatherItem{};
+            auto prefetch_step = [&]() {                               // prefetch one plane, advance the cursor
+                while (pit < nitems && (PI.i0 == PI.i1 || pj >= PI.nplanes)) {
+                    pit += gridDim.x; pj = 0;
+                    if (pit < nitems) PI = gather_item(pit, c, g, ngrids, start_g);
+                }
+                if (pit >= nitems) return;
+                int x = PI.seg_start + pj;
+                if (x >= M) x -= M;
+                tma_prefetch3(&tmap, PI.Z0, PI.Y0, PI.grid * M + x);
+                ++pj;
+            };
             for (int it = blockIdx.x; it < nitems; it += gridDim.x) {
                 const GatherItem I = gather_item(it, c, g, ngrids, start_g);
                 if (I.i0 == I.i1) continue;                            // no support starts here: skipped by everybody
                 int x = I.seg_start;
                 for (int j = 0; j < I.nplanes; ++j) {
+                    while (ahead < GR_PREFETCH + 1) { prefetch_step(); ++ahead; }
                     mbar_wait(empty_bar(sl), par);
                     mbar_expect_tx(full_bar(sl), box_bytes);
                     tma_box3(ring_a + 8u * (uint32_t)(sl * SLOT), &tmap, I.Z0, I.Y0, I.grid * M + x, full_bar(sl));
+                    --ahead;
                     if (++sl == R) { sl = 0; par ^= 1u; }
                     if (++x == M) x = 0;
                 }

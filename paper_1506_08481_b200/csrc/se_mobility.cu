@@ -15,8 +15,8 @@
 #include "se_spread.cuh"
 #include "se_kspace.cuh"
 #include "se_xfft.cuh"
-#include "se_zfft.cuh"
 #include "se_xyfft.cuh"
+#include "se_zfft.cuh"
 #include "se_gather.cuh"
 
 #ifndef M_PI
@@ -81,6 +81,7 @@ struct se_plan {
     double2 *d_wtab;               // exp(-2 pi i q / M), q < M
     double *d_etab;                // exp(-(1 - eta_se) k_q^2 / 4 xi^2), q < M (k-space pass of se_xyfft.cuh)
     int xy_path;                   // SE_OPT_XY_PATH: 0 = own y / fused x kernels, 1 = cuFFT 2-D plans + k_kspace
+    int yz_fused;                  // SE_OPT_YZ_FUSED: (y,z) transforms in one cluster kernel per direction (se_zfft.cuh)
     size_t fft_bytes;
     cudaEvent_t ev[SE_NUM_STAGES + 1];
     bool have_events, timed;
@@ -391,6 +392,59 @@ static void launch_xmid(const SeConst &c, cudaStream_t s, const double2 *Hk, con
 
 #define FOR_EACH_LM(X) X(5) X(6) X(7) X(8) X(9)
 
+// (y,z) transforms by thread-block clusters of M/32 CTAs (se_zfft.cuh); M = 512 needs the non-portable cluster size 16.
+template <int LM>
+static cudaError_t prepare_yz()
+{
+    cudaError_t e = raise_smem_limit(k_yz_r2c<LM>);
+    if (e == cudaSuccess) e = raise_smem_limit(k_yz_c2r<LM>);
+    if (e == cudaSuccess && YzTraits<LM>::CS > 8) {
+        e = cudaFuncSetAttribute(k_yz_r2c<LM>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_yz_c2r<LM>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    }
+    return e;
+}
+
+template <int LM>
+static cudaError_t launch_yz(bool inv, cudaStream_t s, int ngrids, const double *H, double2 *spec, double *R, const double2 *wtab,
+                             int MYp, int MZp, int halo)
+{
+    using TR = YzTraits<LM>;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(ngrids * TR::M * TR::CS));
+    cfg.blockDim = dim3(TR::NT);
+    cfg.dynamicSmemBytes = TR::SMEM;
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = TR::CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    if (inv) return cudaLaunchKernelEx(&cfg, k_yz_c2r<LM>, (const double2 *)spec, R, wtab, MYp, MZp, halo);
+    return cudaLaunchKernelEx(&cfg, k_yz_r2c<LM>, H, spec, wtab);
+}
+
+static cudaError_t dispatch_prepare_yz(int lM)
+{
+    switch (lM) {
+#define X(v) case v: return prepare_yz<v>();
+        FOR_EACH_LM(X)
+#undef X
+    }
+    return cudaErrorInvalidValue;
+}
+
+static cudaError_t dispatch_yz(int lM, bool inv, cudaStream_t s, int ngrids, const double *H, double2 *spec, double *R,
+                               const double2 *wtab, int MYp, int MZp, int halo)
+{
+    switch (lM) {
+#define X(v) case v: return launch_yz<v>(inv, s, ngrids, H, spec, R, wtab, MYp, MZp, halo);
+        FOR_EACH_LM(X)
+#undef X
+    }
+    return cudaErrorInvalidValue;
+}
+
 static cudaError_t dispatch_prepare_xy(int lM)
 {
     switch (lM) {
@@ -450,10 +504,11 @@ static se_status ensure_zt(se_plan *p)
     while ((1 << p->lM) < M) ++p->lM;
     {
         se_status ste = upload_etab(p);
-        if (ste == SE_OK && dispatch_prepare_xy(p->lM) != cudaSuccess) { cudaGetLastError(); ste = fail(p, SE_ERR_CUDA, "ensure_zt", "shared-memory limit"); }
+        if (ste == SE_OK && (dispatch_prepare_xy(p->lM) != cudaSuccess || dispatch_prepare_yz(p->lM) != cudaSuccess)) { cudaGetLastError(); ste = fail(p, SE_ERR_CUDA, "ensure_zt", "shared-memory limit"); }
         if (ste != SE_OK) { cufftDestroy(p->fftz_fwd); cufftDestroy(p->fftz_inv); return ste; }
     }
     p->have_zt = true;
+    p->yz_fused = M <= 128 ? 1 : 0;          // measured: clusters of 8 (M = 256) lose to the separate z and y kernels
     p->fft_bytes += tot;
     p->bytes += tot;
     return SE_OK;
@@ -585,6 +640,7 @@ extern "C" se_status se_plan_set_option(se_plan *p, int key, int value)
     case SE_OPT_REAL_OVERLAP: if (value > 2) return SE_ERR_INVALID_ARG; p->real_overlap = value; break;
     case SE_OPT_REAL_CTAS: p->real_side_ctas = value; break;
     case SE_OPT_XY_PATH: if (value > 1) return SE_ERR_INVALID_ARG; p->xy_path = value; break;
+    case SE_OPT_YZ_FUSED: if (value > 1) return SE_ERR_INVALID_ARG; p->yz_fused = value; break;
     default: return SE_ERR_INVALID_ARG;
     }
     return SE_OK;
@@ -837,7 +893,15 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     }
     if (fork && p->real_overlap == 2) { se_status sf = fork_real(); if (sf != SE_OK) return sf; }
     MARK();
-    if (on(SE_STAGE_FFT_FWD) && use_zt) {
+    const bool yz = use_zt && p->xy_path == 0 && p->yz_fused != 0;
+    if (on(SE_STAGE_FFT_FWD) && yz) {
+        CUDA_TRY(p, dispatch_yz(p->lM, false, s, 3, p->d_real, p->d_Hk, nullptr, p->d_wtab, 0, 0, 0));
+        p->last_launches += 1;
+        if (comp_in) {
+            CUDA_TRY(p, dispatch_yz(p->lM, false, s, 1, p->d_real_p, p->d_Hk_s, nullptr, p->d_wtab, 0, 0, 0));
+            p->last_launches += 1;
+        }
+    } else if (on(SE_STAGE_FFT_FWD) && use_zt) {
         const int M = c.M;
         if (zt_threads(M) <= 128) k_zfft_r2c<128><<<3 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_real, p->d_Hk, p->d_wtab);
         else k_zfft_r2c<256><<<3 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_real, p->d_Hk, p->d_wtab);
@@ -887,7 +951,16 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
         CUDA_TRY(p, cudaGetLastError());
     }
     MARK();
-    if (on(SE_STAGE_FFT_INV) && use_zt) {
+    if (on(SE_STAGE_FFT_INV) && yz) {
+        const int MYp = p->gg.MYp, MZp = p->gg.MZp, halo = c.P - 1;
+        CUDA_TRY(p, dispatch_yz(p->lM, true, s, 6, nullptr, p->d_Gk, p->d_real, p->d_wtab, MYp, MZp, halo));
+        p->last_launches += 1;
+        if (comp_out) {
+            CUDA_TRY(p, dispatch_yz(p->lM, true, s, 1, nullptr, p->d_Gk_p, p->d_real_p, p->d_wtab, MYp, MZp, halo));
+            p->last_launches += 1;
+            p->real_p_padded = true;
+        }
+    } else if (on(SE_STAGE_FFT_INV) && use_zt) {
         const int M = c.M, MYp = p->gg.MYp, MZp = p->gg.MZp, halo = c.P - 1;
         if (p->xy_path == 0) {
             dispatch_yfft(p->lM, s, p->d_Gk, p->d_wtab, 6, true);

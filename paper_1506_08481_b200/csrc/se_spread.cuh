@@ -52,6 +52,7 @@ __device__ __forceinline__ void spread_hit(const SeConst &c, const double *__res
         c2[1] = gyz * (f1 * Fy + s1 * sg1);
         c2[2] = gyz * (f1 * Fz + s1 * sg2);
         c3[0] = gyz * s1 * Sxx; c3[1] = gyz * s1 * Sxy; c3[2] = gyz * s1 * Sxz;
+#ifdef SPREAD_TABLES
         // acc[k][a] += sum_n (gx dx^n)(k) c_n[a]: four passes of 3P independent FMAs, accumulated in place
         const double *__restrict__ X0 = rec + SE_REC_HDR, *__restrict__ X1 = rec + SE_REC_HDR + 3 * P;
 #pragma unroll
@@ -67,6 +68,25 @@ __device__ __forceinline__ void spread_hit(const SeConst &c, const double *__res
             }
             if (NC == 4) acc[k][NC - 1] = fma(x0, gyz * rec[REC_SP], acc[k][NC - 1]);
         }
+#else
+        // acc[k][a] += gx(k) ((c3 dx + c2) dx + c1) dx + c0)[a], dx = d0x + k Delta: 3P independent chains of four FMAs,
+        // one table value per plane
+        const double *__restrict__ X0 = rec + SE_REC_HDR;
+        const double d0x = rec[REC_D0];
+        const double gsp = NC == 4 ? gyz * rec[REC_SP] : 0.0;
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+            const double gx = X0[k], dx = fma((double)k, Delta, d0x);
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                double t = fma(c3[a], dx, c2[a]);
+                t = fma(t, dx, c1[a]);
+                t = fma(t, dx, c0[a]);
+                acc[k][a] = fma(gx, t, acc[k][a]);
+            }
+            if (NC == 4) acc[k][NC - 1] = fma(gx, gsp, acc[k][NC - 1]);
+        }
+#endif
     }
 }
 
