@@ -89,6 +89,24 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def config_dict(name, wl, world):
+    """The `config` object of the JSON line; identical in both arms (--impl ours / reference)."""
+    return {"workload": f"{name}: N={wl.N}, M={wl.M}, P={wl.P}, phi={wl.phi}, radii={wl.meta['radii']}, "
+                        f"positions={wl.meta['positions']}", "N": wl.N, "M": wl.M, "P": wl.P, "xi": wl.xi, "r_c": wl.rc,
+            "parallelism": "replicas only" if world > 1 else "single GPU",
+            "l2": "no flush: the per-step working set (grids + spectra, > 2 GB at c4) is far larger than the 126 MB L2"}
+
+
+def load_counters():
+    """ncu counters of the own kernels (profiles/r02_counters.json, written from the tracked capture by
+    `python -m paper_1506_08481_b200.profile_counters`); None when the file is absent."""
+    path = os.path.join(ROOT, "profiles", "r02_counters.json")
+    try:
+        return json.load(open(path))
+    except Exception:
+        return None
+
+
 def cpu_oracle_seconds(wl, repeats=1):
     """One full O2 product of the workload on the host cores, as the oracle stands."""
     import oracle as O
@@ -143,6 +161,18 @@ def measure_config(name, dev, peak, steps):
     return out
 
 
+def real_pairs(wl):
+    """Ordered pairs with minimum-image distance below r_c (the work of the real-space kernel), counted with a k-d tree."""
+    try:
+        from scipy.spatial import cKDTree
+        pos = np.mod(wl.pos, wl.L)
+        pos[pos >= wl.L] = 0.0
+        t = cKDTree(pos, boxsize=wl.L)
+        return float(t.count_neighbors(t, wl.rc) - wl.N)          # ordered pairs, self pairs removed
+    except Exception:
+        return float("nan")
+
+
 def run_reference(args, rank, world):
     """--impl reference: the CPU oracle timed on the host cores, rank 0 only."""
     if rank != 0:
@@ -162,10 +192,10 @@ def run_reference(args, rank, world):
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "ns_per_particle": 1e9 * dt / args.steps / wl.N,
-        "config": {"workload": f"{args.config}: N={wl.N}, M={wl.M}, P={wl.P}, phi={wl.phi}, radii={wl.meta['radii']}",
-                   "N": wl.N, "M": wl.M, "P": wl.P, "xi": wl.xi, "r_c": wl.rc},
+        "config": config_dict(args.config, wl, world),
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle",
-                         "sample": f"full {args.config} product (oracle O2, gcc -O2 -fopenmp) per step"},
+                         "sample": f"full {args.config} product per step (oracle O2 as it stands, gcc -O2 -fopenmp; its spreading "
+                                   "loop and line FFTs are serial, only the gather, k-space and real-space loops are threaded)"},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -228,14 +258,15 @@ def main():
     if rank == 0:
         sampler.start()
         time.sleep(0.15)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     barrier()
-    e0.record(stream)
-    for _ in range(args.steps):
+    ev[0].record(stream)
+    for k in range(args.steps):
         plan.apply(pos, F, T, S, U, Om, E)
-    e1.record(stream)
+        ev[k + 1].record(stream)
     barrier()
-    ms_total = e0.elapsed_time(e1)
+    ms_total = ev[0].elapsed_time(ev[-1])
+    ms_median = statistics.median(ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps))
     launches = plan.last_launch_count() * args.steps
     clocks = sampler.stop() if rank == 0 else None
     if dist is not None:
@@ -262,11 +293,12 @@ def main():
 
     # ---- per-stage CUDA-event times (library events on the launch stream), averaged over K steps ----
     plan.set_flags(pk.SE_TIMING)
-    stage = {k: 0.0 for k in pk.STAGE_NAMES}
+    samples = {k: [] for k in pk.STAGE_NAMES}
     for _ in range(args.steps):
         plan.apply(pos, F, T, S, U, Om, E)
         for k, v in plan.timings().items():
-            stage[k] += v / args.steps
+            samples[k].append(v)
+    stage = {k: statistics.median(v) for k, v in samples.items()}          # median over the timed steps
     plan.set_flags(0)
 
     # ---- end to end through the C-ABI host entry point: pinned host buffers, H2D + D2H inside the timed region ----
@@ -292,44 +324,78 @@ def main():
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant own kernel (cuFFT stages are library calls, reported separately) ----
+    # ---- roofline of the dominant own kernel (stage times above: CUDA events of the library on the launch stream) ----
+    # Algorithmic work per launch: bytes of the three grid kernels, useful FP64 operations of the
+    # three arithmetic-bound ones.  `traffic` and the DFMA counts come from the tracked ncu capture
+    # (profiles/r02_counters.json), never from literals here; absent file or other config -> null.
     peak, peak_src = measured_peaks()
+    NOMINAL_HBM = 8000.0
     G = float(wl.M) ** 3
     Gc = float(wl.M) ** 2 * (wl.M // 2 + 1)
-    alg_bytes = {                                   # algorithmic bytes per launch
+    alg_bytes = {
         "spread": 24.0 * G + 120.0 * wl.N,          # three grids written once + particle data
-        "kspace": 144.0 * Gc,                       # 3 complex grids read, 6 written
+        "kspace": 144.0 * Gc,                       # 3 complex grids read, 6 written (x transforms fused in, no extra traffic)
         "gather": 48.0 * G + 120.0 * wl.N,          # six grids read once + particle data
     }
-    own = {k: stage[k] for k in ("sort", "real", "spread", "kspace", "gather", "epilogue")}
-    dom = max(("spread", "kspace", "gather"), key=lambda k: stage[k])
-    achieved = alg_bytes[dom] / (stage[dom] * 1e-3) / 1e9
-    # dram__bytes_read.sum + dram__bytes_write.sum per launch, from the ncu --set full capture summarised in
-    # profiles/r01g_summary.md (c4 only; other configs have no capture)
-    traffic_c4 = {"spread": 0.0895e9 + 352.0e6, "kspace": 0.4028e9 + 754.1e6, "gather": 1.4570e9 + 21.9e6}
-    traffic = traffic_c4.get(dom) if args.config == "c4" else None
-    # spreading and gather are FP64-issue bound before they are HBM bound: 12 N P^3 DFMA each
     try:
         fp64_peak = pk.measure_fp64_peak()
     except Exception:
         fp64_peak = None
-    sg_flops = 2.0 * 12.0 * wl.N * float(wl.P) ** 3
+    npairs = real_pairs(wl)
+    alg_flops = {
+        "spread": 2.0 * 12.0 * wl.N * float(wl.P) ** 3,      # 12 DFMA per particle and support point
+        "gather": 2.0 * 12.0 * wl.N * float(wl.P) ** 3,
+        "real": 600.0 * npairs,                              # ~600 FP64 instructions per ordered pair
+    }
+    counters = load_counters() if args.config == "c4" else None
+    kname = {"spread": "k_spread", "gather": "k_gather", "kspace": "k_xmid", "real": "k_real"}
+
+    def ncu(kind, key):
+        try:
+            return counters["kernels"][kname[kind]][key]
+        except Exception:
+            return None
+
     per_kernel = {}
-    for k in alg_bytes:
-        gbs = alg_bytes[k] / (stage[k] * 1e-3) / 1e9
-        per_kernel[k] = {"ms": stage[k], "GB/s": gbs, "frac": gbs / peak}
-        if k in ("spread", "gather"):
-            tf = sg_flops / (stage[k] * 1e-3) / 1e12
-            per_kernel[k]["fp64_TFLOP/s"] = tf
-            per_kernel[k]["fp64_frac"] = tf / fp64_peak if fp64_peak else None
-    roofline = {"kernel": dom, "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": traffic, "peak_source": peak_src, "fp64_peak_TFLOP/s": fp64_peak, "all": per_kernel}
+    for k in ("spread", "gather", "kspace", "real"):
+        e = {"ms": stage[k]}
+        if k in alg_bytes:
+            gbs = alg_bytes[k] / (stage[k] * 1e-3) / 1e9
+            e.update({"GB/s": gbs, "hbm_frac_measured_peak": gbs / peak, "hbm_frac_nominal_8TBs": gbs / NOMINAL_HBM})
+            rd, wr = ncu(k, "dram_bytes_read"), ncu(k, "dram_bytes_write")
+            e["traffic"] = (rd + wr) if rd is not None and wr is not None else None
+        if k in alg_flops:
+            tf = alg_flops[k] / (stage[k] * 1e-3) / 1e12
+            e.update({"fp64_TFLOP/s": tf, "fp64_frac": tf / fp64_peak if fp64_peak else None,
+                      "fp64_pipe_busy_pct_ncu": ncu(k, "fp64_pipe_active_pct")})
+        per_kernel[k] = e
+    own = {k: stage[k] for k in ("sort", "real", "spread", "kspace", "gather", "epilogue")}
+    dom = max(("spread", "kspace", "gather", "real"), key=lambda k: stage[k])
+    if dom in ("spread", "gather", "real"):         # FP64-issue bound before HBM bound: report against the FP64 peak
+        achieved = alg_flops[dom] / (stage[dom] * 1e-3) / 1e12
+        roofline = {"kernel": dom, "bound": "alu", "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
+                    "frac": achieved / fp64_peak if fp64_peak else None, "traffic": per_kernel[dom].get("traffic"),
+                    "peak_source": "measured on this run: independent DFMA chains (se_measure_fp64_peak); nominal 148 SM x 64 DFMA/clk x 2 x 1.965 GHz = 37.2"}
+    else:
+        achieved = alg_bytes[dom] / (stage[dom] * 1e-3) / 1e9
+        roofline = {"kernel": dom, "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                    "traffic": per_kernel[dom].get("traffic"), "peak_source": peak_src}
+    roofline.update({"hbm_peak_GB/s": peak, "hbm_peak_source": peak_src, "hbm_nominal_GB/s": NOMINAL_HBM, "fp64_peak_TFLOP/s": fp64_peak,
+                     "counters": "profiles/r02_counters.json" if counters else None, "all": per_kernel})
 
     cpu = None
     if not args.no_cpu_baseline:
+        import oracle as O
         sec, threads = cpu_oracle_seconds(wl)
-        cpu = {"value": 1.0 / sec, "unit": UNIT, "cores": threads, "kind": "oracle",
-               "sample": f"one full {args.config} product (oracle O2 as it stands, gcc -O2 -fopenmp), {sec:.2f} s"}
+        parts = {}
+        for nm, fl in (("real", O.PART_REAL), ("wave", O.PART_WAVE)):
+            t0 = time.perf_counter()
+            O.o2_apply(wl.pos, wl.radii, wl.L, wl.xi, wl.rc, wl.M, wl.P, wl.F, wl.T, wl.S, parts=fl)
+            parts[nm] = time.perf_counter() - t0
+        cpu = {"value": 1.0 / sec, "unit": UNIT, "cores": threads, "kind": "oracle", "stage_seconds": parts,
+               "sample": f"one full {args.config} product (oracle O2 as it stands, gcc -O2 -fopenmp), {sec:.2f} s; real-space part alone "
+                         f"{parts['real']:.2f} s, wave-space part alone {parts['wave']:.2f} s; the oracle's spreading loop and line FFTs are "
+                         "serial, only its gather, k-space and real-space loops use the cores"}
 
     others = {}
     if world == 1 and not args.no_other_configs and not args.no_cpu_baseline:
@@ -344,10 +410,9 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "ns_per_particle": 1e6 * ms_step / wl.N,
-        "config": {"workload": f"{args.config}: N={wl.N}, M={wl.M}, P={wl.P}, phi={wl.phi}, radii={wl.meta['radii']}, "
-                               f"positions={wl.meta['positions']}", "N": wl.N, "M": wl.M, "P": wl.P, "xi": wl.xi, "r_c": wl.rc,
-                   "parallelism": "replicas only" if world > 1 else "single GPU",
-                   "l2": "no flush: per-step working set (grids + spectra) is %.1f GB >> 126 MB L2" % (plan.workspace_bytes() / 1e9)},
+        "ms_per_step_median": ms_median,
+        "config": config_dict(args.config, wl, world),
+        "workspace_GB": plan.workspace_bytes() / 1e9,
         "warm_ms_per_step": warm_ms, "stages_ms": stage, "fft_ms": stage["fft_fwd"] + stage["fft_inv"], "own_kernels_ms": sum(own.values()),
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 14 * 8 * wl.N, "d2h_bytes_per_step": 11 * 8 * wl.N,

@@ -33,7 +33,6 @@ struct SeConst {
 //   [9..11] F  [12..14] T  [15..20] S (xx,xy,xz,yy,yz,zz)
 //   [21] cF = a^2/6  [22] cS = a^2/10  [23] pressure moment s (a9; 0 without)
 //   [24..24+P) gx * (al/pi)^{3/2}   [24+P..24+2P) gy   [24+2P..24+3P) gz     per-axis Gaussians
-//   [24+3P..24+6P)  gx dx, gx dx^2, gx dx^3 with dx_k = d0x + k Delta     x-moment tables (P each)
 #define REC_D0 2
 #define REC_POLY 5
 #define REC_F 9
@@ -42,7 +41,7 @@ struct SeConst {
 #define REC_CF 21
 #define REC_CS 22
 #define REC_SP 23
-__host__ __device__ inline int se_rec_stride(int P) { return (SE_REC_HDR + 6 * P + 1) & ~1; }
+__host__ __device__ inline int se_rec_stride(int P) { return (SE_REC_HDR + 3 * P + 1) & ~1; }
 
 // Gather record (grec_stride doubles, 16-byte aligned), in gather order (tile major, starting plane minor):
 //   [0] int2 (y0w, z0w)  [1] int2 (x0w, orig)  [2] d0y  [3] d0z

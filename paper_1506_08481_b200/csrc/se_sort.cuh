@@ -127,8 +127,8 @@ __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const doubl
                           double *__restrict__ grecs, double4 *__restrict__ rs_pos, double *__restrict__ rs_mom, int *__restrict__ rs_orig,
                           double *__restrict__ recs, int2 *__restrict__ dst_rs)   // dst_rs[i] = (cell-order index, record index)
 {
-    extern __shared__ __align__(16) double sc_rows[];          // [SCATTER_THREADS][rec_stride + 1] then int dst[2][SCATTER_THREADS]
-    const int P = c.P, pitch = c.rec_stride + 1;
+    extern __shared__ __align__(16) double sc_rows[];          // [SCATTER_THREADS][(rec_stride + P) | 1] then int dst[2][SCATTER_THREADS]
+    const int P = c.P, pitch = (c.rec_stride + P) | 1;          // a row: the spreading record, then gx dx (gather record only)
     int *sc_dst = reinterpret_cast<int *>(sc_rows + SCATTER_THREADS * pitch), *sc_dg = sc_dst + SCATTER_THREADS;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     sc_dst[threadIdx.x] = -1;
@@ -157,7 +157,7 @@ __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const doubl
     // spreading / gather records
     const int ds = start_s[key_s[i]] + rank_s[i];
     dst_rs[i] = make_int2(dr, ds);
-    double *r = sc_rows + threadIdx.x * pitch;
+    double *r = sc_rows + threadIdx.x * pitch, *gxd = r + c.rec_stride;
     sc_dst[threadIdx.x] = ds;
     sc_dg[threadIdx.x] = start_g[key_g[i]] + rank_g[i];
     int n0w[3];
@@ -174,14 +174,10 @@ __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const doubl
             const double dk = ((double)(n0 + k) - u) * c.Delta;
             const double e = exp(-al * dk * dk);
             g[k] = d == 0 ? c.gnorm * e : e;
-            if (d == 0) {                                   // x-moment tables gx dx^n, n = 1..3
-                double *xm = r + SE_REC_HDR + 3 * P;
-                const double g1 = g[k] * dk, g2 = g1 * dk;
-                xm[k] = g1; xm[P + k] = g2; xm[2 * P + k] = g2 * dk;
-            }
+            if (d == 0) gxd[k] = g[k] * dk;                 // gx dx of the gather record
         }
     }
-    if (c.rec_stride > SE_REC_HDR + 6 * P) r[SE_REC_HDR + 6 * P] = 0.0;
+    if (c.rec_stride > SE_REC_HDR + 3 * P) r[SE_REC_HDR + 3 * P] = 0.0;
     r[0] = __longlong_as_double(((long long)(unsigned)n0w[2] << 32) | (unsigned)n0w[1]);     // int2 (y0w, z0w)
     r[1] = __longlong_as_double(((long long)(unsigned)i << 32) | (unsigned)n0w[0]);          // int2 (x0w, orig)
     r[REC_D0] = d0[0]; r[REC_D0 + 1] = d0[1]; r[REC_D0 + 2] = d0[2];
@@ -210,7 +206,7 @@ __global__ void k_scatter(SeConst c, const double *__restrict__ pos, const doubl
             if (q < 2) v = src[q];
             else if (q < 4) v = src[REC_D0 + q - 1];
             else if (q < 4 + 2 * PP) { const int ax = (q - 4) / PP, k = (q - 4) - ax * PP; v = k < P ? src[SE_REC_HDR + (ax + 1) * P + k] : 0.0; }
-            else { const int e = q - 4 - 2 * PP; v = src[SE_REC_HDR + ((e & 1) ? 3 * P : 0) + (e >> 1)]; }
+            else { const int e = q - 4 - 2 * PP; v = (e & 1) ? src[c.rec_stride + (e >> 1)] : src[SE_REC_HDR + (e >> 1)]; }
             dg[q] = v;
         }
     }
@@ -240,5 +236,5 @@ __global__ void k_moments(SeConst c, const double *__restrict__ F, const double 
 
 static inline size_t scatter_smem_bytes(int P)
 {
-    return (size_t)SCATTER_THREADS * (se_rec_stride(P) + 1) * 8 + 2 * SCATTER_THREADS * 4;
+    return (size_t)SCATTER_THREADS * ((se_rec_stride(P) + P) | 1) * 8 + 2 * SCATTER_THREADS * 4;
 }

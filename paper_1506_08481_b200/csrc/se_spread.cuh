@@ -9,9 +9,9 @@
 // plane p and covers the column, that particle's contribution to all P slots (statically indexed), then
 // stores slot 0 (plane p is now final), shifts the window and moves on.  For a fixed column the summand is
 // a cubic in dx = x_n - x_j times the x-Gaussian:
-//   H_c = gx(k) [ c0 + dx c1 + dx^2 c2 + dx^3 c3 ]_c      -> 4 FMA per component and grid point,
-// with the (y,z) Gaussian folded into the four coefficients and gx dx^n tabulated per particle (a1).  The sweep is cut into segments along x for
-// parallelism; a segment starts P-1 planes early to pick up the particles whose support reaches into it.
+//   H_c = gx(k) [ c0 + dx c1 + dx^2 c2 + dx^3 c3 ]_c      -> 4 FMA per component and grid point (Horner),
+// with the (y,z) Gaussian folded into the four coefficients and gx tabulated per particle (a1).  The sweep is cut into
+// segments along x for parallelism; a segment starts P-1 planes early to pick up the particles whose support reaches into it.
 #pragma once
 #include "se_sweep.cuh"
 
@@ -52,23 +52,6 @@ __device__ __forceinline__ void spread_hit(const SeConst &c, const double *__res
         c2[1] = gyz * (f1 * Fy + s1 * sg1);
         c2[2] = gyz * (f1 * Fz + s1 * sg2);
         c3[0] = gyz * s1 * Sxx; c3[1] = gyz * s1 * Sxy; c3[2] = gyz * s1 * Sxz;
-#ifdef SPREAD_TABLES
-        // acc[k][a] += sum_n (gx dx^n)(k) c_n[a]: four passes of 3P independent FMAs, accumulated in place
-        const double *__restrict__ X0 = rec + SE_REC_HDR, *__restrict__ X1 = rec + SE_REC_HDR + 3 * P;
-#pragma unroll
-        for (int k = 0; k < P; ++k) {
-            const double x0 = X0[k], x1 = X1[k], x2 = X1[P + k], x3 = X1[2 * P + k];
-#pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                double t = acc[k][a];
-                t = fma(x0, c0[a], t);
-                t = fma(x1, c1[a], t);
-                t = fma(x2, c2[a], t);
-                acc[k][a] = fma(x3, c3[a], t);
-            }
-            if (NC == 4) acc[k][NC - 1] = fma(x0, gyz * rec[REC_SP], acc[k][NC - 1]);
-        }
-#else
         // acc[k][a] += gx(k) ((c3 dx + c2) dx + c1) dx + c0)[a], dx = d0x + k Delta: 3P independent chains of four FMAs,
         // one table value per plane
         const double *__restrict__ X0 = rec + SE_REC_HDR;
@@ -86,7 +69,6 @@ __device__ __forceinline__ void spread_hit(const SeConst &c, const double *__res
             }
             if (NC == 4) acc[k][NC - 1] = fma(gx, gsp, acc[k][NC - 1]);
         }
-#endif
     }
 }
 
