@@ -144,6 +144,19 @@ se_status far_mobility_apply_compressible(se_plan *plan, const double *pos, cons
                                           double *U, double *Omega, double *E, double *s_out,
                                           void *cuda_stream);
 
+/* Self-image Ewald blocks (Sec. 4.2: the block-diagonal approximation of the grand
+ * mobility behind the far-field preconditioner -- "for each particle, the approximation only considers the interactions
+ * with its periodic images", by direct Ewald summation).  Writes, for every particle i, the 11 x 11 matrix that maps
+ * its own (F[3], T[3], S[5]) to its own (U[3], Omega[3], E[5]) when only the particle and its periodic images are there:
+ * one-body terms (Eq. 13-15) - wave-space self terms (Eq. 37) + real-space image sum + wave-space sum of the self pair.
+ *   out    DEVICE, [N][11][11] row-major (row = output component, column = input component, stored 5-component S and E),
+ *          OVERWRITTEN
+ * Depends on the radii, L and eta0 only (not on xi, r_c, M, P: the sums are direct and converged to round-off).
+ * Cost O(N): the lattice sums are done for three reference radii (every entry is a quadratic in a_i^2 besides the one-body
+ * term) and interpolated per particle.  Enqueues two kernels on cuda_stream; no synchronisation.
+ * Errors: SE_ERR_INVALID_ARG for NULL; SE_ERR_ALLOC / SE_ERR_CUDA. */
+se_status se_self_image_blocks(se_plan *plan, double *out, void *cuda_stream);
+
 /* End-to-end convenience: the same product with HOST arrays (pinned or pageable).  Copies the inputs
  * to plan-owned device buffers, runs far_mobility_apply on cuda_stream, copies the outputs back and
  * synchronises the stream before returning. */

@@ -62,6 +62,8 @@ def load_library(build_if_missing: bool = True):
     L.far_mobility_apply.argtypes = [P] * 9
     L.far_mobility_apply_compressible.restype = INT
     L.far_mobility_apply_compressible.argtypes = [P] * 11
+    L.se_self_image_blocks.restype = INT
+    L.se_self_image_blocks.argtypes = [P, P, P]
     L.far_mobility_apply_host.restype = INT
     L.far_mobility_apply_host.argtypes = [P] * 9
     L.se_plan_copy_grids.restype = INT
@@ -179,6 +181,12 @@ class SePlan:
             None if s_in is None else _dptr(s_in, N, "s_in"), _dptr(U, 3 * N, "U"), _dptr(Omega, 3 * N, "Omega"),
             _dptr(E, 5 * N, "E"), None if s_out is None else _dptr(s_out, N, "s_out"), sp)
         self._check(st, "far_mobility_apply_compressible")
+
+    def self_image_blocks(self, out, stream=None):
+        """se_self_image_blocks: ``out`` is a CUDA float64 tensor [N, 11, 11], overwritten."""
+        import torch
+        sp = (torch.cuda.current_stream() if stream is None else stream).cuda_stream
+        self._check(self._lib.se_self_image_blocks(self._h, _dptr(out, 121 * self.N, "out"), sp), "se_self_image_blocks")
 
     def apply_raw(self, pos, F, T, S, U, Omega, E, stream_ptr=0):
         """far_mobility_apply on raw device addresses (ints); used to test NULL handling."""

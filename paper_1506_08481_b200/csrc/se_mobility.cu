@@ -18,6 +18,7 @@
 #include "se_xyfft.cuh"
 #include "se_zfft.cuh"
 #include "se_gather.cuh"
+#include "se_blocks.cuh"
 
 #ifndef M_PI
 #define M_PI 3.14159265358979323846
@@ -33,6 +34,8 @@ struct se_plan {
     char err[256];
     // device buffers
     double *d_radii;
+    double a2min, a2max;           // range of a_i^2 (reference radii of the self-image blocks)
+    double *d_blockW;              // [3][11][11] lattice sums of se_self_image_blocks at the reference radii
     int *d_key_r, *d_rank_r, *d_cnt_r, *d_start_r;
     int *d_key_s, *d_rank_s, *d_cnt_s, *d_start_s;
     int *d_key_g, *d_rank_g, *d_cnt_g, *d_start_g;
@@ -226,7 +229,7 @@ extern "C" const char *se_last_error(const se_plan *plan) { return plan ? plan->
 extern "C" se_status se_plan_destroy(se_plan *p)
 {
     if (!p) return SE_OK;
-    cudaFree(p->d_radii);
+    cudaFree(p->d_radii); cudaFree(p->d_blockW);
     cudaFree(p->d_key_r); cudaFree(p->d_rank_r); cudaFree(p->d_key_s); cudaFree(p->d_rank_s);
     cudaFree(p->d_key_g); cudaFree(p->d_rank_g); cudaFree(p->d_grecs);
     cudaFree(p->d_cnt_all); cudaFree(p->d_start_all); cudaFree(p->d_dst_rs);
@@ -523,7 +526,13 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
         M < 2 || (M & 1) || M > 2048 || P < 2 || P > M || !(eta0 > 0.0))
         return SE_ERR_INVALID_ARG;
     if (P > SE_PMAX) return SE_ERR_UNSUPPORTED;
-    for (int64_t i = 0; i < N; ++i) if (!(radii[i] > 0.0)) return SE_ERR_INVALID_ARG;
+    double a2min = 1e300, a2max = 0.0;
+    for (int64_t i = 0; i < N; ++i) {
+        if (!(radii[i] > 0.0)) return SE_ERR_INVALID_ARG;
+        const double t = radii[i] * radii[i];
+        if (t < a2min) a2min = t;
+        if (t > a2max) a2max = t;
+    }
 
     se_plan *p = (se_plan *)aligned_alloc(64, (sizeof(se_plan) + 63) & ~(size_t)63);     // CUtensorMap members: 64-byte aligned
     if (!p) return SE_ERR_ALLOC;
@@ -532,6 +541,7 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
     SeConst &c = p->c;
     c.N = (int)N; c.M = M; c.P = P; c.L = L; c.xi = xi; c.rc2 = r_c * r_c; c.eta0 = eta0;
     p->m = sqrt(M_PI * P);
+    p->a2min = a2min; p->a2max = a2max;
     derive_constants(p);
     {
         int dev = 0, sms = 0;
@@ -1061,6 +1071,28 @@ extern "C" se_status far_mobility_apply_host(se_plan *p, const double *pos, cons
     CUDA_TRY(p, cudaMemcpyAsync(Omega, dW, 3 * N * B, cudaMemcpyDeviceToHost, s));
     CUDA_TRY(p, cudaMemcpyAsync(E, dE, 5 * N * B, cudaMemcpyDeviceToHost, s));
     CUDA_TRY(p, cudaStreamSynchronize(s));
+    return SE_OK;
+}
+
+extern "C" se_status se_self_image_blocks(se_plan *p, double *out, void *cuda_stream)
+{
+    if (!p) return SE_ERR_INVALID_ARG;
+    if (!out) return fail(p, SE_ERR_INVALID_ARG, "se_self_image_blocks", "null pointer");
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    if (!p->d_blockW) { se_status st = dev_alloc(p, &p->d_blockW, 3 * 121); if (st != SE_OK) return st; }
+    // the sums use their own splitting parameter xi_b = sqrt(pi)/L: real and wave parts converge equally fast
+    SeConst cb = p->c;
+    cb.xi = sqrt(M_PI) / cb.L;
+    cb.q = 2.0 * cb.xi / sqrt(M_PI);
+    cb.x2 = cb.xi * cb.xi; cb.x4 = cb.x2 * cb.x2; cb.x6 = cb.x4 * cb.x2; cb.x8 = cb.x4 * cb.x4; cb.x10 = cb.x8 * cb.x2; cb.x12 = cb.x6 * cb.x6;
+    cb.inv4xi2 = 1.0 / (4.0 * cb.xi * cb.xi);
+    // three distinct reference values of t = a^2 spanning the radii (any three distinct values give the same quadratic)
+    const double t0 = p->a2min, t2 = p->a2max > 1.0001 * p->a2min ? p->a2max : 2.0 * p->a2min, t1 = 0.5 * (t0 + t2);
+    k_block_lattice<<<dim3(11, 3), BLK_THREADS, 0, s>>>(cb, t0, t1, t2, p->d_blockW);
+    const size_t n = (size_t)cb.N * 121;
+    k_block_eval<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(cb, t0, t1, t2, p->d_blockW, p->d_radii, out);
+    p->last_launches = 2;
+    CUDA_TRY(p, cudaGetLastError());
     return SE_OK;
 }
 

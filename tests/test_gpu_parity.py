@@ -481,3 +481,37 @@ def test_cached_positions_many_right_hand_sides(pk, oracle, workloads):
     # a new configuration through the normal entry point drops the cache; so does set_shape
     _check_blocks(r.run(), r.oracle(oracle), TOL)
     assert r.plan.apply_raw(None, *[t_.data_ptr() for t_ in (r.F, r.T, r.S, r.U, r.W, r.E)]) == 1
+
+
+# ------------------------------------------------------------------------------------------------
+# f4: self-image Ewald blocks (Sec. 4.2) against the definition O1 on one-particle systems
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["c1", "c2"])
+def test_self_image_blocks_against_direct_ewald_sum(pk, oracle, workloads, name):
+    """Each particle with its own periodic images only: O1 with N = 1 at the particle's radius (pinned by Hasimoto's
+    constant and xi-independence) gives the 11 x 11 block; the library interpolates three reference radii."""
+    import torch
+    wl = workloads.make_workload(name)
+    radii = wl.radii.copy()
+    radii[: min(5, wl.N)] *= np.array([0.7, 1.3, 1.9, 2.6, 3.3])[: min(5, wl.N)]     # radii between and beyond the species'
+    plan = pk.SePlan(wl.N, wl.L, radii, wl.xi, wl.rc, wl.M, wl.P, wl.eta0)
+    out = torch.full((wl.N, 11, 11), float("nan"), device="cuda:0", dtype=torch.float64)
+    plan.self_image_blocks(out)
+    torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    xi = 6.0 / wl.L
+    nimg, kmax = 4, int(np.ceil(6.6 * 2 * xi * wl.L / (2 * np.pi)))
+    checked = {}
+    for i in list(range(min(5, wl.N))) + [wl.N // 2, wl.N - 1]:
+        a = float(radii[i])
+        if a not in checked:
+            A = oracle.o1_matrix(np.array([[0.3, 0.1, 0.7]]) * wl.L, np.array([a]), wl.L, xi, eta0=wl.eta0, nimg=nimg, kmax=kmax)
+            checked[a] = A[:11, :11]
+        ref = checked[a]
+        assert _rel(got[i], ref) <= TOL, (i, a, _rel(got[i], ref))
+        assert np.abs(got[i] - got[i].T).max() <= 1e-13 * np.abs(ref).max()          # symmetric (reciprocity)
+    # cubic lattice: the block is diagonal, and U-F, Omega-T are isotropic
+    off = got[0] - np.diag(np.diag(got[0]))
+    assert np.abs(off).max() <= 1e-12 * np.abs(got[0]).max()
+    assert np.ptp(np.diag(got[0])[:3]) <= 1e-13 and np.ptp(np.diag(got[0])[3:6]) <= 1e-13
+    plan.destroy()
