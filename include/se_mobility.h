@@ -129,6 +129,22 @@ se_status se_plan_set_positions(se_plan *plan, const double *pos, void *cuda_str
 se_status far_mobility_apply(se_plan *plan, const double *pos, const double *F, const double *T,
                              const double *S, double *U, double *Omega, double *E, void *cuda_stream);
 
+/* Several right-hand sides on ONE configuration: the iterative solver applies the operator tens to
+ * hundreds of times per configuration with only (F,T,S) changing (nested GMRES; the paper prebuilds
+ * its real-space matrix per time step for that reason, L332), and block methods apply it to several vectors at once.
+ *   pos    [N][3] DEVICE or NULL (= the configuration of se_plan_set_positions); when given, a1 runs once and the
+ *          configuration stays cached afterwards, exactly as after se_plan_set_positions
+ *   nrhs   number of right-hand sides, >= 1
+ *   F, T   [nrhs][N][3] DEVICE;  S  [nrhs][N][5] DEVICE            (right-hand side r starts at offset r N 3, r N 5)
+ *   U, Omega [nrhs][N][3], E [nrhs][N][5] DEVICE outputs, OVERWRITTEN
+ * Results equal nrhs calls of far_mobility_apply (same arithmetic per right-hand side).  What is shared: the sorts and
+ * per-particle tables (once), and in the real-space sum (a2) the neighbour search and every pair's erfc/exp and radial
+ * functions, evaluated once per pair for up to four right-hand sides per launch.  The wave-space pipeline (a3-a7) runs per
+ * right-hand side.  Flags as for far_mobility_apply.  The first call with a larger nrhs allocates 2 nrhs N 12 doubles
+ * (synchronising the stream).  Errors: SE_ERR_INVALID_ARG, SE_ERR_ALLOC, SE_ERR_CUDA, SE_ERR_CUFFT. */
+se_status far_mobility_apply_batch(se_plan *plan, const double *pos, int nrhs, const double *F, const double *T,
+                                   const double *S, double *U, double *Omega, double *E, void *cuda_stream);
+
 /* Compressible-solvent extension (Sec. 2.3, Eq. 24-34).  As far_mobility_apply with
  *   s_in   [N] DEVICE pressure moments s_j (paper's Eq. 25-26 sign: s > 0 is a fluid source), or NULL for none.
  *          Adds the source field grad psi (Eq. 26, split after Eq. 33-34) to U and E: one more spread grid

@@ -60,6 +60,8 @@ def load_library(build_if_missing: bool = True):
     L.se_plan_set_flags.argtypes = [P, U]
     L.far_mobility_apply.restype = INT
     L.far_mobility_apply.argtypes = [P] * 9
+    L.far_mobility_apply_batch.restype = INT
+    L.far_mobility_apply_batch.argtypes = [P, P, INT, P, P, P, P, P, P, P]
     L.far_mobility_apply_compressible.restype = INT
     L.far_mobility_apply_compressible.argtypes = [P] * 11
     L.se_self_image_blocks.restype = INT
@@ -170,6 +172,16 @@ class SePlan:
                                           _dptr(S, 5 * N, "S"), _dptr(U, 3 * N, "U"), _dptr(Omega, 3 * N, "Omega"),
                                           _dptr(E, 5 * N, "E"), sp)
         self._check(st, "far_mobility_apply")
+
+    def apply_batch(self, pos, F, T, S, U, Omega, E, stream=None):
+        """far_mobility_apply_batch: F, T, U, Omega are CUDA float64 [nrhs, N, 3], S and E [nrhs, N, 5]; pos [N, 3] or None."""
+        import torch
+        N, nrhs = self.N, int(F.shape[0])
+        sp = (torch.cuda.current_stream() if stream is None else stream).cuda_stream
+        st = self._lib.far_mobility_apply_batch(
+            self._h, None if pos is None else _dptr(pos, 3 * N, "pos"), nrhs, _dptr(F, 3 * N * nrhs, "F"), _dptr(T, 3 * N * nrhs, "T"),
+            _dptr(S, 5 * N * nrhs, "S"), _dptr(U, 3 * N * nrhs, "U"), _dptr(Omega, 3 * N * nrhs, "Omega"), _dptr(E, 5 * N * nrhs, "E"), sp)
+        self._check(st, "far_mobility_apply_batch")
 
     def apply_compressible(self, pos, F, T, S, s_in, U, Omega, E, s_out, stream=None):
         """far_mobility_apply_compressible; ``s_in`` / ``s_out`` are CUDA float64 tensors of N entries or None."""

@@ -65,6 +65,9 @@ struct se_plan {
     double2 *d_Hk;                 // [3][M][M][M/2+1]
     double2 *d_Gk;                 // [6][M][M][M/2+1]
     double *d_out_real;            // [N][12] real-space part in caller order (slot 11: pressure, a9)
+    const double *ext_out_real;    // far_mobility_apply_batch: real-space part already computed (k_real is skipped)
+    double *d_mom_b, *d_out_real_b; // batch: moments in cell order and real-space results, [nrhs][N][12]
+    int batch_cap;                 // right-hand sides the batch buffers hold
     // compressible extension (a9): allocated by the first apply that passes s_in or s_out
     double *d_real_p;              // [M][MYp][MZp]: scalar spread grid Hs (first M^3 doubles), then the returned pressure grid p~ (padded)
     double2 *d_Hk_s, *d_Gk_p;      // their spectra
@@ -237,7 +240,7 @@ extern "C" se_status se_plan_destroy(se_plan *p)
     cudaFree(p->d_bsum);
     cudaFree(p->d_rs_pos); cudaFree(p->d_rs_mom); cudaFree(p->d_rs_orig); cudaFree(p->d_recs);
     cudaFree(p->d_real); cudaFree(p->d_Hk); cudaFree(p->d_Gk);
-    cudaFree(p->d_out_real); cudaFree(p->d_moments); cudaFree(p->d_io);
+    cudaFree(p->d_out_real); cudaFree(p->d_moments); cudaFree(p->d_io); cudaFree(p->d_mom_b); cudaFree(p->d_out_real_b);
     if (p->have_comp) {
         cudaFree(p->d_real_p); cudaFree(p->d_Hk_s); cudaFree(p->d_Gk_p); cudaFree(p->d_pmom);
         if (p->have_fft1) { cufftDestroy(p->fft_fwd1); cufftDestroy(p->fft_inv1); }
@@ -845,7 +848,7 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     const SeConst &c = p->c;
     const unsigned fl = p->flags;
     const bool timing = (fl & SE_TIMING) != 0;
-    const bool do_real = !(fl & SE_SKIP_REAL), do_wave = !(fl & SE_SKIP_WAVE);
+    const bool do_real = !(fl & SE_SKIP_REAL) && !p->ext_out_real, do_wave = !(fl & SE_SKIP_WAVE);
     const int stop = p->debug_stop;
     auto on = [&](int stage) { return do_wave && (stop < 0 || stage <= stop); };
     p->last_launches = 0;
@@ -875,8 +878,8 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     auto launch_real = [&](cudaStream_t sr) {
         unsigned nb = (unsigned)(c.ncr > 1 ? p->ncell_r : (c.N + 31) / 32);
         if (sr != s && c.ncr > 1 && p->real_side_ctas > 0 && nb > (unsigned)p->real_side_ctas) nb = (unsigned)p->real_side_ctas;
-        if (comp) k_real<true><<<nb, REAL_WARPS * 32, 0, sr>>>(c, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig, p->d_start_r, p->d_out_real);
-        else k_real<false><<<nb, REAL_WARPS * 32, 0, sr>>>(c, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig, p->d_start_r, p->d_out_real);
+        if (comp) k_real<true, 1><<<nb, REAL_WARPS * 32, 0, sr>>>(c, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig, p->d_start_r, p->d_out_real, 0);
+        else k_real<false, 1><<<nb, REAL_WARPS * 32, 0, sr>>>(c, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig, p->d_start_r, p->d_out_real, 0);
         p->last_launches += 1;
     };
     if (do_real && !fork) {
@@ -1029,7 +1032,7 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     MARK();
     // ---- a8: epilogue ----
     if (fork) CUDA_TRY(p, cudaStreamWaitEvent(s, p->ev_join, 0));
-    k_epilogue<<<nbN, TB, 0, s>>>(c, fl | (wave_done ? 0u : SE_SKIP_WAVE), p->d_radii, F, T, S, p->d_out_real, p->d_moments,
+    k_epilogue<<<nbN, TB, 0, s>>>(c, fl | (wave_done ? 0u : SE_SKIP_WAVE), p->d_radii, F, T, S, p->ext_out_real ? p->ext_out_real : p->d_out_real, p->d_moments,
                                   comp_out && wave_done ? p->d_pmom : nullptr, U, Omega, E, s_out);
     p->last_launches += 1;
     CUDA_TRY(p, cudaGetLastError());
@@ -1050,6 +1053,61 @@ extern "C" se_status far_mobility_apply_compressible(se_plan *p, const double *p
                                                      double *E, double *s_out, void *cuda_stream)
 {
     return apply_impl(p, pos, F, T, S, s_in, U, Omega, E, s_out, cuda_stream, "far_mobility_apply_compressible");
+}
+
+// Several right-hand sides on one configuration: a1 once; the real-space sum for up to four right-hand
+// sides per launch, each pair's radial functions evaluated once (k_real<., NR>); the wave-space pipeline per right-hand side.
+extern "C" se_status far_mobility_apply_batch(se_plan *p, const double *pos, int nrhs, const double *F, const double *T,
+                                              const double *S, double *U, double *Omega, double *E, void *cuda_stream)
+{
+    if (!p) return SE_ERR_INVALID_ARG;
+    if (nrhs < 1 || !F || !T || !S || !U || !Omega || !E) return fail(p, SE_ERR_INVALID_ARG, "far_mobility_apply_batch", "null pointer or nrhs < 1");
+    if (!pos && !p->have_positions) return fail(p, SE_ERR_INVALID_ARG, "far_mobility_apply_batch", "pos is NULL and no positions were set");
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const SeConst &c = p->c;
+    const size_t N = (size_t)c.N, rs = 12 * N;
+    if (nrhs > p->batch_cap) {
+        CUDA_TRY(p, cudaStreamSynchronize(s));                         // an earlier batch may still use the old buffers
+        cudaFree(p->d_mom_b); cudaFree(p->d_out_real_b);
+        p->d_mom_b = nullptr; p->d_out_real_b = nullptr; p->batch_cap = 0;
+        se_status st = dev_alloc(p, &p->d_mom_b, (size_t)nrhs * rs);
+        if (st == SE_OK) st = dev_alloc(p, &p->d_out_real_b, (size_t)nrhs * rs);
+        if (st != SE_OK) return st;
+        p->batch_cap = nrhs;
+    }
+    int launches = 0;
+    if (pos) {
+        const se_status st = se_plan_set_positions(p, pos, cuda_stream);
+        if (st != SE_OK) return st;
+        launches += p->last_launches;
+    }
+    const bool do_real = !(p->flags & SE_SKIP_REAL);
+    const int TB = 128, nbN = (c.N + TB - 1) / TB;
+    if (do_real) {
+        for (int r = 0; r < nrhs; ++r)
+            k_moments<<<nbN, TB, 0, s>>>(c, F + 3 * N * r, T + 3 * N * r, S + 5 * N * r, nullptr, p->d_dst_rs, p->d_mom_b + rs * r, nullptr);
+        launches += nrhs;
+        const unsigned nb = (unsigned)(c.ncr > 1 ? p->ncell_r : (c.N + 31) / 32);
+        for (int r = 0; r < nrhs;) {
+            const double *m = p->d_mom_b + rs * r;
+            double *o = p->d_out_real_b + rs * r;
+            if (nrhs - r >= 4) { k_real<false, 4><<<nb, REAL_WARPS * 32, 0, s>>>(c, p->d_rs_pos, m, p->d_rs_orig, p->d_start_r, o, rs); r += 4; }
+            else if (nrhs - r >= 2) { k_real<false, 2><<<nb, REAL_WARPS * 32, 0, s>>>(c, p->d_rs_pos, m, p->d_rs_orig, p->d_start_r, o, rs); r += 2; }
+            else { k_real<false, 1><<<nb, REAL_WARPS * 32, 0, s>>>(c, p->d_rs_pos, m, p->d_rs_orig, p->d_start_r, o, rs); r += 1; }
+            launches += 1;
+        }
+        CUDA_TRY(p, cudaGetLastError());
+    }
+    se_status st = SE_OK;
+    for (int r = 0; r < nrhs && st == SE_OK; ++r) {
+        p->ext_out_real = do_real ? p->d_out_real_b + rs * r : nullptr;
+        st = apply_impl(p, nullptr, F + 3 * N * r, T + 3 * N * r, S + 5 * N * r, nullptr, U + 3 * N * r, Omega + 3 * N * r, E + 5 * N * r,
+                        nullptr, cuda_stream, "far_mobility_apply_batch");
+        launches += p->last_launches;
+    }
+    p->ext_out_real = nullptr;
+    p->last_launches = launches;
+    return st;
 }
 
 extern "C" se_status far_mobility_apply_host(se_plan *p, const double *pos, const double *F, const double *T,

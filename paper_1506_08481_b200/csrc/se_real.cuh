@@ -28,11 +28,17 @@
 #define REAL_WARPS 4
 #define REAL_QCAP 64
 
-// acc[0..2] U, [3..5] Omega, [6..10] E (xx,xy,xz,yy,yz), still to be multiplied by k0; acc[11] pressure p (COMP).
+// The radial part of a pair: everything that does not depend on the moments.  Evaluated once per pair and then applied
+// to one or several right-hand sides (far_mobility_apply_batch).
+template <bool COMP> struct PairS {
+    double uf_a, uf_b, ut, us_a, us_b;          // U:  uf_a F + (uf_b x.F + us_b x.S.x) x + ut x^T + us_a S.x
+    double of, ot_a, ot_b, os;                  // Om: of x^F + ot_a T + ot_b (x.T) x + os x^(S.x)
+    double a1, a2, a3, a4, ef2, ef3, es3, es4;  // E:  w = a1 F + a2 x^T + a3 S.x; beta = es4 xSx - ef3 xF; kappa = es3 xSx - ef2 xF
+    double cu, ce1, ce2, ctr, pS, pF;           // a9 (COMP): U <- s, E <- s, p <- S, p <- F
+};
+
 template <bool COMP>
-__device__ __forceinline__ void pair_real(const SeConst &c, double x, double y, double z, double r2,
-                                          double cFi, double cSi, double aj, const double *__restrict__ mj,
-                                          double acc[12])
+__device__ __forceinline__ PairS<COMP> pair_scalars(const SeConst &c, double r2, double cFi, double cSi, double aj)
 {
     const double cFj = aj * aj * (1.0 / 6.0), cSj = aj * aj * 0.1;
     const double ir = rsqrt(r2), r = r2 * ir, ir2 = ir * ir;      // one reciprocal square root instead of a root and a division
@@ -61,6 +67,51 @@ __device__ __forceinline__ void pair_real(const SeConst &c, double x, double y, 
     const double D1 = qg * (360.0 * c.x6 + (-256.0 * c.x8 + 32.0 * c.x10 * r2) * r2);
     const double D2 = qg * (-1232.0 * c.x8 + (640.0 * c.x10 - 64.0 * c.x12 * r2) * r2);
 
+    PairS<COMP> o;
+    double s, p;
+    // ---- U ----
+    s = cFi + cFj; p = cFi * cFj;
+    o.uf_a = (B0 + s * C0 + p * D0) - (P1 + s * B1 + p * C1);
+    o.uf_b = -(P2 + s * B2 + p * C2);
+    o.ut = 0.5 * (B1 + cFi * C1);
+    s = cFi + cSj; p = cFi * cSj;
+    const double us_Ps2 = P2 + s * B2 + p * C2;
+    o.us_a = -((B1 + s * C1 + p * D1) - 2.0 * us_Ps2);
+    o.us_b = P3 + s * B3 + p * C3;
+    // ---- Omega ----
+    o.of = 0.5 * (B1 + cFj * C1);
+    o.ot_a = 0.25 * (B1 - C0);
+    o.ot_b = 0.25 * B2;
+    o.os = -0.5 * (B2 + cSj * C2);
+    // ---- E ----
+    s = cSi + cFj; p = cSi * cFj;
+    o.ef2 = P2 + s * B2 + p * C2;
+    o.ef3 = P3 + s * B3 + p * C3;
+    o.a1 = 0.5 * (B1 + s * C1 + p * D1) - o.ef2;
+    o.a2 = 0.25 * (B2 + cSi * C2);
+    s = cSi + cSj; p = cSi * cSj;
+    const double es_Ps2 = P2 + s * B2 + p * C2;
+    o.es3 = P3 + s * B3 + p * C3;
+    o.es4 = P4 + s * B4 + p * C4;
+    o.a3 = -(0.5 * (B2 + s * C2 + p * D2) - 2.0 * o.es3);
+    o.a4 = -((B1 + s * C1 + p * D1) - 2.0 * es_Ps2);
+    if (COMP) {
+        const double L1c = -4.0 * c.x4 * qg, L2c = 8.0 * c.x6 * qg;          // (lap chi)_n, n = 1, 2
+        o.cu = -0.5 * (P2 + cFi * L1c);
+        o.ce1 = -0.5 * (P2 + cSi * L1c);
+        o.ce2 = -0.5 * (P3 + cSi * L2c);
+        o.ctr = (3.0 * o.ce1 + o.ce2 * r2) * (1.0 / 3.0);
+        o.pS = 0.07957747154594767 * (P3 + cSj * L2c);                       // 1/(4 pi)
+        o.pF = 0.07957747154594767 * (P2 + cFj * L1c);
+    }
+    return o;
+}
+
+// acc[0..2] U, [3..5] Omega, [6..10] E (xx,xy,xz,yy,yz), still to be multiplied by k0; acc[11] pressure p (COMP).
+template <bool COMP>
+__device__ __forceinline__ void pair_apply(const PairS<COMP> &o, double x, double y, double z, double r2,
+                                           const double *__restrict__ mj, double acc[12])
+{
     const double Fx = mj[0], Fy = mj[1], Fz = mj[2], Tx = mj[3], Ty = mj[4], Tz = mj[5];
     const double Sxx = mj[6], Sxy = mj[7], Sxz = mj[8], Syy = mj[9], Syz = mj[10], Szz = -(Sxx + Syy);
     const double xF = x * Fx + y * Fy + z * Fz, xT = x * Tx + y * Ty + z * Tz;
@@ -69,60 +120,44 @@ __device__ __forceinline__ void pair_real(const SeConst &c, double x, double y, 
     const double cT0 = y * Tz - z * Ty, cT1 = z * Tx - x * Tz, cT2 = x * Ty - y * Tx;       // x ^ T
     const double cF0 = y * Fz - z * Fy, cF1 = z * Fx - x * Fz, cF2 = x * Fy - y * Fx;       // x ^ F
     const double cS0 = y * Sx2 - z * Sx1, cS1 = z * Sx0 - x * Sx2, cS2 = x * Sx1 - y * Sx0; // x ^ (S.x)
-
-    double s, p;
-    // ---- U ----
-    s = cFi + cFj; p = cFi * cFj;
-    const double uf_a = (B0 + s * C0 + p * D0) - (P1 + s * B1 + p * C1);
-    const double uf_b = -(P2 + s * B2 + p * C2) * xF;
-    const double ut = 0.5 * (B1 + cFi * C1);
-    s = cFi + cSj; p = cFi * cSj;
-    const double us_Ps2 = P2 + s * B2 + p * C2;
-    const double us_a = -((B1 + s * C1 + p * D1) - 2.0 * us_Ps2);
-    const double us_b = (P3 + s * B3 + p * C3) * xSx;
-    const double ux = uf_b + us_b;
-    acc[0] += uf_a * Fx + ux * x + ut * cT0 + us_a * Sx0;
-    acc[1] += uf_a * Fy + ux * y + ut * cT1 + us_a * Sx1;
-    acc[2] += uf_a * Fz + ux * z + ut * cT2 + us_a * Sx2;
-    // ---- Omega ----
-    const double of = 0.5 * (B1 + cFj * C1);
-    const double ot_a = 0.25 * (B1 - C0), ot_b = 0.25 * B2 * xT;
-    const double os = -0.5 * (B2 + cSj * C2);
-    acc[3] += of * cF0 + ot_a * Tx + ot_b * x + os * cS0;
-    acc[4] += of * cF1 + ot_a * Ty + ot_b * y + os * cS1;
-    acc[5] += of * cF2 + ot_a * Tz + ot_b * z + os * cS2;
-    // ---- E ----
-    s = cSi + cFj; p = cSi * cFj;
-    const double ef_Ps2 = P2 + s * B2 + p * C2, ef_Ps3 = P3 + s * B3 + p * C3;
-    const double a1 = 0.5 * (B1 + s * C1 + p * D1) - ef_Ps2;
-    const double a2 = 0.25 * (B2 + cSi * C2);
-    s = cSi + cSj; p = cSi * cSj;
-    const double es_Ps2 = P2 + s * B2 + p * C2, es_Ps3 = P3 + s * B3 + p * C3, es_Ps4 = P4 + s * B4 + p * C4;
-    const double a3 = -(0.5 * (B2 + s * C2 + p * D2) - 2.0 * es_Ps3);
-    const double a4 = -((B1 + s * C1 + p * D1) - 2.0 * es_Ps2);
-    const double beta = es_Ps4 * xSx - ef_Ps3 * xF;
-    const double kappa = es_Ps3 * xSx - ef_Ps2 * xF;
-    const double w0 = a1 * Fx + a2 * cT0 + a3 * Sx0, w1 = a1 * Fy + a2 * cT1 + a3 * Sx1, w2 = a1 * Fz + a2 * cT2 + a3 * Sx2;
-    acc[6] += 2.0 * x * w0 + a4 * Sxx + beta * x * x + kappa;
-    acc[7] += x * w1 + y * w0 + a4 * Sxy + beta * x * y;
-    acc[8] += x * w2 + z * w0 + a4 * Sxz + beta * x * z;
-    acc[9] += 2.0 * y * w1 + a4 * Syy + beta * y * y + kappa;
-    acc[10] += y * w2 + z * w1 + a4 * Syz + beta * y * z;
+    const double ux = o.uf_b * xF + o.us_b * xSx;
+    acc[0] += o.uf_a * Fx + ux * x + o.ut * cT0 + o.us_a * Sx0;
+    acc[1] += o.uf_a * Fy + ux * y + o.ut * cT1 + o.us_a * Sx1;
+    acc[2] += o.uf_a * Fz + ux * z + o.ut * cT2 + o.us_a * Sx2;
+    const double otb = o.ot_b * xT;
+    acc[3] += o.of * cF0 + o.ot_a * Tx + otb * x + o.os * cS0;
+    acc[4] += o.of * cF1 + o.ot_a * Ty + otb * y + o.os * cS1;
+    acc[5] += o.of * cF2 + o.ot_a * Tz + otb * z + o.os * cS2;
+    const double beta = o.es4 * xSx - o.ef3 * xF;
+    const double kappa = o.es3 * xSx - o.ef2 * xF;
+    const double w0 = o.a1 * Fx + o.a2 * cT0 + o.a3 * Sx0, w1 = o.a1 * Fy + o.a2 * cT1 + o.a3 * Sx1, w2 = o.a1 * Fz + o.a2 * cT2 + o.a3 * Sx2;
+    acc[6] += 2.0 * x * w0 + o.a4 * Sxx + beta * x * x + kappa;
+    acc[7] += x * w1 + y * w0 + o.a4 * Sxy + beta * x * y;
+    acc[8] += x * w2 + z * w0 + o.a4 * Sxz + beta * x * z;
+    acc[9] += 2.0 * y * w1 + o.a4 * Syy + beta * y * y + kappa;
+    acc[10] += y * w2 + z * w1 + o.a4 * Syz + beta * y * z;
     if (COMP) {
         const double sj = mj[11];
-        const double L0c = 2.0 * c.x2 * qg, L1c = -4.0 * c.x4 * qg, L2c = 8.0 * c.x6 * qg;   // (lap chi)_n
-        const double us = -0.5 * (P2 + cFi * L1c) * sj;
+        const double us = o.cu * sj;
         acc[0] += us * x; acc[1] += us * y; acc[2] += us * z;
-        const double e1 = -0.5 * (P2 + cSi * L1c) * sj, e2 = -0.5 * (P3 + cSi * L2c) * sj;
-        const double tr3 = (3.0 * e1 + e2 * r2) * (1.0 / 3.0);
+        const double e1 = o.ce1 * sj, e2 = o.ce2 * sj, tr3 = o.ctr * sj;
         acc[6] += e2 * x * x + e1 - tr3;
         acc[7] += e2 * x * y;
         acc[8] += e2 * x * z;
         acc[9] += e2 * y * y + e1 - tr3;
         acc[10] += e2 * y * z;
-        acc[11] += 0.07957747154594767 * ((P3 + cSj * L2c) * xSx - (P2 + cFj * L1c) * xF);   // 1/(4 pi)
-        (void)L0c;
+        acc[11] += o.pS * xSx - o.pF * xF;
+        (void)r2;
     }
+}
+
+template <bool COMP>
+__device__ __forceinline__ void pair_real(const SeConst &c, double x, double y, double z, double r2,
+                                          double cFi, double cSi, double aj, const double *__restrict__ mj,
+                                          double acc[12])
+{
+    const PairS<COMP> o = pair_scalars<COMP>(c, r2, cFi, cSi, aj);
+    pair_apply<COMP>(o, x, y, z, r2, mj, acc);
 }
 
 // One CTA per real-space cell (or, when the box holds fewer than 3 cells per axis, per slice of all
@@ -133,10 +168,13 @@ __device__ __forceinline__ void pair_real(const SeConst &c, double x, double y, 
 // Minimum image as in the oracle, x = d - L rint(d/L), with d/L formed as d * (1/L).
 #define REAL_STAGE 1024
 
-template <bool COMP>
+// NR right-hand sides at once (far_mobility_apply_batch): moments rs_mom[r][N][12], results out_real[r][N][12],
+// r < NR, `rhs_stride` doubles apart; the radial part of a pair is evaluated once and applied NR times.
+template <bool COMP, int NR>
 __global__ void __launch_bounds__(REAL_WARPS * 32) k_real(SeConst c, const double4 *__restrict__ rs_pos,
                                                           const double *__restrict__ rs_mom, const int *__restrict__ rs_orig,
-                                                          const int *__restrict__ start_r, double *__restrict__ out_real)
+                                                          const int *__restrict__ start_r, double *__restrict__ out_real,
+                                                          size_t rhs_stride)
 {
     __shared__ double4 cand[REAL_STAGE];               // (x, y, z, a) of staged candidates
     __shared__ int cand_j[REAL_STAGE];                 // their index in cell order
@@ -204,9 +242,17 @@ __global__ void __launch_bounds__(REAL_WARPS * 32) k_real(SeConst c, const doubl
             const double4 pi = rs_pos[i];
             const double cFi = pi.w * pi.w * (1.0 / 6.0), cSi = pi.w * pi.w * 0.1;
             constexpr int NA = COMP ? 12 : 11;
-            double acc[12];
+            double acc[NR][12];
 #pragma unroll
-            for (int k = 0; k < 12; ++k) acc[k] = 0.0;
+            for (int r = 0; r < NR; ++r)
+#pragma unroll
+                for (int k = 0; k < 12; ++k) acc[r][k] = 0.0;
+            auto pair = [&](const double4 &d, int jj) {
+                const double r2 = d.x * d.x + d.y * d.y + d.z * d.z;
+                const PairS<COMP> o = pair_scalars<COMP>(c, r2, cFi, cSi, d.w);
+#pragma unroll
+                for (int r = 0; r < NR; ++r) pair_apply<COMP>(o, d.x, d.y, d.z, r2, rs_mom + r * rhs_stride + 12 * (size_t)jj, acc[r]);
+            };
             int qn = 0;
             for (int qb = 0; qb < nst; qb += 32) {
                 const int q = qb + lane;
@@ -231,34 +277,33 @@ __global__ void __launch_bounds__(REAL_WARPS * 32) k_real(SeConst c, const doubl
                 qn += __popc(mask);
                 __syncwarp();
                 if (qn >= 32) {
-                    const double4 d = qd[wl][qn - 32 + lane];
-                    const int jj = qj[wl][qn - 32 + lane];
-                    pair_real<COMP>(c, d.x, d.y, d.z, d.x * d.x + d.y * d.y + d.z * d.z, cFi, cSi, d.w, rs_mom + 12 * (size_t)jj, acc);
+                    pair(qd[wl][qn - 32 + lane], qj[wl][qn - 32 + lane]);
                     qn -= 32;
                     __syncwarp();
                 }
             }
-            if (lane < qn) {
-                const double4 d = qd[wl][lane];
-                pair_real<COMP>(c, d.x, d.y, d.z, d.x * d.x + d.y * d.y + d.z * d.z, cFi, cSi, d.w, rs_mom + 12 * (size_t)qj[wl][lane], acc);
-            }
+            if (lane < qn) pair(qd[wl][lane], qj[wl][lane]);
             __syncwarp();
+            const int io = rs_orig[i];
 #pragma unroll
-            for (int k = 0; k < NA; ++k) {
-                double v = acc[k];
+            for (int r = 0; r < NR; ++r) {
 #pragma unroll
-                for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-                acc[k] = v;
-            }
-            if (lane == 0) {
-                double *o = out_real + 12 * (size_t)rs_orig[i];
-                if (COMP) acc[11] *= 1.0 / c.k0;                  // p carries its own prefactor
-                if (base == 0) {
+                for (int k = 0; k < NA; ++k) {
+                    double v = acc[r][k];
 #pragma unroll
-                    for (int k = 0; k < NA; ++k) o[k] = c.k0 * acc[k];
-                } else {
+                    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                    acc[r][k] = v;
+                }
+                if (lane == 0) {
+                    double *o = out_real + r * rhs_stride + 12 * (size_t)io;
+                    if (COMP) acc[r][11] *= 1.0 / c.k0;               // p carries its own prefactor
+                    if (base == 0) {
 #pragma unroll
-                    for (int k = 0; k < NA; ++k) o[k] += c.k0 * acc[k];
+                        for (int k = 0; k < NA; ++k) o[k] = c.k0 * acc[r][k];
+                    } else {
+#pragma unroll
+                        for (int k = 0; k < NA; ++k) o[k] += c.k0 * acc[r][k];
+                    }
                 }
             }
         }

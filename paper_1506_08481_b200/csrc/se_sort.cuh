@@ -223,11 +223,13 @@ __global__ void k_moments(SeConst c, const double *__restrict__ F, const double 
     const size_t i3 = 3 * (size_t)i, i5 = 5 * (size_t)i;
     const int2 d = dst_rs[i];
     const double sp = s_in ? s_in[i] : 0.0;
-    double *m = rs_mom + 12 * (size_t)d.x, *r = recs + (size_t)d.y * c.rec_stride;
+    double *m = rs_mom + 12 * (size_t)d.x;
     const double f0 = F[i3], f1 = F[i3 + 1], f2 = F[i3 + 2], t0 = T[i3], t1 = T[i3 + 1], t2 = T[i3 + 2];
     const double s0 = S[i5], s1 = S[i5 + 1], s2 = S[i5 + 2], s3 = S[i5 + 3], s4 = S[i5 + 4];
     m[0] = f0; m[1] = f1; m[2] = f2; m[3] = t0; m[4] = t1; m[5] = t2;
     m[6] = s0; m[7] = s1; m[8] = s2; m[9] = s3; m[10] = s4; m[11] = sp;
+    if (!recs) return;                                  // batch: the real-space copy only
+    double *r = recs + (size_t)d.y * c.rec_stride;
     r[REC_F] = f0; r[REC_F + 1] = f1; r[REC_F + 2] = f2;
     r[REC_T] = t0; r[REC_T + 1] = t1; r[REC_T + 2] = t2;
     r[REC_S] = s0; r[REC_S + 1] = s1; r[REC_S + 2] = s2; r[REC_S + 3] = s3; r[REC_S + 4] = s4; r[REC_S + 5] = -(s0 + s3);

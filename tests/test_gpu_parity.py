@@ -515,3 +515,37 @@ def test_self_image_blocks_against_direct_ewald_sum(pk, oracle, workloads, name)
     assert np.abs(off).max() <= 1e-12 * np.abs(got[0]).max()
     assert np.ptp(np.diag(got[0])[:3]) <= 1e-13 and np.ptp(np.diag(got[0])[3:6]) <= 1e-13
     plan.destroy()
+
+
+# ------------------------------------------------------------------------------------------------
+# f1: several right-hand sides on one configuration (far_mobility_apply_batch)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,nrhs", [("c2", 7), ("c1", 3), ("c4", 4)])
+def test_batch_of_right_hand_sides(pk, oracle, workloads, name, nrhs):
+    """Per right-hand side parity with O2 (7 = one launch of four, one of two, one of one in the real-space sum);
+    the single-product entry point still works on the cached configuration afterwards."""
+    import torch
+    wl = workloads.make_workload(name)
+    r = Runner(pk, wl)
+    rng = np.random.default_rng([150608481, 77])
+    Fb, Tb, Sb = rng.standard_normal((nrhs, wl.N, 3)), rng.standard_normal((nrhs, wl.N, 3)), rng.standard_normal((nrhs, wl.N, 5))
+    Fb[0], Tb[0], Sb[0] = wl.F, wl.T, wl.S
+    dev = r.pos.device
+    t = lambda a: torch.tensor(a, device=dev, dtype=torch.float64)
+    U = torch.full((nrhs, wl.N, 3), float("nan"), device=dev, dtype=torch.float64)
+    W, E = torch.full_like(U, float("nan")), torch.full((nrhs, wl.N, 5), float("nan"), device=dev, dtype=torch.float64)
+    r.plan.apply_batch(r.pos, t(Fb), t(Tb), t(Sb), U, W, E)
+    torch.cuda.synchronize()
+    for k in range(nrhs if name != "c4" else 2):
+        ref = oracle.o2_apply(wl.pos, wl.radii, wl.L, wl.xi, wl.rc, wl.M, wl.P, Fb[k], Tb[k], Sb[k])
+        _check_blocks((U[k].cpu().numpy(), W[k].cpu().numpy(), E[k].cpu().numpy()), ref, TOL)
+    U0, E0 = U[0].cpu().numpy().copy(), E[0].cpu().numpy().copy()
+    # the configuration stays cached: pos = None, fewer right-hand sides, real-space part alone
+    r.plan.set_flags(pk.SE_SKIP_WAVE | pk.SE_SKIP_SELF | pk.SE_SKIP_ONEBODY)
+    r.plan.apply_batch(None, t(Fb[:2]), t(Tb[:2]), t(Sb[:2]), U[:2], W[:2], E[:2])
+    torch.cuda.synchronize()
+    ref = oracle.o2_apply(wl.pos, wl.radii, wl.L, wl.xi, wl.rc, wl.M, wl.P, Fb[1], Tb[1], Sb[1], parts=oracle.PART_REAL)
+    _check_blocks((U[1].cpu().numpy(), W[1].cpu().numpy(), E[1].cpu().numpy()), ref, TOL_STAGE)
+    # the single-product entry point gives the same as right-hand side 0 of the batch
+    single = r.run()
+    assert _rel(single[0], U0) <= 1e-13 and _rel(single[2], E0) <= 1e-13
