@@ -364,7 +364,13 @@ static se_status upload_etab(se_plan *p)
 }
 
 // y-batch of k_xmid: 4 columns (64-byte runs), 2 where the compressible variant would not fit the register file
-template <int LM, bool COMP> struct XmChoice { static constexpr int YB = (COMP && LM == 9) ? 2 : 4; };
+#ifndef XM_YB8
+#define XM_YB8 4                   // y-batch for M = 256
+#endif
+#ifndef XM_YB9
+#define XM_YB9 4                   // y-batch for M = 512
+#endif
+template <int LM, bool COMP> struct XmChoice { static constexpr int YB = LM == 9 ? (COMP ? 2 : XM_YB9) : (LM == 8 && !COMP ? XM_YB8 : 4); };
 
 template <int LM>
 static cudaError_t prepare_xy()

@@ -27,6 +27,9 @@
 
 #define REAL_WARPS 4
 #define REAL_QCAP 64
+#ifndef REAL_MINB1
+#define REAL_MINB1 3                // resident CTAs per SM the single right-hand-side kernel is compiled for
+#endif
 
 // The radial part of a pair: everything that does not depend on the moments.  Evaluated once per pair and then applied
 // to one or several right-hand sides (far_mobility_apply_batch).
@@ -171,7 +174,7 @@ __device__ __forceinline__ void pair_real(const SeConst &c, double x, double y, 
 // NR right-hand sides at once (far_mobility_apply_batch): moments rs_mom[r][N][12], results out_real[r][N][12],
 // r < NR, `rhs_stride` doubles apart; the radial part of a pair is evaluated once and applied NR times.
 template <bool COMP, int NR>
-__global__ void __launch_bounds__(REAL_WARPS * 32) k_real(SeConst c, const double4 *__restrict__ rs_pos,
+__global__ void __launch_bounds__(REAL_WARPS * 32, (NR == 1 ? REAL_MINB1 : (NR == 2 ? 3 : 2))) k_real(SeConst c, const double4 *__restrict__ rs_pos,
                                                           const double *__restrict__ rs_mom, const int *__restrict__ rs_orig,
                                                           const int *__restrict__ start_r, double *__restrict__ out_real,
                                                           size_t rhs_stride)
