@@ -291,6 +291,26 @@ def main():
     warm_ms = w0.elapsed_time(w1) / args.steps
     plan.set_positions(None)
 
+    # ---- several right-hand sides on the cached configuration: products/s per batch size ----
+    batch = {}
+    plan.set_positions(pos)
+    for nrhs in (1, 4, 8):
+        Fb, Tb, Sb = F.repeat(nrhs, 1, 1), T.repeat(nrhs, 1, 1), S.repeat(nrhs, 1, 1)
+        Ub, Wb, Eb = torch.empty_like(Fb), torch.empty_like(Fb), torch.empty_like(Sb)
+        plan.apply_batch(None, Fb, Tb, Sb, Ub, Wb, Eb)
+        barrier()
+        b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = max(1, args.steps // nrhs)
+        b0.record(stream)
+        for _ in range(reps):
+            plan.apply_batch(None, Fb, Tb, Sb, Ub, Wb, Eb)
+        b1.record(stream)
+        barrier()
+        ms_b = b0.elapsed_time(b1) / reps
+        batch[f"nrhs{nrhs}"] = {"ms_per_batch": ms_b, "ms_per_rhs": ms_b / nrhs, "products_per_s": 1e3 * nrhs / ms_b}
+        del Fb, Tb, Sb, Ub, Wb, Eb
+    plan.set_positions(None)
+
     # ---- per-stage CUDA-event times (library events on the launch stream), averaged over K steps ----
     plan.set_flags(pk.SE_TIMING)
     samples = {k: [] for k in pk.STAGE_NAMES}
@@ -413,7 +433,7 @@ def main():
         "ms_per_step_median": ms_median,
         "config": config_dict(args.config, wl, world),
         "workspace_GB": plan.workspace_bytes() / 1e9,
-        "warm_ms_per_step": warm_ms, "stages_ms": stage, "fft_ms": stage["fft_fwd"] + stage["fft_inv"], "own_kernels_ms": sum(own.values()),
+        "warm_ms_per_step": warm_ms, "batch_cached_positions": batch, "stages_ms": stage, "fft_ms": stage["fft_fwd"] + stage["fft_inv"], "own_kernels_ms": sum(own.values()),
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 14 * 8 * wl.N, "d2h_bytes_per_step": 11 * 8 * wl.N,
                 "ms_per_step": 1e3 * e2e_s / args.steps},
