@@ -132,14 +132,15 @@ def measure_config(name, dev, peak, steps):
     U = torch.empty((wl.N, 3), device=dev, dtype=torch.float64)
     Om = torch.empty_like(U)
     E = torch.empty((wl.N, 5), device=dev, dtype=torch.float64)
-    stream = torch.cuda.current_stream()
+    stream = torch.cuda.Stream()             # not the legacy default stream: the plan-owned CUDA graph (M <= 128) needs a capturable one
+    torch.cuda.synchronize()
     for _ in range(3):
-        plan.apply(pos, F, T, S, U, Om, E)
+        plan.apply(pos, F, T, S, U, Om, E, stream=stream)
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
     for _ in range(steps):
-        plan.apply(pos, F, T, S, U, Om, E)
+        plan.apply(pos, F, T, S, U, Om, E, stream=stream)
     e1.record(stream)
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / steps

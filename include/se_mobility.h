@@ -100,8 +100,14 @@ se_status se_plan_set_tuning(se_plan *plan, int spread_segments, int gather_segm
  *   SE_OPT_YZ_FUSED      with SE_OPT_XY_PATH = 0: 1 = the y and z transforms of a direction in ONE kernel (thread-block
  *                        clusters exchanging through distributed shared memory; default for M <= 128), 0 = separate
  *                        z and y kernels.
+ *   SE_OPT_GRAPH         1 = far_mobility_apply / _compressible keep the whole product as a plan-owned CUDA graph: the
+ *                        first call runs plainly, the second captures the sequence on the caller's stream, later calls
+ *                        with the same pointers, stream, flags and options replay it in one launch (the data behind
+ *                        the pointers may change freely).  Default: 1 for M <= 128, where launch latency dominates,
+ *                        else 0.  Never used on the legacy default stream, inside a caller's own capture, with
+ *                        SE_TIMING or se_plan_debug_stop.
  * Errors: SE_ERR_INVALID_ARG for an unknown key or a value out of range. */
-enum { SE_OPT_REAL_OVERLAP = 0, SE_OPT_REAL_CTAS = 1, SE_OPT_XY_PATH = 2, SE_OPT_YZ_FUSED = 3, SE_NUM_OPTS = 4 };
+enum { SE_OPT_REAL_OVERLAP = 0, SE_OPT_REAL_CTAS = 1, SE_OPT_XY_PATH = 2, SE_OPT_YZ_FUSED = 3, SE_OPT_GRAPH = 4, SE_NUM_OPTS = 5 };
 se_status se_plan_set_option(se_plan *plan, int key, int value);
 
 /* Bitwise OR of the SE_* flags above. */

@@ -86,6 +86,15 @@ struct se_plan {
     int lM;
     double2 *d_wtab;               // exp(-2 pi i q / M), q < M
     double *d_etab;                // exp(-(1 - eta_se) k_q^2 / 4 xi^2), q < M (k-space pass of se_xyfft.cuh)
+    // plan-owned CUDA graph of the whole product (SE_OPT_GRAPH): replayed while the same pointers, flags and options come back
+    int use_graph;                 // 0 off, 1 on (default: on for M <= 128, where launch latency dominates)
+    bool have_graph;
+    cudaGraphExec_t gexec;
+    const void *gkey[10];          // pos F T S s_in U Omega E s_out stream
+    unsigned gflags;
+    long gepoch, epoch;            // epoch: bumped by every setter that changes what apply_impl enqueues
+    int graph_launches;
+    bool warmed[2];                // a plain apply (lazy allocations done) was made: [0] without, [1] with the a9 arguments
     int xy_path;                   // SE_OPT_XY_PATH: 0 = own y / fused x kernels, 1 = cuFFT 2-D plans + k_kspace
     int yz_fused;                  // SE_OPT_YZ_FUSED: (y,z) transforms in one cluster kernel per direction (se_zfft.cuh)
     size_t fft_bytes;
@@ -236,6 +245,7 @@ extern "C" se_status se_plan_destroy(se_plan *p)
     cudaFree(p->d_key_r); cudaFree(p->d_rank_r); cudaFree(p->d_key_s); cudaFree(p->d_rank_s);
     cudaFree(p->d_key_g); cudaFree(p->d_rank_g); cudaFree(p->d_grecs);
     cudaFree(p->d_cnt_all); cudaFree(p->d_start_all); cudaFree(p->d_dst_rs);
+    if (p->have_graph) cudaGraphExecDestroy(p->gexec);
     if (p->have_side) { cudaStreamDestroy(p->side); cudaEventDestroy(p->ev_fork); cudaEventDestroy(p->ev_join); }
     cudaFree(p->d_bsum);
     cudaFree(p->d_rs_pos); cudaFree(p->d_rs_mom); cudaFree(p->d_rs_orig); cudaFree(p->d_recs);
@@ -629,6 +639,7 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
         // takes little from the HBM-bound kernels' occupancy; c4 step 3.57 -> 3.50 ms)
         p->real_side_ctas = p->sms;
         p->real_overlap = 1;
+        p->use_graph = M <= 128 ? 1 : 0;
     }
     if (raise_smem_limit(k_scatter) != cudaSuccess || dispatch_prepare(P) != cudaSuccess) { cudaGetLastError(); se_plan_destroy(p); return SE_ERR_CUDA; }
     *out = p;
@@ -639,6 +650,7 @@ extern "C" se_status se_plan_set_shape(se_plan *p, double m)
 {
     if (!p || !(m > 0.0)) return SE_ERR_INVALID_ARG;
     p->m = m;
+    ++p->epoch;
     derive_constants(p);
     p->have_positions = false;          // the cached Gaussian tables depend on the shape
     if (p->d_etab) return upload_etab(p);
@@ -649,17 +661,20 @@ extern "C" se_status se_plan_set_tuning(se_plan *p, int spread_segments, int gat
 {
     if (!p || spread_segments < 0 || gather_segments < 0) return SE_ERR_INVALID_ARG;
     choose_segments(p, spread_segments, gather_segments);
+    ++p->epoch;
     return SE_OK;
 }
 
 extern "C" se_status se_plan_set_option(se_plan *p, int key, int value)
 {
     if (!p || value < 0) return SE_ERR_INVALID_ARG;
+    ++p->epoch;
     switch (key) {
     case SE_OPT_REAL_OVERLAP: if (value > 2) return SE_ERR_INVALID_ARG; p->real_overlap = value; break;
     case SE_OPT_REAL_CTAS: p->real_side_ctas = value; break;
     case SE_OPT_XY_PATH: if (value > 1) return SE_ERR_INVALID_ARG; p->xy_path = value; break;
     case SE_OPT_YZ_FUSED: if (value > 1) return SE_ERR_INVALID_ARG; p->yz_fused = value; break;
+    case SE_OPT_GRAPH: if (value > 1) return SE_ERR_INVALID_ARG; p->use_graph = value; break;
     default: return SE_ERR_INVALID_ARG;
     }
     return SE_OK;
@@ -669,6 +684,7 @@ extern "C" se_status se_plan_set_flags(se_plan *p, unsigned flags)
 {
     if (!p || (flags & ~0x5fu)) return SE_ERR_INVALID_ARG;
     p->flags = flags;
+    ++p->epoch;
     return SE_OK;
 }
 
@@ -676,6 +692,7 @@ extern "C" se_status se_plan_debug_stop(se_plan *p, int stage)
 {
     if (!p || stage < -1 || stage >= SE_NUM_STAGES) return SE_ERR_INVALID_ARG;
     p->debug_stop = stage;
+    ++p->epoch;
     return SE_OK;
 }
 
@@ -826,6 +843,7 @@ static se_status sort_and_pack(se_plan *p, const double *pos, const double *F, c
 extern "C" se_status se_plan_set_positions(se_plan *p, const double *pos, void *cuda_stream)
 {
     if (!p) return SE_ERR_INVALID_ARG;
+    ++p->epoch;
     if (!pos) { p->have_positions = false; return SE_OK; }            // forget the cached configuration
     p->last_launches = 0;
     p->have_positions = false;
@@ -1048,17 +1066,72 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     return SE_OK;
 }
 
+// The product as a plan-owned CUDA graph (small systems are bound by the latency of ~15 launches): the first call with a
+// given set of pointers runs plainly (lazy allocations), the second captures the same sequence on the caller's stream into
+// a graph, later ones replay it.  Anything that changes what is enqueued (other pointers or stream, flags, options,
+// se_plan_set_positions) captures again.  Not used on the legacy default stream, while the caller is capturing itself,
+// or with SE_TIMING / se_plan_debug_stop.
+static se_status apply_graphed(se_plan *p, const double *pos, const double *F, const double *T, const double *S,
+                               const double *s_in, double *U, double *Omega, double *E, double *s_out, void *cuda_stream,
+                               const char *who)
+{
+    if (!p) return SE_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const int cv = (s_in || s_out) ? 1 : 0;
+    bool plain = !p->use_graph || s == nullptr || s == cudaStreamLegacy || (p->flags & SE_TIMING) || p->debug_stop >= 0 || !p->warmed[cv] ||
+                 !F || !T || !S || !U || !Omega || !E || (!pos && !p->have_positions);
+    if (!plain) {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(s, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) { cudaGetLastError(); plain = true; }
+    }
+    if (plain) {
+        const se_status st = apply_impl(p, pos, F, T, S, s_in, U, Omega, E, s_out, cuda_stream, who);
+        if (st == SE_OK) p->warmed[cv] = true;
+        return st;
+    }
+    const void *key[10] = { pos, F, T, S, s_in, U, Omega, E, s_out, cuda_stream };
+    if (p->have_graph && p->gepoch == p->epoch && p->gflags == p->flags && memcmp(key, p->gkey, sizeof(key)) == 0) {
+        CUDA_TRY(p, cudaGraphLaunch(p->gexec, s));
+        p->last_launches = p->graph_launches;
+        if (pos) p->have_positions = false;
+        return SE_OK;
+    }
+    const bool had_pos = p->have_positions;
+    CUDA_TRY(p, cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
+    const se_status st = apply_impl(p, pos, F, T, S, s_in, U, Omega, E, s_out, cuda_stream, who);
+    cudaGraph_t g = nullptr;
+    const cudaError_t ec = cudaStreamEndCapture(s, &g);
+    if (st != SE_OK || ec != cudaSuccess || !g) {
+        if (g) cudaGraphDestroy(g);
+        cudaGetLastError();
+        p->have_positions = had_pos;
+        if (st != SE_OK) return st;
+        return fail(p, SE_ERR_CUDA, "cudaStreamEndCapture", cudaGetErrorString(ec));
+    }
+    if (p->have_graph) { cudaGraphExecDestroy(p->gexec); p->have_graph = false; }
+    const cudaError_t ei = cudaGraphInstantiate(&p->gexec, g, 0);
+    cudaGraphDestroy(g);
+    if (ei != cudaSuccess) { cudaGetLastError(); return fail(p, SE_ERR_CUDA, "cudaGraphInstantiate", cudaGetErrorString(ei)); }
+    p->have_graph = true;
+    memcpy(p->gkey, key, sizeof(key));
+    p->gflags = p->flags;
+    p->gepoch = p->epoch;
+    p->graph_launches = p->last_launches;
+    CUDA_TRY(p, cudaGraphLaunch(p->gexec, s));
+    return SE_OK;
+}
+
 extern "C" se_status far_mobility_apply(se_plan *p, const double *pos, const double *F, const double *T,
                                         const double *S, double *U, double *Omega, double *E, void *cuda_stream)
 {
-    return apply_impl(p, pos, F, T, S, nullptr, U, Omega, E, nullptr, cuda_stream, "far_mobility_apply");
+    return apply_graphed(p, pos, F, T, S, nullptr, U, Omega, E, nullptr, cuda_stream, "far_mobility_apply");
 }
 
 extern "C" se_status far_mobility_apply_compressible(se_plan *p, const double *pos, const double *F, const double *T,
                                                      const double *S, const double *s_in, double *U, double *Omega,
                                                      double *E, double *s_out, void *cuda_stream)
 {
-    return apply_impl(p, pos, F, T, S, s_in, U, Omega, E, s_out, cuda_stream, "far_mobility_apply_compressible");
+    return apply_graphed(p, pos, F, T, S, s_in, U, Omega, E, s_out, cuda_stream, "far_mobility_apply_compressible");
 }
 
 // Several right-hand sides on one configuration: a1 once; the real-space sum for up to four right-hand

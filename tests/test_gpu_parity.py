@@ -549,3 +549,43 @@ def test_batch_of_right_hand_sides(pk, oracle, workloads, name, nrhs):
     # the single-product entry point gives the same as right-hand side 0 of the batch
     single = r.run()
     assert _rel(single[0], U0) <= 1e-13 and _rel(single[2], E0) <= 1e-13
+
+
+def test_plan_owned_cuda_graph(pk, oracle, workloads):
+    """SE_OPT_GRAPH (default on for M <= 128): on a non-default stream the second call captures the product into a
+    plan-owned graph and later calls replay it; new data behind the same pointers, other pointers, other flags and the
+    cached-positions path must all still give the oracle's result."""
+    import torch
+    wl = workloads.make_workload("c2")
+    r = Runner(pk, wl)
+    st = torch.cuda.Stream()
+    ref = r.oracle(oracle)
+
+    def go(pos, F):
+        r.U.fill_(float("nan")); r.W.fill_(float("nan")); r.E.fill_(float("nan"))
+        torch.cuda.synchronize()
+        r.plan.apply(pos, F, r.T, r.S, r.U, r.W, r.E, stream=st)
+        st.synchronize()
+        return r.U.cpu().numpy(), r.W.cpu().numpy(), r.E.cpu().numpy()
+
+    r.plan.set_flags(0); r.plan.debug_stop(-1)
+    for _ in range(4):                                  # plain, capture, replay, replay
+        _check_blocks(go(r.pos, r.F), ref, TOL)
+    n_graph = r.plan.last_launch_count()
+    r.F.mul_(-2.0)                                      # new data behind the same pointers: replay
+    ref2 = oracle.o2_apply(wl.pos, wl.radii, wl.L, wl.xi, wl.rc, wl.M, wl.P, -2.0 * wl.F, wl.T, wl.S)
+    _check_blocks(go(r.pos, r.F), ref2, TOL)
+    F3 = r.F.clone()                                    # another pointer: capture again
+    _check_blocks(go(r.pos, F3), ref2, TOL)
+    _check_blocks(go(r.pos, F3), ref2, TOL)
+    r.plan.set_flags(pk.SE_SKIP_REAL | pk.SE_SKIP_SELF | pk.SE_SKIP_ONEBODY)      # other flags: capture again
+    refw = oracle.o2_apply(wl.pos, wl.radii, wl.L, wl.xi, wl.rc, wl.M, wl.P, -2.0 * wl.F, wl.T, wl.S, parts=oracle.PART_WAVE)
+    for _ in range(3):
+        _check_blocks(go(r.pos, F3), refw, TOL_STAGE)
+    r.plan.set_flags(0)
+    r.plan.set_positions(r.pos, stream=st)              # cached positions: pos = None
+    for _ in range(3):
+        _check_blocks(go(None, F3), ref2, TOL)
+    assert r.plan.last_launch_count() == n_graph - 3    # a1 is one kernel instead of four, also in the graph
+    r.plan.set_option(pk.SE_OPT_GRAPH, 0)
+    _check_blocks(go(None, F3), ref2, TOL)
