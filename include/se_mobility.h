@@ -84,8 +84,9 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, const double *radii
 /* Gaussian shape parameter m of Eq. 46 (h ~ exp(-m^2/2) at the edge of the support), m > 0. */
 se_status se_plan_set_shape(se_plan *plan, double m);
 
-/* Performance knob: number of segments the x-sweeps of the spreading and gather kernels are cut into
- * (0 = the plan's own choice).  Results do not depend on it beyond summation order. */
+/* Performance knob: number of segments the x-sweep of the spreading kernel is cut into (0 = the plan's own choice);
+ * gather_segments is accepted and ignored (the gather kernel balances its own work over the SMs).
+ * Results do not depend on it beyond summation order. */
 se_status se_plan_set_tuning(se_plan *plan, int spread_segments, int gather_segments);
 
 /* Further performance knobs, one integer each (results do not depend on them beyond summation order):

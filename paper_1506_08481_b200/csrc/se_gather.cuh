@@ -86,25 +86,52 @@ __device__ __forceinline__ void tma_prefetch3(const CUtensorMap *tmap, int c0, i
     asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];" ::"l"(tmap), "r"(c0), "r"(c1), "r"(c2) : "memory");
 }
 
-// Work item `it` of the launch: all tiles of one (grid, segment) are consecutive, so that the CTAs of one round work
-// on neighbouring tiles of the same planes and the halo re-reads hit L2.
+// Work of the launch: items = (returned grid, (y,z) tile), tiles of one grid consecutive, M planes each.  They are dealt
+// to the persistent CTAs round-robin, so that at any moment the CTAs work on neighbouring tiles of the same planes and the
+// halo re-reads hit L2.  The items of the last, incomplete round (768 items on 148 SMs: 28 left after five rounds) are cut
+// along x into floor(gridDim / left) segments each, so that every CTA gets a share of it instead of 28 CTAs a whole sixth
+// item.  A sub-item (item, [x0, x1)): the planes x0 .. x1 + P - 2 stream through the ring, the particles whose support
+// starts in [x0, x1) are gathered.
 struct GatherItem { int grid, seg_start, nplanes, Y0, Z0, i0, i1; };
-__device__ __forceinline__ GatherItem gather_item(int it, const SeConst &c, const GatherGeom &g, int ngrids, const int *__restrict__ start_g)
-{
-    const int ntile = g.NTY * g.NTZ;
-    const int gs = it / ntile, tile = it - gs * ntile;
-    GatherItem r;
-    r.grid = gs % ngrids;
-    const int seg = gs / ngrids;
-    r.seg_start = seg * g.seg_len;
-    const int seg_end = min(r.seg_start + g.seg_len, c.M);
-    r.nplanes = seg_end - r.seg_start + c.P - 1;
-    const int ty = tile / g.NTZ, tz = tile - ty * g.NTZ;
-    r.Y0 = ty * g.TY; r.Z0 = tz * g.TZ;
-    r.i0 = start_g[tile * c.M + r.seg_start];
-    r.i1 = start_g[tile * c.M + seg_end];
-    return r;
-}
+struct GatherWalk {
+    int round, nfull, nitems, left, nsplit;
+    __device__ __forceinline__ GatherWalk(const GatherGeom &g, int ngrids)
+    {
+        nitems = g.NTY * g.NTZ * ngrids;
+        nfull = nitems / (int)gridDim.x;
+        left = nitems - nfull * (int)gridDim.x;
+        nsplit = left > 0 ? (int)gridDim.x / left : 1;
+        round = 0;
+    }
+    // next sub-item with particles; false at the end of this CTA's work
+    __device__ __forceinline__ bool next(GatherItem &r, const SeConst &c, const GatherGeom &g, const int *__restrict__ start_g)
+    {
+        const int M = c.M, ntile = g.NTY * g.NTZ, b = (int)blockIdx.x;
+        while (round <= nfull) {
+            int it, x0 = 0, x1 = M;
+            if (round < nfull) it = round * (int)gridDim.x + b;
+            else {
+                if (b >= left * nsplit) { ++round; break; }
+                const int q = b % nsplit, len = (M + nsplit - 1) / nsplit;
+                it = nfull * (int)gridDim.x + b / nsplit;
+                x0 = q * len; x1 = min(x0 + len, M);
+                if (x0 >= x1) { ++round; break; }
+            }
+            ++round;
+            const int gi = it / ntile, tile = it - gi * ntile;
+            r.i0 = start_g[tile * M + x0];
+            r.i1 = start_g[tile * M + x1];
+            if (r.i0 == r.i1) continue;                               // no support starts here: skipped by everybody
+            r.grid = gi;
+            r.seg_start = x0;
+            r.nplanes = x1 - x0 + c.P - 1;
+            const int ty = tile / g.NTZ, tz = tile - ty * g.NTZ;
+            r.Y0 = ty * g.TY; r.Z0 = tz * g.TZ;
+            return true;
+        }
+        return false;
+    }
+};
 
 template <int P>
 __global__ void __launch_bounds__((GR_WARPS + 1) * 32, 1)
@@ -117,7 +144,6 @@ k_gather(SeConst c, GatherGeom g, const double *__restrict__ grecs, const int *_
     extern __shared__ __align__(128) unsigned char gsm[];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int M = c.M;
-    const int nitems = g.NTY * g.NTZ * ngrids * g.nseg;
 
     double *ring = reinterpret_cast<double *>(gsm);
     double *rbuf = ring + (size_t)R * SLOT;                            // [GR_WARPS][2][NPW][GS] record buffers
@@ -144,22 +170,21 @@ k_gather(SeConst c, GatherGeom g, const double *__restrict__ grecs, const int *_
             // A second cursor runs GR_PREFETCH planes ahead of the loads (across item boundaries) and asks for the boxes
             // to be brought into L2, so that the ring fill itself sees L2 latency only: the ring's slack of R - P planes
             // is too short to cover a DRAM miss under load.
-            int pit = blockIdx.x, pj = 0, ahead = 0;
-            GatherItem PI = pit < nitems ? gather_item(pit, c, g, ngrids, start_g) : GatherItem{};
+            int pj = 0, ahead = 0;
+            GatherWalk pw(g, ngrids);
+            GatherItem PI;
+            bool phave = pw.next(PI, c, g, start_g);
             auto prefetch_step = [&]() {                               // prefetch one plane, advance the cursor
-                while (pit < nitems && (PI.i0 == PI.i1 || pj >= PI.nplanes)) {
-                    pit += gridDim.x; pj = 0;
-                    if (pit < nitems) PI = gather_item(pit, c, g, ngrids, start_g);
-                }
-                if (pit >= nitems) return;
+                while (phave && pj >= PI.nplanes) { phave = pw.next(PI, c, g, start_g); pj = 0; }
+                if (!phave) return;
                 int x = PI.seg_start + pj;
                 if (x >= M) x -= M;
                 tma_prefetch3(&tmap, PI.Z0, PI.Y0, PI.grid * M + x);
                 ++pj;
             };
-            for (int it = blockIdx.x; it < nitems; it += gridDim.x) {
-                const GatherItem I = gather_item(it, c, g, ngrids, start_g);
-                if (I.i0 == I.i1) continue;                            // no support starts here: skipped by everybody
+            GatherWalk lw(g, ngrids);
+            GatherItem I;
+            while (lw.next(I, c, g, start_g)) {
                 int x = I.seg_start;
                 for (int j = 0; j < I.nplanes; ++j) {
                     while (ahead < GR_PREFETCH + 1) { prefetch_step(); ++ahead; }
@@ -188,9 +213,9 @@ k_gather(SeConst c, GatherGeom g, const double *__restrict__ grecs, const int *_
     uint32_t rpar = 0;                                                 // bit b: parity of record buffer b
     const double Delta = c.Delta;
 
-    for (int it = blockIdx.x; it < nitems; it += gridDim.x) {
-        const GatherItem I = gather_item(it, c, g, ngrids, start_g);
-        if (I.i0 == I.i1) continue;
+    GatherWalk cw(g, ngrids);
+    GatherItem I;
+    while (cw.next(I, c, g, start_g)) {
         int jdone = 0, jrel = 0;
         auto observe_next = [&]() {
             mbar_wait(full_bar(sdone), pdone);

@@ -177,18 +177,7 @@ static void choose_segments(se_plan *p, int spread_segments, int gather_segments
     int ns = pick(spread_segments, npatch);
     c.seg_len = (M + ns - 1) / ns;
     c.nseg = (M + c.seg_len - 1) / c.seg_len;
-    // gather (persistent, one CTA per SM): enough (tile, grid, segment) items for ~8 rounds, segments of >= 32 planes
-    GatherGeom &g = p->gg;
-    int ng = gather_segments;
-    if (ng <= 0) {
-        const int items = g.NTY * g.NTZ * 6;
-        ng = (p->sms * 8 + items - 1) / items;
-        if (ng > maxseg) ng = maxseg;
-    }
-    if (ng > M) ng = M;
-    if (ng < 1) ng = 1;
-    g.seg_len = (M + ng - 1) / ng;
-    g.nseg = (M + g.seg_len - 1) / g.seg_len;
+    (void)gather_segments;                        // the gather balances its own work (GatherWalk, se_gather.cuh)
 }
 
 #ifndef FOR_EACH_P                 // a development build may define a shorter list on the command line
@@ -734,8 +723,8 @@ static void launch_gather(se_plan *p, cudaStream_t s, bool pressure)
 {
     const GatherGeom &g = p->gg;
     const int ngrids = pressure ? 1 : 6;
-    const int items = g.NTY * g.NTZ * ngrids * g.nseg;
-    const unsigned blocks = (unsigned)(items < p->sms ? items : p->sms);          // persistent: one CTA per SM
+    const int items = g.NTY * g.NTZ * ngrids;
+    const unsigned blocks = (unsigned)(items < p->sms ? items : p->sms);          // persistent: one CTA per SM (work split: GatherWalk)
     k_gather<P><<<blocks, (GR_WARPS + 1) * 32, p->gather_smem, s>>>(p->c, g, p->d_grecs, p->d_start_g, pressure ? p->tmap_p : p->tmap, ngrids,
                                                              pressure ? p->d_pmom : p->d_moments, pressure ? 12 : GATHER_SUMS);
 }
