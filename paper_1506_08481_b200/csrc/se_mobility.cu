@@ -821,7 +821,7 @@ static se_status sort_and_pack(se_plan *p, const double *pos, const double *F, c
     p->last_launches += 1;
     const se_status st = scan_cells(p, s);
     if (st != SE_OK) return st;
-    k_scatter<<<(c.N + SCATTER_THREADS - 1) / SCATTER_THREADS, SCATTER_THREADS, scatter_smem_bytes(c.P), s>>>(
+    k_scatter<<<(c.N + SCATTER_PART - 1) / SCATTER_PART, SCATTER_THREADS, scatter_smem_bytes(c.P), s>>>(
         c, pos, p->d_radii, F, T, S, s_in, p->d_key_r, p->d_rank_r, p->d_start_r, p->d_key_s, p->d_rank_s, p->d_start_s,
         p->d_key_g, p->d_rank_g, p->d_start_g, p->d_grecs, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig, p->d_recs, p->d_dst_rs);
     p->last_launches += 1;

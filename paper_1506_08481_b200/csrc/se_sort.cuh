@@ -113,88 +113,85 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_add(int *__restrict__ out
     }
 }
 
-#define SCATTER_THREADS 64
-// One thread per particle: write the real-space packed copy (cell order), the spreading record (tile order) and the
-// gather record (gather order) with the per-axis Gaussian tables (Eq. 41 in physical coordinates; the paper's
-// fast Gaussian gridding, Eq. 47, is replaced by P direct exponentials per axis, done once here).
-// The record is built in shared memory (one row per thread, odd row pitch) and copied out by whole warps, contiguous doubles at a time: per-thread stores of whole records were the whole cost of a1.
-__global__ void k_scatter(SeConst c, const double *__restrict__ pos, const double *__restrict__ radii,
-                          const double *__restrict__ F, const double *__restrict__ T, const double *__restrict__ S,
-                          const double *__restrict__ s_in,      // pressure moments (a9) or NULL
-                          const int *__restrict__ key_r, const int *__restrict__ rank_r, const int *__restrict__ start_r,
-                          const int *__restrict__ key_s, const int *__restrict__ rank_s, const int *__restrict__ start_s,
-                          const int *__restrict__ key_g, const int *__restrict__ rank_g, const int *__restrict__ start_g,
-                          double *__restrict__ grecs, double4 *__restrict__ rs_pos, double *__restrict__ rs_mom, int *__restrict__ rs_orig,
-                          double *__restrict__ recs, int2 *__restrict__ dst_rs)   // dst_rs[i] = (cell-order index, record index)
+#define SCATTER_PART 64             // particles per CTA
+#define SCATTER_THREADS (3 * SCATTER_PART)
+// Three threads per particle, one per axis: write the real-space packed copy (cell order), the spreading record (tile
+// order) and the gather record (gather order) with the per-axis Gaussian tables (Eq. 41 in physical coordinates; the
+// paper's fast Gaussian gridding, Eq. 47, is replaced by P direct exponentials per axis, done once here).
+// The record is built in shared memory (one row per particle, odd row pitch) and copied out by whole warps, contiguous
+// doubles at a time: per-thread stores of whole records were the whole cost of a1.
+__global__ void __launch_bounds__(SCATTER_THREADS)
+k_scatter(SeConst c, const double *__restrict__ pos, const double *__restrict__ radii,
+          const double *__restrict__ F, const double *__restrict__ T, const double *__restrict__ S,
+          const double *__restrict__ s_in,      // pressure moments (a9) or NULL
+          const int *__restrict__ key_r, const int *__restrict__ rank_r, const int *__restrict__ start_r,
+          const int *__restrict__ key_s, const int *__restrict__ rank_s, const int *__restrict__ start_s,
+          const int *__restrict__ key_g, const int *__restrict__ rank_g, const int *__restrict__ start_g,
+          double *__restrict__ grecs, double4 *__restrict__ rs_pos, double *__restrict__ rs_mom, int *__restrict__ rs_orig,
+          double *__restrict__ recs, int2 *__restrict__ dst_rs)   // dst_rs[i] = (cell-order index, record index)
 {
-    extern __shared__ __align__(16) double sc_rows[];          // [SCATTER_THREADS][(rec_stride + P) | 1] then int dst[2][SCATTER_THREADS]
+    extern __shared__ __align__(16) double sc_rows[];          // [SCATTER_PART][(rec_stride + P) | 1] then int dst[2][SCATTER_PART]
     const int P = c.P, pitch = (c.rec_stride + P) | 1;          // a row: the spreading record, then gx dx (gather record only)
-    int *sc_dst = reinterpret_cast<int *>(sc_rows + SCATTER_THREADS * pitch), *sc_dg = sc_dst + SCATTER_THREADS;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    sc_dst[threadIdx.x] = -1;
+    int *sc_dst = reinterpret_cast<int *>(sc_rows + SCATTER_PART * pitch), *sc_dg = sc_dst + SCATTER_PART;
+    const int pl = threadIdx.x / 3, d = threadIdx.x - 3 * pl;   // local particle, axis
+    const int i = blockIdx.x * SCATTER_PART + pl;
+    if (d == 0) sc_dst[pl] = -1;
     if (i < c.N) {
-    const size_t i3 = 3 * (size_t)i, i5 = 5 * (size_t)i;
-    const double a = radii[i];
-    double xw[3];
-#pragma unroll
-    for (int d = 0; d < 3; ++d) xw[d] = se_wrap(pos[i3 + d], c.L);
-    // F == NULL: positions only (se_plan_set_positions); the moments are filled in later by k_moments
-    double f[3] = { 0.0, 0.0, 0.0 }, t[3] = { 0.0, 0.0, 0.0 }, s[5] = { 0.0, 0.0, 0.0, 0.0, 0.0 };
-    if (F) {
-        f[0] = F[i3]; f[1] = F[i3 + 1]; f[2] = F[i3 + 2]; t[0] = T[i3]; t[1] = T[i3 + 1]; t[2] = T[i3 + 2];
-        s[0] = S[i5]; s[1] = S[i5 + 1]; s[2] = S[i5 + 2]; s[3] = S[i5 + 3]; s[4] = S[i5 + 4];
-    }
-
-    // real-space copy
-    const int dr = start_r[key_r[i]] + rank_r[i];
-    rs_pos[dr] = make_double4(xw[0], xw[1], xw[2], a);
-    double *m = rs_mom + 12 * (size_t)dr;
-    m[0] = f[0]; m[1] = f[1]; m[2] = f[2]; m[3] = t[0]; m[4] = t[1]; m[5] = t[2];
-    const double sp = s_in ? s_in[i] : 0.0;
-    m[6] = s[0]; m[7] = s[1]; m[8] = s[2]; m[9] = s[3]; m[10] = s[4]; m[11] = sp;
-    rs_orig[dr] = i;
-
-    // spreading / gather records
-    const int ds = start_s[key_s[i]] + rank_s[i];
-    dst_rs[i] = make_int2(dr, ds);
-    double *r = sc_rows + threadIdx.x * pitch, *gxd = r + c.rec_stride;
-    sc_dst[threadIdx.x] = ds;
-    sc_dg[threadIdx.x] = start_g[key_g[i]] + rank_g[i];
-    int n0w[3];
-    double d0[3];
-    const double cF = a * a / 6.0, cS = a * a / 10.0, al = c.alpha;
-#pragma unroll
-    for (int d = 0; d < 3; ++d) {
-        const double u = xw[d] * c.MoverL;
+        const size_t i3 = 3 * (size_t)i, i5 = 5 * (size_t)i;
+        double *r = sc_rows + pl * pitch, *gxd = r + c.rec_stride;
+        const int dr = start_r[key_r[i]] + rank_r[i];
+        // this thread's axis: wrapped coordinate, support start, Gaussian table
+        const double xw = se_wrap(pos[i3 + d], c.L), al = c.alpha;
+        reinterpret_cast<double *>(rs_pos + dr)[d] = xw;
+        const double u = xw * c.MoverL;
         const int n0 = se_support_start(u, P);
-        n0w[d] = se_mod(n0, c.M);
-        d0[d] = ((double)n0 - u) * c.Delta;
+        r[REC_D0 + d] = ((double)n0 - u) * c.Delta;
+        reinterpret_cast<int *>(r)[d == 0 ? 2 : d - 1] = se_mod(n0, c.M);            // int2 (y0w, z0w), int2 (x0w, orig)
         double *g = r + SE_REC_HDR + d * P;
         for (int k = 0; k < P; ++k) {
             const double dk = ((double)(n0 + k) - u) * c.Delta;
             const double e = exp(-al * dk * dk);
             g[k] = d == 0 ? c.gnorm * e : e;
-            if (d == 0) gxd[k] = g[k] * dk;                 // gx dx of the gather record
+            if (d == 0) gxd[k] = g[k] * dk;                     // gx dx of the gather record
         }
-    }
-    if (c.rec_stride > SE_REC_HDR + 3 * P) r[SE_REC_HDR + 3 * P] = 0.0;
-    r[0] = __longlong_as_double(((long long)(unsigned)n0w[2] << 32) | (unsigned)n0w[1]);     // int2 (y0w, z0w)
-    r[1] = __longlong_as_double(((long long)(unsigned)i << 32) | (unsigned)n0w[0]);          // int2 (x0w, orig)
-    r[REC_D0] = d0[0]; r[REC_D0 + 1] = d0[1]; r[REC_D0 + 2] = d0[2];
-    r[REC_POLY] = 1.0 - 6.0 * al * cF;
-    r[REC_POLY + 1] = 4.0 * al * al * cF;
-    r[REC_POLY + 2] = 2.0 * al * (1.0 - 10.0 * al * cS);
-    r[REC_POLY + 3] = 8.0 * al * al * al * cS;
-    r[REC_F] = f[0]; r[REC_F + 1] = f[1]; r[REC_F + 2] = f[2];
-    r[REC_T] = t[0]; r[REC_T + 1] = t[1]; r[REC_T + 2] = t[2];
-    r[REC_S] = s[0]; r[REC_S + 1] = s[1]; r[REC_S + 2] = s[2]; r[REC_S + 3] = s[3]; r[REC_S + 4] = s[4];
-    r[REC_S + 5] = -(s[0] + s[3]);
-    r[REC_CF] = cF; r[REC_CS] = cS; r[REC_SP] = sp;
+        if (d == 0) {
+            const double a = radii[i];
+            reinterpret_cast<double *>(rs_pos + dr)[3] = a;
+            // F == NULL: positions only (se_plan_set_positions); the moments are filled in later by k_moments
+            double f[3] = { 0.0, 0.0, 0.0 }, t[3] = { 0.0, 0.0, 0.0 }, s[5] = { 0.0, 0.0, 0.0, 0.0, 0.0 };
+            if (F) {
+                f[0] = F[i3]; f[1] = F[i3 + 1]; f[2] = F[i3 + 2]; t[0] = T[i3]; t[1] = T[i3 + 1]; t[2] = T[i3 + 2];
+                s[0] = S[i5]; s[1] = S[i5 + 1]; s[2] = S[i5 + 2]; s[3] = S[i5 + 3]; s[4] = S[i5 + 4];
+            }
+            // real-space copy
+            double *m = rs_mom + 12 * (size_t)dr;
+            m[0] = f[0]; m[1] = f[1]; m[2] = f[2]; m[3] = t[0]; m[4] = t[1]; m[5] = t[2];
+            const double sp = s_in ? s_in[i] : 0.0;
+            m[6] = s[0]; m[7] = s[1]; m[8] = s[2]; m[9] = s[3]; m[10] = s[4]; m[11] = sp;
+            rs_orig[dr] = i;
+            // spreading / gather records
+            const int ds = start_s[key_s[i]] + rank_s[i];
+            dst_rs[i] = make_int2(dr, ds);
+            sc_dst[pl] = ds;
+            sc_dg[pl] = start_g[key_g[i]] + rank_g[i];
+            const double cF = a * a / 6.0, cS = a * a / 10.0;
+            if (c.rec_stride > SE_REC_HDR + 3 * P) r[SE_REC_HDR + 3 * P] = 0.0;
+            reinterpret_cast<int *>(r)[3] = i;
+            r[REC_POLY] = 1.0 - 6.0 * al * cF;
+            r[REC_POLY + 1] = 4.0 * al * al * cF;
+            r[REC_POLY + 2] = 2.0 * al * (1.0 - 10.0 * al * cS);
+            r[REC_POLY + 3] = 8.0 * al * al * al * cS;
+            r[REC_F] = f[0]; r[REC_F + 1] = f[1]; r[REC_F + 2] = f[2];
+            r[REC_T] = t[0]; r[REC_T + 1] = t[1]; r[REC_T + 2] = t[2];
+            r[REC_S] = s[0]; r[REC_S + 1] = s[1]; r[REC_S + 2] = s[2]; r[REC_S + 3] = s[3]; r[REC_S + 4] = s[4];
+            r[REC_S + 5] = -(s[0] + s[3]);
+            r[REC_CF] = cF; r[REC_CS] = cS; r[REC_SP] = sp;
+        }
     }
     __syncthreads();
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int PP = se_grec_pp(P), gstride = c.grec_stride;
-    for (int rr = w; rr < SCATTER_THREADS; rr += SCATTER_THREADS / 32) {
+    for (int rr = w; rr < SCATTER_PART; rr += SCATTER_THREADS / 32) {
         const int ds = sc_dst[rr];
         if (ds < 0) continue;
         const double *__restrict__ src = sc_rows + rr * pitch;
@@ -238,5 +235,5 @@ __global__ void k_moments(SeConst c, const double *__restrict__ F, const double 
 
 static inline size_t scatter_smem_bytes(int P)
 {
-    return (size_t)SCATTER_THREADS * ((se_rec_stride(P) + P) | 1) * 8 + 2 * SCATTER_THREADS * 4;
+    return (size_t)SCATTER_PART * ((se_rec_stride(P) + P) | 1) * 8 + 2 * SCATTER_PART * 4;
 }
