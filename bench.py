@@ -211,6 +211,8 @@ def main():
     ap.add_argument("--config", default="c4", choices=["c1", "c2", "c3", "c4", "c5"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--real-overlap", type=int, default=None, choices=[0, 1, 2],
+                    help="SE_OPT_REAL_OVERLAP of the plan (default: the library's); 0 runs the real-space kernel alone, one CTA per cell")
     ap.add_argument("--no-other-configs", action="store_true", help="skip the c1-c3, c5 lines of 'all_configs'")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -238,6 +240,8 @@ def main():
 
     wl = W.make_workload(args.config)
     plan = pk.SePlan(wl.N, wl.L, wl.radii, wl.xi, wl.rc, wl.M, wl.P, wl.eta0)
+    if args.real_overlap is not None:
+        plan.set_option(pk.SE_OPT_REAL_OVERLAP, args.real_overlap)
     t = lambda a: torch.tensor(np.ascontiguousarray(a), device=dev, dtype=torch.float64)
     pos, F, T, S = t(wl.pos), t(wl.F), t(wl.T), t(wl.S)
     U = torch.empty((wl.N, 3), device=dev, dtype=torch.float64)
