@@ -107,8 +107,15 @@ se_status se_plan_set_tuning(se_plan *plan, int spread_segments, int gather_segm
  *                        the pointers may change freely).  Default: 1 for M <= 128, where launch latency dominates,
  *                        else 0.  Never used on the legacy default stream, inside a caller's own capture, with
  *                        SE_TIMING or se_plan_debug_stop.
+ *   SE_OPT_PAIR_CACHE    1 (default) = se_plan_set_positions also does the neighbour search of the real-space sum and
+ *                        stores, per pair r < r_c, the separation and the 17 radial scalars of the pair (160 bytes + 4);
+ *                        products on the cached configuration (pos == NULL, also far_mobility_apply_batch) then only
+ *                        stream that list.  Costs about 1.3 real-space sums once and 164 bytes per ordered pair
+ *                        (c4: 0.66 GB); 0 = recompute the pairs in every product.  If the list cannot be allocated the
+ *                        products silently recompute.
  * Errors: SE_ERR_INVALID_ARG for an unknown key or a value out of range. */
-enum { SE_OPT_REAL_OVERLAP = 0, SE_OPT_REAL_CTAS = 1, SE_OPT_XY_PATH = 2, SE_OPT_YZ_FUSED = 3, SE_OPT_GRAPH = 4, SE_NUM_OPTS = 5 };
+enum { SE_OPT_REAL_OVERLAP = 0, SE_OPT_REAL_CTAS = 1, SE_OPT_XY_PATH = 2, SE_OPT_YZ_FUSED = 3, SE_OPT_GRAPH = 4, SE_OPT_PAIR_CACHE = 5,
+       SE_NUM_OPTS = 6 };
 se_status se_plan_set_option(se_plan *plan, int key, int value);
 
 /* Bitwise OR of the SE_* flags above. */
@@ -120,7 +127,9 @@ se_status se_plan_set_flags(se_plan *plan, unsigned flags);
  * may be called with pos == NULL and then only refresh the moments (F, T, S, s) of the packed records.
  *   pos    [N][3] DEVICE, as in far_mobility_apply; NULL forgets the cached configuration
  * The cache is dropped by se_plan_set_shape and by any apply that passes pos != NULL.  With a cached configuration
- * the summation order is fixed, so repeated products are bitwise reproducible. */
+ * the summation order is fixed, so repeated products are bitwise reproducible.  With SE_OPT_PAIR_CACHE (default) the call
+ * also builds the pair list of the real-space sum (the paper prebuilds its real-space matrix per configuration likewise,
+ * PAPER.md L332) and synchronises cuda_stream once to size it. */
 se_status se_plan_set_positions(se_plan *plan, const double *pos, void *cuda_stream);
 
 /* The product.  All pointers are DEVICE pointers to arrays the caller owns:

@@ -65,6 +65,12 @@ struct se_plan {
     double2 *d_Hk;                 // [3][M][M][M/2+1]
     double2 *d_Gk;                 // [6][M][M][M/2+1]
     double *d_out_real;            // [N][12] real-space part in caller order (slot 11: pressure, a9)
+    // cached pairs of the real-space sum (se_real.cuh), built by se_plan_set_positions when SE_OPT_PAIR_CACHE is on
+    int pair_cache;                // SE_OPT_PAIR_CACHE
+    bool have_pairs;               // the list below belongs to the cached configuration
+    int *d_pair_start, *d_pair_cursor, *d_pair_bsum, *d_pj;   // [N+1] row starts (count, then scanned), [N], scan scratch, partners
+    double *d_pd;                  // [pairs][PAIR_F] in row-local structure-of-arrays form
+    size_t pair_cap, npairs;
     const double *ext_out_real;    // far_mobility_apply_batch: real-space part already computed (k_real is skipped)
     double *d_mom_b, *d_out_real_b; // batch: moments in cell order and real-space results, [nrhs][N][12]
     int batch_cap;                 // right-hand sides the batch buffers hold
@@ -231,6 +237,7 @@ extern "C" se_status se_plan_destroy(se_plan *p)
 {
     if (!p) return SE_OK;
     cudaFree(p->d_radii); cudaFree(p->d_blockW);
+    cudaFree(p->d_pair_start); cudaFree(p->d_pair_cursor); cudaFree(p->d_pair_bsum); cudaFree(p->d_pj); cudaFree(p->d_pd);
     cudaFree(p->d_key_r); cudaFree(p->d_rank_r); cudaFree(p->d_key_s); cudaFree(p->d_rank_s);
     cudaFree(p->d_key_g); cudaFree(p->d_rank_g); cudaFree(p->d_grecs);
     cudaFree(p->d_cnt_all); cudaFree(p->d_start_all); cudaFree(p->d_dst_rs);
@@ -629,6 +636,7 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
         p->real_side_ctas = p->sms;
         p->real_overlap = 1;
         p->use_graph = M <= 128 ? 1 : 0;
+        p->pair_cache = 1;
     }
     if (raise_smem_limit(k_scatter) != cudaSuccess || dispatch_prepare(P) != cudaSuccess) { cudaGetLastError(); se_plan_destroy(p); return SE_ERR_CUDA; }
     *out = p;
@@ -664,6 +672,7 @@ extern "C" se_status se_plan_set_option(se_plan *p, int key, int value)
     case SE_OPT_XY_PATH: if (value > 1) return SE_ERR_INVALID_ARG; p->xy_path = value; break;
     case SE_OPT_YZ_FUSED: if (value > 1) return SE_ERR_INVALID_ARG; p->yz_fused = value; break;
     case SE_OPT_GRAPH: if (value > 1) return SE_ERR_INVALID_ARG; p->use_graph = value; break;
+    case SE_OPT_PAIR_CACHE: if (value > 1) return SE_ERR_INVALID_ARG; p->pair_cache = value; if (!value) p->have_pairs = false; break;
     default: return SE_ERR_INVALID_ARG;
     }
     return SE_OK;
@@ -815,6 +824,7 @@ static se_status sort_and_pack(se_plan *p, const double *pos, const double *F, c
 {
     const SeConst &c = p->c;
     const int TB = 128, nbN = (c.N + TB - 1) / TB;
+    p->have_pairs = false;                            // a new configuration: the cached pair list is stale
     CUDA_TRY(p, cudaMemsetAsync(p->d_cnt_all, 0, sizeof(int) * (size_t)p->ncell_all, s));
     k_keys<<<nbN, TB, 0, s>>>(c, p->gg, pos, p->d_key_r, p->d_rank_r, p->d_cnt_r, p->d_key_s, p->d_rank_s, p->d_cnt_s,
                               p->d_key_g, p->d_rank_g, p->d_cnt_g);
@@ -829,6 +839,46 @@ static se_status sort_and_pack(se_plan *p, const double *pos, const double *F, c
     return SE_OK;
 }
 
+// Neighbour search and radial scalars of the real-space sum, once per cached configuration (se_real.cuh, "Cached pairs"):
+// count the pairs of every target, scan, size the list (one 8-byte read back: the stream is synchronised), fill.
+static se_status build_pair_cache(se_plan *p, cudaStream_t s)
+{
+    const SeConst &c = p->c;
+    const int N = c.N, n = N + 1, nb = (n + SCAN_BLOCK - 1) / SCAN_BLOCK;
+    if (!p->d_pair_start) {
+        se_status st = dev_alloc(p, &p->d_pair_start, (size_t)n);
+        if (st == SE_OK) st = dev_alloc(p, &p->d_pair_cursor, (size_t)n);
+        if (st == SE_OK) st = dev_alloc(p, &p->d_pair_bsum, (size_t)nb + 1);
+        if (st != SE_OK) return st;
+    }
+    const unsigned grid = (unsigned)(c.ncr > 1 ? p->ncell_r : (c.N + 31) / 32);
+    CUDA_TRY(p, cudaMemsetAsync(p->d_pair_cursor, 0, sizeof(int) * (size_t)n, s));
+    k_pairs<false><<<grid, REAL_WARPS * 32, 0, s>>>(c, p->d_rs_pos, p->d_start_r, p->d_pair_cursor, nullptr, nullptr, nullptr, nullptr);
+    k_scan_local<<<nb, SCAN_THREADS, 0, s>>>(p->d_pair_cursor, p->d_pair_start, p->d_pair_bsum, n);
+    k_scan_add<<<nb, SCAN_THREADS, 0, s>>>(p->d_pair_start, p->d_pair_bsum, n, 0x7fffffff, 0x7fffffff, 0);
+    p->last_launches += 3;
+    int total = 0;
+    CUDA_TRY(p, cudaMemcpyAsync(&total, p->d_pair_start + N, sizeof(int), cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(p, cudaStreamSynchronize(s));
+    if (total < 0) return fail(p, SE_ERR_UNSUPPORTED, "build_pair_cache", "more than 2^31 pairs");
+    if ((size_t)total > p->pair_cap) {
+        cudaFree(p->d_pj); cudaFree(p->d_pd);
+        p->d_pj = nullptr; p->d_pd = nullptr; p->pair_cap = 0;
+        const size_t cap = (size_t)total + (size_t)total / 8 + 1024;
+        se_status st = dev_alloc(p, &p->d_pj, cap);
+        if (st == SE_OK) st = dev_alloc(p, &p->d_pd, cap * PAIR_F);
+        if (st != SE_OK) { cudaFree(p->d_pj); p->d_pj = nullptr; cudaGetLastError(); p->err[0] = 0; return SE_OK; }   // no room: products fall back to k_real
+        p->pair_cap = cap;
+    }
+    p->npairs = (size_t)total;
+    CUDA_TRY(p, cudaMemsetAsync(p->d_pair_cursor, 0, sizeof(int) * (size_t)n, s));
+    k_pairs<true><<<grid, REAL_WARPS * 32, 0, s>>>(c, p->d_rs_pos, p->d_start_r, nullptr, p->d_pair_start, p->d_pair_cursor, p->d_pj, p->d_pd);
+    p->last_launches += 1;
+    CUDA_TRY(p, cudaGetLastError());
+    p->have_pairs = true;
+    return SE_OK;
+}
+
 extern "C" se_status se_plan_set_positions(se_plan *p, const double *pos, void *cuda_stream)
 {
     if (!p) return SE_ERR_INVALID_ARG;
@@ -839,6 +889,8 @@ extern "C" se_status se_plan_set_positions(se_plan *p, const double *pos, void *
     const se_status st = sort_and_pack(p, pos, nullptr, nullptr, nullptr, nullptr, (cudaStream_t)cuda_stream);
     if (st != SE_OK) return st;
     p->have_positions = true;
+    p->have_pairs = false;
+    if (p->pair_cache) return build_pair_cache(p, (cudaStream_t)cuda_stream);
     return SE_OK;
 }
 
@@ -889,6 +941,12 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     // stream, alone, so that every stage is timed by itself.
     const bool fork = do_real && do_wave && !timing && stop < 0 && p->real_overlap > 0;
     auto launch_real = [&](cudaStream_t sr) {
+        if (!pos && !comp && p->have_pairs) {          // cached configuration: stream the pair list
+            const unsigned nbc = (unsigned)((c.N + 7) / 8 < 148 * 16 ? (c.N + 7) / 8 : 148 * 16);
+            k_real_cached<<<nbc, 128, 0, sr>>>(c, p->d_pair_start, p->d_pj, p->d_pd, p->d_rs_mom, p->d_rs_orig, p->d_out_real);
+            p->last_launches += 1;
+            return;
+        }
         unsigned nb = (unsigned)(c.ncr > 1 ? p->ncell_r : (c.N + 31) / 32);
         if (sr != s && c.ncr > 1 && p->real_side_ctas > 0 && nb > (unsigned)p->real_side_ctas) nb = (unsigned)p->real_side_ctas;
         if (comp) k_real<true, 1><<<nb, REAL_WARPS * 32, 0, sr>>>(c, p->d_rs_pos, p->d_rs_mom, p->d_rs_orig, p->d_start_r, p->d_out_real, 0);
@@ -1159,7 +1217,11 @@ extern "C" se_status far_mobility_apply_batch(se_plan *p, const double *pos, int
         for (int r = 0; r < nrhs;) {
             const double *m = p->d_mom_b + rs * r;
             double *o = p->d_out_real_b + rs * r;
-            if (nrhs - r >= 4) { k_real<false, 4><<<nb, REAL_WARPS * 32, 0, s>>>(c, p->d_rs_pos, m, p->d_rs_orig, p->d_start_r, o, rs); r += 4; }
+            if (p->have_pairs) {                      // cached pair list: one streaming pass per right-hand side
+                const unsigned nbc = (unsigned)((c.N + 7) / 8 < 148 * 16 ? (c.N + 7) / 8 : 148 * 16);
+                k_real_cached<<<nbc, 128, 0, s>>>(c, p->d_pair_start, p->d_pj, p->d_pd, m, p->d_rs_orig, o);
+                r += 1;
+            } else if (nrhs - r >= 4) { k_real<false, 4><<<nb, REAL_WARPS * 32, 0, s>>>(c, p->d_rs_pos, m, p->d_rs_orig, p->d_start_r, o, rs); r += 4; }
             else if (nrhs - r >= 2) { k_real<false, 2><<<nb, REAL_WARPS * 32, 0, s>>>(c, p->d_rs_pos, m, p->d_rs_orig, p->d_start_r, o, rs); r += 2; }
             else { k_real<false, 1><<<nb, REAL_WARPS * 32, 0, s>>>(c, p->d_rs_pos, m, p->d_rs_orig, p->d_start_r, o, rs); r += 1; }
             launches += 1;

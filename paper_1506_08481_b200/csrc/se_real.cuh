@@ -314,3 +314,177 @@ __global__ void __launch_bounds__(REAL_WARPS * 32, (NR == 1 ? REAL_MINB1 : (NR =
     // a cell without any candidate at all cannot occur (it contains its own targets), so every target was written
     }
 }
+
+// ------------------------------------------------------------------------------------------------------------
+// Cached pairs (the paper prebuilds its real-space matrix once per configuration for the same reason):
+// with the configuration fixed by se_plan_set_positions, the neighbour search and every pair's erfc/exp and radial scalars
+// are done ONCE; every later product only streams the pair list and contracts it with the new moments.
+//   k_pairs<false>  counts the pairs r < r_c of every target (cell order);   k_pairs<true>  fills, per target i, its row
+//   of the list: pj[row + p] = partner (cell order), pd[row * PAIR_F + f * n_i + p] = field f of pair p (row-local
+//   structure of arrays: x, y, z, then the 17 scalars of PairS<false>), n_i = pairs of the target.
+//   k_real_cached   half a warp per target: lanes stride over the row (coalesced field loads), gather the partner's
+//   moments, apply, reduce over the 16 lanes.
+// Same scan machinery as k_real (27 staged neighbour cells or all pairs, chunks of REAL_STAGE candidates).
+// ------------------------------------------------------------------------------------------------------------
+#define PAIR_F 20
+
+template <bool FILL>
+__global__ void __launch_bounds__(REAL_WARPS * 32) k_pairs(SeConst c, const double4 *__restrict__ rs_pos, const int *__restrict__ start_r,
+                                                           int *__restrict__ cnt,              // [N] pairs per target (count mode: written)
+                                                           const int *__restrict__ row_start,  // [N+1] (fill mode)
+                                                           int *__restrict__ cursor,           // [N] pairs of the target written so far (fill mode; zeroed)
+                                                           int *__restrict__ pj, double *__restrict__ pd)
+{
+    __shared__ double4 cand[REAL_STAGE];
+    __shared__ int cand_j[REAL_STAGE];
+    __shared__ double4 qd[REAL_WARPS][REAL_QCAP];
+    __shared__ int qj[REAL_WARPS][REAL_QCAP];
+    __shared__ int seg_s[27], seg_o[28];
+    const int wl = threadIdx.x >> 5, lane = threadIdx.x & 31, tid = threadIdx.x;
+    const int nc = c.ncr;
+    const double invL = 1.0 / c.L;
+    const int nitems = nc > 1 ? nc * nc * nc : (int)gridDim.x;
+    for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
+    __syncthreads();
+    int t0, t1, nsegs;
+    if (nc > 1) {
+        const int cell = item;
+        t0 = start_r[cell]; t1 = start_r[cell + 1];
+        if (t0 == t1) continue;
+        nsegs = 27;
+        if (tid < 27) {
+            const int cz = cell % nc, cy = (cell / nc) % nc, cx = cell / (nc * nc);
+            const int nx = se_mod(cx + tid / 9 - 1, nc), ny = se_mod(cy + (tid / 3) % 3 - 1, nc), nz = se_mod(cz + tid % 3 - 1, nc);
+            const int nb = (nx * nc + ny) * nc + nz;
+            seg_s[tid] = start_r[nb];
+            seg_o[tid + 1] = start_r[nb + 1] - start_r[nb];
+        }
+    } else {
+        const int per = (c.N + gridDim.x - 1) / gridDim.x;
+        t0 = item * per; t1 = min(t0 + per, c.N);
+        if (t0 >= t1) continue;
+        nsegs = 1;
+        if (tid == 0) { seg_s[0] = 0; seg_o[1] = c.N; }
+    }
+    __syncthreads();
+    if (tid == 0) {
+        int run = 0;
+        seg_o[0] = 0;
+        for (int k = 0; k < nsegs; ++k) { const int n = seg_o[k + 1]; seg_o[k + 1] = run + n; run += n; }
+    }
+    __syncthreads();
+    const int ncand = seg_o[nsegs];
+    const int rounds = (t1 - t0 + REAL_WARPS - 1) / REAL_WARPS;
+    for (int base = 0; base < ncand; base += REAL_STAGE) {
+        const int nst = min(REAL_STAGE, ncand - base);
+        __syncthreads();
+        for (int q = tid; q < nst; q += REAL_WARPS * 32) {
+            const int f = base + q;
+            int k = 0;
+            while (k + 1 < nsegs && seg_o[k + 1] <= f) ++k;
+            const int j = seg_s[k] + (f - seg_o[k]);
+            cand[q] = rs_pos[j];
+            cand_j[q] = j;
+        }
+        __syncthreads();
+        for (int rd = 0; rd < rounds; ++rd) {
+            const int i = t0 + rd * REAL_WARPS + wl;
+            if (i >= t1) break;
+            const double4 pi = rs_pos[i];
+            const double cFi = pi.w * pi.w * (1.0 / 6.0), cSi = pi.w * pi.w * 0.1;
+            int done = 0, row = 0, ni = 0;
+            if (FILL) { row = row_start[i]; ni = row_start[i + 1] - row; done = cursor[i]; }
+            auto emit = [&](const double4 &d, int jj, int p) {          // pair p of the row
+                const PairS<false> o = pair_scalars<false>(c, d.x * d.x + d.y * d.y + d.z * d.z, cFi, cSi, d.w);
+                pj[row + p] = jj;
+                double *f = pd + (size_t)row * PAIR_F + p;
+                const double v[PAIR_F] = { d.x, d.y, d.z, o.uf_a, o.uf_b, o.ut, o.us_a, o.us_b, o.of, o.ot_a, o.ot_b, o.os,
+                                           o.a1, o.a2, o.a3, o.a4, o.ef2, o.ef3, o.es3, o.es4 };
+#pragma unroll
+                for (int q = 0; q < PAIR_F; ++q) f[(size_t)q * ni] = v[q];
+            };
+            int qn = 0;
+            for (int qb = 0; qb < nst; qb += 32) {
+                const int q = qb + lane;
+                bool hit = false;
+                double dx = 0, dy = 0, dz = 0, aj = 0;
+                int j = -1;
+                if (q < nst) {
+                    const double4 pjv = cand[q];
+                    j = cand_j[q];
+                    dx = pi.x - pjv.x; dy = pi.y - pjv.y; dz = pi.z - pjv.z;
+                    dx -= c.L * rint(dx * invL); dy -= c.L * rint(dy * invL); dz -= c.L * rint(dz * invL);
+                    const double r2 = dx * dx + dy * dy + dz * dz;
+                    hit = (j != i) && (r2 < c.rc2) && (r2 > 0.0);
+                    aj = pjv.w;
+                }
+                const unsigned mask = __ballot_sync(0xffffffffu, hit);
+                if (!FILL) { qn += __popc(mask); continue; }
+                if (hit) {
+                    const int slot = qn + __popc(mask & ((1u << lane) - 1u));
+                    qd[wl][slot] = make_double4(dx, dy, dz, aj);
+                    qj[wl][slot] = j;
+                }
+                qn += __popc(mask);
+                __syncwarp();
+                if (qn >= 32) {
+                    emit(qd[wl][qn - 32 + lane], qj[wl][qn - 32 + lane], done + lane);
+                    done += 32;
+                    qn -= 32;
+                    __syncwarp();
+                }
+            }
+            if (FILL) {
+                if (lane < qn) emit(qd[wl][lane], qj[wl][lane], done + lane);
+                done += qn;
+                __syncwarp();
+                if (lane == 0) cursor[i] = done;
+            } else if (lane == 0) {
+                if (base == 0) cnt[i] = qn; else cnt[i] += qn;
+            }
+        }
+    }
+    }
+}
+
+// out_real[rs_orig[i]][0..10] = k0 * sum over the cached pairs of target i (cell order) applied to the moments rs_mom.
+__global__ void __launch_bounds__(128) k_real_cached(SeConst c, const int *__restrict__ row_start, const int *__restrict__ pj,
+                                                     const double *__restrict__ pd, const double *__restrict__ rs_mom,
+                                                     const int *__restrict__ rs_orig, double *__restrict__ out_real)
+{
+    const int hl = threadIdx.x & 15;
+    const int nhw = (int)(gridDim.x * blockDim.x) >> 4;
+    for (int i0 = (int)(blockIdx.x * blockDim.x + threadIdx.x) >> 4; ; i0 += nhw) {
+        // the two halves of a warp walk in step (shuffles below are warp-wide); a half past the end idles
+        const bool live = i0 < c.N;
+        if (!__any_sync(0xffffffffu, live)) break;
+        const int i = live ? i0 : c.N - 1;
+        const int row = row_start[i], n = live ? row_start[i + 1] - row : 0;
+        const double *__restrict__ f = pd + (size_t)row * PAIR_F;
+        double acc[12];
+#pragma unroll
+        for (int k = 0; k < 12; ++k) acc[k] = 0.0;
+        for (int p = hl; p < n; p += 16) {
+            PairS<false> o;
+            const double x = f[p], y = f[(size_t)n + p], z = f[2 * (size_t)n + p];
+            o.uf_a = f[3 * (size_t)n + p]; o.uf_b = f[4 * (size_t)n + p]; o.ut = f[5 * (size_t)n + p]; o.us_a = f[6 * (size_t)n + p];
+            o.us_b = f[7 * (size_t)n + p]; o.of = f[8 * (size_t)n + p]; o.ot_a = f[9 * (size_t)n + p]; o.ot_b = f[10 * (size_t)n + p];
+            o.os = f[11 * (size_t)n + p]; o.a1 = f[12 * (size_t)n + p]; o.a2 = f[13 * (size_t)n + p]; o.a3 = f[14 * (size_t)n + p];
+            o.a4 = f[15 * (size_t)n + p]; o.ef2 = f[16 * (size_t)n + p]; o.ef3 = f[17 * (size_t)n + p]; o.es3 = f[18 * (size_t)n + p];
+            o.es4 = f[19 * (size_t)n + p];
+            pair_apply<false>(o, x, y, z, 0.0, rs_mom + 12 * (size_t)pj[row + p], acc);
+        }
+#pragma unroll
+        for (int k = 0; k < 11; ++k) {
+            double v = acc[k];
+#pragma unroll
+            for (int s = 8; s > 0; s >>= 1) v += __shfl_xor_sync(0xffffffffu, v, s);
+            acc[k] = v;
+        }
+        if (live && hl == 0) {
+            double *o = out_real + 12 * (size_t)rs_orig[i];
+#pragma unroll
+            for (int k = 0; k < 11; ++k) o[k] = c.k0 * acc[k];
+        }
+    }
+}
