@@ -589,3 +589,36 @@ def test_plan_owned_cuda_graph(pk, oracle, workloads):
     assert r.plan.last_launch_count() == n_graph - 3    # a1 is one kernel instead of four, also in the graph
     r.plan.set_option(pk.SE_OPT_GRAPH, 0)
     _check_blocks(go(None, F3), ref2, TOL)
+
+
+def test_pair_cache_dense_all_pairs_and_single_particle(pk, oracle, workloads):
+    """SE_OPT_PAIR_CACHE on the branches c1-c5 never reach: candidate chunks beyond the first (rows filled over several
+    chunks), the all-pairs path, and a system without any pair; with the cache switched off the products agree."""
+    import torch
+    import workloads as W
+    cases = [workloads.make_uniform_system(1, 3000, 0.3, 64, 12, 1.0 / 3.001), workloads.make_uniform_system(1, 3000, 0.3, 64, 12, 0.45)]
+    sysm = workloads.random_small_system(7, 12, 9.0)
+    cases.append(W.Workload(name="one", N=1, L=9.0, radii=sysm["radii"][:1], pos=sysm["pos"][:1], F=sysm["F"][:1], T=sysm["T"][:1],
+                            S=sysm["S"][:1], xi=0.9, rc=4.5, M=24, P=10, m=0.0))
+    for wl in cases:
+        r = Runner(pk, wl)
+        r.plan.set_positions(r.pos)
+        r.plan.set_flags(pk.SE_SKIP_WAVE | pk.SE_SKIP_SELF | pk.SE_SKIP_ONEBODY)
+        r.plan.apply(None, r.F, r.T, r.S, r.U, r.W, r.E)
+        torch.cuda.synchronize()
+        got = (r.U.cpu().numpy().copy(), r.W.cpu().numpy().copy(), r.E.cpu().numpy().copy())
+        if wl.N > 1:
+            _check_blocks(got, r.oracle(oracle, parts=oracle.PART_REAL), TOL_STAGE)
+        else:
+            assert all(np.abs(x).max() == 0.0 for x in got)
+        r.plan.set_option(pk.SE_OPT_PAIR_CACHE, 0)
+        r.plan.apply(None, r.F, r.T, r.S, r.U, r.W, r.E)
+        torch.cuda.synchronize()
+        for a, b in zip((r.U.cpu().numpy(), r.W.cpu().numpy(), r.E.cpu().numpy()), got):
+            assert np.abs(a - b).max() <= 1e-13 * max(1.0, np.abs(b).max())
+        r.plan.set_flags(0)
+        r.plan.set_option(pk.SE_OPT_PAIR_CACHE, 1)
+        r.plan.set_positions(r.pos)
+        r.plan.apply(None, r.F, r.T, r.S, r.U, r.W, r.E)
+        torch.cuda.synchronize()
+        _check_blocks((r.U.cpu().numpy(), r.W.cpu().numpy(), r.E.cpu().numpy()), r.oracle(oracle), TOL)
