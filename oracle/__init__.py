@@ -51,6 +51,10 @@ def lib():
         L.o1_apply.argtypes = [_I64, _D, _P, _P, _D, _D, _INT, _INT, _U, _P, _P, _P, _P, _P, _P, _P, _P]
         L.o2_apply.restype = _INT
         L.o2_apply.argtypes = [_I64, _D, _P, _P, _D, _D, _INT, _INT, _D, _D, _U, _P, _P, _P, _P, _P, _P, _P, _P, _P, _P]
+        L.o1_apply_sheared.restype = _INT
+        L.o1_apply_sheared.argtypes = [_I64, _D, _D, _P, _P, _D, _D, _INT, _INT, _U, _P, _P, _P, _P, _P, _P, _P, _P]
+        L.o2_apply_sheared.restype = _INT
+        L.o2_apply_sheared.argtypes = [_I64, _D, _D, _P, _P, _D, _D, _INT, _INT, _D, _D, _U, _P, _P, _P, _P, _P, _P, _P, _P, _P, _P]
         L.o2_real_targets.restype = _INT
         L.o2_real_targets.argtypes = [_I64, _D, _P, _P, _D, _D, _D, _P, _P, _P, _P, _I64, _P, _P, _P, _P, _P]
         L.oracle_radial.restype = _D
@@ -133,6 +137,60 @@ def o2_apply(pos, radii, L, xi, rc, M, P, F, T, S, s=None, m=None, eta0=1.0, par
                            _ptr(gH), _ptr(gO))
     if rcode:
         raise RuntimeError(f"o2_apply status {rcode}")
+    out = dict(U=U, Omega=W, E=E, s_out=so)
+    if want_grids:
+        out["gridH"], out["gridOut"] = gH, gO
+    return out
+
+
+def o1_apply_sheared(pos, radii, L, gamma, xi, F, T, S, s=None, eta0=1.0, nimg=3, kmax=12, parts=PART_ALL):
+    """Direct Ewald sum on the sheared lattice a1 = (L,0,0), a2 = (gamma L, L, 0), a3 = (0,0,L).  Returns (U, Omega, E, s_out)."""
+    N = len(radii)
+    pos, radii, F, T, S = _c(pos, (N, 3)), _c(radii, (N,)), _c(F, (N, 3)), _c(T, (N, 3)), _c(S, (N, 5))
+    s_in = None if s is None else _c(s, (N,))
+    U, W, E, so = np.zeros((N, 3)), np.zeros((N, 3)), np.zeros((N, 5)), np.zeros(N)
+    rc = lib().o1_apply_sheared(N, L, gamma, _ptr(pos), _ptr(radii), xi, eta0, nimg, kmax, parts,
+                                _ptr(F), _ptr(T), _ptr(S), _ptr(s_in), _ptr(U), _ptr(W), _ptr(E), _ptr(so))
+    if rc:
+        raise RuntimeError(f"o1_apply_sheared status {rc}")
+    return U, W, E, so
+
+
+def o1_matrix_sheared(pos, radii, L, gamma, xi, eta0=1.0, nimg=3, kmax=12, parts=PART_ALL):
+    """Assembled [11N, 11N] grand mobility (stored basis, no pressure row/column) on the sheared lattice."""
+    N = len(radii)
+    A = np.zeros((11 * N, 11 * N))
+    for j in range(N):
+        for c in range(11):
+            F, T, S = np.zeros((N, 3)), np.zeros((N, 3)), np.zeros((N, 5))
+            if c < 3:
+                F[j, c] = 1.0
+            elif c < 6:
+                T[j, c - 3] = 1.0
+            else:
+                S[j, c - 6] = 1.0
+            U, W, E, _ = o1_apply_sheared(pos, radii, L, gamma, xi, F, T, S, None, eta0, nimg, kmax, parts)
+            A[:, 11 * j + c] = np.concatenate([U, W, E], axis=1).reshape(-1)
+    return A
+
+
+def o2_apply_sheared(pos, radii, L, gamma, xi, rc, M, P, F, T, S, s=None, m=None, eta0=1.0, parts=PART_ALL, want_grids=False):
+    """Step-by-step Spectral Ewald product on the sheared lattice.  Returns dict(U, Omega, E, s_out[, gridH, gridOut])."""
+    N = len(radii)
+    pos, radii, F, T, S = _c(pos, (N, 3)), _c(radii, (N,)), _c(F, (N, 3)), _c(T, (N, 3)), _c(S, (N, 5))
+    s_in = None if s is None else _c(s, (N,))
+    if m is None:
+        m = float(np.sqrt(np.pi * P))
+    U, W, E = np.zeros((N, 3)), np.zeros((N, 3)), np.zeros((N, 5))
+    so = None if s is None else np.zeros(N)
+    gH = gO = None
+    if want_grids:
+        gH = np.zeros((4 if s is not None else 3, M, M, M))
+        gO = np.zeros((7 if s is not None else 6, M, M, M))
+    rcode = lib().o2_apply_sheared(N, L, gamma, _ptr(pos), _ptr(radii), xi, rc, M, P, m, eta0, parts,
+                                   _ptr(F), _ptr(T), _ptr(S), _ptr(s_in), _ptr(U), _ptr(W), _ptr(E), _ptr(so), _ptr(gH), _ptr(gO))
+    if rcode:
+        raise RuntimeError(f"o2_apply_sheared status {rcode}")
     out = dict(U=U, Omega=W, E=E, s_out=so)
     if want_grids:
         out["gridH"], out["gridOut"] = gH, gO

@@ -768,3 +768,252 @@ void oracle_se_constants(double L, double xi, int M, int P, double m, double out
     const se_consts c = se_constants(L, xi, M, P, m);
     out[0] = c.Delta; out[1] = c.eta_se; out[2] = c.alpha; out[3] = c.gnorm;
 }
+
+/* ================================================================================================
+ * Sheared (Lees-Edwards) lattice, SURVEY 8f-2.  PAPER.md Sec. 3.1 L245-253 (fractional coordinates t, r = A.t,
+ * k = B.q, k^2 = q.B^T.B.q), Eq. 39-45 (the Gaussian h(t) of Eq. 41 is ISOTROPIC in the fractional coordinate; the
+ * lattice enters through the metric B^T.B of the derivatives and through g1(B.q)), L300-302 (simple shear:
+ * a1 = (L,0,0), a2 = (gamma L, L, 0), a3 = (0,0,L), Eq. 48), L501 (same accuracy at gamma = 0.5).
+ * New functions; the cubic O1 / O2 above are left as they were pinned.  For gamma = 0 they compute the same numbers.
+ *
+ *   A = L [[1, gamma, 0], [0, 1, 0], [0, 0, 1]]  (columns a1, a2, a3),  V = L^3,
+ *   lattice images  R_n = A.n = L (n0 + gamma n1, n1, n2),
+ *   wave vectors    k = 2 pi A^{-T}.j = (2 pi/L) (j0, j1 - gamma j0, j2),    k.r = 2 pi j.t.
+ * ============================================================================================== */
+
+/* O1 under shear: the definition.  Image and mode cubes are widened along the sheared directions so that they still
+ * contain the spheres the cubic version sums over. */
+int o1_apply_sheared(int64_t N, double L, double gamma, const double *pos, const double *rad, double xi, double eta0,
+                     int nimg, int kmax, unsigned parts,
+                     const double *F, const double *T, const double *S5, const double *s_in,
+                     double *U, double *W, double *E5, double *s_out)
+{
+    acc_t *acc = (acc_t *)calloc((size_t)N, sizeof(acc_t));
+    if (!acc) return 1;
+    const double V = L * L * L;
+    const int nx = nimg + (int)ceil(fabs(gamma) * nimg), ky = kmax + (int)ceil(fabs(gamma) * kmax);
+
+    if (parts & PART_REAL) {
+        radtab rt; radtab_build(xi, &rt);
+        #pragma omp parallel for schedule(dynamic)
+        for (int64_t i = 0; i < N; ++i)
+            for (int64_t j = 0; j < N; ++j) {
+                double S[3][3]; s5_to_33(S5 + 5 * j, S);
+                for (int n0 = -nx; n0 <= nx; ++n0) for (int n1 = -nimg; n1 <= nimg; ++n1) for (int n2 = -nimg; n2 <= nimg; ++n2) {
+                    if (i == j && n0 == 0 && n1 == 0 && n2 == 0) continue;
+                    const double x[3] = { pos[3 * i] - pos[3 * j] - L * (n0 + gamma * n1), pos[3 * i + 1] - pos[3 * j + 1] - L * n1,
+                                          pos[3 * i + 2] - pos[3 * j + 2] - L * n2 };
+                    pair_real(&rt, x, rad[i], rad[j], eta0, F + 3 * j, T + 3 * j, S, s_in ? s_in[j] : 0.0, &acc[i]);
+                }
+            }
+    }
+
+    if (parts & PART_WAVE) {
+        for (int j0 = -kmax; j0 <= kmax; ++j0) for (int j1 = -ky; j1 <= ky; ++j1) for (int j2 = -kmax; j2 <= kmax; ++j2) {
+            if (j0 == 0 && j1 == 0 && j2 == 0) continue;
+            const double k[3] = { 2.0 * M_PI * j0 / L, 2.0 * M_PI * (j1 - gamma * j0) / L, 2.0 * M_PI * j2 / L };
+            const double k2 = k[0] * k[0] + k[1] * k[1] + k[2] * k[2];
+            double complex f[3] = { 0, 0, 0 }, sk = 0;
+            for (int64_t j = 0; j < N; ++j) {
+                double S[3][3]; s5_to_33(S5 + 5 * j, S);
+                const double cF = rad[j] * rad[j] / 6.0, cS = rad[j] * rad[j] / 10.0;
+                const double *Fj = F + 3 * j, *Tj = T + 3 * j;
+                const double complex ph = cexp(I * (k[0] * pos[3 * j] + k[1] * pos[3 * j + 1] + k[2] * pos[3 * j + 2]));
+                const double Txk[3] = { Tj[1] * k[2] - Tj[2] * k[1], Tj[2] * k[0] - Tj[0] * k[2], Tj[0] * k[1] - Tj[1] * k[0] };
+                for (int a = 0; a < 3; ++a) {
+                    const double Sk = S[a][0] * k[0] + S[a][1] * k[1] + S[a][2] * k[2];
+                    f[a] += ph * ((1.0 - cF * k2) * Fj[a] + 0.5 * I * Txk[a] + I * (1.0 - cS * k2) * Sk);
+                }
+                if (s_in) sk += ph * s_in[j];
+            }
+            const double ew = exp(-k2 / (4.0 * xi * xi));
+            const double hk = (1.0 + k2 / (4.0 * xi * xi)) * ew;
+            const double complex kf = k[0] * f[0] + k[1] * f[1] + k[2] * f[2];
+            double complex v[3];
+            for (int a = 0; a < 3; ++a)
+                v[a] = hk / (eta0 * V * k2) * (f[a] - k[a] * kf / k2) + I * k[a] / (4.0 * eta0 * V * k2) * ew * sk;
+            const double complex pk = I * kf / (V * k2) * ew;
+            for (int64_t i = 0; i < N; ++i) {
+                const double cF = rad[i] * rad[i] / 6.0, cS = rad[i] * rad[i] / 10.0;
+                const double complex ph = cexp(-I * (k[0] * pos[3 * i] + k[1] * pos[3 * i + 1] + k[2] * pos[3 * i + 2]));
+                double complex g[3] = { -I * k[0], -I * k[1], -I * k[2] };
+                for (int a = 0; a < 3; ++a) acc[i].U[a] += creal((1.0 - cF * k2) * ph * v[a]);
+                acc[i].W[0] += creal(0.5 * ph * (g[1] * v[2] - g[2] * v[1]));
+                acc[i].W[1] += creal(0.5 * ph * (g[2] * v[0] - g[0] * v[2]));
+                acc[i].W[2] += creal(0.5 * ph * (g[0] * v[1] - g[1] * v[0]));
+                for (int a = 0; a < 3; ++a) for (int b = 0; b < 3; ++b)
+                    acc[i].E[a][b] += creal((1.0 - cS * k2) * ph * 0.5 * (g[a] * v[b] + g[b] * v[a]));
+                acc[i].p += creal(ph * pk);
+            }
+        }
+    }
+    add_self_onebody(acc, N, rad, xi, eta0, parts, F, T, S5);
+    acc_finish(acc, N, rad, U, W, E5, s_out);
+    free(acc);
+    return 0;
+}
+
+/* Minimum image on the sheared lattice (r_c <= L/2: at most one image of a pair lies within r_c, and it is this one):
+ * the y and z images are fixed by rounding, then the x image given the shift gamma L of the chosen y image. */
+static void min_image_sheared(const double *ri, const double *rj, double L, double gamma, double x[3])
+{
+    const double dy = ri[1] - rj[1], dz = ri[2] - rj[2];
+    const double n1 = nearbyint(dy / L);
+    const double dx = (ri[0] - rj[0]) - gamma * L * n1;
+    x[0] = dx - L * nearbyint(dx / L);
+    x[1] = dy - L * n1;
+    x[2] = dz - L * nearbyint(dz / L);
+}
+
+/* O2 under shear, step by step.  Differences from o2_apply:
+ *   2. fractional coordinates t = A^{-1} r = ((x - gamma y)/L, y/L, z/L), wrapped to [0,1); u_d = t_d M; same support rule.
+ *   3. grid offsets d_d = (n_d - u_d) Delta (fractional offset times L); the Gaussian is isotropic in them (Eq. 41),
+ *      gam = (alpha/pi)^{3/2} e^{-alpha |d|^2}; its physical gradient is grad gam = -2 alpha D gam with the metric vector
+ *          D = L^2 A^{-T}A^{-1} (r - r_j) = (d0, d1 - gamma d0, d2),    Mt = L^2 A^{-T}A^{-1} = [[1,-gamma,0],[-gamma,1+gamma^2,0],[0,0,1]],
+ *      lap gam = (4 alpha^2 D.D - 2 alpha tr Mt) gam,  grad lap gam = [8 alpha^2 Mt.D - 2 alpha D (4 alpha^2 D.D - 2 alpha tr Mt)] gam
+ *      (the braces of Eq. 48: tr Mt = 3 + gamma^2, D.D = (1+gamma^2) d0^2 + d1^2 + d2^2 - 2 gamma d0 d1), so
+ *          H = gam { F [1 + cF (4 al^2 D.D - 2 al trMt)] - al D x T + 2 al (S.D) [1 + cS (4 al^2 D.D - 2 al trMt)] - 8 al^2 cS S.(Mt.D) }
+ *      = F (1 + cF lap) gam + (1/2) grad gam x T - S.grad (1 + cS lap) gam, as in the cubic case.
+ *   5. k = (2 pi/L)(j0, j1 - gamma j0, j2) in the Green's function, the projector and w = -k^2 u; the deconvolution of the two
+ *      Gaussians uses the FRACTIONAL wave number: e^{+eta_se kq^2/4xi^2}, kq^2 = (2 pi/L)^2 |j|^2 (theta q^2 of Eq. 39, 43).
+ *   7. gather with D in place of d:  Omega = D^3 sum al gam D x u~,  E = D^3 sum al gam (D q + q D).
+ *   8. real part: all pairs, sheared minimum image, r^2 < r_c^2 (brute force: this oracle is for N <= ~1e4).         */
+int o2_apply_sheared(int64_t N, double L, double gamma, const double *pos, const double *rad, double xi, double rc,
+                     int M, int P, double m, double eta0, unsigned parts,
+                     const double *F, const double *T, const double *S5, const double *s_in,
+                     double *U, double *W, double *E5, double *s_out, double *gridH, double *gridOut)
+{
+    if (N < 1 || M < 2 || (M % 2) || P < 2 || P > M || !(rc > 0.0) || rc > 0.5 * L) return 2;
+    acc_t *acc = (acc_t *)calloc((size_t)N, sizeof(acc_t));
+    double *uu = (double *)malloc(sizeof(double) * 3 * (size_t)N);              /* u_d = wrapped fractional coordinate * M */
+    if (!acc || !uu) { free(acc); free(uu); return 1; }
+    const double invL = 1.0 / L;
+    for (int64_t i = 0; i < N; ++i) {
+        const double t[3] = { (pos[3 * i] - gamma * pos[3 * i + 1]) * invL, pos[3 * i + 1] * invL, pos[3 * i + 2] * invL };
+        for (int d = 0; d < 3; ++d) uu[3 * i + d] = (t[d] - floor(t[d])) * (double)M;
+    }
+    int status = 0;
+
+    if (parts & PART_REAL) {
+        radtab rt; radtab_build(xi, &rt);
+        #pragma omp parallel for schedule(dynamic, 16)
+        for (int64_t i = 0; i < N; ++i)
+            for (int64_t j = 0; j < N; ++j) {
+                if (j == i) continue;
+                double x[3]; min_image_sheared(pos + 3 * i, pos + 3 * j, L, gamma, x);
+                const double r2 = x[0] * x[0] + x[1] * x[1] + x[2] * x[2];
+                if (!(r2 < rc * rc) || r2 == 0.0) continue;
+                double S[3][3]; s5_to_33(S5 + 5 * j, S);
+                pair_real(&rt, x, rad[i], rad[j], eta0, F + 3 * j, T + 3 * j, S, s_in ? s_in[j] : 0.0, &acc[i]);
+            }
+    }
+
+    if (parts & PART_WAVE) {
+        const se_consts c = se_constants(L, xi, M, P, m);
+        const double al = c.alpha, D = c.Delta, V = L * L * L, trM = 3.0 + gamma * gamma;
+        const int64_t G = (int64_t)M * M * M;
+        const int nin = s_in ? 4 : 3, nout = s_out ? 7 : 6;
+        double *H = (double *)calloc((size_t)(nin * G), sizeof(double));
+        double complex *Hk = (double complex *)malloc(sizeof(double complex) * (size_t)(nin * G));
+        double *Gr = (double *)malloc(sizeof(double) * (size_t)(nout * G));
+        double complex *work = (double complex *)malloc(sizeof(double complex) * (size_t)G);
+        if (!H || !Hk || !Gr || !work) status = 1;
+
+        if (!status) {
+            for (int64_t j = 0; j < N; ++j) {                                         /* step 3 */
+                double S[3][3]; s5_to_33(S5 + 5 * j, S);
+                const double cF = rad[j] * rad[j] / 6.0, cS = rad[j] * rad[j] / 10.0;
+                const double *Fj = F + 3 * j, *Tj = T + 3 * j, *u = uu + 3 * j;
+                int n0[3];
+                for (int d = 0; d < 3; ++d) n0[d] = support_start(u[d], P);
+                for (int a0 = 0; a0 < P; ++a0) for (int a1 = 0; a1 < P; ++a1) for (int a2 = 0; a2 < P; ++a2) {
+                    const double d[3] = { ((n0[0] + a0) - u[0]) * D, ((n0[1] + a1) - u[1]) * D, ((n0[2] + a2) - u[2]) * D };
+                    const double gam = c.gnorm * exp(-al * (d[0] * d[0] + d[1] * d[1] + d[2] * d[2]));
+                    const double Dv[3] = { d[0], d[1] - gamma * d[0], d[2] };
+                    const double MD[3] = { Dv[0] - gamma * Dv[1], -gamma * Dv[0] + (1.0 + gamma * gamma) * Dv[1], Dv[2] };
+                    const double DD = Dv[0] * Dv[0] + Dv[1] * Dv[1] + Dv[2] * Dv[2];
+                    const double lapf = 4.0 * al * al * DD - 2.0 * al * trM;
+                    const double DxT[3] = { Dv[1] * Tj[2] - Dv[2] * Tj[1], Dv[2] * Tj[0] - Dv[0] * Tj[2], Dv[0] * Tj[1] - Dv[1] * Tj[0] };
+                    const int64_t idx = gidx(M, n0[0] + a0, n0[1] + a1, n0[2] + a2);
+                    for (int a = 0; a < 3; ++a) {
+                        const double SD = S[a][0] * Dv[0] + S[a][1] * Dv[1] + S[a][2] * Dv[2];
+                        const double SMD = S[a][0] * MD[0] + S[a][1] * MD[1] + S[a][2] * MD[2];
+                        H[a * G + idx] += gam * (Fj[a] * (1.0 + cF * lapf) - al * DxT[a] + 2.0 * al * SD * (1.0 + cS * lapf)
+                                                 - 8.0 * al * al * cS * SMD);
+                    }
+                    if (s_in) H[3 * G + idx] += gam * s_in[j];
+                }
+            }
+            if (gridH) memcpy(gridH, H, sizeof(double) * (size_t)(nin * G));
+            for (int64_t q = 0; q < nin * G; ++q) Hk[q] = H[q];                       /* step 4: e^{+2 pi i j.t_n} */
+            for (int a = 0; a < nin && !status; ++a) status = fft3d(Hk + a * G, M, +1);
+        }
+
+        for (int og = 0; og < nout && !status; ++og) {                               /* steps 5-6 */
+            #pragma omp parallel for
+            for (int i0 = 0; i0 < M; ++i0) for (int i1 = 0; i1 < M; ++i1) for (int i2 = 0; i2 < M; ++i2) {
+                const int j0 = i0 < M / 2 ? i0 : i0 - M, j1 = i1 < M / 2 ? i1 : i1 - M, j2 = i2 < M / 2 ? i2 : i2 - M;
+                const int64_t q = ((int64_t)i0 * M + i1) * M + i2;
+                if ((j0 == 0 && j1 == 0 && j2 == 0) || j0 == -M / 2 || j1 == -M / 2 || j2 == -M / 2) { work[q] = 0; continue; }
+                const double k[3] = { 2.0 * M_PI * j0 / L, 2.0 * M_PI * (j1 - gamma * j0) / L, 2.0 * M_PI * j2 / L };
+                const double k2 = k[0] * k[0] + k[1] * k[1] + k[2] * k[2];
+                const double kq2 = (2.0 * M_PI / L) * (2.0 * M_PI / L) * ((double)j0 * j0 + (double)j1 * j1 + (double)j2 * j2);
+                const double dec = exp(-k2 / (4.0 * xi * xi) + c.eta_se * kq2 / (4.0 * xi * xi));
+                const double sc = D * D * D / (eta0 * V) * (1.0 + k2 / (4.0 * xi * xi)) * dec / k2;
+                const double complex h[3] = { Hk[q], Hk[G + q], Hk[2 * G + q] };
+                const double complex kh = k[0] * h[0] + k[1] * h[1] + k[2] * h[2];
+                if (og < 6) {
+                    const int a = og % 3;
+                    double complex uk = sc * (h[a] - k[a] * kh / k2);
+                    if (s_in) uk += D * D * D / (4.0 * eta0 * V) * (I * k[a] / k2) * dec * Hk[3 * G + q];
+                    work[q] = (og < 3) ? uk : -k2 * uk;
+                } else {
+                    work[q] = D * D * D / V * (I * kh / k2) * dec;
+                }
+            }
+            status = fft3d(work, M, -1);
+            if (!status) for (int64_t q = 0; q < G; ++q) Gr[og * G + q] = creal(work[q]);
+        }
+        if (!status && gridOut) memcpy(gridOut, Gr, sizeof(double) * (size_t)(nout * G));
+
+        if (!status) {                                                                /* step 7 */
+            const double D3 = D * D * D;
+            #pragma omp parallel for schedule(static)
+            for (int64_t i = 0; i < N; ++i) {
+                const double cF = rad[i] * rad[i] / 6.0, cS = rad[i] * rad[i] / 10.0;
+                const double *u = uu + 3 * i;
+                int n0[3];
+                for (int d = 0; d < 3; ++d) n0[d] = support_start(u[d], P);
+                double aU[3] = { 0, 0, 0 }, aW[3] = { 0, 0, 0 }, aE[3][3] = { { 0 } }, ap = 0.0;
+                for (int a0 = 0; a0 < P; ++a0) for (int a1 = 0; a1 < P; ++a1) for (int a2 = 0; a2 < P; ++a2) {
+                    const double d[3] = { ((n0[0] + a0) - u[0]) * D, ((n0[1] + a1) - u[1]) * D, ((n0[2] + a2) - u[2]) * D };
+                    const double gam = c.gnorm * exp(-al * (d[0] * d[0] + d[1] * d[1] + d[2] * d[2]));
+                    const double Dv[3] = { d[0], d[1] - gamma * d[0], d[2] };
+                    const int64_t idx = gidx(M, n0[0] + a0, n0[1] + a1, n0[2] + a2);
+                    const double ut[3] = { Gr[idx], Gr[G + idx], Gr[2 * G + idx] };
+                    const double wt[3] = { Gr[3 * G + idx], Gr[4 * G + idx], Gr[5 * G + idx] };
+                    double q[3];
+                    for (int a = 0; a < 3; ++a) { aU[a] += gam * (ut[a] + cF * wt[a]); q[a] = ut[a] + cS * wt[a]; }
+                    aW[0] += al * gam * (Dv[1] * ut[2] - Dv[2] * ut[1]);
+                    aW[1] += al * gam * (Dv[2] * ut[0] - Dv[0] * ut[2]);
+                    aW[2] += al * gam * (Dv[0] * ut[1] - Dv[1] * ut[0]);
+                    for (int a = 0; a < 3; ++a) for (int b = 0; b < 3; ++b) aE[a][b] += al * gam * (Dv[a] * q[b] + q[a] * Dv[b]);
+                    if (s_out) ap += gam * Gr[6 * G + idx];
+                }
+                for (int a = 0; a < 3; ++a) {
+                    acc[i].U[a] += D3 * aU[a]; acc[i].W[a] += D3 * aW[a];
+                    for (int b = 0; b < 3; ++b) acc[i].E[a][b] += D3 * aE[a][b];
+                }
+                acc[i].p += D3 * ap;
+            }
+        }
+        free(H); free(Hk); free(Gr); free(work);
+    }
+
+    if (!status) {
+        add_self_onebody(acc, N, rad, xi, eta0, parts, F, T, S5);
+        acc_finish(acc, N, rad, U, W, E5, s_out);
+    }
+    free(acc); free(uu);
+    return status;
+}
