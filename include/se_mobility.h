@@ -84,6 +84,16 @@ se_status se_plan_create(se_plan **out, int64_t N, double L, const double *radii
 /* Gaussian shape parameter m of Eq. 46 (h ~ exp(-m^2/2) at the edge of the support), m > 0. */
 se_status se_plan_set_shape(se_plan *plan, double m);
 
+/* Lees-Edwards strain (Sec. 3.1, Sec. 3.2 L300-302 with Eq. 48): the periodic lattice
+ * becomes a1 = (L,0,0), a2 = (gamma L, L, 0), a3 = (0,0,L) -- simple shear, flow along x, gradient along y.  Positions stay
+ * physical Cartesian coordinates (any real value; wrapped on the sheared lattice internally).  The grid lives in the
+ * fractional coordinate t = A^{-1} r, in which the Gaussian of Eq. 41 is isotropic; the strain enters through the metric
+ * B^T.B of its derivatives when spreading and gathering (Eq. 42, 45, 48), through k = B.q in the Green's function (Eq. 43),
+ * through the sheared minimum image of the real-space sum, and in se_self_image_blocks.  gamma = 0 (default) is the cubic
+ * box and takes exactly the original code paths.  Any finite gamma is accepted; gamma and gamma + 1 describe the same
+ * lattice.  Drops the cached configuration.  Errors: SE_ERR_INVALID_ARG for a non-finite value. */
+se_status se_plan_set_strain(se_plan *plan, double gamma);
+
 /* Performance knob: number of segments the x-sweep of the spreading kernel is cut into (0 = the plan's own choice);
  * gather_segments is accepted and ignored (the gather kernel balances its own work over the SMs).
  * Results do not depend on it beyond summation order. */

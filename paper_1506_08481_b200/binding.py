@@ -50,6 +50,8 @@ def load_library(build_if_missing: bool = True):
     L.se_plan_create.argtypes = [ctypes.POINTER(P), I64, D, P, D, D, INT, INT, D]
     L.se_plan_set_shape.restype = INT
     L.se_plan_set_shape.argtypes = [P, D]
+    L.se_plan_set_strain.restype = INT
+    L.se_plan_set_strain.argtypes = [P, D]
     L.se_plan_set_tuning.restype = INT
     L.se_plan_set_tuning.argtypes = [P, INT, INT]
     L.se_plan_set_option.restype = INT
@@ -143,6 +145,10 @@ class SePlan:
 
     def set_shape(self, m):
         self._check(self._lib.se_plan_set_shape(self._h, float(m)), "se_plan_set_shape")
+
+    def set_strain(self, gamma):
+        """se_plan_set_strain: Lees-Edwards strain of the lattice, a2 = (gamma L, L, 0)."""
+        self._check(self._lib.se_plan_set_strain(self._h, float(gamma)), "se_plan_set_strain")
 
     def set_tuning(self, spread_segments=0, gather_segments=0):
         self._check(self._lib.se_plan_set_tuning(self._h, int(spread_segments), int(gather_segments)), "se_plan_set_tuning")

@@ -40,22 +40,26 @@ __global__ void __launch_bounds__(BLK_THREADS) k_block_lattice(SeConst cb, doubl
 #pragma unroll
     for (int q = 0; q < 11; ++q) accw[q] = 0.0;
     // real-space images R_n = L n, n != 0: separation x = r_i - r_j - R_n = -R_n
+    // sheared lattice: R_n = L (n0 + gamma n1, n1, n2); the x range is widened so that the cube still holds the cutoff sphere
     constexpr int NI = 2 * BLK_NIMG + 1;
-    for (int q = tid; q < NI * NI * NI; q += BLK_THREADS) {
-        const int nx = q / (NI * NI) - BLK_NIMG, ny = (q / NI) % NI - BLK_NIMG, nz = q % NI - BLK_NIMG;
+    const int wx = (int)ceil(fabs(cb.gamma) * BLK_NIMG), NX = NI + 2 * wx;
+    for (int q = tid; q < NX * NI * NI; q += BLK_THREADS) {
+        const int nx = q / (NI * NI) - BLK_NIMG - wx, ny = (q / NI) % NI - BLK_NIMG, nz = q % NI - BLK_NIMG;
         if (nx == 0 && ny == 0 && nz == 0) continue;
-        const double x = -cb.L * nx, y = -cb.L * ny, z = -cb.L * nz;
+        const double x = -cb.L * (nx + cb.gamma * ny), y = -cb.L * ny, z = -cb.L * nz;
         pair_real<false>(cb, x, y, z, x * x + y * y + z * z, cF, cS, a, mj, acc);
     }
     // wave vectors k = (2 pi / L) j, j != 0
     const double Fx = mj[0], Fy = mj[1], Fz = mj[2], Tx = mj[3], Ty = mj[4], Tz = mj[5];
     const double Sxx = mj[6], Sxy = mj[7], Sxz = mj[8], Syy = mj[9], Syz = mj[10], Szz = -(Sxx + Syy);
     const double V = cb.L * cb.L * cb.L;
+    // k = (2 pi/L)(j0, j1 - gamma j0, j2); the j1 range is widened likewise
     constexpr int NK = 2 * BLK_KMAX + 1;
-    for (int q = tid; q < NK * NK * NK; q += BLK_THREADS) {
-        const int jx = q / (NK * NK) - BLK_KMAX, jy = (q / NK) % NK - BLK_KMAX, jz = q % NK - BLK_KMAX;
+    const int wy = (int)ceil(fabs(cb.gamma) * BLK_KMAX), NY = NK + 2 * wy;
+    for (int q = tid; q < NK * NY * NK; q += BLK_THREADS) {
+        const int jx = q / (NY * NK) - BLK_KMAX, jy = (q / NK) % NY - BLK_KMAX - wy, jz = q % NK - BLK_KMAX;
         if (jx == 0 && jy == 0 && jz == 0) continue;
-        const double kx = cb.twopiL * jx, ky = cb.twopiL * jy, kz = cb.twopiL * jz;
+        const double kx = cb.twopiL * jx, ky = cb.twopiL * (jy - cb.gamma * jx), kz = cb.twopiL * jz;
         const double k2 = kx * kx + ky * ky + kz * kz, e = k2 * cb.inv4xi2;
         const double G = (1.0 + e) * exp(-e) / (cb.eta0 * V * k2);
         const double f = 1.0 - cF * k2, s = 1.0 - cS * k2;

@@ -23,7 +23,37 @@ struct SeConst {
     // k-space: scale0 = Delta^3/(eta0 V), inv4xi2 = 1/(4 xi^2), dec = (1 - eta_se)/(4 xi^2), twopiL = 2 pi/L
     double scale0, inv4xi2, dec, twopiL;
     double D3;                     // Delta^3 (gather quadrature weight)
+    // sheared (Lees-Edwards) lattice a1 = (L,0,0), a2 = (gamma L, L, 0), a3 = (0,0,L):
+    double gamma, invL;            // strain (0 = cubic box: every kernel then takes its original path); 1/L
 };
+
+// Position of a particle on the grid axis d.  Cubic box: the wrapped coordinate x - L floor(x/L) (returned in *xw) times M/L.
+// Sheared lattice: the wrapped FRACTIONAL coordinate t = A^{-1} r = ((x - gamma y)/L, y/L, z/L), t - floor(t) (returned in
+// *xw, times L), times M -- evaluated without fused multiply-adds, in the order the oracle uses, so that both sides choose
+// the same support for a particle that sits on a grid plane.
+__device__ __forceinline__ double se_grid_coord(const SeConst &c, const double *__restrict__ pos3, int d, double *xw)
+{
+    if (c.gamma == 0.0) {
+        const double x = pos3[d];
+        *xw = x - c.L * floor(x / c.L);
+        return *xw * c.MoverL;
+    }
+    const double t = d == 0 ? __dmul_rn(__dsub_rn(pos3[0], __dmul_rn(c.gamma, pos3[1])), c.invL) : __dmul_rn(pos3[d], c.invL);
+    const double tw = t - floor(t);
+    *xw = tw * c.L;
+    return __dmul_rn(tw, (double)c.M);
+}
+
+// Minimum image of a separation (r_c <= L/2: at most one image lies within r_c, and it is this one).  Sheared lattice: the
+// y and z images by rounding, then the x image given the shift gamma L of the chosen y image.
+__device__ __forceinline__ void se_min_image(const SeConst &c, double &dx, double &dy, double &dz)
+{
+    const double n1 = rint(dy * c.invL);
+    dy -= c.L * n1;
+    if (c.gamma != 0.0) dx -= c.gamma * c.L * n1;
+    dx -= c.L * rint(dx * c.invL);
+    dz -= c.L * rint(dz * c.invL);
+}
 
 // Spreading record (AoS, rec_stride doubles, 16-byte aligned), in spreading-tile order:
 //   [0]  int2 (y0w, z0w)   wrapped first support index along y, z

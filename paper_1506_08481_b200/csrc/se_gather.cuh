@@ -373,12 +373,15 @@ __global__ void k_epilogue(SeConst c, unsigned flags, const double *__restrict__
         const double *m = moments + (size_t)GATHER_SUMS * i;
         const double cF = a * a / 6.0, cS = a * a / 10.0, D3 = c.D3, aD3 = c.alpha * c.D3;
         double A0[3], A1[3], Ay[3], Az[3], C1[3], Cy[3], Cz[3];
+        // sheared lattice: the gathered offsets are fractional (times L); the physical gradient of the Gaussian carries the
+        // metric vector D = (dx, dy - gamma dx, dz) (se_spread.cuh), so only the y moments change
+        const double gm = c.gamma;
 #pragma unroll
         for (int g = 0; g < 3; ++g) {
-            A0[g] = m[g]; A1[g] = m[3 + g]; Ay[g] = m[6 + g]; Az[g] = m[9 + g];
+            A0[g] = m[g]; A1[g] = m[3 + g]; Ay[g] = m[6 + g] - gm * m[3 + g]; Az[g] = m[9 + g];
             v[g] += D3 * (A0[g] + cF * m[12 + g]);
             C1[g] = A1[g] + cS * m[15 + g];
-            Cy[g] = Ay[g] + cS * m[18 + g];
+            Cy[g] = Ay[g] + cS * (m[18 + g] - gm * m[15 + g]);
             Cz[g] = Az[g] + cS * m[21 + g];
         }
         v[3] += aD3 * (Ay[2] - Az[1]);

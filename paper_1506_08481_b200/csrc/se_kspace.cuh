@@ -31,9 +31,11 @@ __global__ void __launch_bounds__(KSPACE_THREADS) k_kspace(SeConst c, const doub
     double2 u0 = make_double2(0.0, 0.0), u1 = u0, u2 = u0, w0 = u0, w1 = u0, w2 = u0, pk = u0;
     const bool zero = (ix == 0 && iy == 0 && iz == 0) || ix == M / 2 || iy == M / 2 || iz == M / 2;
     if (!zero) {
-        const double kx = c.twopiL * jx, ky = c.twopiL * jy, kz = c.twopiL * jz;
+        // sheared lattice: k = (2 pi/L)(jx, jy - gamma jx, jz); deconvolution in the fractional wave number kq (se_xyfft.cuh)
+        const double kx = c.twopiL * jx, ky = c.twopiL * ((double)jy - c.gamma * (double)jx), kz = c.twopiL * jz;
         const double k2 = kx * kx + ky * ky + kz * kz;
-        const double dec = exp(-c.dec * k2);
+        const double kq2 = c.twopiL * c.twopiL * ((double)jx * jx + (double)jy * jy + (double)jz * jz);
+        const double dec = c.gamma == 0.0 ? exp(-c.dec * k2) : exp(-k2 * c.inv4xi2 + c.eta_se * kq2 * c.inv4xi2);
         const double sc = c.scale0 * (1.0 + k2 * c.inv4xi2) * dec / k2;
         const double2 h0 = Hk[q], h1 = Hk[Gc + q], h2 = Hk[2 * Gc + q];
         const double pr = (kx * h0.x + ky * h1.x + kz * h2.x) / k2, pi = (kx * h0.y + ky * h1.y + kz * h2.y) / k2;

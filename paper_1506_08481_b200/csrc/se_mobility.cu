@@ -45,6 +45,8 @@ struct se_plan {
     int *d_cnt_all, *d_start_all;  // the three count / start tables, concatenated (one pad element after each)
     int *d_bsum;
     int ncell_r, ncell_s, ncell_g, ncell_all;
+    int ncell_r_alloc;             // cells the count / start tables were laid out for (strain 0)
+    double r_c;
     cudaStream_t side;             // the real-space sum runs here, beside the wave-space pipeline
     cudaEvent_t ev_fork, ev_join;
     bool have_side;
@@ -163,6 +165,20 @@ static void derive_constants(se_plan *p)
     c.inv4xi2 = 1.0 / (4.0 * c.xi * c.xi);
     c.dec = (1.0 - c.eta_se) / (4.0 * c.xi * c.xi);
     c.twopiL = 2.0 * M_PI / c.L;
+    c.invL = 1.0 / c.L;
+}
+
+// Real-space cell grid: cells of edge >= r_c in the cubic box; on the sheared lattice the cells live in the fractional
+// coordinate, where a separation r < r_c has |dt1| <= r_c sqrt(1 + gamma^2)/L, |dt2|, |dt3| <= r_c/L.
+static void choose_real_cells(se_plan *p)
+{
+    SeConst &c = p->c;
+    int ncr = (int)floor(c.L / (p->r_c * sqrt(1.0 + c.gamma * c.gamma)));
+    if (ncr < 3) ncr = 1;
+    if (ncr > 1024) ncr = 1024;
+    c.ncr = ncr;
+    c.hr = c.L / ncr;
+    p->ncell_r = ncr * ncr * ncr;
 }
 
 // Sweep segments along x.  Spreading re-processes the particles of the P-1 planes before a segment, the
@@ -362,7 +378,10 @@ static se_status upload_etab(se_plan *p)
     if (!p->d_etab) { se_status st = dev_alloc(p, &p->d_etab, (size_t)M); if (st != SE_OK) return st; }
     double *et = (double *)malloc(sizeof(double) * (size_t)M);
     if (!et) return fail(p, SE_ERR_ALLOC, "malloc", "exp table");
-    for (int q = 0; q < M; ++q) { const double k = p->c.twopiL * (q < M / 2 ? q : q - M); et[q] = exp(-p->c.dec * k * k); }
+    for (int q = 0; q < M; ++q) {           // sheared lattice: only the deconvolution e^{+eta_se kq^2/4xi^2} is separable (se_xyfft.cuh)
+        const double k = p->c.twopiL * (q < M / 2 ? q : q - M);
+        et[q] = p->c.gamma == 0.0 ? exp(-p->c.dec * k * k) : exp(p->c.eta_se * p->c.inv4xi2 * k * k);
+    }
     const cudaError_t e = cudaMemcpy(p->d_etab, et, sizeof(double) * (size_t)M, cudaMemcpyHostToDevice);
     free(et);
     if (e != cudaSuccess) { cudaGetLastError(); return fail(p, SE_ERR_CUDA, "cudaMemcpy", "exp table"); }
@@ -383,8 +402,10 @@ static cudaError_t prepare_xy()
 {
     cudaError_t e = raise_smem_limit(k_yfft<LM, false>);
     if (e == cudaSuccess) e = raise_smem_limit(k_yfft<LM, true>);
-    if (e == cudaSuccess) e = raise_smem_limit(k_xmid<LM, XmChoice<LM, false>::YB, false>);
-    if (e == cudaSuccess) e = raise_smem_limit(k_xmid<LM, XmChoice<LM, true>::YB, true>);
+    if (e == cudaSuccess) e = raise_smem_limit(k_xmid<LM, XmChoice<LM, false>::YB, false, false>);
+    if (e == cudaSuccess) e = raise_smem_limit(k_xmid<LM, XmChoice<LM, true>::YB, true, false>);
+    if (e == cudaSuccess) e = raise_smem_limit(k_xmid<LM, XmChoice<LM, false>::YB, false, true>);
+    if (e == cudaSuccess) e = raise_smem_limit(k_xmid<LM, XmChoice<LM, true>::YB, true, true>);
     return e;
 }
 
@@ -405,7 +426,8 @@ static void launch_xmid(const SeConst &c, cudaStream_t s, const double2 *Hk, con
     constexpr int YB = XmChoice<LM, COMP>::YB;
     using TR = XmTraits<LM, YB, COMP>;
     const unsigned nb = (unsigned)((TR::M / 2 + 1) * (TR::M / YB));
-    k_xmid<LM, YB, COMP><<<nb, TR::NT, TR::SMEM, s>>>(c, Hk, Hsk, Gk, Pk, wtab, etab);
+    if (c.gamma != 0.0) k_xmid<LM, YB, COMP, true><<<nb, TR::NT, TR::SMEM, s>>>(c, Hk, Hsk, Gk, Pk, wtab, etab);
+    else k_xmid<LM, YB, COMP, false><<<nb, TR::NT, TR::SMEM, s>>>(c, Hk, Hsk, Gk, Pk, wtab, etab);
 }
 
 #define FOR_EACH_LM(X) X(5) X(6) X(7) X(8) X(9)
@@ -566,12 +588,9 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
     }
 
     // real-space cell grid: edge >= r_c, at least 3 cells per axis, else all pairs (one cell)
-    int ncr = (int)floor(L / r_c);
-    if (ncr < 3) ncr = 1;
-    if (ncr > 1024) ncr = 1024;
-    c.ncr = ncr;
-    c.hr = L / ncr;
-    p->ncell_r = ncr * ncr * ncr;
+    p->r_c = r_c;
+    choose_real_cells(p);
+    p->ncell_r_alloc = p->ncell_r;                     // a strain only makes the cells larger
     // spreading tile bins (plane-thin): M x ceil(M/4) x ceil(M/8)
     c.NBY = (M + SE_TILE_Y - 1) / SE_TILE_Y;
     c.NBZ = (M + SE_TILE_Z - 1) / SE_TILE_Z;
@@ -654,6 +673,21 @@ extern "C" se_status se_plan_set_shape(se_plan *p, double m)
     return SE_OK;
 }
 
+// Lees-Edwards strain of the lattice.  The count / start tables keep the layout of the unstrained box (their
+// real-space part is only used up to the current number of cells).
+extern "C" se_status se_plan_set_strain(se_plan *p, double gamma)
+{
+    if (!p || !(gamma == gamma) || fabs(gamma) > 1e6) return SE_ERR_INVALID_ARG;
+    p->c.gamma = gamma;
+    ++p->epoch;
+    p->have_positions = false;
+    p->have_pairs = false;
+    choose_real_cells(p);
+    if (p->ncell_r > p->ncell_r_alloc) return fail(p, SE_ERR_UNSUPPORTED, "se_plan_set_strain", "cell grid larger than allocated");
+    if (p->d_etab) return upload_etab(p);
+    return SE_OK;
+}
+
 extern "C" se_status se_plan_set_tuning(se_plan *p, int spread_segments, int gather_segments)
 {
     if (!p || spread_segments < 0 || gather_segments < 0) return SE_ERR_INVALID_ARG;
@@ -709,7 +743,7 @@ static se_status scan_cells(se_plan *p, cudaStream_t s)
 {
     const int n = p->ncell_all, nb = (n + SCAN_BLOCK - 1) / SCAN_BLOCK;
     k_scan_local<<<nb, SCAN_THREADS, 0, s>>>(p->d_cnt_all, p->d_start_all, p->d_bsum, n);
-    k_scan_add<<<nb, SCAN_THREADS, 0, s>>>(p->d_start_all, p->d_bsum, n, p->ncell_r + 1, p->ncell_r + p->ncell_s + 2, p->c.N);
+    k_scan_add<<<nb, SCAN_THREADS, 0, s>>>(p->d_start_all, p->d_bsum, n, p->ncell_r_alloc + 1, p->ncell_r_alloc + p->ncell_s + 2, p->c.N);
     p->last_launches += 2;
     CUDA_TRY(p, cudaGetLastError());
     return SE_OK;
@@ -721,10 +755,14 @@ static void launch_spread(se_plan *p, cudaStream_t s, bool comp_in)
     const SeConst &c = p->c;
     const long long warps = (long long)c.NBY * c.NBZ * c.nseg;
     const int blocks = (int)((warps + SWEEP_WARPS - 1) / SWEEP_WARPS);
-    if (comp_in)
-        k_spread<P, 4><<<blocks, SWEEP_WARPS * 32, sweep_smem_bytes(c.rec_stride), s>>>(c, p->d_recs, p->d_start_s, p->d_real, p->d_real_p);
+    const size_t sm = sweep_smem_bytes(c.rec_stride);
+    if (c.gamma != 0.0) {
+        if (comp_in) k_spread<P, 4, true><<<blocks, SWEEP_WARPS * 32, sm, s>>>(c, p->d_recs, p->d_start_s, p->d_real, p->d_real_p);
+        else k_spread<P, 3, true><<<blocks, SWEEP_WARPS * 32, sm, s>>>(c, p->d_recs, p->d_start_s, p->d_real, nullptr);
+    } else if (comp_in)
+        k_spread<P, 4, false><<<blocks, SWEEP_WARPS * 32, sm, s>>>(c, p->d_recs, p->d_start_s, p->d_real, p->d_real_p);
     else
-        k_spread<P, 3><<<blocks, SWEEP_WARPS * 32, sweep_smem_bytes(c.rec_stride), s>>>(c, p->d_recs, p->d_start_s, p->d_real, nullptr);
+        k_spread<P, 3, false><<<blocks, SWEEP_WARPS * 32, sm, s>>>(c, p->d_recs, p->d_start_s, p->d_real, nullptr);
 }
 
 template <int P>
@@ -741,8 +779,10 @@ static void launch_gather(se_plan *p, cudaStream_t s, bool pressure)
 template <int P>
 static cudaError_t prepare_sweeps()
 {
-    cudaError_t e = raise_smem_limit(k_spread<P, 3>);
-    if (e == cudaSuccess) e = raise_smem_limit(k_spread<P, 4>);
+    cudaError_t e = raise_smem_limit(k_spread<P, 3, false>);
+    if (e == cudaSuccess) e = raise_smem_limit(k_spread<P, 4, false>);
+    if (e == cudaSuccess) e = raise_smem_limit(k_spread<P, 3, true>);
+    if (e == cudaSuccess) e = raise_smem_limit(k_spread<P, 4, true>);
     if (e == cudaSuccess) e = raise_smem_limit(k_gather<P>);
     return e;
 }

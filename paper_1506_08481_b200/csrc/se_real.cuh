@@ -186,7 +186,6 @@ __global__ void __launch_bounds__(REAL_WARPS * 32, (NR == 1 ? REAL_MINB1 : (NR =
     __shared__ int seg_s[27], seg_o[28];               // neighbour cell ranges: first particle, exclusive offsets
     const int wl = threadIdx.x >> 5, lane = threadIdx.x & 31, tid = threadIdx.x;
     const int nc = c.ncr;
-    const double invL = 1.0 / c.L;
 
     // Work items: the cells (grid-stride loop, so that a small persistent grid can run beside the HBM-bound
     // wave-space kernels without taking their SM resources), or one slice of all particles per CTA.
@@ -266,7 +265,7 @@ __global__ void __launch_bounds__(REAL_WARPS * 32, (NR == 1 ? REAL_MINB1 : (NR =
                     const double4 pj = cand[q];
                     j = cand_j[q];
                     dx = pi.x - pj.x; dy = pi.y - pj.y; dz = pi.z - pj.z;
-                    dx -= c.L * rint(dx * invL); dy -= c.L * rint(dy * invL); dz -= c.L * rint(dz * invL);
+                    se_min_image(c, dx, dy, dz);
                     const double r2 = dx * dx + dy * dy + dz * dz;
                     hit = (j != i) && (r2 < c.rc2) && (r2 > 0.0);
                     aj = pj.w;
@@ -342,7 +341,6 @@ __global__ void __launch_bounds__(REAL_WARPS * 32) k_pairs(SeConst c, const doub
     __shared__ int seg_s[27], seg_o[28];
     const int wl = threadIdx.x >> 5, lane = threadIdx.x & 31, tid = threadIdx.x;
     const int nc = c.ncr;
-    const double invL = 1.0 / c.L;
     const int nitems = nc > 1 ? nc * nc * nc : (int)gridDim.x;
     for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
     __syncthreads();
@@ -413,7 +411,7 @@ __global__ void __launch_bounds__(REAL_WARPS * 32) k_pairs(SeConst c, const doub
                     const double4 pjv = cand[q];
                     j = cand_j[q];
                     dx = pi.x - pjv.x; dy = pi.y - pjv.y; dz = pi.z - pjv.z;
-                    dx -= c.L * rint(dx * invL); dy -= c.L * rint(dy * invL); dz -= c.L * rint(dz * invL);
+                    se_min_image(c, dx, dy, dz);
                     const double r2 = dx * dx + dy * dy + dz * dz;
                     hit = (j != i) && (r2 < c.rc2) && (r2 > 0.0);
                     aj = pjv.w;

@@ -25,9 +25,10 @@ __global__ void k_keys(SeConst c, GatherGeom g, const double *__restrict__ pos, 
     int cc[3], n0[3];
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
-        const double xw = se_wrap(pos[3 * (size_t)i + d], c.L);
-        cc[d] = se_mod((int)floor(xw / c.hr), c.ncr);
-        n0[d] = se_mod(se_support_start(xw * c.MoverL, c.P), c.M);
+        double xw;
+        const double u = se_grid_coord(c, pos + 3 * (size_t)i, d, &xw);
+        cc[d] = se_mod((int)floor(xw / c.hr), c.ncr);                 // sheared: cells in the fractional coordinate (xw = t L)
+        n0[d] = se_mod(se_support_start(u, c.P), c.M);
     }
     const int kr = (cc[0] * c.ncr + cc[1]) * c.ncr + cc[2];
     const int ks = (n0[0] * c.NBY + n0[1] / SE_TILE_Y) * c.NBZ + n0[2] / SE_TILE_Z;
@@ -141,9 +142,13 @@ k_scatter(SeConst c, const double *__restrict__ pos, const double *__restrict__ 
         double *r = sc_rows + pl * pitch, *gxd = r + c.rec_stride;
         const int dr = start_r[key_r[i]] + rank_r[i];
         // this thread's axis: wrapped coordinate, support start, Gaussian table
-        const double xw = se_wrap(pos[i3 + d], c.L), al = c.alpha;
-        reinterpret_cast<double *>(rs_pos + dr)[d] = xw;
-        const double u = xw * c.MoverL;
+        double xw;
+        const double u = se_grid_coord(c, pos + i3, d, &xw), al = c.alpha;
+        if (c.gamma != 0.0 && d == 0) {                     // real-space copy: a physical position, x = L (t1 + gamma t2)
+            double yw;
+            se_grid_coord(c, pos + i3, 1, &yw);
+            reinterpret_cast<double *>(rs_pos + dr)[0] = xw + c.gamma * yw;
+        } else reinterpret_cast<double *>(rs_pos + dr)[d] = xw;
         const int n0 = se_support_start(u, P);
         r[REC_D0 + d] = ((double)n0 - u) * c.Delta;
         reinterpret_cast<int *>(r)[d == 0 ? 2 : d - 1] = se_mod(n0, c.M);            // int2 (y0w, z0w), int2 (x0w, orig)
@@ -177,9 +182,15 @@ k_scatter(SeConst c, const double *__restrict__ pos, const double *__restrict__ 
             const double cF = a * a / 6.0, cS = a * a / 10.0;
             if (c.rec_stride > SE_REC_HDR + 3 * P) r[SE_REC_HDR + 3 * P] = 0.0;
             reinterpret_cast<int *>(r)[3] = i;
-            r[REC_POLY] = 1.0 - 6.0 * al * cF;
+            if (c.gamma == 0.0) {
+                r[REC_POLY] = 1.0 - 6.0 * al * cF;
+                r[REC_POLY + 2] = 2.0 * al * (1.0 - 10.0 * al * cS);
+            } else {                                        // metric trace 3 + gamma^2 (Eq. 48); the anisotropic S term is separate (k_spread)
+                const double trM = 3.0 + c.gamma * c.gamma;
+                r[REC_POLY] = 1.0 - 2.0 * al * trM * cF;
+                r[REC_POLY + 2] = 2.0 * al * (1.0 - 2.0 * al * trM * cS);
+            }
             r[REC_POLY + 1] = 4.0 * al * al * cF;
-            r[REC_POLY + 2] = 2.0 * al * (1.0 - 10.0 * al * cS);
             r[REC_POLY + 3] = 8.0 * al * al * al * cS;
             r[REC_F] = f[0]; r[REC_F + 1] = f[1]; r[REC_F + 2] = f[2];
             r[REC_T] = t[0]; r[REC_T + 1] = t[1]; r[REC_T + 2] = t[2];

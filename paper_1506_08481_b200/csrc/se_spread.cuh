@@ -17,7 +17,12 @@
 
 // NC = 3: the three force-density grids; NC = 4: plus the scalar grid of the pressure moments (a9),
 // Hs(x_n) = sum_j gamma(d) s_j, one more FMA per grid point.
-template <int P, int NC>
+// SHEAR: sheared lattice (Eq. 48).  The Gaussian is isotropic in the grid offsets (dx, dy, dz) = fractional
+// offsets times L; its physical gradient is -2 al D gam with the metric vector D = (dx, dy - g dx, dz), lap gam =
+// (4 al^2 D.D - 2 al (3 + g^2)) gam and grad lap gam carries the extra term 8 al^2 Mt.D, Mt = [[1,-g,0],[-g,1+g^2,0],[0,0,1]]:
+//   H = gam { F [f0 + f1 D.D] - al D x T + (S.D) [s0 + s1 D.D] - 8 al^2 cS S.(Mt.D) },   f0, s0 with the trace 3 + g^2 (a1),
+// still a cubic in dx for a fixed column: D = D0 + dx D1, D0 = (0, dy, dz), D1 = (1, -g, 0).
+template <int P, int NC, bool SHEAR>
 __device__ __forceinline__ void spread_hit(const SeConst &c, const double *__restrict__ rec, int y, int z, bool active,
                                            double (&acc)[P][NC])
 {
@@ -52,6 +57,25 @@ __device__ __forceinline__ void spread_hit(const SeConst &c, const double *__res
         c2[1] = gyz * (f1 * Fy + s1 * sg1);
         c2[2] = gyz * (f1 * Fz + s1 * sg2);
         c3[0] = gyz * s1 * Sxx; c3[1] = gyz * s1 * Sxy; c3[2] = gyz * s1 * Sxz;
+        if (SHEAR) {
+            const double g = c.gamma, g1 = 1.0 + g * g, kap = 8.0 * al * al * rec[REC_CS];
+            const double A1 = -2.0 * g * dy * f1, A2 = g1 * f1, B1 = -2.0 * g * dy * s1, B2 = g1 * s1;
+            const double Fv[3] = { Fx, Fy, Fz };
+            const double Sx_[3] = { Sxx, Sxy, Sxz }, Sy_[3] = { Sxy, Syy, Syz }, Sz_[3] = { Sxz, Syz, Szz };
+            const double t0v[3] = { t00, t01, t02 };                                  // D0 x T
+            const double t1v[3] = { -g * Tz, -Tz, Ty + g * Tx };                      // D1 x T
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                const double sg = Sy_[a] * dy + Sz_[a] * dz;                          // (S.D0)_a
+                const double sd = Sx_[a] - g * Sy_[a];                                // (S.D1)_a
+                const double m0 = -g * dy * Sx_[a] + g1 * dy * Sy_[a] + dz * Sz_[a];  // (S.Mt.D0)_a
+                const double m1 = g1 * Sx_[a] - g * (2.0 + g * g) * Sy_[a];           // (S.Mt.D1)_a
+                c0[a] = gyz * (fa * Fv[a] - al * t0v[a] + sa * sg - kap * m0);
+                c1[a] = gyz * (A1 * Fv[a] - al * t1v[a] + B1 * sg + sa * sd - kap * m1);
+                c2[a] = gyz * (A2 * Fv[a] + B2 * sg + B1 * sd);
+                c3[a] = gyz * (B2 * sd);
+            }
+        }
         // acc[k][a] += gx(k) ((c3 dx + c2) dx + c1) dx + c0)[a], dx = d0x + k Delta: 3P independent chains of four FMAs,
         // one table value per plane
         const double *__restrict__ X0 = rec + SE_REC_HDR;
@@ -72,8 +96,8 @@ __device__ __forceinline__ void spread_hit(const SeConst &c, const double *__res
     }
 }
 
-template <int P, int NC>
-__global__ void __launch_bounds__(SWEEP_WARPS * 32, NC == 3 ? SWEEP_MIN_BLOCKS : 2) k_spread(SeConst c, const double *__restrict__ recs,
+template <int P, int NC, bool SHEAR>
+__global__ void __launch_bounds__(SWEEP_WARPS * 32, (NC == 3 && !SHEAR) ? SWEEP_MIN_BLOCKS : 2) k_spread(SeConst c, const double *__restrict__ recs,
                                                               const int *__restrict__ start_s, double *__restrict__ H,
                                                               double *__restrict__ Hs)
 {
@@ -128,10 +152,10 @@ __global__ void __launch_bounds__(SWEEP_WARPS * 32, NC == 3 ? SWEEP_MIN_BLOCKS :
             parity ^= 1u << buf;
             const double *__restrict__ sl = buf ? slot1 : slot0;
             const int ns = min(cur.n, SWEEP_CAP);
-            for (int ci = 0; ci < ns; ++ci) spread_hit<P, NC>(c, sl + (size_t)ci * stride, y, z, active, acc);
+            for (int ci = 0; ci < ns; ++ci) spread_hit<P, NC, SHEAR>(c, sl + (size_t)ci * stride, y, z, active, acc);
             for (int ci = SWEEP_CAP; ci < cur.n; ++ci) {
                 const int j = sweep_overflow_index(cur, ci);
-                spread_hit<P, NC>(c, recs + (size_t)j * stride, y, z, active, acc);
+                spread_hit<P, NC, SHEAR>(c, recs + (size_t)j * stride, y, z, active, acc);
             }
             __syncwarp();                           // slot fully read before it is refilled
         }

@@ -146,7 +146,10 @@ template <int LM, int YB, bool COMP> struct XmTraits {
     static constexpr size_t SMEM = ((size_t)NG * PITCH * YB + M) * 16 + (size_t)M * 8;
 };
 
-template <int LM, int YB, bool COMP>
+// SHEAR: k = (2 pi/L)(jx, jy - gamma jx, jz) in the Green's function, the projector and w = -k^2 u; the Gaussians are
+// deconvolved in the FRACTIONAL wave number, so the factor is e^{-k^2/4xi^2} (one exponential per mode) times the separable
+// e^{+eta_se kq^2/4xi^2} from the table (then Etab holds that factor).
+template <int LM, int YB, bool COMP, bool SHEAR>
 __global__ void __launch_bounds__(XmTraits<LM, YB, COMP>::NT, (XmTraits<LM, YB, COMP>::NT <= 192 ? 2 : 1))
 k_xmid(SeConst c, const double2 *__restrict__ Hk, const double2 *__restrict__ Hsk, double2 *__restrict__ Gk,
        double2 *__restrict__ Pk, const double2 *__restrict__ Wtab, const double *__restrict__ Etab)
@@ -205,18 +208,19 @@ k_xmid(SeConst c, const double2 *__restrict__ Hk, const double2 *__restrict__ Hs
     __syncthreads();
     cplx uu[16];
     const int jy = iy < Nh ? iy : iy - M;
-    const double ky = c.twopiL * jy, kzv = c.twopiL * kz;
-    const double eyz = ET[iy] * ET[kz], kyz2 = ky * ky + kzv * kzv;
+    const double ky0 = c.twopiL * jy, kzv = c.twopiL * kz;
+    const double eyz = ET[iy] * ET[kz], kyz2 = ky0 * ky0 + kzv * kzv;
     const cplx *E0 = E + y, *E1 = E0 + (size_t)PITCH * YB, *E2 = E1 + (size_t)PITCH * YB, *E3 = E2 + (size_t)PITCH * YB;
 #pragma unroll
     for (int q = 0; q < 16; ++q) {
         const int ix = jj + q * M16, ps = xf_sk<4>(ix) * YB;
         const int jx = ix < Nh ? ix : ix - M;
         const double kx = c.twopiL * jx;
-        const double k2 = kx * kx + kyz2;
+        const double ky = SHEAR ? c.twopiL * ((double)jy - c.gamma * (double)jx) : ky0;
+        const double k2 = SHEAR ? kx * kx + ky * ky + kzv * kzv : kx * kx + kyz2;
         const bool zero = (ix == 0 && iy == 0 && kz == 0) || ix == Nh || iy == Nh;
         const double inv = zero ? 0.0 : 1.0 / k2;
-        const double dec = ET[ix] * eyz;
+        const double dec = SHEAR ? exp(-k2 * c.inv4xi2) * (ET[ix] * eyz) : ET[ix] * eyz;
         const cplx h0 = grp == 0 ? v[q] : E0[ps], h1 = grp == 1 ? v[q] : E1[ps], h2 = grp == 2 ? v[q] : E2[ps];
         const double pr = (kx * h0.x + ky * h1.x + kzv * h2.x) * inv, pi = (kx * h0.y + ky * h1.y + kzv * h2.y) * inv;
         cplx r;
@@ -250,7 +254,8 @@ k_xmid(SeConst c, const double2 *__restrict__ Hk, const double2 *__restrict__ Hs
 #pragma unroll
     for (int q = 0; q < 16; ++q) {
         const int ix = jj + q * M16, jx = ix < Nh ? ix : ix - M;
-        const double kx = c.twopiL * jx, k2 = kx * kx + kyz2;
+        const double kx = c.twopiL * jx, kys = c.twopiL * ((double)jy - c.gamma * (double)jx);
+        const double k2 = SHEAR ? kx * kx + kys * kys + kzv * kzv : kx * kx + kyz2;
         v[q] = { -k2 * uu[q].x, -k2 * uu[q].y };
     }
     fft16<LM, true>(v, W, jj, st, ld, group_sync, group_sync);

@@ -622,3 +622,88 @@ def test_pair_cache_dense_all_pairs_and_single_particle(pk, oracle, workloads):
         r.plan.apply(None, r.F, r.T, r.S, r.U, r.W, r.E)
         torch.cuda.synchronize()
         _check_blocks((r.U.cpu().numpy(), r.W.cpu().numpy(), r.E.cpu().numpy()), r.oracle(oracle), TOL)
+
+
+# ------------------------------------------------------------------------------------------------
+# f2: sheared (Lees-Edwards) lattice, se_plan_set_strain -- against o2_apply_sheared
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,gamma", [("c1", 0.3), ("c2", 0.5), ("c2", -0.37), ("c3", 0.5)])
+def test_sheared_lattice_stage_and_full_parity(pk, oracle, workloads, name, gamma):
+    """PAPER.md L245-253, L300-302 (Eq. 48), L501 (gamma = 0.5).  Positions are spread over several sheared cells and moved by
+    random lattice vectors, so the fractional wrap, the sheared minimum image and the fractional cell list all work."""
+    import torch
+    wl = workloads.make_workload(name)
+    rng = np.random.default_rng([150608481, 5])
+    A = wl.L * np.array([[1.0, gamma, 0.0], [0.0, 1.0, 0.0], [0.0, 0.0, 1.0]])
+    wl.pos = wl.pos + rng.integers(-2, 3, size=wl.pos.shape) @ A.T
+    r = Runner(pk, wl)
+    r.plan.set_strain(gamma)
+
+    def ref(parts, **kw):
+        return oracle.o2_apply_sheared(wl.pos, wl.radii, wl.L, gamma, wl.xi, wl.rc, wl.M, wl.P, wl.F, wl.T, wl.S, parts=parts, **kw)
+
+    full = ref(oracle.PART_ALL, want_grids=True)
+    _check_blocks(r.run(flags=pk.SE_SKIP_WAVE | pk.SE_SKIP_SELF | pk.SE_SKIP_ONEBODY), ref(oracle.PART_REAL), TOL_STAGE)
+    r.run(stop=2)
+    assert _rel(r.plan.copy_grids(0), full["gridH"]) <= TOL_STAGE
+    r.run(stop=5)
+    Gr = r.plan.copy_grids(1)
+    for g in range(6):
+        assert _rel(Gr[g], full["gridOut"][g]) <= TOL_STAGE, g
+    _check_blocks(r.run(flags=pk.SE_SKIP_REAL | pk.SE_SKIP_SELF | pk.SE_SKIP_ONEBODY), ref(oracle.PART_WAVE), TOL_STAGE)
+    got = r.run()
+    _check_blocks(got, full, TOL)
+    # the strain matters (the test is not vacuous) and can be taken back
+    r.plan.set_strain(0.0)
+    plain = r.run()
+    assert _rel(plain[0], got[0]) > 1e-3
+    _check_blocks(plain, r.oracle(oracle), TOL)
+
+
+def test_sheared_lattice_other_paths(pk, oracle, workloads):
+    """Strain with the cuFFT 3-D transforms (grid size that is not a power of two), the compressible extension, cached
+    positions with the pair cache, a batch, and the self-image blocks on the sheared lattice (against O1, N = 1)."""
+    import torch
+    gamma = 0.41
+    wl = workloads.make_workload("c1")
+    r = Runner(pk, wl, M=36, P=9)
+    r.plan.set_strain(gamma)
+    o2 = lambda **kw: oracle.o2_apply_sheared(wl.pos, wl.radii, wl.L, gamma, wl.xi, wl.rc, kw.pop("M", wl.M), kw.pop("P", wl.P), wl.F, wl.T, wl.S, **kw)
+    _check_blocks(r.run(), o2(M=36, P=9), TOL)
+    wl2 = workloads.make_workload("c2")
+    r2 = Runner(pk, wl2)
+    r2.plan.set_strain(gamma)
+    s_np = _pressure_moments(wl2)
+    dev = r2.pos.device
+    s_in = torch.tensor(s_np, device=dev, dtype=torch.float64)
+    s_out = torch.empty((wl2.N,), device=dev, dtype=torch.float64)
+    r2.plan.apply_compressible(r2.pos, r2.F, r2.T, r2.S, s_in, r2.U, r2.W, r2.E, s_out)
+    torch.cuda.synchronize()
+    refc = oracle.o2_apply_sheared(wl2.pos, wl2.radii, wl2.L, gamma, wl2.xi, wl2.rc, wl2.M, wl2.P, wl2.F, wl2.T, wl2.S, s=s_np)
+    _check_blocks((r2.U.cpu().numpy(), r2.W.cpu().numpy(), r2.E.cpu().numpy()), refc, TOL)
+    assert _rel(s_out.cpu().numpy(), refc["s_out"]) <= TOL
+    # cached positions (pair cache) and a batch
+    ref2 = oracle.o2_apply_sheared(wl2.pos, wl2.radii, wl2.L, gamma, wl2.xi, wl2.rc, wl2.M, wl2.P, wl2.F, wl2.T, wl2.S)
+    r2.plan.set_positions(r2.pos)
+    r2.plan.apply(None, r2.F, r2.T, r2.S, r2.U, r2.W, r2.E)
+    torch.cuda.synchronize()
+    _check_blocks((r2.U.cpu().numpy(), r2.W.cpu().numpy(), r2.E.cpu().numpy()), ref2, TOL)
+    Fb, Tb, Sb = torch.stack([r2.F, -r2.F]), torch.stack([r2.T, 2 * r2.T]), torch.stack([r2.S, r2.S])
+    Ub, Wb, Eb = torch.empty_like(Fb), torch.empty_like(Fb), torch.empty_like(Sb)
+    r2.plan.apply_batch(None, Fb, Tb, Sb, Ub, Wb, Eb)
+    torch.cuda.synchronize()
+    _check_blocks((Ub[0].cpu().numpy(), Wb[0].cpu().numpy(), Eb[0].cpu().numpy()), ref2, TOL)
+    ref3 = oracle.o2_apply_sheared(wl2.pos, wl2.radii, wl2.L, gamma, wl2.xi, wl2.rc, wl2.M, wl2.P, -wl2.F, 2 * wl2.T, wl2.S)
+    _check_blocks((Ub[1].cpu().numpy(), Wb[1].cpu().numpy(), Eb[1].cpu().numpy()), ref3, TOL)
+    # self-image blocks: no longer diagonal, still symmetric; against the definition on a one-particle system
+    out = torch.empty((wl2.N, 11, 11), device=dev, dtype=torch.float64)
+    r2.plan.self_image_blocks(out)
+    torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    xi = 6.0 / wl2.L
+    kmax = int(np.ceil(6.6 * 2 * xi * wl2.L / (2 * np.pi)))
+    for i in (0, wl2.N - 1):
+        a = float(wl2.radii[i])
+        A = oracle.o1_matrix_sheared(np.array([[0.3, 0.1, 0.7]]) * wl2.L, np.array([a]), wl2.L, gamma, xi, eta0=wl2.eta0, nimg=4, kmax=kmax)
+        assert _rel(got[i], A) <= TOL, (i, _rel(got[i], A))
+    assert np.abs(got[0] - np.diag(np.diag(got[0]))).max() > 1e-6 * np.abs(got[0]).max()
