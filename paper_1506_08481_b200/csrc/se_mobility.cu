@@ -983,7 +983,7 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     auto launch_real = [&](cudaStream_t sr) {
         if (!pos && !comp && p->have_pairs) {          // cached configuration: stream the pair list
             const unsigned nbc = (unsigned)((c.N + 7) / 8 < 148 * 16 ? (c.N + 7) / 8 : 148 * 16);
-            k_real_cached<<<nbc, 128, 0, sr>>>(c, p->d_pair_start, p->d_pj, p->d_pd, p->d_rs_mom, p->d_rs_orig, p->d_out_real);
+            k_real_cached<1><<<nbc, 128, 0, sr>>>(c, p->d_pair_start, p->d_pj, p->d_pd, p->d_rs_mom, p->d_rs_orig, p->d_out_real, 0);
             p->last_launches += 1;
             return;
         }
@@ -1257,10 +1257,11 @@ extern "C" se_status far_mobility_apply_batch(se_plan *p, const double *pos, int
         for (int r = 0; r < nrhs;) {
             const double *m = p->d_mom_b + rs * r;
             double *o = p->d_out_real_b + rs * r;
-            if (p->have_pairs) {                      // cached pair list: one streaming pass per right-hand side
+            if (p->have_pairs) {                      // cached pair list: one streaming pass for up to four right-hand sides
                 const unsigned nbc = (unsigned)((c.N + 7) / 8 < 148 * 16 ? (c.N + 7) / 8 : 148 * 16);
-                k_real_cached<<<nbc, 128, 0, s>>>(c, p->d_pair_start, p->d_pj, p->d_pd, m, p->d_rs_orig, o);
-                r += 1;
+                if (nrhs - r >= 4) { k_real_cached<4><<<nbc, 128, 0, s>>>(c, p->d_pair_start, p->d_pj, p->d_pd, m, p->d_rs_orig, o, rs); r += 4; }
+                else if (nrhs - r >= 2) { k_real_cached<2><<<nbc, 128, 0, s>>>(c, p->d_pair_start, p->d_pj, p->d_pd, m, p->d_rs_orig, o, rs); r += 2; }
+                else { k_real_cached<1><<<nbc, 128, 0, s>>>(c, p->d_pair_start, p->d_pj, p->d_pd, m, p->d_rs_orig, o, rs); r += 1; }
             } else if (nrhs - r >= 4) { k_real<false, 4><<<nb, REAL_WARPS * 32, 0, s>>>(c, p->d_rs_pos, m, p->d_rs_orig, p->d_start_r, o, rs); r += 4; }
             else if (nrhs - r >= 2) { k_real<false, 2><<<nb, REAL_WARPS * 32, 0, s>>>(c, p->d_rs_pos, m, p->d_rs_orig, p->d_start_r, o, rs); r += 2; }
             else { k_real<false, 1><<<nb, REAL_WARPS * 32, 0, s>>>(c, p->d_rs_pos, m, p->d_rs_orig, p->d_start_r, o, rs); r += 1; }

@@ -445,10 +445,12 @@ __global__ void __launch_bounds__(REAL_WARPS * 32) k_pairs(SeConst c, const doub
     }
 }
 
-// out_real[rs_orig[i]][0..10] = k0 * sum over the cached pairs of target i (cell order) applied to the moments rs_mom.
+// out_real[r][rs_orig[i]][0..10] = k0 * sum over the cached pairs of target i (cell order) applied to the moments rs_mom[r],
+// r < NR right-hand sides `rhs_stride` doubles apart: the list is streamed once for all of them.
+template <int NR>
 __global__ void __launch_bounds__(128) k_real_cached(SeConst c, const int *__restrict__ row_start, const int *__restrict__ pj,
                                                      const double *__restrict__ pd, const double *__restrict__ rs_mom,
-                                                     const int *__restrict__ rs_orig, double *__restrict__ out_real)
+                                                     const int *__restrict__ rs_orig, double *__restrict__ out_real, size_t rhs_stride)
 {
     const int hl = threadIdx.x & 15;
     const int nhw = (int)(gridDim.x * blockDim.x) >> 4;
@@ -459,9 +461,11 @@ __global__ void __launch_bounds__(128) k_real_cached(SeConst c, const int *__res
         const int i = live ? i0 : c.N - 1;
         const int row = row_start[i], n = live ? row_start[i + 1] - row : 0;
         const double *__restrict__ f = pd + (size_t)row * PAIR_F;
-        double acc[12];
+        double acc[NR][12];
 #pragma unroll
-        for (int k = 0; k < 12; ++k) acc[k] = 0.0;
+        for (int r = 0; r < NR; ++r)
+#pragma unroll
+            for (int k = 0; k < 12; ++k) acc[r][k] = 0.0;
         for (int p = hl; p < n; p += 16) {
             PairS<false> o;
             const double x = f[p], y = f[(size_t)n + p], z = f[2 * (size_t)n + p];
@@ -470,19 +474,31 @@ __global__ void __launch_bounds__(128) k_real_cached(SeConst c, const int *__res
             o.os = f[11 * (size_t)n + p]; o.a1 = f[12 * (size_t)n + p]; o.a2 = f[13 * (size_t)n + p]; o.a3 = f[14 * (size_t)n + p];
             o.a4 = f[15 * (size_t)n + p]; o.ef2 = f[16 * (size_t)n + p]; o.ef3 = f[17 * (size_t)n + p]; o.es3 = f[18 * (size_t)n + p];
             o.es4 = f[19 * (size_t)n + p];
-            pair_apply<false>(o, x, y, z, 0.0, rs_mom + 12 * (size_t)pj[row + p], acc);
+            const double *__restrict__ mj = rs_mom + 12 * (size_t)pj[row + p];
+#pragma unroll
+            for (int r = 0; r < NR; ++r) {
+                double m[12];
+                const double2 *__restrict__ m2 = reinterpret_cast<const double2 *>(mj + r * rhs_stride);     // rows of 96 bytes: 16-byte aligned
+#pragma unroll
+                for (int q = 0; q < 6; ++q) { const double2 t = m2[q]; m[2 * q] = t.x; m[2 * q + 1] = t.y; }
+                pair_apply<false>(o, x, y, z, 0.0, m, acc[r]);
+            }
         }
+        const int io = rs_orig[i];
 #pragma unroll
-        for (int k = 0; k < 11; ++k) {
-            double v = acc[k];
+        for (int r = 0; r < NR; ++r) {
 #pragma unroll
-            for (int s = 8; s > 0; s >>= 1) v += __shfl_xor_sync(0xffffffffu, v, s);
-            acc[k] = v;
-        }
-        if (live && hl == 0) {
-            double *o = out_real + 12 * (size_t)rs_orig[i];
+            for (int k = 0; k < 11; ++k) {
+                double v = acc[r][k];
 #pragma unroll
-            for (int k = 0; k < 11; ++k) o[k] = c.k0 * acc[k];
+                for (int s = 8; s > 0; s >>= 1) v += __shfl_xor_sync(0xffffffffu, v, s);
+                acc[r][k] = v;
+            }
+            if (live && hl == 0) {
+                double *o = out_real + r * rhs_stride + 12 * (size_t)io;
+#pragma unroll
+                for (int k = 0; k < 11; ++k) o[k] = c.k0 * acc[r][k];
+            }
         }
     }
 }
