@@ -45,11 +45,10 @@ typedef enum {
 #define SE_SKIP_SELF     0x4u         /* do not subtract the wave-space self terms (Eq. 37)           */
 #define SE_SKIP_ONEBODY  0x8u         /* do not add the one-body Faxen terms (Eq. 13-15)              */
 #define SE_TIMING        0x10u        /* record CUDA events between stages (se_plan_get_timings)      */
-#define SE_CUFFT3D       0x40u        /* a4/a6 by cuFFT's batched 3-D real transforms.  Without this flag, power-of-two
-                                         grids 32 <= M <= 512 take the faster default: the z transforms (real <->
-                                         half-complex) by own kernels that keep the spectra transposed, [kz][x][y], so
-                                         that cuFFT only runs contiguous batched 2-D complex plans over (x,y).  Other
-                                         M always use the 3-D transforms.                                           */
+#define SE_CUFFT3D       0x40u        /* a4/a6 by cuFFT's batched 3-D real transforms and a separate k-space kernel.
+                                         Without this flag, power-of-two grids 32 <= M <= 512 take the faster default:
+                                         own transform kernels on transposed half spectra [kz][x][y], the x transforms
+                                         fused with the k-space scaling (no cuFFT).  Other M always use cuFFT.       */
 
 /* stage indices of se_plan_get_timings */
 enum {
@@ -105,10 +104,9 @@ se_status se_plan_set_tuning(se_plan *plan, int spread_segments, int gather_segm
  *                        beside the whole wave pipeline; 2 = on that stream, started after the spreading (beside the
  *                        HBM-bound transforms).  Joined before the epilogue in every case.
  *   SE_OPT_REAL_CTAS     CTAs of the real-space kernel when it runs beside the wave pipeline (0 = one per cell).
- *   SE_OPT_XY_PATH       (x,y) transforms of power-of-two grids: 0 = own kernels, the y transforms and ONE kernel that
- *                        fuses the x transforms with the k-space scaling (default); 1 = cuFFT's batched 2-D complex plans
- *                        and a separate k-space kernel.
- *   SE_OPT_YZ_FUSED      with SE_OPT_XY_PATH = 0: 1 = the y and z transforms of a direction in ONE kernel (thread-block
+ *   SE_OPT_XY_PATH       reserved (round 1's cuFFT 2-D path was removed when the own y / fused x kernels replaced it);
+ *                        SE_ERR_INVALID_ARG.
+ *   SE_OPT_YZ_FUSED      1 = the y and z transforms of a direction in ONE kernel (thread-block
  *                        clusters exchanging through distributed shared memory; default for M <= 128), 0 = separate
  *                        z and y kernels.
  *   SE_OPT_GRAPH         1 = far_mobility_apply / _compressible keep the whole product as a plan-owned CUDA graph: the

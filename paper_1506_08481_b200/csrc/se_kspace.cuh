@@ -15,8 +15,8 @@
 
 #define KSPACE_THREADS 256
 
-// TR: spectra stored [kz][x][y] (own z transforms, se_zfft.cuh) instead of cuFFT's [x][y][kz].
-template <bool TR>
+// Used on the cuFFT 3-D path only (grids that are not powers of two, or flag SE_CUFFT3D); power-of-two grids run k_xmid
+// (se_xyfft.cuh), which fuses this arithmetic with the x transforms.
 __global__ void __launch_bounds__(KSPACE_THREADS) k_kspace(SeConst c, const double2 *__restrict__ Hk, double2 *__restrict__ Gk,
                                                            const double2 *__restrict__ Hsk, double2 *__restrict__ Pk)
 {
@@ -25,8 +25,7 @@ __global__ void __launch_bounds__(KSPACE_THREADS) k_kspace(SeConst c, const doub
     const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (q >= Gc) return;
     int ix, iy, iz;
-    if (TR) { iy = (int)(q % M); const size_t t = q / M; ix = (int)(t % M); iz = (int)(t / M); }
-    else { iz = (int)(q % Zc); const size_t t = q / Zc; iy = (int)(t % M); ix = (int)(t / M); }
+    { iz = (int)(q % Zc); const size_t t = q / Zc; iy = (int)(t % M); ix = (int)(t / M); }
     const int jx = ix < M / 2 ? ix : ix - M, jy = iy < M / 2 ? iy : iy - M, jz = iz;
     double2 u0 = make_double2(0.0, 0.0), u1 = u0, u2 = u0, w0 = u0, w1 = u0, w2 = u0, pk = u0;
     const bool zero = (ix == 0 && iy == 0 && iz == 0) || ix == M / 2 || iy == M / 2 || iz == M / 2;

@@ -1,5 +1,5 @@
 // C-ABI of the far-field mobility product (include/se_mobility.h): plan, orchestration, cuFFT calls.
-// Hand-written CUDA for sm_100a; cuFFT is used for the 3-D transforms only (a4, a6).
+// Hand-written CUDA for sm_100a; cuFFT is used only for grids that are not powers of two (batched 3-D real plans, a4 / a6).
 #include "../../include/se_mobility.h"
 
 #include <cuda_runtime.h>
@@ -81,15 +81,12 @@ struct se_plan {
     double2 *d_Hk_s, *d_Gk_p;      // their spectra
     double *d_pmom;                // [N][12] gathered pressure sums
     cufftHandle fft_fwd1, fft_inv1;
-    cufftHandle fftz_1;            // 2-D complex plan over (x,y), M/2+1 planes: the scalar / pressure grid on the own-z path
-    bool have_fftz1;
     bool have_comp;
     double *d_moments;             // [N][24] gathered wave-space sums in caller order
     // host-API staging
     double *d_io;                  // pos3 F3 T3 S5 U3 W3 E5 = 25 N doubles
     cufftHandle fft_fwd, fft_inv;  // 3-D batched plans (unfused path), made when first needed
     bool have_fwd, have_inv, have_fft1;
-    cufftHandle fftz_fwd, fftz_inv; // contiguous batched 2-D complex plans (x,y) of the own-z-transform path (se_zfft.cuh)
     bool have_zt;
     int lM;
     double2 *d_wtab;               // exp(-2 pi i q / M), q < M
@@ -103,7 +100,6 @@ struct se_plan {
     long gepoch, epoch;            // epoch: bumped by every setter that changes what apply_impl enqueues
     int graph_launches;
     bool warmed[2];                // a plain apply (lazy allocations done) was made: [0] without, [1] with the a9 arguments
-    int xy_path;                   // SE_OPT_XY_PATH: 0 = own y / fused x kernels, 1 = cuFFT 2-D plans + k_kspace
     int yz_fused;                  // SE_OPT_YZ_FUSED: (y,z) transforms in one cluster kernel per direction (se_zfft.cuh)
     size_t fft_bytes;
     cudaEvent_t ev[SE_NUM_STAGES + 1];
@@ -266,9 +262,7 @@ extern "C" se_status se_plan_destroy(se_plan *p)
     if (p->have_comp) {
         cudaFree(p->d_real_p); cudaFree(p->d_Hk_s); cudaFree(p->d_Gk_p); cudaFree(p->d_pmom);
         if (p->have_fft1) { cufftDestroy(p->fft_fwd1); cufftDestroy(p->fft_inv1); }
-        if (p->have_fftz1) cufftDestroy(p->fftz_1);
     }
-    if (p->have_zt) { cufftDestroy(p->fftz_fwd); cufftDestroy(p->fftz_inv); }
     cudaFree(p->d_wtab); cudaFree(p->d_etab);
     if (p->have_fwd) cufftDestroy(p->fft_fwd);
     if (p->have_inv) cufftDestroy(p->fft_inv);
@@ -514,43 +508,28 @@ static void dispatch_xmid(int lM, bool comp, const SeConst &c, cudaStream_t s, c
     }
 }
 
-// Plans of the own-z-transform path (se_zfft.cuh): contiguous batched 2-D complex transforms over (x,y), 3 (M/2+1)
-// planes forward and 6 (M/2+1) inverse, in place.
+// Tables and kernel attributes of the own-transform path (se_zfft.cuh, se_xyfft.cuh): power-of-two grids, no cuFFT.
 static se_status ensure_zt(se_plan *p)
 {
     if (p->have_zt) return SE_OK;
-    const int M = p->c.M, Zc = M / 2 + 1;
+    const int M = p->c.M;
     se_status st = ensure_wtab(p);
     if (st != SE_OK) return st;
-    int n2[2] = { M, M };
-    size_t ws = 0, tot = 0;
-    cufftResult r = cufftCreate(&p->fftz_fwd);
-    bool c1 = (r == CUFFT_SUCCESS), c2 = false;
-    if (c1) { r = cufftMakePlanMany(p->fftz_fwd, 2, n2, NULL, 1, 0, NULL, 1, 0, CUFFT_Z2Z, 3 * Zc, &ws); tot += ws; }
-    if (r == CUFFT_SUCCESS) { r = cufftCreate(&p->fftz_inv); c2 = (r == CUFFT_SUCCESS); }
-    if (r == CUFFT_SUCCESS) { r = cufftMakePlanMany(p->fftz_inv, 2, n2, NULL, 1, 0, NULL, 1, 0, CUFFT_Z2Z, 6 * Zc, &ws); tot += ws; }
-    if (r == CUFFT_SUCCESS &&
-        (raise_smem_limit(k_zfft_r2c<128>) != cudaSuccess || raise_smem_limit(k_zfft_c2r<128>) != cudaSuccess ||
-         raise_smem_limit(k_zfft_r2c<256>) != cudaSuccess || raise_smem_limit(k_zfft_c2r<256>) != cudaSuccess)) {
+    if (raise_smem_limit(k_zfft_r2c<128>) != cudaSuccess || raise_smem_limit(k_zfft_c2r<128>) != cudaSuccess ||
+        raise_smem_limit(k_zfft_r2c<256>) != cudaSuccess || raise_smem_limit(k_zfft_c2r<256>) != cudaSuccess) {
         cudaGetLastError();
-        r = CUFFT_INTERNAL_ERROR;
-    }
-    if (r != CUFFT_SUCCESS) {
-        if (c1) cufftDestroy(p->fftz_fwd);
-        if (c2) cufftDestroy(p->fftz_inv);
-        return fail(p, r == CUFFT_ALLOC_FAILED ? SE_ERR_ALLOC : SE_ERR_CUFFT, "ensure_zt", "2-D complex plans");
+        return fail(p, SE_ERR_CUDA, "ensure_zt", "shared-memory limit");
     }
     p->lM = 0;
     while ((1 << p->lM) < M) ++p->lM;
-    {
-        se_status ste = upload_etab(p);
-        if (ste == SE_OK && (dispatch_prepare_xy(p->lM) != cudaSuccess || dispatch_prepare_yz(p->lM) != cudaSuccess)) { cudaGetLastError(); ste = fail(p, SE_ERR_CUDA, "ensure_zt", "shared-memory limit"); }
-        if (ste != SE_OK) { cufftDestroy(p->fftz_fwd); cufftDestroy(p->fftz_inv); return ste; }
+    st = upload_etab(p);
+    if (st == SE_OK && (dispatch_prepare_xy(p->lM) != cudaSuccess || dispatch_prepare_yz(p->lM) != cudaSuccess)) {
+        cudaGetLastError();
+        st = fail(p, SE_ERR_CUDA, "ensure_zt", "shared-memory limit");
     }
+    if (st != SE_OK) return st;
     p->have_zt = true;
     p->yz_fused = M <= 128 ? 1 : 0;          // measured: clusters of 8 (M = 256) lose to the separate z and y kernels
-    p->fft_bytes += tot;
-    p->bytes += tot;
     return SE_OK;
 }
 
@@ -703,7 +682,6 @@ extern "C" se_status se_plan_set_option(se_plan *p, int key, int value)
     switch (key) {
     case SE_OPT_REAL_OVERLAP: if (value > 2) return SE_ERR_INVALID_ARG; p->real_overlap = value; break;
     case SE_OPT_REAL_CTAS: p->real_side_ctas = value; break;
-    case SE_OPT_XY_PATH: if (value > 1) return SE_ERR_INVALID_ARG; p->xy_path = value; break;
     case SE_OPT_YZ_FUSED: if (value > 1) return SE_ERR_INVALID_ARG; p->yz_fused = value; break;
     case SE_OPT_GRAPH: if (value > 1) return SE_ERR_INVALID_ARG; p->use_graph = value; break;
     case SE_OPT_PAIR_CACHE: if (value > 1) return SE_ERR_INVALID_ARG; p->pair_cache = value; if (!value) p->have_pairs = false; break;
@@ -838,24 +816,10 @@ static se_status ensure_compressible(se_plan *p)
     return SE_OK;
 }
 
-// Single-grid cuFFT plans of the compressible extension: the 2-D complex plan of the own-z-transform path, or the 3-D pair.
+// Single-grid cuFFT plans of the compressible extension (cuFFT 3-D path only; the own transforms need none).
 static se_status ensure_comp_plans(se_plan *p, bool zt)
 {
-    if (!zt) return ensure_fft3d(p, true);
-    if (p->have_fftz1) return SE_OK;
-    const int M = p->c.M;
-    int n2[2] = { M, M };
-    size_t ws = 0;
-    cufftResult r = cufftCreate(&p->fftz_1);
-    if (r == CUFFT_SUCCESS) {
-        r = cufftMakePlanMany(p->fftz_1, 2, n2, NULL, 1, 0, NULL, 1, 0, CUFFT_Z2Z, M / 2 + 1, &ws);
-        if (r != CUFFT_SUCCESS) cufftDestroy(p->fftz_1);
-    }
-    if (r != CUFFT_SUCCESS) return fail(p, r == CUFFT_ALLOC_FAILED ? SE_ERR_ALLOC : SE_ERR_CUFFT, "cufftMakePlanMany", "2-D plan of the compressible extension");
-    p->have_fftz1 = true;
-    p->fft_bytes += ws;
-    p->bytes += ws;
-    return SE_OK;
+    return zt ? SE_OK : ensure_fft3d(p, true);
 }
 
 // a1: wrap, the three counting sorts, packed records and real-space copies (F == NULL: zero moments).
@@ -948,7 +912,7 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     const bool use_zt = !(p->flags & SE_CUFFT3D) && xf_supported(p->c.M);
     if (use_zt) { se_status stf = ensure_zt(p); if (stf != SE_OK) return stf; }
     if (!use_zt) { se_status stf = ensure_fft3d(p, false); if (stf != SE_OK) return stf; }
-    if (comp && !(use_zt && p->xy_path == 0)) { se_status stf = ensure_comp_plans(p, use_zt); if (stf != SE_OK) return stf; }
+    if (comp) { se_status stf = ensure_comp_plans(p, use_zt); if (stf != SE_OK) return stf; }
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const SeConst &c = p->c;
     const unsigned fl = p->flags;
@@ -1017,7 +981,7 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     }
     if (fork && p->real_overlap == 2) { se_status sf = fork_real(); if (sf != SE_OK) return sf; }
     MARK();
-    const bool yz = use_zt && p->xy_path == 0 && p->yz_fused != 0;
+    const bool yz = use_zt && p->yz_fused != 0;
     if (on(SE_STAGE_FFT_FWD) && yz) {
         CUDA_TRY(p, dispatch_yz(p->lM, false, s, 3, p->d_real, p->d_Hk, nullptr, p->d_wtab, 0, 0, 0));
         p->last_launches += 1;
@@ -1031,27 +995,17 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
         else k_zfft_r2c<256><<<3 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_real, p->d_Hk, p->d_wtab);
         p->last_launches += 1;
         CUDA_TRY(p, cudaGetLastError());
-        if (p->xy_path == 0) {
-            dispatch_yfft(p->lM, s, p->d_Hk, p->d_wtab, 3, false);
-            p->last_launches += 1;
-            CUDA_TRY(p, cudaGetLastError());
-        } else {
-            CUFFT_TRY(p, cufftSetStream(p->fftz_fwd, s));
-            CUFFT_TRY(p, cufftExecZ2Z(p->fftz_fwd, (cufftDoubleComplex *)p->d_Hk, (cufftDoubleComplex *)p->d_Hk, CUFFT_FORWARD));
-        }
+        dispatch_yfft(p->lM, s, p->d_Hk, p->d_wtab, 3, false);
+        p->last_launches += 1;
+        CUDA_TRY(p, cudaGetLastError());
         if (comp_in) {
             if (zt_threads(M) <= 128) k_zfft_r2c<128><<<M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_real_p, p->d_Hk_s, p->d_wtab);
             else k_zfft_r2c<256><<<M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_real_p, p->d_Hk_s, p->d_wtab);
             p->last_launches += 1;
             CUDA_TRY(p, cudaGetLastError());
-            if (p->xy_path == 0) {
-                dispatch_yfft(p->lM, s, p->d_Hk_s, p->d_wtab, 1, false);
-                p->last_launches += 1;
-                CUDA_TRY(p, cudaGetLastError());
-            } else {
-                CUFFT_TRY(p, cufftSetStream(p->fftz_1, s));
-                CUFFT_TRY(p, cufftExecZ2Z(p->fftz_1, (cufftDoubleComplex *)p->d_Hk_s, (cufftDoubleComplex *)p->d_Hk_s, CUFFT_FORWARD));
-            }
+            dispatch_yfft(p->lM, s, p->d_Hk_s, p->d_wtab, 1, false);
+            p->last_launches += 1;
+            CUDA_TRY(p, cudaGetLastError());
         }
     } else if (on(SE_STAGE_FFT_FWD)) {
         CUFFT_TRY(p, cufftSetStream(p->fft_fwd, s));
@@ -1065,11 +1019,9 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     if (on(SE_STAGE_KSPACE)) {
         const size_t Gc = (size_t)c.M * c.M * (c.M / 2 + 1);
         const unsigned nbk = (unsigned)((Gc + KSPACE_THREADS - 1) / KSPACE_THREADS);
-        if (use_zt && p->xy_path == 0) dispatch_xmid(p->lM, comp, c, s, p->d_Hk, comp_in ? p->d_Hk_s : nullptr, p->d_Gk, comp_out ? p->d_Gk_p : nullptr,
-                                                      p->d_wtab, p->d_etab);
-        else if (use_zt) k_kspace<true><<<nbk, KSPACE_THREADS, 0, s>>>(c, p->d_Hk, p->d_Gk, comp_in ? p->d_Hk_s : nullptr,
-                                                                  comp_out ? p->d_Gk_p : nullptr);
-        else k_kspace<false><<<nbk, KSPACE_THREADS, 0, s>>>(c, p->d_Hk, p->d_Gk, comp_in ? p->d_Hk_s : nullptr,
+        if (use_zt) dispatch_xmid(p->lM, comp, c, s, p->d_Hk, comp_in ? p->d_Hk_s : nullptr, p->d_Gk, comp_out ? p->d_Gk_p : nullptr,
+                                  p->d_wtab, p->d_etab);
+        else k_kspace<<<nbk, KSPACE_THREADS, 0, s>>>(c, p->d_Hk, p->d_Gk, comp_in ? p->d_Hk_s : nullptr,
                                                             comp_out ? p->d_Gk_p : nullptr);
         p->last_launches += 1;
         CUDA_TRY(p, cudaGetLastError());
@@ -1086,27 +1038,17 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
         }
     } else if (on(SE_STAGE_FFT_INV) && use_zt) {
         const int M = c.M, MYp = p->gg.MYp, MZp = p->gg.MZp, halo = c.P - 1;
-        if (p->xy_path == 0) {
-            dispatch_yfft(p->lM, s, p->d_Gk, p->d_wtab, 6, true);
-            p->last_launches += 1;
-            CUDA_TRY(p, cudaGetLastError());
-        } else {
-            CUFFT_TRY(p, cufftSetStream(p->fftz_inv, s));
-            CUFFT_TRY(p, cufftExecZ2Z(p->fftz_inv, (cufftDoubleComplex *)p->d_Gk, (cufftDoubleComplex *)p->d_Gk, CUFFT_INVERSE));
-        }
+        dispatch_yfft(p->lM, s, p->d_Gk, p->d_wtab, 6, true);
+        p->last_launches += 1;
+        CUDA_TRY(p, cudaGetLastError());
         if (zt_threads(M) <= 128) k_zfft_c2r<128><<<6 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk, p->d_real, p->d_wtab, MYp, MZp, halo);
         else k_zfft_c2r<256><<<6 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk, p->d_real, p->d_wtab, MYp, MZp, halo);
         p->last_launches += 1;
         CUDA_TRY(p, cudaGetLastError());
         if (comp_out) {
-            if (p->xy_path == 0) {
-                dispatch_yfft(p->lM, s, p->d_Gk_p, p->d_wtab, 1, true);
-                p->last_launches += 1;
-                CUDA_TRY(p, cudaGetLastError());
-            } else {
-                CUFFT_TRY(p, cufftSetStream(p->fftz_1, s));
-                CUFFT_TRY(p, cufftExecZ2Z(p->fftz_1, (cufftDoubleComplex *)p->d_Gk_p, (cufftDoubleComplex *)p->d_Gk_p, CUFFT_INVERSE));
-            }
+            dispatch_yfft(p->lM, s, p->d_Gk_p, p->d_wtab, 1, true);
+            p->last_launches += 1;
+            CUDA_TRY(p, cudaGetLastError());
             if (zt_threads(M) <= 128) k_zfft_c2r<128><<<M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk_p, p->d_real_p, p->d_wtab, MYp, MZp, halo);
             else k_zfft_c2r<256><<<M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk_p, p->d_real_p, p->d_wtab, MYp, MZp, halo);
             p->last_launches += 1;
