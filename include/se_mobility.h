@@ -241,7 +241,7 @@ const char *se_last_error(const se_plan *plan);
 /* Release everything.  NULL is allowed. */
 se_status se_plan_destroy(se_plan *plan);
 
-/* Library version string, e.g. "se_mobility 0.1 (sm_100a)". */
+/* Library version string, e.g. "se_mobility 0.2 (sm_100a)". */
 const char *se_version(void);
 
 #ifdef __cplusplus

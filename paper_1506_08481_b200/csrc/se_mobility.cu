@@ -241,7 +241,7 @@ static cudaError_t raise_smem_limit(K kernel)
 
 static cudaError_t dispatch_prepare(int P);
 
-extern "C" const char *se_version(void) { return "se_mobility 0.1 (sm_100a)"; }
+extern "C" const char *se_version(void) { return "se_mobility 0.2 (sm_100a)"; }
 
 extern "C" const char *se_last_error(const se_plan *plan) { return plan ? plan->err : "null plan"; }
 
