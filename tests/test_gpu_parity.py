@@ -707,3 +707,18 @@ def test_sheared_lattice_other_paths(pk, oracle, workloads):
         A = oracle.o1_matrix_sheared(np.array([[0.3, 0.1, 0.7]]) * wl2.L, np.array([a]), wl2.L, gamma, xi, eta0=wl2.eta0, nimg=4, kmax=kmax)
         assert _rel(got[i], A) <= TOL, (i, _rel(got[i], A))
     assert np.abs(got[0] - np.diag(np.diag(got[0]))).max() > 1e-6 * np.abs(got[0]).max()
+
+
+def test_sheared_lattice_tiny_system_all_pairs_and_wrapping_supports(pk, oracle, workloads):
+    """Strain with fewer than three real-space cells per axis (all-pairs loop with the sheared minimum image) and with supports
+    that wrap onto themselves (P = M)."""
+    import workloads as W
+    sysm = workloads.random_small_system(7, 12, 9.0)
+    for M, P, gamma in ((24, 10, 0.5), (12, 12, -0.25)):
+        wl = W.Workload(name="tiny", N=12, L=9.0, radii=sysm["radii"], pos=sysm["pos"], F=sysm["F"], T=sysm["T"], S=sysm["S"],
+                        xi=0.9, rc=4.5, M=M, P=P, m=0.0)
+        r = Runner(pk, wl)
+        r.plan.set_strain(gamma)
+        assert r.plan.constants()["real_cells"] == 1
+        ref = oracle.o2_apply_sheared(wl.pos, wl.radii, wl.L, gamma, wl.xi, wl.rc, M, P, wl.F, wl.T, wl.S)
+        _check_blocks(r.run(), ref, TOL)
