@@ -946,7 +946,7 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     const bool fork = do_real && do_wave && !timing && stop < 0 && p->real_overlap > 0;
     auto launch_real = [&](cudaStream_t sr) {
         if (!pos && !comp && p->have_pairs) {          // cached configuration: stream the pair list
-            const unsigned nbc = (unsigned)((c.N + 7) / 8 < 148 * 16 ? (c.N + 7) / 8 : 148 * 16);
+            const unsigned nbc = (unsigned)((c.N + 7) / 8 < p->sms * 16 ? (c.N + 7) / 8 : p->sms * 16);   // 8 targets per CTA pass, 16 CTAs per SM
             k_real_cached<1><<<nbc, 128, 0, sr>>>(c, p->d_pair_start, p->d_pj, p->d_pd, p->d_rs_mom, p->d_rs_orig, p->d_out_real, 0);
             p->last_launches += 1;
             return;
@@ -1200,7 +1200,7 @@ extern "C" se_status far_mobility_apply_batch(se_plan *p, const double *pos, int
             const double *m = p->d_mom_b + rs * r;
             double *o = p->d_out_real_b + rs * r;
             if (p->have_pairs) {                      // cached pair list: one streaming pass for up to four right-hand sides
-                const unsigned nbc = (unsigned)((c.N + 7) / 8 < 148 * 16 ? (c.N + 7) / 8 : 148 * 16);
+                const unsigned nbc = (unsigned)((c.N + 7) / 8 < p->sms * 16 ? (c.N + 7) / 8 : p->sms * 16);   // 8 targets per CTA pass, 16 CTAs per SM
                 if (nrhs - r >= 4) { k_real_cached<4><<<nbc, 128, 0, s>>>(c, p->d_pair_start, p->d_pj, p->d_pd, m, p->d_rs_orig, o, rs); r += 4; }
                 else if (nrhs - r >= 2) { k_real_cached<2><<<nbc, 128, 0, s>>>(c, p->d_pair_start, p->d_pj, p->d_pd, m, p->d_rs_orig, o, rs); r += 2; }
                 else { k_real_cached<1><<<nbc, 128, 0, s>>>(c, p->d_pair_start, p->d_pj, p->d_pd, m, p->d_rs_orig, o, rs); r += 1; }
