@@ -136,6 +136,9 @@ __global__ void __launch_bounds__(YF_THREADS, 4) k_yfft(double2 *__restrict__ sp
 // ------------------------------------------------------------------------------------------------------------
 // x transforms fused with the k-space pass
 // ------------------------------------------------------------------------------------------------------------
+#ifndef XM_MINB
+#define XM_MINB 2                  // resident CTAs per SM k_xmid is compiled for when a CTA has <= 192 threads (3: spills, slower)
+#endif
 template <int LM, int YB, bool COMP> struct XmTraits {
     static constexpr int M = 1 << LM, M16 = M >> 4;
     static constexpr int NG = COMP ? 4 : 3;                           // thread groups: H_x, H_y, H_z (, Hs)
@@ -150,7 +153,7 @@ template <int LM, int YB, bool COMP> struct XmTraits {
 // deconvolved in the FRACTIONAL wave number, so the factor is e^{-k^2/4xi^2} (one exponential per mode) times the separable
 // e^{+eta_se kq^2/4xi^2} from the table (then Etab holds that factor).
 template <int LM, int YB, bool COMP, bool SHEAR>
-__global__ void __launch_bounds__(XmTraits<LM, YB, COMP>::NT, (XmTraits<LM, YB, COMP>::NT <= 192 ? 2 : 1))
+__global__ void __launch_bounds__(XmTraits<LM, YB, COMP>::NT, (XmTraits<LM, YB, COMP>::NT <= 192 ? XM_MINB : 1))
 k_xmid(SeConst c, const double2 *__restrict__ Hk, const double2 *__restrict__ Hsk, double2 *__restrict__ Gk,
        double2 *__restrict__ Pk, const double2 *__restrict__ Wtab, const double *__restrict__ Etab)
 {
