@@ -1017,3 +1017,192 @@ int o2_apply_sheared(int64_t N, double L, double gamma, const double *pos, const
     free(acc); free(uu);
     return status;
 }
+
+/* ------------------------------------------------------------------------------------------------
+ * O2, the other two ways of bringing in the particle size (Sec. 3.2), cubic box.
+ * Both differ from o2_apply (the hybrid approach) in the wave part only; steps are numbered as there.
+ *
+ *   variant 1, "real space" (L298-304): the size terms are derivatives of the shape function on BOTH sides.
+ *     spread  : H of Eq. 42 as in o2_apply (step 3);
+ *     k space : u_k only (steps 5-6 without w_k): 3 grids to wave space, 3 back (+1 +1 for the pressure);
+ *     gather  : U_i = D^3 sum_n [(1 + cF lap) gamma](d) u~            = D^3 sum gamma (1 + cF (4 al^2 d^2 -  6 al)) u~
+ *               E_i = D^3 sum_n -(1/2)[grad (1 + cS lap) gamma] u~ + T = D^3 sum al gamma (1 + cS (4 al^2 d^2 - 10 al)) (d u~ + u~ d)
+ *               Om_i as in o2_apply.          (lap gamma = (4 al^2 d^2 - 6 al) gamma, grad gamma = -2 al d gamma)
+ *
+ *   variant 2, "wave space" (L306-322, Eq. 49-52): only gamma itself is spread and gathered; every derivative is a
+ *     multiplication by the wave vector.  With the transform conventions of o2_apply (H_k = sum_n H e^{+ik.x},
+ *     returned grids sum_k (.) e^{-ik.x}) a gradient acting on gamma(x - r_j) in the spreading becomes -ik, and a
+ *     gradient acting on a returned grid becomes -ik as well.
+ *     spread  : H'_F = sum gamma F, H''_F = sum gamma a^2 F, H_T = sum gamma T, H'_S = sum gamma S, H''_S = sum gamma a^2 S   (Eq. 49)
+ *     k space : Heff_k = (H'_F - (k^2/6) H''_F) - (i/2) k x H_T + i (H'_S - (k^2/10) H''_S).k                     (Eq. 50, bracket)
+ *               [this is the transform of Eq. 42's H: F (1 + a^2/6 lap) gamma + (1/2) grad gamma x T - (1 + a^2/10 lap) S.grad gamma]
+ *               u_k as in o2_apply from Heff_k;   w_k = -k^2 u_k (Eq. 51);   om_k = -(i/2) k x u_k;
+ *               e0_k[ab] = -(i/2)(k_a u_b + k_b u_a);   e2_k = -k^2 e0_k
+ *     gather  : U_i = D^3 sum gamma (u~ + cF_i w~) (Eq. 52);  Om_i = D^3 sum gamma om~;  E_i = D^3 sum gamma (e0~ + cS_i e2~).
+ *     Grid count: the paper quotes 20 pairs with a symmetric S of six components; this restatement carries six
+ *     components for S, a^2 S, e0 and e2 (21 to wave space, 21 back) and removes the trace at the end like o2_apply.
+ *   Pressure moment and pressure (a9): the scalar grid Hs and the returned p~ carry no size terms and are spread and
+ *   gathered with gamma in every variant; p_k uses Heff_k in variant 2.
+ * ---------------------------------------------------------------------------------------------- */
+int o2_apply_variant(int variant, int64_t N, double L, const double *pos, const double *rad, double xi, double rc,
+                     int M, int P, double m, double eta0, unsigned parts,
+                     const double *F, const double *T, const double *S5, const double *s_in,
+                     double *U, double *W, double *E5, double *s_out)
+{
+    if (variant != 1 && variant != 2) return 2;
+    if (N < 1 || M < 2 || (M % 2) || P < 2 || P > M || !(rc > 0.0) || rc > 0.5 * L) return 2;
+    acc_t *acc = (acc_t *)calloc((size_t)N, sizeof(acc_t));
+    double *posw = (double *)malloc(sizeof(double) * 3 * (size_t)N);
+    if (!acc || !posw) { free(acc); free(posw); return 1; }
+    for (int64_t i = 0; i < 3 * N; ++i) posw[i] = wrap_box(pos[i], L);
+    int status = 0;
+
+    if (parts & PART_REAL) status = real_celllist(N, L, posw, rad, xi, rc, eta0, F, T, S5, s_in, acc);   /* step 8 */
+
+    if (!status && (parts & PART_WAVE)) {
+        const se_consts c = se_constants(L, xi, M, P, m);
+        const double al = c.alpha, D = c.Delta, V = L * L * L, D3 = D * D * D;
+        const int64_t G = (int64_t)M * M * M;
+        /* grid tables.  variant 1: in 0-2 H (3 s);            out 0-2 u~ (3 p~)
+         *               variant 2: in 0-2 F, 3-5 a^2 F, 6-8 T, 9-14 S, 15-20 a^2 S (21 s);
+         *                          out 0-2 u~, 3-5 w~, 6-8 om~, 9-14 e0~, 15-20 e2~ (21 p~);  pairs (a,b) in the order below */
+        static const int PA[6] = { 0, 0, 0, 1, 1, 2 }, PB[6] = { 0, 1, 2, 1, 2, 2 };
+        const int nbase = variant == 1 ? 3 : 21;
+        const int nin = nbase + (s_in ? 1 : 0), nout = nbase + (s_out ? 1 : 0);
+        double *H = (double *)calloc((size_t)(nin * G), sizeof(double));
+        double complex *Hk = (double complex *)malloc(sizeof(double complex) * (size_t)(nin * G));
+        double *Gr = (double *)malloc(sizeof(double) * (size_t)(nout * G));
+        double complex *work = (double complex *)malloc(sizeof(double complex) * (size_t)G);
+        if (!H || !Hk || !Gr || !work) status = 1;
+
+        if (!status) {                                                              /* step 3: spread */
+            for (int64_t j = 0; j < N; ++j) {
+                double S[3][3]; s5_to_33(S5 + 5 * j, S);
+                const double a2 = rad[j] * rad[j], cF = a2 / 6.0, cS = a2 / 10.0;
+                const double *Fj = F + 3 * j, *Tj = T + 3 * j;
+                double u[3]; int n0[3];
+                for (int d = 0; d < 3; ++d) { u[d] = posw[3 * j + d] * ((double)M / L); n0[d] = support_start(u[d], P); }
+                for (int a0 = 0; a0 < P; ++a0) for (int a1 = 0; a1 < P; ++a1) for (int a2i = 0; a2i < P; ++a2i) {
+                    const double d[3] = { ((n0[0] + a0) - u[0]) * D, ((n0[1] + a1) - u[1]) * D, ((n0[2] + a2i) - u[2]) * D };
+                    const double d2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+                    const double gam = c.gnorm * exp(-al * d2);
+                    const int64_t idx = gidx(M, n0[0] + a0, n0[1] + a1, n0[2] + a2i);
+                    if (variant == 1) {
+                        const double dxT[3] = { d[1] * Tj[2] - d[2] * Tj[1], d[2] * Tj[0] - d[0] * Tj[2], d[0] * Tj[1] - d[1] * Tj[0] };
+                        for (int a = 0; a < 3; ++a) {
+                            const double Sd = S[a][0] * d[0] + S[a][1] * d[1] + S[a][2] * d[2];
+                            H[a * G + idx] += gam * (Fj[a] * (1.0 + cF * (4.0 * al * al * d2 - 6.0 * al)) - al * dxT[a]
+                                                     + 2.0 * al * Sd * (1.0 + cS * (4.0 * al * al * d2 - 10.0 * al)));
+                        }
+                    } else {
+                        for (int a = 0; a < 3; ++a) {
+                            H[a * G + idx] += gam * Fj[a];
+                            H[(3 + a) * G + idx] += gam * a2 * Fj[a];
+                            H[(6 + a) * G + idx] += gam * Tj[a];
+                        }
+                        for (int e = 0; e < 6; ++e) {
+                            H[(9 + e) * G + idx] += gam * S[PA[e]][PB[e]];
+                            H[(15 + e) * G + idx] += gam * a2 * S[PA[e]][PB[e]];
+                        }
+                    }
+                    if (s_in) H[nbase * G + idx] += gam * s_in[j];
+                }
+            }
+            for (int64_t q = 0; q < nin * G; ++q) Hk[q] = H[q];                     /* step 4 */
+            for (int a = 0; a < nin && !status; ++a) status = fft3d(Hk + a * G, M, +1);
+        }
+
+        for (int og = 0; og < nout && !status; ++og) {                              /* steps 5-6, one returned grid at a time */
+            #pragma omp parallel for
+            for (int i0 = 0; i0 < M; ++i0) for (int i1 = 0; i1 < M; ++i1) for (int i2 = 0; i2 < M; ++i2) {
+                const int j0 = i0 < M / 2 ? i0 : i0 - M, j1 = i1 < M / 2 ? i1 : i1 - M, j2 = i2 < M / 2 ? i2 : i2 - M;
+                const int64_t q = ((int64_t)i0 * M + i1) * M + i2;
+                if ((j0 == 0 && j1 == 0 && j2 == 0) || j0 == -M / 2 || j1 == -M / 2 || j2 == -M / 2) { work[q] = 0; continue; }
+                const double k[3] = { 2.0 * M_PI * j0 / L, 2.0 * M_PI * j1 / L, 2.0 * M_PI * j2 / L };
+                const double k2 = k[0] * k[0] + k[1] * k[1] + k[2] * k[2];
+                const double dec = exp(-(1.0 - c.eta_se) * k2 / (4.0 * xi * xi));
+                const double sc = D3 / (eta0 * V) * (1.0 + k2 / (4.0 * xi * xi)) * dec / k2;
+                double complex h[3];
+                if (variant == 1) { h[0] = Hk[q]; h[1] = Hk[G + q]; h[2] = Hk[2 * G + q]; }
+                else {
+                    double complex Tk[3], Sk[3][3];
+                    for (int a = 0; a < 3; ++a) Tk[a] = Hk[(6 + a) * G + q];
+                    for (int e = 0; e < 6; ++e)
+                        Sk[PA[e]][PB[e]] = Sk[PB[e]][PA[e]] = Hk[(9 + e) * G + q] - (k2 / 10.0) * Hk[(15 + e) * G + q];
+                    const double complex kxT[3] = { k[1] * Tk[2] - k[2] * Tk[1], k[2] * Tk[0] - k[0] * Tk[2], k[0] * Tk[1] - k[1] * Tk[0] };
+                    for (int a = 0; a < 3; ++a)
+                        h[a] = Hk[a * G + q] - (k2 / 6.0) * Hk[(3 + a) * G + q] - 0.5 * I * kxT[a]
+                               + I * (Sk[a][0] * k[0] + Sk[a][1] * k[1] + Sk[a][2] * k[2]);
+                }
+                const double complex kh = k[0] * h[0] + k[1] * h[1] + k[2] * h[2];
+                double complex uk[3];
+                for (int a = 0; a < 3; ++a) {
+                    uk[a] = sc * (h[a] - k[a] * kh / k2);
+                    if (s_in) uk[a] += D3 / (4.0 * eta0 * V) * (I * k[a] / k2) * dec * Hk[nbase * G + q];
+                }
+                if (og == nbase) work[q] = D3 / V * (I * kh / k2) * dec;                                   /* p_k */
+                else if (og < 3) work[q] = uk[og];
+                else if (og < 6) work[q] = -k2 * uk[og - 3];
+                else if (og < 9) {
+                    const double complex kxu[3] = { k[1] * uk[2] - k[2] * uk[1], k[2] * uk[0] - k[0] * uk[2], k[0] * uk[1] - k[1] * uk[0] };
+                    work[q] = -0.5 * I * kxu[og - 6];
+                } else {
+                    const int e = (og - 9) % 6, a = PA[e], b = PB[e];
+                    const double complex e0 = -0.5 * I * (k[a] * uk[b] + k[b] * uk[a]);
+                    work[q] = og < 15 ? e0 : -k2 * e0;
+                }
+            }
+            status = fft3d(work, M, -1);
+            if (!status) for (int64_t q = 0; q < G; ++q) Gr[og * G + q] = creal(work[q]);
+        }
+
+        if (!status) {                                                              /* step 7: gather */
+            #pragma omp parallel for schedule(static)
+            for (int64_t i = 0; i < N; ++i) {
+                const double cF = rad[i] * rad[i] / 6.0, cS = rad[i] * rad[i] / 10.0;
+                double u[3]; int n0[3];
+                for (int d = 0; d < 3; ++d) { u[d] = posw[3 * i + d] * ((double)M / L); n0[d] = support_start(u[d], P); }
+                double aU[3] = { 0, 0, 0 }, aW[3] = { 0, 0, 0 }, aE[3][3] = { { 0 } }, ap = 0.0;
+                for (int a0 = 0; a0 < P; ++a0) for (int a1 = 0; a1 < P; ++a1) for (int a2i = 0; a2i < P; ++a2i) {
+                    const double d[3] = { ((n0[0] + a0) - u[0]) * D, ((n0[1] + a1) - u[1]) * D, ((n0[2] + a2i) - u[2]) * D };
+                    const double d2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+                    const double gam = c.gnorm * exp(-al * d2);
+                    const int64_t idx = gidx(M, n0[0] + a0, n0[1] + a1, n0[2] + a2i);
+                    if (variant == 1) {
+                        const double ut[3] = { Gr[idx], Gr[G + idx], Gr[2 * G + idx] };
+                        const double fU = 1.0 + cF * (4.0 * al * al * d2 - 6.0 * al), fE = 1.0 + cS * (4.0 * al * al * d2 - 10.0 * al);
+                        for (int a = 0; a < 3; ++a) aU[a] += gam * fU * ut[a];
+                        aW[0] += al * gam * (d[1] * ut[2] - d[2] * ut[1]);
+                        aW[1] += al * gam * (d[2] * ut[0] - d[0] * ut[2]);
+                        aW[2] += al * gam * (d[0] * ut[1] - d[1] * ut[0]);
+                        for (int a = 0; a < 3; ++a) for (int b = 0; b < 3; ++b) aE[a][b] += al * gam * fE * (d[a] * ut[b] + ut[a] * d[b]);
+                    } else {
+                        for (int a = 0; a < 3; ++a) {
+                            aU[a] += gam * (Gr[a * G + idx] + cF * Gr[(3 + a) * G + idx]);
+                            aW[a] += gam * Gr[(6 + a) * G + idx];
+                        }
+                        for (int e = 0; e < 6; ++e) {
+                            const double v = gam * (Gr[(9 + e) * G + idx] + cS * Gr[(15 + e) * G + idx]);
+                            aE[PA[e]][PB[e]] += v;
+                            if (PA[e] != PB[e]) aE[PB[e]][PA[e]] += v;
+                        }
+                    }
+                    if (s_out) ap += gam * Gr[nbase * G + idx];
+                }
+                for (int a = 0; a < 3; ++a) {
+                    acc[i].U[a] += D3 * aU[a]; acc[i].W[a] += D3 * aW[a];
+                    for (int b = 0; b < 3; ++b) acc[i].E[a][b] += D3 * aE[a][b];
+                }
+                acc[i].p += D3 * ap;
+            }
+        }
+        free(H); free(Hk); free(Gr); free(work);
+    }
+
+    if (!status) {
+        add_self_onebody(acc, N, rad, xi, eta0, parts, F, T, S5);                    /* step 9 */
+        acc_finish(acc, N, rad, U, W, E5, s_out);
+    }
+    free(acc); free(posw);
+    return status;
+}
