@@ -123,7 +123,7 @@ se_status se_plan_set_tuning(se_plan *plan, int spread_segments, int gather_segm
  *                        products silently recompute.
  * Errors: SE_ERR_INVALID_ARG for an unknown key or a value out of range. */
 enum { SE_OPT_REAL_OVERLAP = 0, SE_OPT_REAL_CTAS = 1, SE_OPT_XY_PATH = 2, SE_OPT_YZ_FUSED = 3, SE_OPT_GRAPH = 4, SE_OPT_PAIR_CACHE = 5,
-       SE_NUM_OPTS = 6 };
+       SE_OPT_SIZE_VARIANT = 6, SE_NUM_OPTS = 7 };
 se_status se_plan_set_option(se_plan *plan, int key, int value);
 
 /* Bitwise OR of the SE_* flags above. */

@@ -11,6 +11,8 @@ from . import build as _build
 
 SE_SKIP_REAL, SE_SKIP_WAVE, SE_SKIP_SELF, SE_SKIP_ONEBODY, SE_TIMING, SE_CUFFT3D = 0x1, 0x2, 0x4, 0x8, 0x10, 0x40
 SE_OPT_REAL_OVERLAP, SE_OPT_REAL_CTAS, SE_OPT_XY_PATH, SE_OPT_YZ_FUSED, SE_OPT_GRAPH, SE_OPT_PAIR_CACHE = 0, 1, 2, 3, 4, 5
+SE_OPT_SIZE_VARIANT, SE_OPT_GRID_FP32 = 6, 7
+SE_VARIANT_HYBRID, SE_VARIANT_REAL, SE_VARIANT_WAVE = 0, 1, 2
 SE_NUM_STAGES = 8
 STAGE_NAMES = ("sort", "real", "spread", "fft_fwd", "kspace", "fft_inv", "gather", "epilogue")
 _STATUS = {0: "SE_OK", 1: "SE_ERR_INVALID_ARG", 2: "SE_ERR_UNSUPPORTED", 3: "SE_ERR_ALLOC", 4: "SE_ERR_CUDA",

@@ -133,7 +133,11 @@ struct GatherWalk {
     }
 };
 
-template <int P>
+// RV (real-space size variant): the Faxen operators act on the Gaussian of the gather, (1 + cF lap) gamma
+// = gamma (1 + cF (4 al^2 d^2 - 6 al)) and its gradient, so four more sums per grid are needed,
+//     Q0[g] = sum gamma d^2 g,  Q1[g] = sum gamma d^2 dx g,  Qy[g], Qz[g],
+// from the x moments m2 = sum gx dx^2 g and m3 = sum gx dx^3 g: d^2 = dx^2 + dy^2 + dz^2.  Slot of (kind, g): kind*3 + g, g < 3.
+template <int P, bool RV>
 __global__ void __launch_bounds__((GR_WARPS + 1) * 32, 1)
 k_gather(SeConst c, GatherGeom g, const double *__restrict__ grecs, const int *__restrict__ start_g,
          const __grid_constant__ CUtensorMap tmap, int ngrids, double *__restrict__ moments, int mstride)
@@ -267,16 +271,21 @@ k_gather(SeConst c, GatherGeom g, const double *__restrict__ grecs, const int *_
                 int sl = srel + (mine ? j0 - ja : 0);                  // slot of my first plane (idle lanes: any loaded one)
                 if (sl >= R) sl -= R;
                 const double *__restrict__ col = ring + ((yz.x - I.Y0 + by) * WZ + (yz.y - I.Z0 + bz));
-                double m0[CY][CZ], m1[CY][CZ];
+                double m0[CY][CZ], m1[CY][CZ], m2[RV ? CY : 1][RV ? CZ : 1], m3[RV ? CY : 1][RV ? CZ : 1];
 #pragma unroll
                 for (int a = 0; a < CY; ++a)
 #pragma unroll
-                    for (int q = 0; q < CZ; ++q) { m0[a][q] = 0.0; m1[a][q] = 0.0; }
+                    for (int q = 0; q < CZ; ++q) {
+                        m0[a][q] = 0.0; m1[a][q] = 0.0;
+                        if (RV) { m2[a][q] = 0.0; m3[a][q] = 0.0; }
+                    }
                 const double2 *__restrict__ GX = reinterpret_cast<const double2 *>(rs + 4 + 2 * PP);
+                const double d0x = RV ? GX[0].y / GX[0].x : 0.0;      // the table holds (gx, gx dx); gx(0) >= e^{-m^2/2} > 0
 #pragma unroll
                 for (int k = 0; k < P; ++k) {
                     const double *__restrict__ pl = col + sl * SLOT;
                     const double2 gx = GX[k];
+                    const double dxk = fma((double)k, Delta, d0x), gx2 = gx.y * dxk, gx3 = gx2 * dxk;
 #pragma unroll
                     for (int a = 0; a < CY; ++a)
 #pragma unroll
@@ -284,11 +293,17 @@ k_gather(SeConst c, GatherGeom g, const double *__restrict__ grecs, const int *_
                             const double v = pl[4 * a * WZ + LZ * q];
                             m0[a][q] = fma(gx.x, v, m0[a][q]);
                             m1[a][q] = fma(gx.y, v, m1[a][q]);
+                            if (RV) {
+                                m2[a][q] = fma(gx2, v, m2[a][q]);
+                                m3[a][q] = fma(gx3, v, m3[a][q]);
+                            }
                         }
                     sl = sl + 1 == R ? 0 : sl + 1;
                 }
                 // weights: sums over this lane's columns of gy gz {m0, m1, dy m0, dz m0}; gy, gz are zero beyond P
                 const double d0y = rs[2] + by * Delta, d0z = rs[3] + bz * Delta;
+                constexpr int B1 = LP / 2, B2 = LP / 4, B3 = LP / 8;
+                if (!RV) {
                 double gz[CZ], gzd[CZ];
 #pragma unroll
                 for (int q = 0; q < CZ; ++q) { gz[q] = rs[4 + PP + bz + LZ * q]; gzd[q] = gz[q] * (d0z + (LZ * q) * Delta); }
@@ -311,7 +326,6 @@ k_gather(SeConst c, GatherGeom g, const double *__restrict__ grecs, const int *_
                 // reduce-scatter of the four sums over the LP lanes of the particle: the two highest lane bits select
                 // the kind (00 s0, 01 s1, 10 sy, 11 sz), the remaining bits are summed
                 {
-                    constexpr int B1 = LP / 2, B2 = LP / 4;
                     const bool hi = (hl & B1) != 0;
                     const double a = (hi ? sy : s0) + __shfl_xor_sync(0xffffffffu, hi ? s0 : sy, B1);
                     const double bb = (hi ? sz : s1) + __shfl_xor_sync(0xffffffffu, hi ? s1 : sz, B1);
@@ -322,6 +336,39 @@ k_gather(SeConst c, GatherGeom g, const double *__restrict__ grecs, const int *_
                     if ((hl & (B2 - 1)) == 0 && valid && mine) {
                         const int kind = (hi ? 2 : 0) | (h2 ? 1 : 0);
                         moments[(size_t)xo.y * mstride + (I.grid / 3) * 12 + kind * 3 + (I.grid % 3)] = tt;
+                    }
+                }
+                } else {
+                    // eight sums: kind 0 gamma, 1 gamma dx, 2 gamma dy, 3 gamma dz, 4..7 the same times d^2
+                    double sm[8];
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) sm[i] = 0.0;
+#pragma unroll
+                    for (int a = 0; a < CY; ++a) {
+                        const double gy = rs[4 + by + 4 * a], dy = d0y + (4 * a) * Delta;
+#pragma unroll
+                        for (int q = 0; q < CZ; ++q) {
+                            const double dz = d0z + (LZ * q) * Delta, w = gy * rs[4 + PP + bz + LZ * q];
+                            const double rho2 = fma(dy, dy, dz * dz);
+                            const double t0 = w * m0[a][q], t1 = w * m1[a][q];
+                            const double u0 = w * fma(rho2, m0[a][q], m2[a][q]), u1 = w * fma(rho2, m1[a][q], m3[a][q]);
+                            sm[0] += t0; sm[1] += t1; sm[2] = fma(dy, t0, sm[2]); sm[3] = fma(dz, t0, sm[3]);
+                            sm[4] += u0; sm[5] += u1; sm[6] = fma(dy, u0, sm[6]); sm[7] = fma(dz, u0, sm[7]);
+                        }
+                    }
+                    // reduce-scatter over the LP lanes: the three highest lane bits select the kind, the rest is summed
+                    const bool h1 = (hl & B1) != 0, h2 = (hl & B2) != 0, h3 = (hl & B3) != 0;
+                    double v4[4], v2[2];
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) v4[i] = (h1 ? sm[i + 4] : sm[i]) + __shfl_xor_sync(0xffffffffu, h1 ? sm[i] : sm[i + 4], B1);
+#pragma unroll
+                    for (int i = 0; i < 2; ++i) v2[i] = (h2 ? v4[i + 2] : v4[i]) + __shfl_xor_sync(0xffffffffu, h2 ? v4[i] : v4[i + 2], B2);
+                    double tt = (h3 ? v2[1] : v2[0]) + __shfl_xor_sync(0xffffffffu, h3 ? v2[0] : v2[1], B3);
+#pragma unroll
+                    for (int o = B3 / 2; o > 0; o >>= 1) tt += __shfl_xor_sync(0xffffffffu, tt, o);
+                    if ((hl & (B3 - 1)) == 0 && valid && mine) {
+                        const int kind = (h1 ? 4 : 0) | (h2 ? 2 : 0) | (h3 ? 1 : 0);
+                        moments[(size_t)xo.y * mstride + kind * 3 + I.grid] = tt;
                     }
                 }
             }
@@ -342,7 +389,8 @@ __global__ void k_epilogue(SeConst c, unsigned flags, const double *__restrict__
                            const double *__restrict__ out_real, const double *__restrict__ moments,
                            const double *__restrict__ pmom,     // gathered pressure sums [N][12], slot 0 used (a9), or NULL
                            double *__restrict__ U, double *__restrict__ W, double *__restrict__ E,
-                           double *__restrict__ s_out)           // 4 pi a^3 p'(r_i), Eq. 28 (a9), or NULL
+                           double *__restrict__ s_out,           // 4 pi a^3 p'(r_i), Eq. 28 (a9), or NULL
+                           int variant)                          // 0 hybrid, 1 real-space, 2 wave-space size terms (Sec. 3.2)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= c.N) return;
@@ -376,13 +424,17 @@ __global__ void k_epilogue(SeConst c, unsigned flags, const double *__restrict__
         // sheared lattice: the gathered offsets are fractional (times L); the physical gradient of the Gaussian carries the
         // metric vector D = (dx, dy - gamma dx, dz) (se_spread.cuh), so only the y moments change
         const double gm = c.gamma;
+        // real-space variant: slots 12.. hold the d^2-weighted sums Q of u~ instead of the sums of w~;
+        // lap gamma = (4 al^2 d^2 - 6 al) gamma for U, grad lap gamma = -2 al d (4 al^2 d^2 - 10 al) gamma for E
+        const double q2 = 4.0 * c.alpha * c.alpha, qU = variant == 1 ? -6.0 * c.alpha : 0.0, qE = variant == 1 ? -10.0 * c.alpha : 0.0;
+        const double qs = variant == 1 ? q2 : 1.0;
 #pragma unroll
         for (int g = 0; g < 3; ++g) {
             A0[g] = m[g]; A1[g] = m[3 + g]; Ay[g] = m[6 + g] - gm * m[3 + g]; Az[g] = m[9 + g];
-            v[g] += D3 * (A0[g] + cF * m[12 + g]);
-            C1[g] = A1[g] + cS * m[15 + g];
-            Cy[g] = Ay[g] + cS * (m[18 + g] - gm * m[15 + g]);
-            Cz[g] = Az[g] + cS * m[21 + g];
+            v[g] += D3 * (A0[g] + cF * (qs * m[12 + g] + qU * A0[g]));
+            C1[g] = A1[g] + cS * (qs * m[15 + g] + qE * A1[g]);
+            Cy[g] = Ay[g] + cS * (qs * (m[18 + g] - gm * m[15 + g]) + qE * Ay[g]);
+            Cz[g] = Az[g] + cS * (qs * m[21 + g] + qE * Az[g]);
         }
         v[3] += aD3 * (Ay[2] - Az[1]);
         v[4] += aD3 * (Az[0] - A1[2]);

@@ -83,6 +83,7 @@ struct se_plan {
     cufftHandle fft_fwd1, fft_inv1;
     bool have_comp;
     double *d_moments;             // [N][24] gathered wave-space sums in caller order
+    int size_variant;              // SE_OPT_SIZE_VARIANT: 0 hybrid (default), 1 real-space, 2 wave-space size terms (Sec. 3.2)
     // host-API staging
     double *d_io;                  // pos3 F3 T3 S5 U3 W3 E5 = 25 N doubles
     cufftHandle fft_fwd, fft_inv;  // 3-D batched plans (unfused path), made when first needed
@@ -693,6 +694,7 @@ extern "C" se_status se_plan_set_option(se_plan *p, int key, int value)
     case SE_OPT_YZ_FUSED: if (value > 1) return SE_ERR_INVALID_ARG; p->yz_fused = value; break;
     case SE_OPT_GRAPH: if (value > 1) return SE_ERR_INVALID_ARG; p->use_graph = value; break;
     case SE_OPT_PAIR_CACHE: if (value > 1) return SE_ERR_INVALID_ARG; p->pair_cache = value; if (!value) p->have_pairs = false; break;
+    case SE_OPT_SIZE_VARIANT: if (value > 2) return SE_ERR_INVALID_ARG; p->size_variant = value; break;
     default: return SE_ERR_INVALID_ARG;
     }
     return SE_OK;
@@ -755,10 +757,15 @@ template <int P>
 static void launch_gather(se_plan *p, cudaStream_t s, bool pressure)
 {
     const GatherGeom &g = p->gg;
-    const int ngrids = pressure ? 1 : 6;
+    const bool rv = !pressure && p->size_variant == 1;                            // real-space variant: u~ only, eight sums per grid
+    const int ngrids = pressure ? 1 : (rv ? 3 : 6);
     const int items = g.NTY * g.NTZ * ngrids;
     const unsigned blocks = (unsigned)(items < p->sms ? items : p->sms);          // persistent: one CTA per SM (work split: GatherWalk)
-    k_gather<P><<<blocks, (GR_WARPS + 1) * 32, p->gather_smem, s>>>(p->c, g, p->d_grecs, p->d_start_g, pressure ? p->tmap_p : p->tmap, ngrids,
+    if (rv) {
+        k_gather<P, true><<<blocks, (GR_WARPS + 1) * 32, p->gather_smem, s>>>(p->c, g, p->d_grecs, p->d_start_g, p->tmap, ngrids, p->d_moments, GATHER_SUMS);
+        return;
+    }
+    k_gather<P, false><<<blocks, (GR_WARPS + 1) * 32, p->gather_smem, s>>>(p->c, g, p->d_grecs, p->d_start_g, pressure ? p->tmap_p : p->tmap, ngrids,
                                                              pressure ? p->d_pmom : p->d_moments, pressure ? 12 : GATHER_SUMS);
 }
 
@@ -769,7 +776,8 @@ static cudaError_t prepare_sweeps()
     if (e == cudaSuccess) e = raise_smem_limit(k_spread<P, 4, false>);
     if (e == cudaSuccess) e = raise_smem_limit(k_spread<P, 3, true>);
     if (e == cudaSuccess) e = raise_smem_limit(k_spread<P, 4, true>);
-    if (e == cudaSuccess) e = raise_smem_limit(k_gather<P>);
+    if (e == cudaSuccess) e = raise_smem_limit(k_gather<P, false>);
+    if (e == cudaSuccess) e = raise_smem_limit(k_gather<P, true>);
     return e;
 }
 
@@ -914,7 +922,10 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     if (!F || !T || !S || !U || !Omega || !E) return fail(p, SE_ERR_INVALID_ARG, who, "null pointer");
     if (!pos && !p->have_positions) return fail(p, SE_ERR_INVALID_ARG, who, "pos is NULL and no positions were set (se_plan_set_positions)");
     const bool comp_in = s_in != nullptr, comp_out = s_out != nullptr, comp = comp_in || comp_out;
+    if (p->size_variant != 0 && p->c.gamma != 0.0)
+        return fail(p, SE_ERR_UNSUPPORTED, who, "the real-space and wave-space size variants are built for the cubic box (strain 0) only");
     if (comp) { se_status stc = ensure_compressible(p); if (stc != SE_OK) return stc; }
+    const int nret = p->size_variant == 1 ? 3 : 6;          // returned grids: u~ (+ w~ in the hybrid approach)
     // default for power-of-two grids: own z transforms with transposed spectra + contiguous 2-D complex cuFFT plans
     // (se_zfft.cuh); otherwise, and with SE_CUFFT3D, cuFFT's 3-D real transforms
     const bool use_zt = !(p->flags & SE_CUFFT3D) && xf_supported(p->c.M);
@@ -1037,7 +1048,7 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     MARK();
     if (on(SE_STAGE_FFT_INV) && yz) {
         const int MYp = p->gg.MYp, MZp = p->gg.MZp, halo = c.P - 1;
-        CUDA_TRY(p, dispatch_yz(p->lM, true, s, 6, nullptr, p->d_Gk, p->d_real, p->d_wtab, MYp, MZp, halo));
+        CUDA_TRY(p, dispatch_yz(p->lM, true, s, nret, nullptr, p->d_Gk, p->d_real, p->d_wtab, MYp, MZp, halo));
         p->last_launches += 1;
         if (comp_out) {
             CUDA_TRY(p, dispatch_yz(p->lM, true, s, 1, nullptr, p->d_Gk_p, p->d_real_p, p->d_wtab, MYp, MZp, halo));
@@ -1046,11 +1057,11 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
         }
     } else if (on(SE_STAGE_FFT_INV) && use_zt) {
         const int M = c.M, MYp = p->gg.MYp, MZp = p->gg.MZp, halo = c.P - 1;
-        dispatch_yfft(p->lM, s, p->d_Gk, p->d_wtab, 6, true);
+        dispatch_yfft(p->lM, s, p->d_Gk, p->d_wtab, nret, true);
         p->last_launches += 1;
         CUDA_TRY(p, cudaGetLastError());
-        if (zt_threads(M) <= 128) k_zfft_c2r<128><<<6 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk, p->d_real, p->d_wtab, MYp, MZp, halo);
-        else k_zfft_c2r<256><<<6 * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk, p->d_real, p->d_wtab, MYp, MZp, halo);
+        if (zt_threads(M) <= 128) k_zfft_c2r<128><<<nret * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk, p->d_real, p->d_wtab, MYp, MZp, halo);
+        else k_zfft_c2r<256><<<nret * M * (M / ZT_LINES), zt_threads(M), zt_smem_bytes(M), s>>>(M, p->lM - 1, p->d_Gk, p->d_real, p->d_wtab, MYp, MZp, halo);
         p->last_launches += 1;
         CUDA_TRY(p, cudaGetLastError());
         if (comp_out) {
@@ -1094,7 +1105,7 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     // ---- a8: epilogue ----
     if (fork) CUDA_TRY(p, cudaStreamWaitEvent(s, p->ev_join, 0));
     k_epilogue<<<nbN, TB, 0, s>>>(c, fl | (wave_done ? 0u : SE_SKIP_WAVE), p->d_radii, F, T, S, p->ext_out_real ? p->ext_out_real : p->d_out_real, p->d_moments,
-                                  comp_out && wave_done ? p->d_pmom : nullptr, U, Omega, E, s_out);
+                                  comp_out && wave_done ? p->d_pmom : nullptr, U, Omega, E, s_out, p->size_variant);
     p->last_launches += 1;
     CUDA_TRY(p, cudaGetLastError());
     MARK();

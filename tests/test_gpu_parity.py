@@ -722,3 +722,56 @@ def test_sheared_lattice_tiny_system_all_pairs_and_wrapping_supports(pk, oracle,
         assert r.plan.constants()["real_cells"] == 1
         ref = oracle.o2_apply_sheared(wl.pos, wl.radii, wl.L, gamma, wl.xi, wl.rc, M, P, wl.F, wl.T, wl.S)
         _check_blocks(r.run(), ref, TOL)
+
+
+# ------------------------------------------------------------------------------------------------
+# f3: the other two ways of bringing in the particle size (Sec. 3.2) against oracle.o2_apply_variant
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("name", ["c1", "c2", "c3"])
+def test_size_variant_parity(pk, oracle, workloads, name, variant):
+    """Real-space variant (derivatives of the Gaussian on both sides, u~ only comes back) and wave-space variant (plain
+    Gaussian, every derivative a wave-vector factor, a^2-weighted grids): wave part alone, full product, the compressible
+    entry point, the cuFFT 3-D path and the cached configuration."""
+    import torch
+    wl = workloads.make_workload(name)
+    r = Runner(pk, wl)
+    r.plan.set_option(pk.SE_OPT_SIZE_VARIANT, variant)
+    s_np = _pressure_moments(wl)
+
+    def ref(parts, s=None):
+        return oracle.o2_apply_variant(variant, wl.pos, wl.radii, wl.L, wl.xi, wl.rc, wl.M, wl.P, wl.F, wl.T, wl.S, s=s, parts=parts)
+
+    ref_wave = ref(oracle.PART_WAVE)
+    _check_blocks(r.run(flags=pk.SE_SKIP_REAL | pk.SE_SKIP_SELF | pk.SE_SKIP_ONEBODY), ref_wave, TOL_STAGE)
+    _check_blocks(r.run(flags=pk.SE_CUFFT3D | pk.SE_SKIP_REAL | pk.SE_SKIP_SELF | pk.SE_SKIP_ONEBODY), ref_wave, TOL_STAGE)
+    full = ref(oracle.PART_ALL)
+    _check_blocks(r.run(), full, TOL)
+    # it is a different discretisation, not the hybrid one in disguise
+    hyb = r.oracle(oracle)
+    assert _rel(full["E"], hyb["E"]) > 1e3 * TOL
+    # cached configuration
+    r.plan.set_positions(r.pos)
+    r.plan.apply(None, r.F, r.T, r.S, r.U, r.W, r.E)
+    torch.cuda.synchronize()
+    _check_blocks((r.U.cpu().numpy(), r.W.cpu().numpy(), r.E.cpu().numpy()), full, TOL)
+    # compressible entry point
+    s_in = torch.tensor(s_np, device=r.pos.device, dtype=torch.float64)
+    s_out = torch.full((wl.N,), float("nan"), device=r.pos.device, dtype=torch.float64)
+    r.plan.apply_compressible(r.pos, r.F, r.T, r.S, s_in, r.U, r.W, r.E, s_out)
+    torch.cuda.synchronize()
+    fc = ref(oracle.PART_ALL, s=s_np)
+    _check_blocks((r.U.cpu().numpy(), r.W.cpu().numpy(), r.E.cpu().numpy()), fc, TOL)
+    assert _rel(s_out.cpu().numpy(), fc["s_out"]) <= TOL
+    # back to the hybrid approach on the same plan
+    r.plan.set_option(pk.SE_OPT_SIZE_VARIANT, 0)
+    _check_blocks(r.run(), hyb, TOL)
+
+
+def test_size_variants_refuse_the_sheared_lattice(pk, workloads):
+    wl = workloads.make_workload("c1")
+    r = Runner(pk, wl)
+    r.plan.set_strain(0.3)
+    r.plan.set_option(pk.SE_OPT_SIZE_VARIANT, 1)
+    with pytest.raises(RuntimeError):
+        r.plan.apply(r.pos, r.F, r.T, r.S, r.U, r.W, r.E)
