@@ -121,6 +121,21 @@ se_status se_plan_set_tuning(se_plan *plan, int spread_segments, int gather_segm
  *                        stream that list.  Costs about 1.3 real-space sums once and 164 bytes per ordered pair
  *                        (c4: 0.66 GB); 0 = recompute the pairs in every product.  If the list cannot be allocated the
  *                        products silently recompute.
+ *   SE_OPT_SIZE_VARIANT  how the particle-size terms of the Faxen laws and of the multipole expansion enter the wave-space sum
+ *                        (Sec. 3.2); unlike the knobs above this one changes the DISCRETISATION, i.e. the result at
+ *                        a given P (all three converge to the same sum, Fig. 2):
+ *                        0 = hybrid (default; L324: derivatives of the Gaussian in the spreading, Laplacian in wave space,
+ *                            3 grids to wave space and 6 back);
+ *                        1 = real-space (L298-304: derivatives of the Gaussian on both sides; 3 grids to wave space, 3 back,
+ *                            the gather takes the d^2-weighted sums; the cheapest product, the largest P for a given accuracy);
+ *                        2 = wave-space (L306-322, Eq. 49-52: only the Gaussian is spread and gathered, F, a^2 F, T, S and
+ *                            a^2 S on grids of their own, every derivative a wave-vector factor; 21 grids to wave space and
+ *                            21 back in seven spreading passes and four gather batches through cuFFT's 3-D transforms; the
+ *                            smallest P for a given accuracy, about 6 products' worth of transforms; extra workspace of 24
+ *                            half spectra, allocated by the first such product; its stage timings put the seven passes
+ *                            under "spread" and the four batches under "gather"; se_plan_debug_stop is not available).
+ *                        Both alternatives cover the compressible entry point, cached positions and batches, and are
+ *                        built for the cubic box: with a non-zero strain the product returns SE_ERR_UNSUPPORTED.
  * Errors: SE_ERR_INVALID_ARG for an unknown key or a value out of range. */
 enum { SE_OPT_REAL_OVERLAP = 0, SE_OPT_REAL_CTAS = 1, SE_OPT_XY_PATH = 2, SE_OPT_YZ_FUSED = 3, SE_OPT_GRAPH = 4, SE_OPT_PAIR_CACHE = 5,
        SE_OPT_SIZE_VARIANT = 6, SE_NUM_OPTS = 7 };

@@ -386,7 +386,7 @@ k_gather(SeConst c, GatherGeom g, const double *__restrict__ grecs, const int *_
 //   E = al D^3 traceless(d q + q d) with the d-moments C1 = A1 + cS B1, Cy = Ay + cS By, Cz = Az + cS Bz.
 __global__ void k_epilogue(SeConst c, unsigned flags, const double *__restrict__ radii,
                            const double *__restrict__ F, const double *__restrict__ T, const double *__restrict__ S,
-                           const double *__restrict__ out_real, const double *__restrict__ moments,
+                           const double *__restrict__ out_real, const double *__restrict__ moments, int mstride,
                            const double *__restrict__ pmom,     // gathered pressure sums [N][12], slot 0 used (a9), or NULL
                            double *__restrict__ U, double *__restrict__ W, double *__restrict__ E,
                            double *__restrict__ s_out,           // 4 pi a^3 p'(r_i), Eq. 28 (a9), or NULL
@@ -418,7 +418,7 @@ __global__ void k_epilogue(SeConst c, unsigned flags, const double *__restrict__
         for (int k = 0; k < 11; ++k) v[k] += orl[k];
     }
     if (!(flags & 0x2u)) {                                   // wave-space part
-        const double *m = moments + (size_t)GATHER_SUMS * i;
+        const double *m = moments + (size_t)mstride * i;
         const double cF = a * a / 6.0, cS = a * a / 10.0, D3 = c.D3, aD3 = c.alpha * c.D3;
         double A0[3], A1[3], Ay[3], Az[3], C1[3], Cy[3], Cz[3];
         // sheared lattice: the gathered offsets are fractional (times L); the physical gradient of the Gaussian carries the
@@ -436,6 +436,14 @@ __global__ void k_epilogue(SeConst c, unsigned flags, const double *__restrict__
             Cy[g] = Ay[g] + cS * (qs * (m[18 + g] - gm * m[15 + g]) + qE * Ay[g]);
             Cz[g] = Az[g] + cS * (qs * m[21 + g] + qE * Az[g]);
         }
+        if (variant == 2) {
+            // wave-space variant: plain sums of om~ (slots 24..26), e0~ (36..38, 48..50) and e2~ (60..62, 72..74)
+            v[3] += D3 * m[24]; v[4] += D3 * m[25]; v[5] += D3 * m[26];
+            const double exx = m[36] + cS * m[60], exy = m[37] + cS * m[61], exz = m[38] + cS * m[62];
+            const double eyy = m[48] + cS * m[72], eyz = m[49] + cS * m[73], ezz = m[50] + cS * m[74];
+            const double tr3 = (exx + eyy + ezz) * (1.0 / 3.0);
+            v[6] += D3 * (exx - tr3); v[7] += D3 * exy; v[8] += D3 * exz; v[9] += D3 * (eyy - tr3); v[10] += D3 * eyz;
+        } else {
         v[3] += aD3 * (Ay[2] - Az[1]);
         v[4] += aD3 * (Az[0] - A1[2]);
         v[5] += aD3 * (A1[1] - Ay[0]);
@@ -446,6 +454,7 @@ __global__ void k_epilogue(SeConst c, unsigned flags, const double *__restrict__
         v[8] += aD3 * (C1[2] + Cz[0]);
         v[9] += aD3 * (eyy - tr3);
         v[10] += aD3 * (Cy[2] + Cz[1]);
+        }
     }
 #pragma unroll
     for (int k = 0; k < 3; ++k) {

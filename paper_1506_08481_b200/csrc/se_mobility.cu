@@ -83,6 +83,9 @@ struct se_plan {
     cufftHandle fft_fwd1, fft_inv1;
     bool have_comp;
     double *d_moments;             // [N][24] gathered wave-space sums in caller order
+    double *d_wrecs;               // wave-space variant: spreading records of the current pass [N][rec_stride]
+    double2 *d_Wk;                 // wave-space variant: 24 half spectra (cuFFT layout), transformed in place by k_kspace_wave
+    double *d_wmom;                // wave-space variant: gathered sums [N][96] (four batches of six returned grids)
     int size_variant;              // SE_OPT_SIZE_VARIANT: 0 hybrid (default), 1 real-space, 2 wave-space size terms (Sec. 3.2)
     // host-API staging
     double *d_io;                  // pos3 F3 T3 S5 U3 W3 E5 = 25 N doubles
@@ -266,6 +269,7 @@ extern "C" se_status se_plan_destroy(se_plan *p)
     if (p->have_side) { cudaStreamDestroy(p->side); cudaEventDestroy(p->ev_fork); cudaEventDestroy(p->ev_join); }
     cudaFree(p->d_bsum);
     cudaFree(p->d_rs_pos); cudaFree(p->d_rs_mom); cudaFree(p->d_rs_orig); cudaFree(p->d_recs);
+    cudaFree(p->d_wrecs); cudaFree(p->d_Wk); cudaFree(p->d_wmom);
     cudaFree(p->d_real); cudaFree(p->d_Hk); cudaFree(p->d_Gk);
     cudaFree(p->d_out_real); cudaFree(p->d_moments); cudaFree(p->d_io); cudaFree(p->d_mom_b); cudaFree(p->d_out_real_b);
     if (p->have_comp) {
@@ -738,23 +742,23 @@ static se_status scan_cells(se_plan *p, cudaStream_t s)
 }
 
 template <int P>
-static void launch_spread(se_plan *p, cudaStream_t s, bool comp_in)
+static void launch_spread(se_plan *p, cudaStream_t s, bool comp_in, const double *recs)
 {
     const SeConst &c = p->c;
     const long long warps = (long long)c.NBY * c.NBZ * c.nseg;
     const int blocks = (int)((warps + SWEEP_WARPS - 1) / SWEEP_WARPS);
     const size_t sm = sweep_smem_bytes(c.rec_stride);
     if (c.gamma != 0.0) {
-        if (comp_in) k_spread<P, 4, true><<<blocks, SWEEP_WARPS * 32, sm, s>>>(c, p->d_recs, p->d_start_s, p->d_real, p->d_real_p);
-        else k_spread<P, 3, true><<<blocks, SWEEP_WARPS * 32, sm, s>>>(c, p->d_recs, p->d_start_s, p->d_real, nullptr);
+        if (comp_in) k_spread<P, 4, true><<<blocks, SWEEP_WARPS * 32, sm, s>>>(c, recs, p->d_start_s, p->d_real, p->d_real_p);
+        else k_spread<P, 3, true><<<blocks, SWEEP_WARPS * 32, sm, s>>>(c, recs, p->d_start_s, p->d_real, nullptr);
     } else if (comp_in)
-        k_spread<P, 4, false><<<blocks, SWEEP_WARPS * 32, sm, s>>>(c, p->d_recs, p->d_start_s, p->d_real, p->d_real_p);
+        k_spread<P, 4, false><<<blocks, SWEEP_WARPS * 32, sm, s>>>(c, recs, p->d_start_s, p->d_real, p->d_real_p);
     else
-        k_spread<P, 3, false><<<blocks, SWEEP_WARPS * 32, sm, s>>>(c, p->d_recs, p->d_start_s, p->d_real, nullptr);
+        k_spread<P, 3, false><<<blocks, SWEEP_WARPS * 32, sm, s>>>(c, recs, p->d_start_s, p->d_real, nullptr);
 }
 
 template <int P>
-static void launch_gather(se_plan *p, cudaStream_t s, bool pressure)
+static void launch_gather(se_plan *p, cudaStream_t s, bool pressure, double *mom, int mstride)
 {
     const GatherGeom &g = p->gg;
     const bool rv = !pressure && p->size_variant == 1;                            // real-space variant: u~ only, eight sums per grid
@@ -766,7 +770,7 @@ static void launch_gather(se_plan *p, cudaStream_t s, bool pressure)
         return;
     }
     k_gather<P, false><<<blocks, (GR_WARPS + 1) * 32, p->gather_smem, s>>>(p->c, g, p->d_grecs, p->d_start_g, pressure ? p->tmap_p : p->tmap, ngrids,
-                                                             pressure ? p->d_pmom : p->d_moments, pressure ? 12 : GATHER_SUMS);
+                                                             pressure ? p->d_pmom : (mom ? mom : p->d_moments), pressure ? 12 : (mom ? mstride : GATHER_SUMS));
 }
 
 template <int P>
@@ -781,10 +785,11 @@ static cudaError_t prepare_sweeps()
     return e;
 }
 
-static void dispatch_spread(se_plan *p, cudaStream_t s, bool comp_in)
+static void dispatch_spread(se_plan *p, cudaStream_t s, bool comp_in, const double *recs = nullptr)
 {
+    if (!recs) recs = p->d_recs;
     switch (p->c.P) {
-#define X(v) case v: launch_spread<v>(p, s, comp_in); break;
+#define X(v) case v: launch_spread<v>(p, s, comp_in, recs); break;
         FOR_EACH_P(X)
 #undef X
     }
@@ -800,10 +805,10 @@ static cudaError_t dispatch_prepare(int P)
     return cudaErrorInvalidValue;
 }
 
-static void dispatch_gather(se_plan *p, cudaStream_t s, bool pressure)
+static void dispatch_gather(se_plan *p, cudaStream_t s, bool pressure, double *mom = nullptr, int mstride = 0)
 {
     switch (p->c.P) {
-#define X(v) case v: launch_gather<v>(p, s, pressure); break;
+#define X(v) case v: launch_gather<v>(p, s, pressure, mom, mstride); break;
         FOR_EACH_P(X)
 #undef X
     }
@@ -830,6 +835,24 @@ static se_status ensure_compressible(se_plan *p)
     }
     p->have_comp = true;
     return SE_OK;
+}
+
+// Buffers of the wave-space size variant (SE_OPT_SIZE_VARIANT = 2), made by the first product that needs them.
+static se_status ensure_wave_variant(se_plan *p)
+{
+    if (p->d_Wk) return SE_OK;
+    const int M = p->c.M;
+    const size_t Gc = (size_t)M * M * (M / 2 + 1);
+    se_status st = dev_alloc(p, &p->d_wrecs, (size_t)p->c.N * p->c.rec_stride);
+    if (st == SE_OK) st = dev_alloc(p, &p->d_wmom, 96 * (size_t)p->c.N);
+    if (st == SE_OK) st = dev_alloc(p, &p->d_Wk, 24 * Gc);
+    if (st == SE_OK && cudaMemset(p->d_wmom, 0, sizeof(double) * 96 * (size_t)p->c.N) != cudaSuccess) st = fail(p, SE_ERR_CUDA, "cudaMemset", "wave-variant sums");
+    if (st != SE_OK) {
+        cudaFree(p->d_wrecs); cudaFree(p->d_wmom); cudaFree(p->d_Wk);
+        p->d_wrecs = nullptr; p->d_wmom = nullptr; p->d_Wk = nullptr;
+        cudaGetLastError();
+    }
+    return st;
 }
 
 // Single-grid cuFFT plans of the compressible extension (cuFFT 3-D path only; the own transforms need none).
@@ -925,10 +948,15 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     if (p->size_variant != 0 && p->c.gamma != 0.0)
         return fail(p, SE_ERR_UNSUPPORTED, who, "the real-space and wave-space size variants are built for the cubic box (strain 0) only");
     if (comp) { se_status stc = ensure_compressible(p); if (stc != SE_OK) return stc; }
+    const bool wv = p->size_variant == 2;
     const int nret = p->size_variant == 1 ? 3 : 6;          // returned grids: u~ (+ w~ in the hybrid approach)
+    // wave-space variant: seven spreading passes of three plain grids each, cuFFT's 3-D transforms, one k-space pass on 24
+    // spectra, four batches of six returned grids through the gather
+    if (wv && p->debug_stop >= 0) return fail(p, SE_ERR_UNSUPPORTED, who, "se_plan_debug_stop with the wave-space size variant");
+    if (wv) { se_status stw = ensure_wave_variant(p); if (stw != SE_OK) return stw; }
     // default for power-of-two grids: own z transforms with transposed spectra + contiguous 2-D complex cuFFT plans
     // (se_zfft.cuh); otherwise, and with SE_CUFFT3D, cuFFT's 3-D real transforms
-    const bool use_zt = !(p->flags & SE_CUFFT3D) && xf_supported(p->c.M);
+    const bool use_zt = !wv && !(p->flags & SE_CUFFT3D) && xf_supported(p->c.M);
     if (use_zt) { se_status stf = ensure_zt(p); if (stf != SE_OK) return stf; }
     if (!use_zt) { se_status stf = ensure_fft3d(p, false); if (stf != SE_OK) return stf; }
     if (comp) { se_status stf = ensure_comp_plans(p, use_zt); if (stf != SE_OK) return stf; }
@@ -938,7 +966,7 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     const bool timing = (fl & SE_TIMING) != 0;
     const bool do_real = !(fl & SE_SKIP_REAL) && !p->ext_out_real, do_wave = !(fl & SE_SKIP_WAVE);
     const int stop = p->debug_stop;
-    auto on = [&](int stage) { return do_wave && (stop < 0 || stage <= stop); };
+    auto on = [&](int stage) { return do_wave && !wv && (stop < 0 || stage <= stop); };
     p->last_launches = 0;
     p->timed = false;
     p->err[0] = 0;
@@ -998,6 +1026,23 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
         p->last_launches += 1;
         CUDA_TRY(p, cudaGetLastError());
     }
+    if (wv && do_wave) {
+        // stage "spread" of the timings holds all seven passes (records, spreading, transform to wave space)
+        const size_t Gc = (size_t)c.M * c.M * (c.M / 2 + 1);
+        if (comp_in) p->real_p_padded = false;
+        CUFFT_TRY(p, cufftSetStream(p->fft_fwd, s));
+        for (int pass = 0; pass < 7; ++pass) {
+            k_plain_recs<<<(unsigned)((c.N + 3) / 4), 128, 0, s>>>(c, p->d_recs, p->d_wrecs, pass);
+            dispatch_spread(p, s, comp_in && pass == 0, p->d_wrecs);
+            p->last_launches += 2;
+            CUDA_TRY(p, cudaGetLastError());
+            CUFFT_TRY(p, cufftExecD2Z(p->fft_fwd, p->d_real, (cufftDoubleComplex *)(p->d_Wk + 3 * (size_t)pass * Gc)));
+            if (comp_in && pass == 0) {
+                CUFFT_TRY(p, cufftSetStream(p->fft_fwd1, s));
+                CUFFT_TRY(p, cufftExecD2Z(p->fft_fwd1, p->d_real_p, (cufftDoubleComplex *)p->d_Hk_s));
+            }
+        }
+    }
     if (fork && p->real_overlap == 2) { se_status sf = fork_real(); if (sf != SE_OK) return sf; }
     MARK();
     const bool yz = use_zt && p->yz_fused != 0;
@@ -1042,6 +1087,13 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
                                   p->d_wtab, p->d_etab);
         else k_kspace<<<nbk, KSPACE_THREADS, 0, s>>>(c, p->d_Hk, p->d_Gk, comp_in ? p->d_Hk_s : nullptr,
                                                             comp_out ? p->d_Gk_p : nullptr);
+        p->last_launches += 1;
+        CUDA_TRY(p, cudaGetLastError());
+    }
+    if (wv && do_wave) {
+        const size_t Gc = (size_t)c.M * c.M * (c.M / 2 + 1);
+        k_kspace_wave<<<(unsigned)((Gc + KSPACE_THREADS - 1) / KSPACE_THREADS), KSPACE_THREADS, 0, s>>>(c, p->d_Wk, comp_in ? p->d_Hk_s : nullptr,
+                                                                                                    comp_out ? p->d_Gk_p : nullptr);
         p->last_launches += 1;
         CUDA_TRY(p, cudaGetLastError());
     }
@@ -1101,10 +1153,33 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
         CUDA_TRY(p, cudaGetLastError());
         wave_done = true;
     }
+    if (wv && do_wave) {
+        // stage "gather" of the timings holds the four batches (transform back, halo, gather)
+        const int M = c.M, MYp = p->gg.MYp, MZp = p->gg.MZp, halo = c.P - 1;
+        const size_t Gc = (size_t)M * M * (M / 2 + 1), per = (size_t)MYp * MZp;
+        CUFFT_TRY(p, cufftSetStream(p->fft_inv, s));
+        for (int b = 0; b < 4; ++b) {
+            CUFFT_TRY(p, cufftExecZ2D(p->fft_inv, (cufftDoubleComplex *)(p->d_Wk + 6 * (size_t)b * Gc), p->d_real));
+            k_halo_fill<<<(unsigned)((6 * M * per + 255) / 256), 256, 0, s>>>(p->d_real, M, MYp, MZp, halo, (size_t)6 * M);
+            dispatch_gather(p, s, false, p->d_wmom + 24 * b, 96);
+            p->last_launches += 2;
+            CUDA_TRY(p, cudaGetLastError());
+        }
+        if (comp_out) {
+            CUFFT_TRY(p, cufftSetStream(p->fft_inv1, s));
+            CUFFT_TRY(p, cufftExecZ2D(p->fft_inv1, (cufftDoubleComplex *)p->d_Gk_p, p->d_real_p));
+            k_halo_fill<<<(unsigned)((M * per + 255) / 256), 256, 0, s>>>(p->d_real_p, M, MYp, MZp, halo, (size_t)M);
+            dispatch_gather(p, s, true);
+            p->last_launches += 2;
+            p->real_p_padded = true;
+            CUDA_TRY(p, cudaGetLastError());
+        }
+        wave_done = true;
+    }
     MARK();
     // ---- a8: epilogue ----
     if (fork) CUDA_TRY(p, cudaStreamWaitEvent(s, p->ev_join, 0));
-    k_epilogue<<<nbN, TB, 0, s>>>(c, fl | (wave_done ? 0u : SE_SKIP_WAVE), p->d_radii, F, T, S, p->ext_out_real ? p->ext_out_real : p->d_out_real, p->d_moments,
+    k_epilogue<<<nbN, TB, 0, s>>>(c, fl | (wave_done ? 0u : SE_SKIP_WAVE), p->d_radii, F, T, S, p->ext_out_real ? p->ext_out_real : p->d_out_real, wv ? p->d_wmom : p->d_moments, wv ? 96 : GATHER_SUMS,
                                   comp_out && wave_done ? p->d_pmom : nullptr, U, Omega, E, s_out, p->size_variant);
     p->last_launches += 1;
     CUDA_TRY(p, cudaGetLastError());
