@@ -136,9 +136,18 @@ se_status se_plan_set_tuning(se_plan *plan, int spread_segments, int gather_segm
  *                            under "spread" and the four batches under "gather"; se_plan_debug_stop is not available).
  *                        Both alternatives cover the compressible entry point, cached positions and batches, and are
  *                        built for the cubic box: with a non-zero strain the product returns SE_ERR_UNSUPPORTED.
+ *   SE_OPT_GRID_FP32     1 = single-precision mesh (Fig. 6: the paper's GPU code computes in single precision): the
+ *                        spread grids are rounded to fp32, transformed, scaled and transformed back in fp32 (cuFFT's 3-D
+ *                        R2C / C2R) and widened again for the gather; everything on the particle side (Gaussians, the
+ *                        accumulation of the spreading and of the gather, the real-space sum, the epilogue) stays fp64.
+ *                        Changes the RESULT: relative error about 3e-7 .. 3e-6 against the fp64 product (bound 1e-5 in the
+ *                        tests), the error floor of Fig. 6a.  Hybrid and real-space size variants, cubic or sheared box,
+ *                        compressible entry point included; with the wave-space variant the product returns
+ *                        SE_ERR_UNSUPPORTED.  Extra workspace (7 fp32 grids, 11 fp32 half spectra, cuFFT plans) is
+ *                        allocated by the first such product.  0 (default) = double precision throughout.
  * Errors: SE_ERR_INVALID_ARG for an unknown key or a value out of range. */
 enum { SE_OPT_REAL_OVERLAP = 0, SE_OPT_REAL_CTAS = 1, SE_OPT_XY_PATH = 2, SE_OPT_YZ_FUSED = 3, SE_OPT_GRAPH = 4, SE_OPT_PAIR_CACHE = 5,
-       SE_OPT_SIZE_VARIANT = 6, SE_NUM_OPTS = 7 };
+       SE_OPT_SIZE_VARIANT = 6, SE_OPT_GRID_FP32 = 7, SE_NUM_OPTS = 8 };
 se_status se_plan_set_option(se_plan *plan, int key, int value);
 
 /* Bitwise OR of the SE_* flags above. */

@@ -17,8 +17,16 @@
 
 // Used on the cuFFT 3-D path only (grids that are not powers of two, or flag SE_CUFFT3D); power-of-two grids run k_xmid
 // (se_xyfft.cuh), which fuses this arithmetic with the x transforms.
-__global__ void __launch_bounds__(KSPACE_THREADS) k_kspace(SeConst c, const double2 *__restrict__ Hk, double2 *__restrict__ Gk,
-                                                           const double2 *__restrict__ Hsk, double2 *__restrict__ Pk)
+// T2 = double2, or float2 for the single-precision mesh (SE_OPT_GRID_FP32): the spectra are then stored in fp32, the
+// factors are still formed in fp64.
+template <typename T2> __device__ __forceinline__ double2 ks_load(const T2 *p, size_t i) { const T2 v = p[i]; return make_double2((double)v.x, (double)v.y); }
+template <typename T2> __device__ __forceinline__ void ks_store(T2 *p, size_t i, double2 v);
+template <> __device__ __forceinline__ void ks_store<double2>(double2 *p, size_t i, double2 v) { p[i] = v; }
+template <> __device__ __forceinline__ void ks_store<float2>(float2 *p, size_t i, double2 v) { p[i] = make_float2((float)v.x, (float)v.y); }
+
+template <typename T2>
+__global__ void __launch_bounds__(KSPACE_THREADS) k_kspace(SeConst c, const T2 *__restrict__ Hk, T2 *__restrict__ Gk,
+                                                           const T2 *__restrict__ Hsk, T2 *__restrict__ Pk)
 {
     const int M = c.M, Zc = M / 2 + 1;
     const size_t Gc = (size_t)M * M * Zc;
@@ -36,13 +44,13 @@ __global__ void __launch_bounds__(KSPACE_THREADS) k_kspace(SeConst c, const doub
         const double kq2 = c.twopiL * c.twopiL * ((double)jx * jx + (double)jy * jy + (double)jz * jz);
         const double dec = c.gamma == 0.0 ? exp(-c.dec * k2) : exp(-k2 * c.inv4xi2 + c.eta_se * kq2 * c.inv4xi2);
         const double sc = c.scale0 * (1.0 + k2 * c.inv4xi2) * dec / k2;
-        const double2 h0 = Hk[q], h1 = Hk[Gc + q], h2 = Hk[2 * Gc + q];
+        const double2 h0 = ks_load(Hk, q), h1 = ks_load(Hk, Gc + q), h2 = ks_load(Hk, 2 * Gc + q);
         const double pr = (kx * h0.x + ky * h1.x + kz * h2.x) / k2, pi = (kx * h0.y + ky * h1.y + kz * h2.y) / k2;
         u0 = make_double2(sc * (h0.x - kx * pr), sc * (h0.y - kx * pi));
         u1 = make_double2(sc * (h1.x - ky * pr), sc * (h1.y - ky * pi));
         u2 = make_double2(sc * (h2.x - kz * pr), sc * (h2.y - kz * pi));
         if (Hsk) {                                   // -i (x + i y) = y - i x
-            const double2 hs = Hsk[q];
+            const double2 hs = ks_load(Hsk, q);
             const double cs = 0.25 * c.scale0 * dec / k2;
             u0.x += cs * kx * hs.y; u0.y -= cs * kx * hs.x;
             u1.x += cs * ky * hs.y; u1.y -= cs * ky * hs.x;
@@ -56,9 +64,29 @@ __global__ void __launch_bounds__(KSPACE_THREADS) k_kspace(SeConst c, const doub
         w1 = make_double2(-k2 * u1.x, -k2 * u1.y);
         w2 = make_double2(-k2 * u2.x, -k2 * u2.y);
     }
-    Gk[q] = u0; Gk[Gc + q] = u1; Gk[2 * Gc + q] = u2;
-    Gk[3 * Gc + q] = w0; Gk[4 * Gc + q] = w1; Gk[5 * Gc + q] = w2;
-    if (Pk) Pk[q] = pk;
+    ks_store(Gk, q, u0); ks_store(Gk, Gc + q, u1); ks_store(Gk, 2 * Gc + q, u2);
+    ks_store(Gk, 3 * Gc + q, w0); ks_store(Gk, 4 * Gc + q, w1); ks_store(Gk, 5 * Gc + q, w2);
+    if (Pk) ks_store(Pk, q, pk);
+}
+
+// Single-precision mesh: H (fp64, plain [n][M][M][M]) -> fp32 copy for the transforms.
+__global__ void k_grid_to_f32(const double *__restrict__ src, float *__restrict__ dst, size_t n)
+{
+    const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q < n) dst[q] = (float)src[q];
+}
+
+// Single-precision mesh: returned fp32 grids (plain [n][M][M][M]) -> the padded fp64 planes [MYp][MZp] the gather reads,
+// periodic halo included (rows M .. M+halo-1 and columns M .. M+halo repeat the first ones, as k_halo_fill writes them).
+__global__ void k_grid_from_f32(const float *__restrict__ src, double *__restrict__ Rg, int M, int MYp, int MZp, int halo, size_t nplanes)
+{
+    const size_t per = (size_t)MYp * MZp;
+    const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= nplanes * per) return;
+    const size_t pl = q / per;
+    const int r = (int)(q - pl * per), y = r / MZp, z = r - y * MZp;
+    if (y >= M + halo || z >= M + halo + 1) return;
+    Rg[q] = (double)src[(pl * M + (size_t)(y % M)) * M + (z % M)];
 }
 
 // Wave-space size variant (Eq. 49-52; SE_OPT_SIZE_VARIANT = 2): only the Gaussian itself is spread and

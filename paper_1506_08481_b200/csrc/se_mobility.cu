@@ -86,6 +86,11 @@ struct se_plan {
     double *d_wrecs;               // wave-space variant: spreading records of the current pass [N][rec_stride]
     double2 *d_Wk;                 // wave-space variant: 24 half spectra (cuFFT layout), transformed in place by k_kspace_wave
     double *d_wmom;                // wave-space variant: gathered sums [N][96] (four batches of six returned grids)
+    int grid_fp32;                 // SE_OPT_GRID_FP32: mesh (H, spectra, transforms, returned grids) in single precision
+    float *d_realf;                // fp32 mesh: [7][M^3] real grids (6 + pressure)
+    float2 *d_Hkf, *d_Gkf;         // fp32 mesh: [4][Gc] and [7][Gc] half spectra (3 + pressure moment, 6 + pressure)
+    cufftHandle fftf_fwd, fftf_inv, fftf_fwd1, fftf_inv1;
+    bool have_f32;
     int size_variant;              // SE_OPT_SIZE_VARIANT: 0 hybrid (default), 1 real-space, 2 wave-space size terms (Sec. 3.2)
     // host-API staging
     double *d_io;                  // pos3 F3 T3 S5 U3 W3 E5 = 25 N doubles
@@ -270,6 +275,8 @@ extern "C" se_status se_plan_destroy(se_plan *p)
     cudaFree(p->d_bsum);
     cudaFree(p->d_rs_pos); cudaFree(p->d_rs_mom); cudaFree(p->d_rs_orig); cudaFree(p->d_recs);
     cudaFree(p->d_wrecs); cudaFree(p->d_Wk); cudaFree(p->d_wmom);
+    cudaFree(p->d_realf); cudaFree(p->d_Hkf); cudaFree(p->d_Gkf);
+    if (p->have_f32) { cufftDestroy(p->fftf_fwd); cufftDestroy(p->fftf_inv); cufftDestroy(p->fftf_fwd1); cufftDestroy(p->fftf_inv1); }
     cudaFree(p->d_real); cudaFree(p->d_Hk); cudaFree(p->d_Gk);
     cudaFree(p->d_out_real); cudaFree(p->d_moments); cudaFree(p->d_io); cudaFree(p->d_mom_b); cudaFree(p->d_out_real_b);
     if (p->have_comp) {
@@ -699,6 +706,7 @@ extern "C" se_status se_plan_set_option(se_plan *p, int key, int value)
     case SE_OPT_GRAPH: if (value > 1) return SE_ERR_INVALID_ARG; p->use_graph = value; break;
     case SE_OPT_PAIR_CACHE: if (value > 1) return SE_ERR_INVALID_ARG; p->pair_cache = value; if (!value) p->have_pairs = false; break;
     case SE_OPT_SIZE_VARIANT: if (value > 2) return SE_ERR_INVALID_ARG; p->size_variant = value; break;
+    case SE_OPT_GRID_FP32: if (value > 1) return SE_ERR_INVALID_ARG; p->grid_fp32 = value; break;
     default: return SE_ERR_INVALID_ARG;
     }
     return SE_OK;
@@ -837,6 +845,41 @@ static se_status ensure_compressible(se_plan *p)
     return SE_OK;
 }
 
+// Buffers and cuFFT plans of the single-precision mesh (SE_OPT_GRID_FP32), made by the first product that needs them.
+static se_status ensure_f32(se_plan *p)
+{
+    if (p->have_f32) return SE_OK;
+    const int M = p->c.M;
+    const size_t G = (size_t)M * M * M, Gc = (size_t)M * M * (M / 2 + 1);
+    se_status st = dev_alloc(p, &p->d_realf, 7 * G);
+    if (st == SE_OK) st = dev_alloc(p, &p->d_Hkf, 4 * Gc);
+    if (st == SE_OK) st = dev_alloc(p, &p->d_Gkf, 7 * Gc);
+    int n3[3] = { M, M, M };
+    cufftHandle *h[4] = { &p->fftf_fwd, &p->fftf_inv, &p->fftf_fwd1, &p->fftf_inv1 };
+    const cufftType ty[4] = { CUFFT_R2C, CUFFT_C2R, CUFFT_R2C, CUFFT_C2R };
+    const int nb[4] = { 3, 6, 1, 1 };
+    int made = 0;
+    size_t tot = 0;
+    cufftResult r = CUFFT_SUCCESS;
+    for (int i = 0; i < 4 && st == SE_OK && r == CUFFT_SUCCESS; ++i) {
+        size_t ws = 0;
+        r = cufftCreate(h[i]);
+        if (r == CUFFT_SUCCESS) { ++made; r = cufftMakePlanMany(*h[i], 3, n3, NULL, 1, 0, NULL, 1, 0, ty[i], nb[i], &ws); tot += ws; }
+    }
+    if (st == SE_OK && r != CUFFT_SUCCESS) st = fail(p, r == CUFFT_ALLOC_FAILED ? SE_ERR_ALLOC : SE_ERR_CUFFT, "cufftMakePlanMany", "single-precision 3-D plans");
+    if (st != SE_OK) {
+        for (int i = 0; i < made; ++i) cufftDestroy(*h[i]);
+        cudaFree(p->d_realf); cudaFree(p->d_Hkf); cudaFree(p->d_Gkf);
+        p->d_realf = nullptr; p->d_Hkf = nullptr; p->d_Gkf = nullptr;
+        cudaGetLastError();
+        return st;
+    }
+    p->fft_bytes += tot;
+    p->bytes += tot;
+    p->have_f32 = true;
+    return SE_OK;
+}
+
 // Buffers of the wave-space size variant (SE_OPT_SIZE_VARIANT = 2), made by the first product that needs them.
 static se_status ensure_wave_variant(se_plan *p)
 {
@@ -956,10 +999,13 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     if (wv) { se_status stw = ensure_wave_variant(p); if (stw != SE_OK) return stw; }
     // default for power-of-two grids: own z transforms with transposed spectra + contiguous 2-D complex cuFFT plans
     // (se_zfft.cuh); otherwise, and with SE_CUFFT3D, cuFFT's 3-D real transforms
-    const bool use_zt = !wv && !(p->flags & SE_CUFFT3D) && xf_supported(p->c.M);
+    const bool f32 = p->grid_fp32 != 0 && !wv;
+    if (p->grid_fp32 != 0 && wv) return fail(p, SE_ERR_UNSUPPORTED, who, "the single-precision mesh is built for the hybrid and real-space size variants");
+    if (f32) { se_status st3 = ensure_f32(p); if (st3 != SE_OK) return st3; }
+    const bool use_zt = !wv && !f32 && !(p->flags & SE_CUFFT3D) && xf_supported(p->c.M);
     if (use_zt) { se_status stf = ensure_zt(p); if (stf != SE_OK) return stf; }
-    if (!use_zt) { se_status stf = ensure_fft3d(p, false); if (stf != SE_OK) return stf; }
-    if (comp) { se_status stf = ensure_comp_plans(p, use_zt); if (stf != SE_OK) return stf; }
+    if (!use_zt && !f32) { se_status stf = ensure_fft3d(p, false); if (stf != SE_OK) return stf; }
+    if (comp && !f32) { se_status stf = ensure_comp_plans(p, use_zt); if (stf != SE_OK) return stf; }
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const SeConst &c = p->c;
     const unsigned fl = p->flags;
@@ -1071,6 +1117,20 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
             p->last_launches += 1;
             CUDA_TRY(p, cudaGetLastError());
         }
+    } else if (on(SE_STAGE_FFT_FWD) && f32) {
+        const size_t G = (size_t)c.M * c.M * c.M;
+        k_grid_to_f32<<<(unsigned)((3 * G + 255) / 256), 256, 0, s>>>(p->d_real, p->d_realf, 3 * G);
+        p->last_launches += 1;
+        CUFFT_TRY(p, cufftSetStream(p->fftf_fwd, s));
+        CUFFT_TRY(p, cufftExecR2C(p->fftf_fwd, p->d_realf, (cufftComplex *)p->d_Hkf));
+        if (comp_in) {
+            const size_t Gc = (size_t)c.M * c.M * (c.M / 2 + 1);
+            k_grid_to_f32<<<(unsigned)((G + 255) / 256), 256, 0, s>>>(p->d_real_p, p->d_realf + 6 * G, G);
+            p->last_launches += 1;
+            CUFFT_TRY(p, cufftSetStream(p->fftf_fwd1, s));
+            CUFFT_TRY(p, cufftExecR2C(p->fftf_fwd1, p->d_realf + 6 * G, (cufftComplex *)(p->d_Hkf + 3 * Gc)));
+        }
+        CUDA_TRY(p, cudaGetLastError());
     } else if (on(SE_STAGE_FFT_FWD)) {
         CUFFT_TRY(p, cufftSetStream(p->fft_fwd, s));
         CUFFT_TRY(p, cufftExecD2Z(p->fft_fwd, p->d_real, (cufftDoubleComplex *)p->d_Hk));
@@ -1085,7 +1145,9 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
         const unsigned nbk = (unsigned)((Gc + KSPACE_THREADS - 1) / KSPACE_THREADS);
         if (use_zt) dispatch_xmid(p->lM, comp, c, s, p->d_Hk, comp_in ? p->d_Hk_s : nullptr, p->d_Gk, comp_out ? p->d_Gk_p : nullptr,
                                   p->d_wtab, p->d_etab);
-        else k_kspace<<<nbk, KSPACE_THREADS, 0, s>>>(c, p->d_Hk, p->d_Gk, comp_in ? p->d_Hk_s : nullptr,
+        else if (f32) k_kspace<float2><<<nbk, KSPACE_THREADS, 0, s>>>(c, p->d_Hkf, p->d_Gkf, comp_in ? p->d_Hkf + 3 * Gc : nullptr,
+                                                                     comp_out ? p->d_Gkf + 6 * Gc : nullptr);
+        else k_kspace<double2><<<nbk, KSPACE_THREADS, 0, s>>>(c, p->d_Hk, p->d_Gk, comp_in ? p->d_Hk_s : nullptr,
                                                             comp_out ? p->d_Gk_p : nullptr);
         p->last_launches += 1;
         CUDA_TRY(p, cudaGetLastError());
@@ -1126,6 +1188,21 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
             CUDA_TRY(p, cudaGetLastError());
             p->real_p_padded = true;
         }
+    } else if (on(SE_STAGE_FFT_INV) && f32) {
+        const int M = c.M, MYp = p->gg.MYp, MZp = p->gg.MZp, halo = c.P - 1;
+        const size_t per = (size_t)MYp * MZp, G = (size_t)M * M * M, Gc = (size_t)M * M * (M / 2 + 1);
+        CUFFT_TRY(p, cufftSetStream(p->fftf_inv, s));
+        CUFFT_TRY(p, cufftExecC2R(p->fftf_inv, (cufftComplex *)p->d_Gkf, p->d_realf));       // all six; the real-space variant gathers three
+        k_grid_from_f32<<<(unsigned)((nret * M * per + 255) / 256), 256, 0, s>>>(p->d_realf, p->d_real, M, MYp, MZp, halo, (size_t)nret * M);
+        p->last_launches += 1;
+        if (comp_out) {
+            CUFFT_TRY(p, cufftSetStream(p->fftf_inv1, s));
+            CUFFT_TRY(p, cufftExecC2R(p->fftf_inv1, (cufftComplex *)(p->d_Gkf + 6 * Gc), p->d_realf + 6 * G));
+            k_grid_from_f32<<<(unsigned)((M * per + 255) / 256), 256, 0, s>>>(p->d_realf + 6 * G, p->d_real_p, M, MYp, MZp, halo, (size_t)M);
+            p->last_launches += 1;
+            p->real_p_padded = true;
+        }
+        CUDA_TRY(p, cudaGetLastError());
     } else if (on(SE_STAGE_FFT_INV)) {
         const int M = c.M, MYp = p->gg.MYp, MZp = p->gg.MZp, halo = c.P - 1;
         const size_t per = (size_t)MYp * MZp;
