@@ -326,6 +326,31 @@ def main():
     stage = {k: statistics.median(v) for k, v in samples.items()}          # median over the timed steps
     plan.set_flags(0)
 
+    # ---- the other size-effect variants and the single-precision mesh, same workload, cold products.  They change
+    # the discretisation (or the precision), so they are reported beside the headline, never as it. ----
+    variants = {}
+    if world == 1 and not args.no_other_configs:
+        for key, opts, reps in (("real_space", {pk.SE_OPT_SIZE_VARIANT: 1}, args.steps), ("wave_space", {pk.SE_OPT_SIZE_VARIANT: 2}, max(2, args.steps // 5)),
+                                ("fp32_mesh", {pk.SE_OPT_GRID_FP32: 1}, args.steps), ("real_space_fp32_mesh", {pk.SE_OPT_SIZE_VARIANT: 1, pk.SE_OPT_GRID_FP32: 1}, args.steps)):
+            try:
+                for k, v in opts.items():
+                    plan.set_option(k, v)
+                for _ in range(2):
+                    plan.apply(pos, F, T, S, U, Om, E)
+                barrier()
+                v0, v1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                v0.record(stream)
+                for _ in range(reps):
+                    plan.apply(pos, F, T, S, U, Om, E)
+                v1.record(stream)
+                barrier()
+                variants[key] = {"ms_per_step": v0.elapsed_time(v1) / reps, "gpu_launches": plan.last_launch_count()}
+            except Exception as exc:               # e.g. the 24 extra spectra of the wave-space variant do not fit
+                variants[key] = {"error": str(exc)[:200]}
+            finally:
+                plan.set_option(pk.SE_OPT_SIZE_VARIANT, 0)
+                plan.set_option(pk.SE_OPT_GRID_FP32, 0)
+
     # ---- end to end through the C-ABI host entry point: pinned host buffers, H2D + D2H inside the timed region ----
     hp = lambda a: torch.tensor(np.ascontiguousarray(a), dtype=torch.float64).pin_memory().numpy()
     hpos, hF, hT, hS = hp(wl.pos), hp(wl.F), hp(wl.T), hp(wl.S)
@@ -445,6 +470,7 @@ def main():
         "gpu_launches": launches,
         "roofline": roofline,
         "cpu_baseline": cpu,
+        "size_variants": variants,
         "all_configs": others,
     }
     print(json.dumps(line), flush=True)
