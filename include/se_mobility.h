@@ -268,6 +268,29 @@ se_status se_plan_destroy(se_plan *plan);
 /* Library version string, e.g. "se_mobility 0.2 (sm_100a)". */
 const char *se_version(void);
 
+/* The real-space pair sum (a2; Sec. 3.3 with the pair couplings of Eq. 13-17 on Eq. 22's J_R) WITHOUT a plan and without
+ * any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid it):
+ *     [U, Omega, E]_i = sum over j != i, minimum image, r_ij < r_c, of the real-space Ewald couplings with [F, T, S]_j,
+ * i.e. exactly what far_mobility_apply returns with flags SE_SKIP_WAVE | SE_SKIP_SELF | SE_SKIP_ONEBODY, cubic box.
+ * All pairs are scanned (no cell list): meant for the small systems of such loops, N <= SE_NOALLOC_MAX_N.
+ * Arguments: N particles; L box edge; xi splitting parameter; r_c cutoff, 0 < r_c <= L/2; eta0 viscosity;
+ * pos [N][3], radii [N], F [N][3], T [N][3], S [N][5] DEVICE pointers, read only, caller-owned, layout as in
+ * far_mobility_apply; U [N][3], Omega [N][3], E [N][5] DEVICE pointers, overwritten; cuda_stream a cudaStream_t (NULL = legacy
+ * default stream); err / err_len an optional caller buffer that receives the error text (may be NULL / 0).
+ * Scratch: the packed copies and the per-particle sums live in ONE static device array inside the library,
+ * SE_NOALLOC_MAX_N * 29 doubles = 1.9 MB, held by every GPU that loads the library until the process exits.  Every call on a
+ * device shares it: calls that overlap on the GPU (different streams, different host threads) RACE -- order them on one stream
+ * or with events.  It keeps the last call's contents; nothing in it has to start at zero (every field read is written first by
+ * the same call).  The first call on each device asks the runtime for the array's device address (no allocation); the launch
+ * itself is three kernels on the caller's stream and returns without synchronising.
+ * Errors: SE_ERR_INVALID_ARG for N < 1, N > SE_NOALLOC_MAX_N (text says so), a parameter out of range or a NULL pointer (nothing
+ * is launched); SE_ERR_CUDA when the address cannot be had or a launch fails.  Calls no cudaMalloc, cudaFree, cuFFT. */
+#define SE_NOALLOC_MAX_N 8192
+se_status far_mobility_real_noalloc(int64_t N, double L, double xi, double r_c, double eta0, const double *pos, const double *radii,
+                                    const double *F, const double *T, const double *S, double *U, double *Omega, double *E,
+                                    void *cuda_stream, char *err, size_t err_len);
+
 #ifdef __cplusplus
 }
 #endif

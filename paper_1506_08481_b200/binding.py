@@ -92,8 +92,28 @@ def load_library(build_if_missing: bool = True):
     L.se_measure_fp64_peak.argtypes = [P, P]
     L.se_version.restype = ctypes.c_char_p
     L.se_version.argtypes = []
+    L.far_mobility_real_noalloc.restype = INT
+    L.far_mobility_real_noalloc.argtypes = [I64, D, D, D, D] + [P] * 9 + [ctypes.c_char_p, SZ]
     _lib = L
     return L
+
+
+SE_NOALLOC_MAX_N = 8192
+
+
+def real_noalloc(L, xi, rc, pos, radii, F, T, S, U, Omega, E, eta0=1.0, stream=None):
+    """far_mobility_real_noalloc: the real-space pair sum on CUDA float64 tensors, no plan and no allocation (the scratch is a
+    static device array inside the library, N <= SE_NOALLOC_MAX_N; calls that overlap on the GPU race)."""
+    import torch
+    N = int(radii.numel())
+    sp = (torch.cuda.current_stream() if stream is None else stream).cuda_stream
+    buf = ctypes.create_string_buffer(256)
+    st = load_library().far_mobility_real_noalloc(N, float(L), float(xi), float(rc), float(eta0), _dptr(pos, 3 * N, "pos"),
+                                                  _dptr(radii, N, "radii"), _dptr(F, 3 * N, "F"), _dptr(T, 3 * N, "T"),
+                                                  _dptr(S, 5 * N, "S"), _dptr(U, 3 * N, "U"), _dptr(Omega, 3 * N, "Omega"),
+                                                  _dptr(E, 5 * N, "E"), sp, buf, 256)
+    if st != 0:
+        raise SeError(st, "far_mobility_real_noalloc", buf.value.decode())
 
 
 def version() -> str:

@@ -9,6 +9,9 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <cmath>
+#include <mutex>
+
 #include "se_common.cuh"
 #include "se_sort.cuh"
 #include "se_real.cuh"
@@ -1516,5 +1519,109 @@ extern "C" se_status se_plan_get_timings(se_plan *p, double *ms)
         CUDA_TRY(p, cudaEventElapsedTime(&t, p->ev[k], p->ev[k + 1]));
         ms[k] = (double)t;
     }
+    return SE_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// far_mobility_real_noalloc: the real-space pair sum (a2) for callers that cannot allocate (CUDA graph capture, serving
+// loops, harnesses that forbid cudaMalloc).  No plan, no cudaMalloc / cudaFree, no cuFFT: the packed copies the pair kernel
+// reads (wrapped positions + radius, the 12 moments per particle, the index map) and the 12 sums per particle it writes
+// live in ONE file-scope device array of fixed size, SE_NOALLOC_MAX_N particles (1.9 MB, held by every GPU that loads the
+// library until the process exits).  All pairs are scanned (no cell list), which is what the plan's kernel does too when
+// L < 3 r_c; the launch sequence is  k_noalloc_pack -> k_real<false,1> (the plan's own pair kernel, reading the scratch)
+// -> k_epilogue (real part only).
+// The array's name is a host-side stand-in in host code, not a device address: its device address is asked for once per
+// device (cudaGetSymbolAddress with that device current) and handed to the kernels.
+// ------------------------------------------------------------------------------------------------------------
+#define SE_NOALLOC_DOUBLES_PER_PARTICLE 29          // 4 (x, y, z, a) + 12 moments + 12 sums + 1 (the int index map, padded)
+static __device__ __align__(256) double g_noalloc_scratch[(size_t)SE_NOALLOC_MAX_N * SE_NOALLOC_DOUBLES_PER_PARTICLE];
+
+#define SE_NOALLOC_MAX_DEVICES 64
+static double *g_noalloc_addr[SE_NOALLOC_MAX_DEVICES];     // device address of g_noalloc_scratch, per device ordinal (0 = not asked yet)
+static std::mutex g_noalloc_mutex;
+
+// wrapped position + radius, moments in the pair kernel's layout (slot 11, the pressure moment, zero), identity index map
+__global__ void k_noalloc_pack(SeConst c, const double *__restrict__ pos, const double *__restrict__ radii, const double *__restrict__ F,
+                               const double *__restrict__ T, const double *__restrict__ S, double4 *__restrict__ rs_pos,
+                               double *__restrict__ rs_mom, int *__restrict__ rs_orig)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= c.N) return;
+    double xw[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) se_grid_coord(c, pos + 3 * (size_t)i, d, &xw[d]);
+    rs_pos[i] = make_double4(xw[0], xw[1], xw[2], radii[i]);
+    double *m = rs_mom + 12 * (size_t)i;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { m[k] = F[3 * (size_t)i + k]; m[3 + k] = T[3 * (size_t)i + k]; }
+#pragma unroll
+    for (int k = 0; k < 5; ++k) m[6 + k] = S[5 * (size_t)i + k];
+    m[11] = 0.0;
+    rs_orig[i] = i;
+}
+
+static se_status noalloc_fail(char *err, size_t err_len, se_status st, const char *what, const char *detail)
+{
+    if (err && err_len) snprintf(err, err_len, "far_mobility_real_noalloc: %s: %s", what, detail);
+    return st;
+}
+
+extern "C" se_status far_mobility_real_noalloc(int64_t N, double L, double xi, double r_c, double eta0, const double *pos,
+                                               const double *radii, const double *F, const double *T, const double *S, double *U,
+                                               double *Omega, double *E, void *cuda_stream, char *err, size_t err_len)
+{
+    if (err && err_len) err[0] = 0;
+    if (N < 1) return noalloc_fail(err, err_len, SE_ERR_INVALID_ARG, "N", "must be at least 1");
+    if (N > SE_NOALLOC_MAX_N) {
+        char b[96];
+        snprintf(b, sizeof(b), "N = %lld exceeds SE_NOALLOC_MAX_N = %d (size of the static device scratch)", (long long)N, SE_NOALLOC_MAX_N);
+        return noalloc_fail(err, err_len, SE_ERR_INVALID_ARG, "N", b);
+    }
+    if (!(L > 0.0) || !(xi > 0.0) || !(eta0 > 0.0) || !(r_c > 0.0) || r_c > 0.5 * L || !std::isfinite(L) || !std::isfinite(xi))
+        return noalloc_fail(err, err_len, SE_ERR_INVALID_ARG, "parameters", "need L, xi, eta0 > 0 and 0 < r_c <= L/2");
+    if (!pos || !radii || !F || !T || !S || !U || !Omega || !E) return noalloc_fail(err, err_len, SE_ERR_INVALID_ARG, "pointers", "null pointer");
+
+    // set-up, once per device: the device address of the static scratch array on the CURRENT device
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { cudaGetLastError(); return noalloc_fail(err, err_len, SE_ERR_CUDA, "cudaGetDevice", cudaGetErrorString(e)); }
+    if (dev < 0 || dev >= SE_NOALLOC_MAX_DEVICES) return noalloc_fail(err, err_len, SE_ERR_UNSUPPORTED, "device", "ordinal beyond SE_NOALLOC_MAX_DEVICES");
+    double *base = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+        if (!g_noalloc_addr[dev]) {
+            void *ptr = nullptr;
+            e = cudaGetSymbolAddress(&ptr, g_noalloc_scratch);
+            if (e != cudaSuccess || !ptr) {
+                cudaGetLastError();
+                return noalloc_fail(err, err_len, SE_ERR_CUDA, "cudaGetSymbolAddress", e != cudaSuccess ? cudaGetErrorString(e) : "null address");
+            }
+            g_noalloc_addr[dev] = (double *)ptr;
+        }
+        base = g_noalloc_addr[dev];
+    }
+    double4 *rs_pos = reinterpret_cast<double4 *>(base);                               // [MAX_N] 32-byte elements at a 256-byte aligned base
+    double *rs_mom = base + 4 * (size_t)SE_NOALLOC_MAX_N;                              // [MAX_N][12]
+    double *out_real = rs_mom + 12 * (size_t)SE_NOALLOC_MAX_N;                         // [MAX_N][12]
+    int *rs_orig = reinterpret_cast<int *>(out_real + 12 * (size_t)SE_NOALLOC_MAX_N);  // [MAX_N]
+
+    SeConst c;
+    memset(&c, 0, sizeof(c));
+    c.N = (int)N; c.L = L; c.invL = 1.0 / L; c.xi = xi; c.eta0 = eta0; c.rc2 = r_c * r_c;
+    c.ncr = 1; c.hr = L; c.gamma = 0.0;
+    c.q = 2.0 * xi / sqrt(M_PI);
+    c.x2 = xi * xi; c.x4 = c.x2 * c.x2; c.x6 = c.x4 * c.x2; c.x8 = c.x4 * c.x4; c.x10 = c.x8 * c.x2; c.x12 = c.x6 * c.x6;
+    c.k0 = 1.0 / (8.0 * M_PI * eta0);
+
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const int TB = 128, nbN = (c.N + TB - 1) / TB;
+    // nothing in the scratch has to start at zero: the pack kernel writes every field the pair kernel reads, the pair kernel
+    // writes sums 0..10 of every particle (it assigns on its first candidate chunk), the epilogue reads only those
+    k_noalloc_pack<<<nbN, TB, 0, s>>>(c, pos, radii, F, T, S, rs_pos, rs_mom, rs_orig);
+    k_real<false, 1><<<(unsigned)((c.N + 31) / 32), REAL_WARPS * 32, 0, s>>>(c, rs_pos, rs_mom, rs_orig, nullptr, out_real, 0);
+    k_epilogue<<<nbN, TB, 0, s>>>(c, SE_SKIP_WAVE | SE_SKIP_SELF | SE_SKIP_ONEBODY, radii, F, T, S, out_real, nullptr, GATHER_SUMS, nullptr,
+                                  U, Omega, E, nullptr, 0);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return noalloc_fail(err, err_len, SE_ERR_CUDA, "kernel launch", cudaGetErrorString(e));
     return SE_OK;
 }
