@@ -227,6 +227,14 @@ se_status se_self_image_blocks(se_plan *plan, double *out, void *cuda_stream);
 se_status far_mobility_apply_host(se_plan *plan, const double *pos, const double *F, const double *T,
                                   const double *S, double *U, double *Omega, double *E, void *cuda_stream);
 
+/* The same without the final synchronisation: the three copies in, the product and the three copies out are enqueued on
+ * cuda_stream and the call returns.  With PINNED host arrays nothing blocks, so a caller with independent products can keep two
+ * in flight -- two plans on two streams -- and the copies of one overlap the kernels of the other (bench.py's "e2e" does this).
+ * The host arrays must stay valid, and the outputs must not be read, until the stream is synchronised; one plan carries one
+ * product at a time (its device buffers are reused by the next call on it).  Errors as far_mobility_apply. */
+se_status far_mobility_apply_host_async(se_plan *plan, const double *pos, const double *F, const double *T,
+                                  const double *S, double *U, double *Omega, double *E, void *cuda_stream);
+
 /* Staged outputs for parity tests (valid after the stream of the last apply has been synchronised).
  * which = 0: the three spread grids H_x,H_y,H_z, [3][M][M][M];  which = 1: the six returned grids
  * u~ (3), w~ (3), [6][M][M][M];  which = 2: the scalar grid of the compressible extension, [M][M][M]

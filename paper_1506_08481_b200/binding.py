@@ -72,6 +72,8 @@ def load_library(build_if_missing: bool = True):
     L.se_self_image_blocks.argtypes = [P, P, P]
     L.far_mobility_apply_host.restype = INT
     L.far_mobility_apply_host.argtypes = [P] * 9
+    L.far_mobility_apply_host_async.restype = INT
+    L.far_mobility_apply_host_async.argtypes = [P] * 9
     L.se_plan_copy_grids.restype = INT
     L.se_plan_copy_grids.argtypes = [P, INT, P]
     L.se_plan_debug_stop.restype = INT
@@ -241,6 +243,16 @@ class SePlan:
                                                _hptr(S, 5 * N, "S"), _hptr(U, 3 * N, "U"), _hptr(Omega, 3 * N, "Omega"),
                                                _hptr(E, 5 * N, "E"), sp)
         self._check(st, "far_mobility_apply_host")
+
+    def apply_host_async(self, pos, F, T, S, U, Omega, E, stream=None):
+        """far_mobility_apply_host_async on (pinned) numpy float64 arrays: enqueues copies and product, does not synchronise."""
+        import torch
+        N = self.N
+        sp = (torch.cuda.current_stream() if stream is None else stream).cuda_stream
+        st = self._lib.far_mobility_apply_host_async(self._h, _hptr(pos, 3 * N, "pos"), _hptr(F, 3 * N, "F"), _hptr(T, 3 * N, "T"),
+                                                     _hptr(S, 5 * N, "S"), _hptr(U, 3 * N, "U"), _hptr(Omega, 3 * N, "Omega"),
+                                                     _hptr(E, 5 * N, "E"), sp)
+        self._check(st, "far_mobility_apply_host_async")
 
     def copy_grids(self, which):
         out = np.empty(({0: 3, 1: 6, 2: 1}[which], self.M, self.M, self.M))

@@ -1397,8 +1397,8 @@ extern "C" se_status far_mobility_apply_batch(se_plan *p, const double *pos, int
     return st;
 }
 
-extern "C" se_status far_mobility_apply_host(se_plan *p, const double *pos, const double *F, const double *T,
-                                             const double *S, double *U, double *Omega, double *E, void *cuda_stream)
+extern "C" se_status far_mobility_apply_host_async(se_plan *p, const double *pos, const double *F, const double *T,
+                                                   const double *S, double *U, double *Omega, double *E, void *cuda_stream)
 {
     if (!p) return SE_ERR_INVALID_ARG;
     if (!pos || !F || !T || !S || !U || !Omega || !E) return fail(p, SE_ERR_INVALID_ARG, "far_mobility_apply_host", "null pointer");
@@ -1415,7 +1415,15 @@ extern "C" se_status far_mobility_apply_host(se_plan *p, const double *pos, cons
     CUDA_TRY(p, cudaMemcpyAsync(U, dU, 3 * N * B, cudaMemcpyDeviceToHost, s));
     CUDA_TRY(p, cudaMemcpyAsync(Omega, dW, 3 * N * B, cudaMemcpyDeviceToHost, s));
     CUDA_TRY(p, cudaMemcpyAsync(E, dE, 5 * N * B, cudaMemcpyDeviceToHost, s));
-    CUDA_TRY(p, cudaStreamSynchronize(s));
+    return SE_OK;
+}
+
+extern "C" se_status far_mobility_apply_host(se_plan *p, const double *pos, const double *F, const double *T,
+                                             const double *S, double *U, double *Omega, double *E, void *cuda_stream)
+{
+    const se_status st = far_mobility_apply_host_async(p, pos, F, T, S, U, Omega, E, cuda_stream);
+    if (st != SE_OK) return st;
+    CUDA_TRY(p, cudaStreamSynchronize((cudaStream_t)cuda_stream));
     return SE_OK;
 }
 

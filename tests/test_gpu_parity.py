@@ -204,6 +204,28 @@ def test_host_entry_point_and_stage_timings(pk, oracle, workloads):
     assert r.plan.workspace_bytes() > 6 * 8 * wl.M ** 3
 
 
+def test_async_host_entry_point_two_products_in_flight(pk, oracle, workloads):
+    """far_mobility_apply_host_async: two plans on two streams with pinned host arrays, several products each, different
+    right-hand sides per plan; results only read after the streams are synchronised, equal to the oracle's."""
+    import torch
+    wl = workloads.make_workload("c2")
+    pin = lambda a: torch.tensor(np.ascontiguousarray(a), dtype=torch.float64).pin_memory().numpy()
+    hpos = pin(wl.pos)
+    ins = [(pin(wl.F), pin(wl.T), pin(wl.S)), (pin(2.0 * wl.F), pin(-wl.T), pin(0.5 * wl.S))]
+    outs = [tuple(pin(np.full((wl.N, k), np.nan)) for k in (3, 3, 5)) for _ in range(2)]
+    plans = [pk.SePlan(wl.N, wl.L, wl.radii, wl.xi, wl.rc, wl.M, wl.P, wl.eta0) for _ in range(2)]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    for i in range(6):
+        j = i & 1
+        streams[j].synchronize()
+        plans[j].apply_host_async(hpos, *ins[j], *outs[j], stream=streams[j])
+    for st in streams:
+        st.synchronize()
+    refs = [oracle.o2_apply(wl.pos, wl.radii, wl.L, wl.xi, wl.rc, wl.M, wl.P, F, T, S) for (F, T, S) in ins]
+    for o, ref in zip(outs, refs):
+        _check_blocks(o, ref, TOL)
+
+
 def test_api_errors_on_device(pk, workloads):
     wl = workloads.make_workload("c1")
     r = Runner(pk, wl)
