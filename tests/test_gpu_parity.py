@@ -904,3 +904,37 @@ def test_fig6a_single_precision_floor(pk, oracle, workloads):
         assert abs(e32[P] - e64[P]) <= 0.02 * e64[P], (P, e64, e32)
     assert e64[21] < 1e-9 and 1e-8 < e32[21] < TOL_F32, (e64, e32)
     assert e32[21] <= 3.0 * e32[17], e32
+
+
+@pytest.mark.parametrize("variant", [1, 2])
+def test_size_variants_in_batches(pk, oracle, workloads, variant):
+    """far_mobility_apply_batch under SE_OPT_SIZE_VARIANT: per right-hand side parity with oracle.o2_apply_variant."""
+    import torch
+    wl = workloads.make_workload("c2")
+    r = Runner(pk, wl)
+    r.plan.set_option(pk.SE_OPT_SIZE_VARIANT, variant)
+    nrhs = 3
+    rng = np.random.default_rng([150608481, 91])
+    Fb, Tb, Sb = rng.standard_normal((nrhs, wl.N, 3)), rng.standard_normal((nrhs, wl.N, 3)), rng.standard_normal((nrhs, wl.N, 5))
+    dev = r.pos.device
+    t = lambda a: torch.tensor(a, device=dev, dtype=torch.float64)
+    U = torch.full((nrhs, wl.N, 3), float("nan"), device=dev, dtype=torch.float64)
+    W, E = torch.full_like(U, float("nan")), torch.full((nrhs, wl.N, 5), float("nan"), device=dev, dtype=torch.float64)
+    r.plan.apply_batch(r.pos, t(Fb), t(Tb), t(Sb), U, W, E)
+    torch.cuda.synchronize()
+    for k in range(nrhs):
+        ref = oracle.o2_apply_variant(variant, wl.pos, wl.radii, wl.L, wl.xi, wl.rc, wl.M, wl.P, Fb[k], Tb[k], Sb[k])
+        _check_blocks((U[k].cpu().numpy(), W[k].cpu().numpy(), E[k].cpu().numpy()), ref, TOL)
+
+
+def test_single_precision_mesh_on_the_sheared_lattice(pk, oracle, workloads):
+    """SE_OPT_GRID_FP32 with a strain: the fp32 k-space pass takes k = B.q as the fp64 one does."""
+    wl = workloads.make_workload("c2")
+    gamma = 0.3
+    r = Runner(pk, wl)
+    r.plan.set_strain(gamma)
+    r.plan.set_option(pk.SE_OPT_GRID_FP32, 1)
+    ref = oracle.o2_apply_sheared(wl.pos, wl.radii, wl.L, gamma, wl.xi, wl.rc, wl.M, wl.P, wl.F, wl.T, wl.S)
+    got = r.run()
+    _check_blocks(got, ref, TOL_F32)
+    assert _rel(got[0], ref["U"]) > 1e-10                    # really single precision on the mesh
