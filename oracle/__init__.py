@@ -57,6 +57,8 @@ def lib():
         L.o2_apply_sheared.argtypes = [_I64, _D, _D, _P, _P, _D, _D, _INT, _INT, _D, _D, _U, _P, _P, _P, _P, _P, _P, _P, _P, _P, _P]
         L.o2_apply_variant.restype = _INT
         L.o2_apply_variant.argtypes = [_INT, _I64, _D, _P, _P, _D, _D, _INT, _INT, _D, _D, _U, _P, _P, _P, _P, _P, _P, _P, _P]
+        L.o2_apply_variant_sheared.restype = _INT
+        L.o2_apply_variant_sheared.argtypes = [_INT, _I64, _D, _D, _P, _P, _D, _D, _INT, _INT, _D, _D, _U, _P, _P, _P, _P, _P, _P, _P, _P]
         L.o2_real_targets.restype = _INT
         L.o2_real_targets.argtypes = [_I64, _D, _P, _P, _D, _D, _D, _P, _P, _P, _P, _I64, _P, _P, _P, _P, _P]
         L.oracle_radial.restype = _D
@@ -218,6 +220,24 @@ def o2_apply_variant(variant, pos, radii, L, xi, rc, M, P, F, T, S, s=None, m=No
                                    _ptr(F), _ptr(T), _ptr(S), _ptr(s_in), _ptr(U), _ptr(W), _ptr(E), _ptr(so))
     if rcode:
         raise RuntimeError(f"o2_apply_variant status {rcode}")
+    return dict(U=U, Omega=W, E=E, s_out=so)
+
+
+def o2_apply_variant_sheared(variant, pos, radii, L, gamma, xi, rc, M, P, F, T, S, s=None, m=None, eta0=1.0, parts=PART_ALL):
+    """The real-space (1) or wave-space (2) size variant on the sheared lattice; variant 0 is o2_apply_sheared."""
+    if variant == VARIANT_HYBRID:
+        return o2_apply_sheared(pos, radii, L, gamma, xi, rc, M, P, F, T, S, s, m=m, eta0=eta0, parts=parts)
+    N = len(radii)
+    pos, radii, F, T, S = _c(pos, (N, 3)), _c(radii, (N,)), _c(F, (N, 3)), _c(T, (N, 3)), _c(S, (N, 5))
+    s_in = None if s is None else _c(s, (N,))
+    if m is None:
+        m = float(np.sqrt(np.pi * P))
+    U, W, E = np.zeros((N, 3)), np.zeros((N, 3)), np.zeros((N, 5))
+    so = None if s is None else np.zeros(N)
+    rcode = lib().o2_apply_variant_sheared(variant, N, L, gamma, _ptr(pos), _ptr(radii), xi, rc, M, P, m, eta0, parts,
+                                           _ptr(F), _ptr(T), _ptr(S), _ptr(s_in), _ptr(U), _ptr(W), _ptr(E), _ptr(so))
+    if rcode:
+        raise RuntimeError(f"o2_apply_variant_sheared status {rcode}")
     return dict(U=U, Omega=W, E=E, s_out=so)
 
 

@@ -1206,3 +1206,198 @@ int o2_apply_variant(int variant, int64_t N, double L, const double *pos, const 
     free(acc); free(posw);
     return status;
 }
+
+/* ------------------------------------------------------------------------------------------------
+ * The real-space and wave-space size variants on the SHEARED lattice (Fig. 2 shows both at gamma = 0.5).
+ * o2_apply_variant with the changes o2_apply_sheared makes to o2_apply (its header): wrapped fractional coordinates, the
+ * Gaussian isotropic in the grid offsets d, physical derivatives through D = (d0, d1 - gamma d0, d2) and Mt, k = B.q in every
+ * wave-vector factor, deconvolution in the fractional wave number, brute-force real part with the sheared minimum image.
+ *   variant 1: spread as o2_apply_sheared; u~ only; gather with the SAME operators on the Gaussian (the adjoint of the spreading):
+ *       U  = D^3 sum gam [1 + cF lapf] u~,                           lapf = 4 al^2 D.D - 2 al tr Mt
+ *       Om = D^3 sum al gam D x u~
+ *       E  = D^3 sum gam { al [1 + cS lapf] (D u~ + u~ D) - 4 al^2 cS (Mt.D u~ + u~ Mt.D) }     [-(1/2) grad (1 + cS lap) gam, symmetrised]
+ *   variant 2: plain gam on both sides, k = B.q in H_eff, u, w, om, e0, e2 as in o2_apply_variant.
+ * ---------------------------------------------------------------------------------------------- */
+int o2_apply_variant_sheared(int variant, int64_t N, double L, double gamma, const double *pos, const double *rad, double xi, double rc,
+                             int M, int P, double m, double eta0, unsigned parts,
+                             const double *F, const double *T, const double *S5, const double *s_in,
+                             double *U, double *W, double *E5, double *s_out)
+{
+    if (variant != 1 && variant != 2) return 2;
+    if (N < 1 || M < 2 || (M % 2) || P < 2 || P > M || !(rc > 0.0) || rc > 0.5 * L) return 2;
+    acc_t *acc = (acc_t *)calloc((size_t)N, sizeof(acc_t));
+    double *uu = (double *)malloc(sizeof(double) * 3 * (size_t)N);
+    if (!acc || !uu) { free(acc); free(uu); return 1; }
+    const double invL = 1.0 / L;
+    for (int64_t i = 0; i < N; ++i) {                                              /* step 2 */
+        const double t[3] = { (pos[3 * i] - gamma * pos[3 * i + 1]) * invL, pos[3 * i + 1] * invL, pos[3 * i + 2] * invL };
+        for (int d = 0; d < 3; ++d) uu[3 * i + d] = (t[d] - floor(t[d])) * (double)M;
+    }
+    int status = 0;
+
+    if (parts & PART_REAL) {                                                        /* step 8 */
+        radtab rt; radtab_build(xi, &rt);
+        #pragma omp parallel for schedule(dynamic, 16)
+        for (int64_t i = 0; i < N; ++i)
+            for (int64_t j = 0; j < N; ++j) {
+                if (j == i) continue;
+                double x[3]; min_image_sheared(pos + 3 * i, pos + 3 * j, L, gamma, x);
+                const double r2 = x[0] * x[0] + x[1] * x[1] + x[2] * x[2];
+                if (!(r2 < rc * rc) || r2 == 0.0) continue;
+                double S[3][3]; s5_to_33(S5 + 5 * j, S);
+                pair_real(&rt, x, rad[i], rad[j], eta0, F + 3 * j, T + 3 * j, S, s_in ? s_in[j] : 0.0, &acc[i]);
+            }
+    }
+
+    if (parts & PART_WAVE) {
+        const se_consts c = se_constants(L, xi, M, P, m);
+        const double al = c.alpha, D = c.Delta, V = L * L * L, D3 = D * D * D, trM = 3.0 + gamma * gamma;
+        const int64_t G = (int64_t)M * M * M;
+        static const int PA[6] = { 0, 0, 0, 1, 1, 2 }, PB[6] = { 0, 1, 2, 1, 2, 2 };
+        const int nbase = variant == 1 ? 3 : 21;
+        const int nin = nbase + (s_in ? 1 : 0), nout = nbase + (s_out ? 1 : 0);
+        double *H = (double *)calloc((size_t)(nin * G), sizeof(double));
+        double complex *Hk = (double complex *)malloc(sizeof(double complex) * (size_t)(nin * G));
+        double *Gr = (double *)malloc(sizeof(double) * (size_t)(nout * G));
+        double complex *work = (double complex *)malloc(sizeof(double complex) * (size_t)G);
+        if (!H || !Hk || !Gr || !work) status = 1;
+
+        if (!status) {                                                              /* step 3 */
+            for (int64_t j = 0; j < N; ++j) {
+                double S[3][3]; s5_to_33(S5 + 5 * j, S);
+                const double a2 = rad[j] * rad[j], cF = a2 / 6.0, cS = a2 / 10.0;
+                const double *Fj = F + 3 * j, *Tj = T + 3 * j, *u = uu + 3 * j;
+                int n0[3];
+                for (int d = 0; d < 3; ++d) n0[d] = support_start(u[d], P);
+                for (int a0 = 0; a0 < P; ++a0) for (int a1 = 0; a1 < P; ++a1) for (int a2i = 0; a2i < P; ++a2i) {
+                    const double d[3] = { ((n0[0] + a0) - u[0]) * D, ((n0[1] + a1) - u[1]) * D, ((n0[2] + a2i) - u[2]) * D };
+                    const double gam = c.gnorm * exp(-al * (d[0] * d[0] + d[1] * d[1] + d[2] * d[2]));
+                    const int64_t idx = gidx(M, n0[0] + a0, n0[1] + a1, n0[2] + a2i);
+                    if (variant == 1) {
+                        const double Dv[3] = { d[0], d[1] - gamma * d[0], d[2] };
+                        const double MD[3] = { Dv[0] - gamma * Dv[1], -gamma * Dv[0] + (1.0 + gamma * gamma) * Dv[1], Dv[2] };
+                        const double lapf = 4.0 * al * al * (Dv[0] * Dv[0] + Dv[1] * Dv[1] + Dv[2] * Dv[2]) - 2.0 * al * trM;
+                        const double DxT[3] = { Dv[1] * Tj[2] - Dv[2] * Tj[1], Dv[2] * Tj[0] - Dv[0] * Tj[2], Dv[0] * Tj[1] - Dv[1] * Tj[0] };
+                        for (int a = 0; a < 3; ++a) {
+                            const double SD = S[a][0] * Dv[0] + S[a][1] * Dv[1] + S[a][2] * Dv[2];
+                            const double SMD = S[a][0] * MD[0] + S[a][1] * MD[1] + S[a][2] * MD[2];
+                            H[a * G + idx] += gam * (Fj[a] * (1.0 + cF * lapf) - al * DxT[a] + 2.0 * al * SD * (1.0 + cS * lapf)
+                                                     - 8.0 * al * al * cS * SMD);
+                        }
+                    } else {
+                        for (int a = 0; a < 3; ++a) {
+                            H[a * G + idx] += gam * Fj[a];
+                            H[(3 + a) * G + idx] += gam * a2 * Fj[a];
+                            H[(6 + a) * G + idx] += gam * Tj[a];
+                        }
+                        for (int e = 0; e < 6; ++e) {
+                            H[(9 + e) * G + idx] += gam * S[PA[e]][PB[e]];
+                            H[(15 + e) * G + idx] += gam * a2 * S[PA[e]][PB[e]];
+                        }
+                    }
+                    if (s_in) H[nbase * G + idx] += gam * s_in[j];
+                }
+            }
+            for (int64_t q = 0; q < nin * G; ++q) Hk[q] = H[q];                     /* step 4 */
+            for (int a = 0; a < nin && !status; ++a) status = fft3d(Hk + a * G, M, +1);
+        }
+
+        for (int og = 0; og < nout && !status; ++og) {                              /* steps 5-6 */
+            #pragma omp parallel for
+            for (int i0 = 0; i0 < M; ++i0) for (int i1 = 0; i1 < M; ++i1) for (int i2 = 0; i2 < M; ++i2) {
+                const int j0 = i0 < M / 2 ? i0 : i0 - M, j1 = i1 < M / 2 ? i1 : i1 - M, j2 = i2 < M / 2 ? i2 : i2 - M;
+                const int64_t q = ((int64_t)i0 * M + i1) * M + i2;
+                if ((j0 == 0 && j1 == 0 && j2 == 0) || j0 == -M / 2 || j1 == -M / 2 || j2 == -M / 2) { work[q] = 0; continue; }
+                const double k[3] = { 2.0 * M_PI * j0 / L, 2.0 * M_PI * (j1 - gamma * j0) / L, 2.0 * M_PI * j2 / L };
+                const double k2 = k[0] * k[0] + k[1] * k[1] + k[2] * k[2];
+                const double kq2 = (2.0 * M_PI / L) * (2.0 * M_PI / L) * ((double)j0 * j0 + (double)j1 * j1 + (double)j2 * j2);
+                const double dec = exp(-k2 / (4.0 * xi * xi) + c.eta_se * kq2 / (4.0 * xi * xi));
+                const double sc = D3 / (eta0 * V) * (1.0 + k2 / (4.0 * xi * xi)) * dec / k2;
+                double complex h[3];
+                if (variant == 1) { h[0] = Hk[q]; h[1] = Hk[G + q]; h[2] = Hk[2 * G + q]; }
+                else {
+                    double complex Tk[3], Sk[3][3];
+                    for (int a = 0; a < 3; ++a) Tk[a] = Hk[(6 + a) * G + q];
+                    for (int e = 0; e < 6; ++e)
+                        Sk[PA[e]][PB[e]] = Sk[PB[e]][PA[e]] = Hk[(9 + e) * G + q] - (k2 / 10.0) * Hk[(15 + e) * G + q];
+                    const double complex kxT[3] = { k[1] * Tk[2] - k[2] * Tk[1], k[2] * Tk[0] - k[0] * Tk[2], k[0] * Tk[1] - k[1] * Tk[0] };
+                    for (int a = 0; a < 3; ++a)
+                        h[a] = Hk[a * G + q] - (k2 / 6.0) * Hk[(3 + a) * G + q] - 0.5 * I * kxT[a]
+                               + I * (Sk[a][0] * k[0] + Sk[a][1] * k[1] + Sk[a][2] * k[2]);
+                }
+                const double complex kh = k[0] * h[0] + k[1] * h[1] + k[2] * h[2];
+                double complex uk[3];
+                for (int a = 0; a < 3; ++a) {
+                    uk[a] = sc * (h[a] - k[a] * kh / k2);
+                    if (s_in) uk[a] += D3 / (4.0 * eta0 * V) * (I * k[a] / k2) * dec * Hk[nbase * G + q];
+                }
+                if (og == nbase) work[q] = D3 / V * (I * kh / k2) * dec;
+                else if (og < 3) work[q] = uk[og];
+                else if (og < 6) work[q] = -k2 * uk[og - 3];
+                else if (og < 9) {
+                    const double complex kxu[3] = { k[1] * uk[2] - k[2] * uk[1], k[2] * uk[0] - k[0] * uk[2], k[0] * uk[1] - k[1] * uk[0] };
+                    work[q] = -0.5 * I * kxu[og - 6];
+                } else {
+                    const int e = (og - 9) % 6, a = PA[e], b = PB[e];
+                    const double complex e0 = -0.5 * I * (k[a] * uk[b] + k[b] * uk[a]);
+                    work[q] = og < 15 ? e0 : -k2 * e0;
+                }
+            }
+            status = fft3d(work, M, -1);
+            if (!status) for (int64_t q = 0; q < G; ++q) Gr[og * G + q] = creal(work[q]);
+        }
+
+        if (!status) {                                                              /* step 7 */
+            #pragma omp parallel for schedule(static)
+            for (int64_t i = 0; i < N; ++i) {
+                const double cF = rad[i] * rad[i] / 6.0, cS = rad[i] * rad[i] / 10.0;
+                const double *u = uu + 3 * i;
+                int n0[3];
+                for (int d = 0; d < 3; ++d) n0[d] = support_start(u[d], P);
+                double aU[3] = { 0, 0, 0 }, aW[3] = { 0, 0, 0 }, aE[3][3] = { { 0 } }, ap = 0.0;
+                for (int a0 = 0; a0 < P; ++a0) for (int a1 = 0; a1 < P; ++a1) for (int a2i = 0; a2i < P; ++a2i) {
+                    const double d[3] = { ((n0[0] + a0) - u[0]) * D, ((n0[1] + a1) - u[1]) * D, ((n0[2] + a2i) - u[2]) * D };
+                    const double gam = c.gnorm * exp(-al * (d[0] * d[0] + d[1] * d[1] + d[2] * d[2]));
+                    const int64_t idx = gidx(M, n0[0] + a0, n0[1] + a1, n0[2] + a2i);
+                    if (variant == 1) {
+                        const double Dv[3] = { d[0], d[1] - gamma * d[0], d[2] };
+                        const double MD[3] = { Dv[0] - gamma * Dv[1], -gamma * Dv[0] + (1.0 + gamma * gamma) * Dv[1], Dv[2] };
+                        const double lapf = 4.0 * al * al * (Dv[0] * Dv[0] + Dv[1] * Dv[1] + Dv[2] * Dv[2]) - 2.0 * al * trM;
+                        const double ut[3] = { Gr[idx], Gr[G + idx], Gr[2 * G + idx] };
+                        for (int a = 0; a < 3; ++a) aU[a] += gam * (1.0 + cF * lapf) * ut[a];
+                        aW[0] += al * gam * (Dv[1] * ut[2] - Dv[2] * ut[1]);
+                        aW[1] += al * gam * (Dv[2] * ut[0] - Dv[0] * ut[2]);
+                        aW[2] += al * gam * (Dv[0] * ut[1] - Dv[1] * ut[0]);
+                        for (int a = 0; a < 3; ++a) for (int b = 0; b < 3; ++b)
+                            aE[a][b] += gam * (al * (1.0 + cS * lapf) * (Dv[a] * ut[b] + ut[a] * Dv[b])
+                                               - 4.0 * al * al * cS * (MD[a] * ut[b] + ut[a] * MD[b]));
+                    } else {
+                        for (int a = 0; a < 3; ++a) {
+                            aU[a] += gam * (Gr[a * G + idx] + cF * Gr[(3 + a) * G + idx]);
+                            aW[a] += gam * Gr[(6 + a) * G + idx];
+                        }
+                        for (int e = 0; e < 6; ++e) {
+                            const double v = gam * (Gr[(9 + e) * G + idx] + cS * Gr[(15 + e) * G + idx]);
+                            aE[PA[e]][PB[e]] += v;
+                            if (PA[e] != PB[e]) aE[PB[e]][PA[e]] += v;
+                        }
+                    }
+                    if (s_out) ap += gam * Gr[nbase * G + idx];
+                }
+                for (int a = 0; a < 3; ++a) {
+                    acc[i].U[a] += D3 * aU[a]; acc[i].W[a] += D3 * aW[a];
+                    for (int b = 0; b < 3; ++b) acc[i].E[a][b] += D3 * aE[a][b];
+                }
+                acc[i].p += D3 * ap;
+            }
+        }
+        free(H); free(Hk); free(Gr); free(work);
+    }
+
+    if (!status) {
+        add_self_onebody(acc, N, rad, xi, eta0, parts, F, T, S5);                    /* step 9 */
+        acc_finish(acc, N, rad, U, W, E5, s_out);
+    }
+    free(acc); free(uu);
+    return status;
+}

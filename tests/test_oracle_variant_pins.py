@@ -96,3 +96,47 @@ def test_variant_wave_part_is_reciprocal(oracle, workloads, variant):
     lhs = _dot(x, (ry["U"], ry["Omega"], ry["E"]))
     rhs = _dot(y, (rx["U"], rx["Omega"], rx["E"]))
     assert abs(lhs - rhs) < 1e-12 * max(abs(lhs), abs(rhs))
+
+
+# ------------------------------------------------------------------------------------------------
+# the two variants on the sheared lattice (oracle.o2_apply_variant_sheared)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", [1, 2])
+def test_sheared_variants_reduce_to_the_cubic_ones_at_zero_strain(oracle, workloads, variant):
+    sysm = workloads.random_small_system(4, 9, 9.0)
+    a = (sysm["pos"], sysm["radii"], sysm["L"])
+    b = (0.7, 0.45 * sysm["L"], 16, 9, sysm["F"], sysm["T"], sysm["S"], sysm["s"])
+    cub = oracle.o2_apply_variant(variant, *a, *b)
+    she = oracle.o2_apply_variant_sheared(variant, *a, 0.0, *b)
+    for k in ("U", "Omega", "E", "s_out"):
+        assert _rel(she[k], cub[k]) < 1e-13, k
+
+
+@pytest.mark.parametrize("variant", [1, 2])
+def test_sheared_variants_converge_to_the_sheared_direct_ewald_sum(oracle, workloads, variant):
+    """PAPER.md L501 / Fig. 2 (dashed lines): at gamma = 0.5 every variant converges as in the cubic box."""
+    sysm = workloads.random_small_system(2, 10, 10.0)
+    xi, gamma = 0.6, 0.5
+    mom = (sysm["F"], sysm["T"], sysm["S"], sysm["s"])
+    ref = oracle.o1_apply_sheared(sysm["pos"], sysm["radii"], sysm["L"], gamma, xi, *mom, nimg=4, kmax=16, parts=oracle.PART_WAVE)
+    errs = {}
+    for P in (8, 16, 24):
+        r = oracle.o2_apply_variant_sheared(variant, sysm["pos"], sysm["radii"], sysm["L"], gamma, xi, 0.5 * sysm["L"], 32, P, *mom,
+                                            parts=oracle.PART_WAVE)
+        errs[P] = max(_rel(r["U"], ref[0]), _rel(r["Omega"], ref[1]), _rel(r["E"], ref[2]), _rel(r["s_out"], ref[3]))
+    assert errs[24] < 2e-10 and errs[16] < 1e-3 * errs[8], errs
+
+
+@pytest.mark.parametrize("variant", [1, 2])
+def test_sheared_variant_wave_part_is_reciprocal(oracle, workloads, variant):
+    sysm = workloads.random_small_system(5, 12, 9.0)
+    rng = np.random.default_rng(12)
+    N = len(sysm["radii"])
+    x = (rng.standard_normal((N, 3)), rng.standard_normal((N, 3)), rng.standard_normal((N, 5)))
+    y = (rng.standard_normal((N, 3)), rng.standard_normal((N, 3)), rng.standard_normal((N, 5)))
+    a = (sysm["pos"], sysm["radii"], sysm["L"], 0.35, 0.7, 0.5 * sysm["L"], 16, 8)
+    rx = oracle.o2_apply_variant_sheared(variant, *a, *x, parts=oracle.PART_WAVE)
+    ry = oracle.o2_apply_variant_sheared(variant, *a, *y, parts=oracle.PART_WAVE)
+    lhs = _dot(x, (ry["U"], ry["Omega"], ry["E"]))
+    rhs = _dot(y, (rx["U"], rx["Omega"], rx["E"]))
+    assert abs(lhs - rhs) < 1e-12 * max(abs(lhs), abs(rhs))
