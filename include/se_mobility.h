@@ -134,8 +134,8 @@ se_status se_plan_set_tuning(se_plan *plan, int spread_segments, int gather_segm
  *                            smallest P for a given accuracy, about 6 products' worth of transforms; extra workspace of 24
  *                            half spectra, allocated by the first such product; its stage timings put the seven passes
  *                            under "spread" and the four batches under "gather"; se_plan_debug_stop is not available).
- *                        Both alternatives cover the compressible entry point, cached positions and batches, and are
- *                        built for the cubic box: with a non-zero strain the product returns SE_ERR_UNSUPPORTED.
+ *                        Both alternatives cover the compressible entry point, cached positions, batches and the
+ *                        sheared lattice (se_plan_set_strain; Fig. 2 shows them at gamma = 0.5 as well).
  *   SE_OPT_GRID_FP32     1 = single-precision mesh (Fig. 6: the paper's GPU code computes in single precision): the
  *                        spread grids are rounded to fp32, transformed, scaled and transformed back in fp32 (cuFFT's 3-D
  *                        R2C / C2R) and widened again for the gather; everything on the particle side (Gaussians, the

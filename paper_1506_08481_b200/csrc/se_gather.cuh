@@ -339,7 +339,8 @@ k_gather(SeConst c, GatherGeom g, const double *__restrict__ grecs, const int *_
                     }
                 }
                 } else {
-                    // eight sums: kind 0 gamma, 1 gamma dx, 2 gamma dy, 3 gamma dz, 4..7 the same times d^2
+                    // eight sums: kind 0 gamma, 1 gamma dx, 2 gamma dy, 3 gamma dz, 4..7 the same times D.D (d^2 in the cubic box)
+                    const double g1 = 1.0 + c.gamma * c.gamma, gdy2 = -2.0 * c.gamma;
                     double sm[8];
 #pragma unroll
                     for (int i = 0; i < 8; ++i) sm[i] = 0.0;
@@ -351,7 +352,9 @@ k_gather(SeConst c, GatherGeom g, const double *__restrict__ grecs, const int *_
                             const double dz = d0z + (LZ * q) * Delta, w = gy * rs[4 + PP + bz + LZ * q];
                             const double rho2 = fma(dy, dy, dz * dz);
                             const double t0 = w * m0[a][q], t1 = w * m1[a][q];
-                            const double u0 = w * fma(rho2, m0[a][q], m2[a][q]), u1 = w * fma(rho2, m1[a][q], m3[a][q]);
+                            // weight D.D = (1 + g^2) dx^2 - 2 g dx dy + dy^2 + dz^2 (sheared lattice; g = 0: d^2)
+                            const double u0 = w * fma(rho2, m0[a][q], fma(gdy2 * dy, m1[a][q], g1 * m2[a][q]));
+                            const double u1 = w * fma(rho2, m1[a][q], fma(gdy2 * dy, m2[a][q], g1 * m3[a][q]));
                             sm[0] += t0; sm[1] += t1; sm[2] = fma(dy, t0, sm[2]); sm[3] = fma(dz, t0, sm[3]);
                             sm[4] += u0; sm[5] += u1; sm[6] = fma(dy, u0, sm[6]); sm[7] = fma(dz, u0, sm[7]);
                         }
@@ -424,17 +427,22 @@ __global__ void k_epilogue(SeConst c, unsigned flags, const double *__restrict__
         // sheared lattice: the gathered offsets are fractional (times L); the physical gradient of the Gaussian carries the
         // metric vector D = (dx, dy - gamma dx, dz) (se_spread.cuh), so only the y moments change
         const double gm = c.gamma;
-        // real-space variant: slots 12.. hold the d^2-weighted sums Q of u~ instead of the sums of w~;
-        // lap gamma = (4 al^2 d^2 - 6 al) gamma for U, grad lap gamma = -2 al d (4 al^2 d^2 - 10 al) gamma for E
-        const double q2 = 4.0 * c.alpha * c.alpha, qU = variant == 1 ? -6.0 * c.alpha : 0.0, qE = variant == 1 ? -10.0 * c.alpha : 0.0;
+        // real-space variant: slots 12.. hold the D.D-weighted sums Q of u~ instead of the sums of w~ (D.D = d^2 in the cubic box):
+        // lap gamma = (4 al^2 D.D - 2 al tr) gamma for U; for E the gradient of (1 + cS lap) gamma is
+        // -2 al D (1 + cS (4 al^2 D.D - 2 al tr)) gamma + 8 al^2 cS Mt.D gamma, tr = 3 + g^2 (se_spread.cuh); with g = 0, Mt.D = D and
+        // the last term turns -6 al into the -10 al of the cubic formula
+        const double tr = 3.0 + gm * gm, g1 = 1.0 + gm * gm;
+        const double q2 = 4.0 * c.alpha * c.alpha, qU = variant == 1 ? -2.0 * c.alpha * tr : 0.0, qE = qU, qM = variant == 1 ? -4.0 * c.alpha : 0.0;
         const double qs = variant == 1 ? q2 : 1.0;
 #pragma unroll
         for (int g = 0; g < 3; ++g) {
             A0[g] = m[g]; A1[g] = m[3 + g]; Ay[g] = m[6 + g] - gm * m[3 + g]; Az[g] = m[9 + g];
             v[g] += D3 * (A0[g] + cF * (qs * m[12 + g] + qU * A0[g]));
-            C1[g] = A1[g] + cS * (qs * m[15 + g] + qE * A1[g]);
-            Cy[g] = Ay[g] + cS * (qs * (m[18 + g] - gm * m[15 + g]) + qE * Ay[g]);
-            Cz[g] = Az[g] + cS * (qs * m[21 + g] + qE * Az[g]);
+            // Mt.D from the raw first moments (d = grid offsets): ((1+g^2) dx - g dy, -g (2+g^2) dx + (1+g^2) dy, dz)
+            const double M1 = g1 * m[3 + g] - gm * m[6 + g], My = -gm * (2.0 + gm * gm) * m[3 + g] + g1 * m[6 + g], Mz = m[9 + g];
+            C1[g] = A1[g] + cS * (qs * m[15 + g] + qE * A1[g] + qM * M1);
+            Cy[g] = Ay[g] + cS * (qs * (m[18 + g] - gm * m[15 + g]) + qE * Ay[g] + qM * My);
+            Cz[g] = Az[g] + cS * (qs * m[21 + g] + qE * Az[g] + qM * Mz);
         }
         if (variant == 2) {
             // wave-space variant: plain sums of om~ (slots 24..26), e0~ (36..38, 48..50) and e2~ (60..62, 72..74)

@@ -113,9 +113,11 @@ __global__ void __launch_bounds__(KSPACE_THREADS) k_kspace_wave(SeConst c, doubl
     for (int g = 0; g < 21; ++g) out[g] = z0;
     const bool zero = (ix == 0 && iy == 0 && iz == 0) || ix == M / 2 || iy == M / 2 || iz == M / 2;
     if (!zero) {
-        const double k[3] = { c.twopiL * jx, c.twopiL * jy, c.twopiL * jz };
+        // sheared lattice: k = (2 pi/L)(jx, jy - gamma jx, jz) in every factor; deconvolution in the fractional wave number (k_kspace)
+        const double k[3] = { c.twopiL * jx, c.twopiL * ((double)jy - c.gamma * (double)jx), c.twopiL * jz };
         const double k2 = k[0] * k[0] + k[1] * k[1] + k[2] * k[2];
-        const double dec = exp(-c.dec * k2);
+        const double kq2 = c.twopiL * c.twopiL * ((double)jx * jx + (double)jy * jy + (double)jz * jz);
+        const double dec = c.gamma == 0.0 ? exp(-c.dec * k2) : exp(-k2 * c.inv4xi2 + c.eta_se * kq2 * c.inv4xi2);
         const double sc = c.scale0 * (1.0 + k2 * c.inv4xi2) * dec / k2;
         const int PA[6] = { 0, 0, 0, 1, 1, 2 }, PB[6] = { 0, 1, 2, 1, 2, 2 };
         double2 h[3], Tk[3], Sk[3][3];

@@ -991,8 +991,6 @@ static se_status apply_impl(se_plan *p, const double *pos, const double *F, cons
     if (!F || !T || !S || !U || !Omega || !E) return fail(p, SE_ERR_INVALID_ARG, who, "null pointer");
     if (!pos && !p->have_positions) return fail(p, SE_ERR_INVALID_ARG, who, "pos is NULL and no positions were set (se_plan_set_positions)");
     const bool comp_in = s_in != nullptr, comp_out = s_out != nullptr, comp = comp_in || comp_out;
-    if (p->size_variant != 0 && p->c.gamma != 0.0)
-        return fail(p, SE_ERR_UNSUPPORTED, who, "the real-space and wave-space size variants are built for the cubic box (strain 0) only");
     if (comp) { se_status stc = ensure_compressible(p); if (stc != SE_OK) return stc; }
     const bool wv = p->size_variant == 2;
     const int nret = p->size_variant == 1 ? 3 : 6;          // returned grids: u~ (+ w~ in the hybrid approach)

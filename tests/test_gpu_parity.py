@@ -790,13 +790,30 @@ def test_size_variant_parity(pk, oracle, workloads, name, variant):
     _check_blocks(r.run(), hyb, TOL)
 
 
-def test_size_variants_refuse_the_sheared_lattice(pk, workloads):
-    wl = workloads.make_workload("c1")
+@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("name,gamma", [("c1", 0.3), ("c2", 0.5), ("c3", -0.37)])
+def test_size_variants_on_the_sheared_lattice(pk, oracle, workloads, name, gamma, variant):
+    """PAPER.md Fig. 2 shows the real-space and the wave-space approach at gamma = 0.5 too: wave part alone and full product against
+    oracle.o2_apply_variant_sheared, the compressible entry point included."""
+    import torch
+    wl = workloads.make_workload(name)
     r = Runner(pk, wl)
-    r.plan.set_strain(0.3)
-    r.plan.set_option(pk.SE_OPT_SIZE_VARIANT, 1)
-    with pytest.raises(RuntimeError):
-        r.plan.apply(r.pos, r.F, r.T, r.S, r.U, r.W, r.E)
+    r.plan.set_strain(gamma)
+    r.plan.set_option(pk.SE_OPT_SIZE_VARIANT, variant)
+
+    def ref(parts, s=None):
+        return oracle.o2_apply_variant_sheared(variant, wl.pos, wl.radii, wl.L, gamma, wl.xi, wl.rc, wl.M, wl.P, wl.F, wl.T, wl.S, s=s, parts=parts)
+
+    _check_blocks(r.run(flags=pk.SE_SKIP_REAL | pk.SE_SKIP_SELF | pk.SE_SKIP_ONEBODY), ref(oracle.PART_WAVE), TOL_STAGE)
+    _check_blocks(r.run(), ref(oracle.PART_ALL), TOL)
+    s_np = _pressure_moments(wl)
+    s_in = torch.tensor(s_np, device=r.pos.device, dtype=torch.float64)
+    s_out = torch.full((wl.N,), float("nan"), device=r.pos.device, dtype=torch.float64)
+    r.plan.apply_compressible(r.pos, r.F, r.T, r.S, s_in, r.U, r.W, r.E, s_out)
+    torch.cuda.synchronize()
+    fc = ref(oracle.PART_ALL, s=s_np)
+    _check_blocks((r.U.cpu().numpy(), r.W.cpu().numpy(), r.E.cpu().numpy()), fc, TOL)
+    assert _rel(s_out.cpu().numpy(), fc["s_out"]) <= TOL
 
 
 def _accuracy_runner(pk, oracle, workloads):
