@@ -816,13 +816,17 @@ def test_size_variants_on_the_sheared_lattice(pk, oracle, workloads, name, gamma
     assert _rel(s_out.cpu().numpy(), fc["s_out"]) <= TOL
 
 
-def _accuracy_runner(pk, oracle, workloads):
+def _accuracy_runner(pk, oracle, workloads, gamma=0.0):
     """The paper's accuracy system (N = 50, phi = 0.05, M = 64, xi a1 = 0.1), its wave part by the direct Ewald
     sum O1 and the error measure e_inf,r(E) of Eq. 78 against it."""
     import torch
     sysm = workloads.make_accuracy_system()
     xi, L, N = 0.1, sysm["L"], sysm["N"]
-    ref = oracle.o1_apply(sysm["pos"], sysm["radii"], L, xi, sysm["F"], sysm["T"], sysm["S"], nimg=0, kmax=8, parts=oracle.PART_WAVE)[2]
+    if gamma == 0.0:
+        ref = oracle.o1_apply(sysm["pos"], sysm["radii"], L, xi, sysm["F"], sysm["T"], sysm["S"], nimg=0, kmax=8, parts=oracle.PART_WAVE)[2]
+    else:
+        ref = oracle.o1_apply_sheared(sysm["pos"], sysm["radii"], L, gamma, xi, sysm["F"], sysm["T"], sysm["S"], None, nimg=0, kmax=9,
+                                      parts=oracle.PART_WAVE)[2]
     dev = torch.device("cuda:0")
     t = lambda a: torch.tensor(np.ascontiguousarray(a), device=dev, dtype=torch.float64)
     pos, F, T, S = t(sysm["pos"]), t(sysm["F"]), t(sysm["T"]), t(sysm["S"])
@@ -835,6 +839,8 @@ def _accuracy_runner(pk, oracle, workloads):
 
     def wave_E(P, variant=0, f32=0, m=None):
         plan = pk.SePlan(N, L, sysm["radii"], xi, 0.5 * L, 64, P, 1.0)
+        if gamma != 0.0:
+            plan.set_strain(gamma)
         if m is not None:
             plan.set_shape(m)
         plan.set_option(pk.SE_OPT_SIZE_VARIANT, variant)
@@ -847,13 +853,15 @@ def _accuracy_runner(pk, oracle, workloads):
     return sysm, einf, wave_E
 
 
-def test_fig2_P_ladder_of_the_variants_on_the_gpu(pk, oracle, workloads):
-    """PAPER.md L508 / Fig. 2: e_inf,r(E) ~ 1e-4 needs P = 15, 13, 9 with the real-space, hybrid and wave-space size terms.  The
-    CUDA path reproduces the ladder (crossings within +-2, reading 11) and agrees with the oracle's variant at every P."""
+@pytest.mark.parametrize("gamma", [0.0, 0.5])
+def test_fig2_P_ladder_of_the_variants_on_the_gpu(pk, oracle, workloads, gamma):
+    """PAPER.md L508 / Fig. 2: e_inf,r(E) ~ 1e-4 needs P = 15, 13, 9 with the real-space, hybrid and wave-space size terms, in the
+    orthogonal (solid lines) and in the sheared box, gamma = 0.5 (dashed lines, "almost identical", L501).  The CUDA path
+    reproduces the ladder (crossings within +-2, reading 11) and agrees with the oracle's variant at every P."""
     import math, os
     with open(os.path.join(os.path.dirname(__file__), "golden", "paper_variant_claims.txt")) as f:
         claims = [int(x) for x in [ln for ln in f if not ln.startswith("#")][0].split()]
-    sysm, einf, wave_E = _accuracy_runner(pk, oracle, workloads)
+    sysm, einf, wave_E = _accuracy_runner(pk, oracle, workloads, gamma)
     L = sysm["L"]
     for variant, p_paper, Ps in ((1, claims[0], (11, 13, 15, 17)), (0, claims[1], (9, 11, 13, 15)), (2, claims[2], (5, 7, 9, 11))):
         errs = {}
@@ -862,8 +870,8 @@ def test_fig2_P_ladder_of_the_variants_on_the_gpu(pk, oracle, workloads):
             for f in (0.9, 1.0):
                 m = f * math.sqrt(math.pi * P)
                 Eg = wave_E(P, variant, m=m)
-                Eo = oracle.o2_apply_variant(variant, sysm["pos"], sysm["radii"], L, 0.1, 0.5 * L, 64, P, sysm["F"], sysm["T"], sysm["S"],
-                                             m=m, parts=oracle.PART_WAVE)["E"]
+                Eo = oracle.o2_apply_variant_sheared(variant, sysm["pos"], sysm["radii"], L, gamma, 0.1, 0.5 * L, 64, P, sysm["F"], sysm["T"],
+                                                     sysm["S"], m=m, parts=oracle.PART_WAVE)["E"]
                 assert _rel(Eg, Eo) <= TOL_STAGE, (variant, P, f)
                 best = einf(Eg) if best is None else min(best, einf(Eg))
             errs[P] = best
