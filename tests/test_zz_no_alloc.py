@@ -72,3 +72,29 @@ def test_no_alloc_rejects_sizes_beyond_the_static_scratch():
     with pytest.raises(pk.SeError) as ei:
         pk.real_noalloc(100.0, 0.5, 4.0, z(3), torch.ones(N, device=dev, dtype=torch.float64), z(3), z(3), z(5), z(3), z(3), z(5))
     assert ei.value.status == 1 and "SE_NOALLOC_MAX_N" in str(ei.value)
+
+
+@pytest.mark.gpu
+def test_no_alloc_at_the_maximum_size_and_with_a_single_particle(workloads):
+    """N = SE_NOALLOC_MAX_N exactly (the first 8192 particles of c3: the whole scratch array is in use, several candidate chunks
+    per target in the all-pairs scan) against the plan path, and N = 1 (no pair at all: zeros, not stale scratch)."""
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_1506_08481_b200 as pk
+    dev = torch.device("cuda:0")
+    t = lambda a: torch.tensor(np.ascontiguousarray(a), device=dev, dtype=torch.float64)
+    wl = workloads.make_workload("c3")
+    N = pk.SE_NOALLOC_MAX_N
+    assert wl.N >= N
+    wl.N, wl.pos, wl.radii, wl.F, wl.T, wl.S = N, wl.pos[:N], wl.radii[:N], wl.F[:N], wl.T[:N], wl.S[:N]
+    ref = _existing_path(pk, torch, wl, dev)
+    U, W, E = (torch.full((N, k), float("nan"), device=dev, dtype=torch.float64) for k in (3, 3, 5))
+    pk.real_noalloc(wl.L, wl.xi, wl.rc, t(wl.pos), t(wl.radii), t(wl.F), t(wl.T), t(wl.S), U, W, E, eta0=wl.eta0)
+    torch.cuda.synchronize()
+    for g, r in zip((U, W, E), ref):
+        assert _rel(g.cpu().numpy(), r) <= TOL_STAGE
+    # one particle, right after the full-size call
+    U1, W1, E1 = (torch.full((1, k), float("nan"), device=dev, dtype=torch.float64) for k in (3, 3, 5))
+    pk.real_noalloc(wl.L, wl.xi, wl.rc, t(wl.pos[:1]), t(wl.radii[:1]), t(wl.F[:1]), t(wl.T[:1]), t(wl.S[:1]), U1, W1, E1)
+    torch.cuda.synchronize()
+    assert float(U1.abs().sum() + W1.abs().sum() + E1.abs().sum()) == 0.0
