@@ -653,8 +653,11 @@ extern "C" se_status se_plan_create(se_plan **out, int64_t N, double L, const do
     }
     p->have_side = true;
     {   // beside the wave pipeline a2 runs as a persistent grid of one CTA per SM (measured best on B200: it then
-        // takes little from the HBM-bound kernels' occupancy; c4 step 3.57 -> 3.50 ms)
-        p->real_side_ctas = p->sms;
+        // takes little from the HBM-bound kernels' occupancy; c4 step 3.57 -> 3.50 ms) -- as long as a CTA walks no more than
+        // about 256 cells: beyond that the walk can outlast the wave pipeline and become the critical path (c5, 537 cells per
+        // CTA: 26.8 ... 29.1 ms from run to run with one CTA per SM, 26.98 ms every time with two or three)
+        const int per_sm = (p->ncell_r + 256 * p->sms - 1) / (256 * p->sms);
+        p->real_side_ctas = p->sms * (per_sm < 1 ? 1 : (per_sm > 3 ? 3 : per_sm));
         p->real_overlap = 1;
         p->use_graph = M <= 128 ? 1 : 0;
         p->pair_cache = 1;
