@@ -103,7 +103,8 @@ se_status se_plan_set_tuning(se_plan *plan, int spread_segments, int gather_segm
  *                        0 = on the caller's stream before the spreading; 1 = on a plan-owned low-priority stream
  *                        beside the whole wave pipeline; 2 = on that stream, started after the spreading (beside the
  *                        HBM-bound transforms).  Joined before the epilogue in every case.
- *   SE_OPT_REAL_CTAS     CTAs of the real-space kernel when it runs beside the wave pipeline (0 = one per cell).
+ *   SE_OPT_REAL_CTAS     CTAs of the real-space kernel when it runs beside the wave pipeline (0 = one per cell).  Default: a
+ *                        persistent grid of one CTA per SM and per 256 cells to walk, at most three per SM.
  *   SE_OPT_XY_PATH       reserved (round 1's cuFFT 2-D path was removed when the own y / fused x kernels replaced it);
  *                        SE_ERR_INVALID_ARG.
  *   SE_OPT_YZ_FUSED      1 = the y and z transforms of a direction in ONE kernel (thread-block
